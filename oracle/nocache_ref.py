@@ -1,0 +1,95 @@
+"""Independent no-cache model of the dense decoder — TEST INFRASTRUCTURE ONLY (pins the C oracle).
+
+A separately written float64 numpy routine that runs the WHOLE prefix at once: library matmul,
+explicit causal mask, library softmax pieces, RoPE in complex form.  It shares nothing with
+oracle/spd_oracle.c (different language, no KV cache, no token loop), so a dropped term, a wrong
+sign/index or a transposed operand in either one shows up as a mismatch.
+
+Architecture (BASELINE.json configs; SURVEY C-2.13): pre-norm, no biases, no QK-norm, GQA, SwiGLU,
+RoPE (rotate-half pairing, base from the config) on all head dims, scale 1/sqrt(hd), causal incl.
+self.  K and V are rounded to bf16 as the cache stores them (C-2.17); bf16 rounding here is torch's.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+
+def _w(bits: np.ndarray) -> np.ndarray:
+    """bf16 bits -> float64 via torch's own bf16 type (not the generator's shift)."""
+    t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16)
+    return t.to(torch.float64).numpy()
+
+
+def _round_bf16(x: np.ndarray) -> np.ndarray:
+    return torch.from_numpy(x.astype(np.float32)).to(torch.bfloat16).to(torch.float64).numpy()
+
+
+def _rmsnorm(x: np.ndarray, gain: np.ndarray, eps: float) -> np.ndarray:
+    return x / np.sqrt(np.mean(x * x, axis=-1, keepdims=True) + eps) * gain
+
+
+def _rope(x: np.ndarray, positions: np.ndarray, base: float) -> np.ndarray:
+    """x: [T, H, hd].  Pair (i, i+hd/2) is the complex number x_i + 1j*x_{i+hd/2}, multiplied by
+    exp(1j * pos * base^(-2i/hd)).  cos/sin are rounded to fp32 as the contract says (C-2.14)."""
+    T, H, hd = x.shape
+    half = hd // 2
+    theta = float(base) ** (-2.0 * np.arange(half, dtype=np.float64) / hd)
+    ang = positions.astype(np.float64)[:, None] * theta[None, :]
+    rot = np.cos(ang).astype(np.float32).astype(np.float64) + 1j * np.sin(ang).astype(np.float32).astype(np.float64)
+    z = (x[..., :half] + 1j * x[..., half:]) * rot[:, None, :]
+    return np.concatenate([z.real, z.imag], axis=-1)
+
+
+def forward_nocache(shape, weights, tokens, keep_hidden: bool = False) -> dict:
+    """Full-sequence forward.  Returns {"logits": [T, V] f64, "final": [T, d] pre-norm final hidden,
+    "k": [L][T, Hkv*hd] bf16-rounded f64, "v": same, "hidden": [L+1, T, d] if keep_hidden}."""
+    tokens = np.asarray(tokens, dtype=np.int64)
+    T = len(tokens)
+    d, Hq, Hkv, hd = shape.d_model, shape.n_q_heads, shape.n_kv_heads, shape.head_dim
+    eps, base = float(np.float32(shape.rms_eps)), float(np.float32(shape.rope_base))
+    E = _w(weights["embed"])
+    h = E[tokens]                                           # [T, d]
+    pos = np.arange(T)
+    causal = np.tril(np.ones((T, T), dtype=bool))           # row = query position, col = key position
+    hidden = [h.copy()] if keep_hidden else None
+    ks, vs = [], []
+    for l in range(shape.n_layers):
+        x = _rmsnorm(h, _w(weights["attn_norm"][l]), eps)
+        q = (x @ _w(weights["wq"][l]).T).astype(np.float32).astype(np.float64).reshape(T, Hq, hd)
+        k = (x @ _w(weights["wk"][l]).T).astype(np.float32).astype(np.float64).reshape(T, Hkv, hd)
+        v = (x @ _w(weights["wv"][l]).T).astype(np.float32).astype(np.float64).reshape(T, Hkv, hd)
+        q = _rope(q, pos, base)
+        k = _round_bf16(_rope(k, pos, base))
+        v = _round_bf16(v)
+        ks.append(k.reshape(T, Hkv * hd))
+        vs.append(v.reshape(T, Hkv * hd))
+        kx = np.repeat(k, Hq // Hkv, axis=1)                # kv-head hq // group serves q-head hq
+        vx = np.repeat(v, Hq // Hkv, axis=1)
+        s = np.einsum("qhe,khe->hqk", q, kx) / np.sqrt(hd)
+        s = np.where(causal[None], s, -np.inf)
+        s = s - s.max(axis=-1, keepdims=True)
+        w = np.exp(s)
+        w = w / w.sum(axis=-1, keepdims=True)
+        o = np.einsum("hqk,khe->qhe", w, vx).reshape(T, Hq * hd)
+        h = h + o @ _w(weights["wo"][l]).T
+        x = _rmsnorm(h, _w(weights["mlp_norm"][l]), eps)
+        g = x @ _w(weights["w_gate"][l]).T
+        u = x @ _w(weights["w_up"][l]).T
+        h = h + ((g / (1.0 + np.exp(-g))) * u) @ _w(weights["w_down"][l]).T
+        if keep_hidden:
+            hidden.append(h.copy())
+    logits = _rmsnorm(h, _w(weights["final_norm"]), eps) @ E.T
+    out = {"logits": logits, "final": h, "k": ks, "v": vs}
+    if keep_hidden:
+        out["hidden"] = np.stack(hidden)
+    return out
+
+
+def pdm_ref(shape, weights, feats: np.ndarray) -> dict:
+    """The simplified PDM (BASELINE.json north_star) as a pure function of its n slot vectors:
+    u = W_p . concat(f_0..f_{n-1}); z = RMSNorm(u; g_pdm); logits = E . z.   feats: [n, d]."""
+    f = np.asarray(feats, dtype=np.float64).reshape(-1)
+    u = _w(weights["pdm_proj"]) @ f
+    z = _rmsnorm(u, _w(weights["pdm_norm"]), float(np.float32(shape.rms_eps)))
+    return {"u": u, "logits": _w(weights["embed"]) @ z}

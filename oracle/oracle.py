@@ -1,0 +1,319 @@
+"""ctypes wrapper over oracle/spd_oracle.c.  Argument marshalling only — no arithmetic here."""
+from __future__ import annotations
+
+import ctypes as C
+from typing import NamedTuple
+
+import numpy as np
+
+from . import build as _build
+
+_LAYER_NAMES = ["attn_norm", "wq", "wk", "wv", "wo", "mlp_norm", "w_gate", "w_up", "w_down"]
+
+
+class _Cfg(C.Structure):
+    _fields_ = [(k, C.c_int32) for k in ("d_model", "n_layers", "n_stages", "n_q_heads", "n_kv_heads",
+                                          "head_dim", "d_ffn", "vocab", "max_seq")] + \
+               [("rms_eps", C.c_float), ("rope_base", C.c_float)]
+
+
+_PP = C.POINTER(C.c_void_p)
+
+
+class _Weights(C.Structure):
+    _fields_ = [("embed", C.c_void_p)] + [(k, _PP) for k in _LAYER_NAMES] + \
+               [("final_norm", C.c_void_p), ("pdm_proj", C.c_void_p), ("pdm_norm", C.c_void_p)]
+
+
+class _Res(C.Structure):
+    _fields_ = [(k, C.c_int32) for k in ("step_index", "fill", "exited", "accepted", "emitted_token",
+                                          "draft_token", "draft_forced", "discarded", "committed_len")]
+
+
+class StepResult(NamedTuple):
+    step_index: int
+    fill: int
+    exited: int
+    accepted: int
+    emitted_token: int
+    draft_token: int
+    draft_forced: int
+    discarded: int
+    committed_len: int
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        L.ora_create.restype = C.c_void_p
+        L.ora_create.argtypes = [C.POINTER(_Cfg), C.POINTER(_Weights)]
+        L.ora_destroy.argtypes = [C.c_void_p]
+        L.ora_prefill.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_int32)]
+        L.ora_step.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_Res)]
+        L.ora_rollback.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+        L.ora_set_forced.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_float, C.c_uint64]
+        L.ora_ar_step.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+        L.ora_ar_set_trace.argtypes = [C.c_void_p, C.c_void_p]
+        L.ora_set_forward_order.argtypes = [C.c_void_p, C.c_int32]
+        L.ora_committed_len.argtypes = [C.c_void_p]
+        L.ora_fill.argtypes = [C.c_void_p]
+        L.ora_steps.argtypes = [C.c_void_p]
+        L.ora_steps.restype = C.c_int64
+        L.ora_emitted.argtypes = [C.c_void_p]
+        L.ora_get_kv_len.argtypes = [C.c_void_p, C.c_void_p]
+        L.ora_get_kv.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p]
+        L.ora_get_ring.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
+                                   C.POINTER(C.c_int32), C.c_void_p]
+        L.ora_get_hfin.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+        L.ora_get_last.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+        L.ora_get_margin.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        L.ora_load_kv.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32]
+        L.ora_assume_prefilled.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+        L.ora_op_rmsnorm.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_float, C.c_void_p]
+        L.ora_op_gemv.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+        L.ora_op_rope.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float]
+        L.ora_op_attention.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
+                                       C.c_int32, C.c_void_p]
+        L.ora_op_silu_mul.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+        L.ora_op_argmax.argtypes = [C.c_void_p, C.c_int32]
+        L.ora_op_f32_to_bf16.argtypes = [C.c_float]
+        L.ora_op_f32_to_bf16.restype = C.c_uint16
+        L.ora_op_splitmix64.argtypes = [C.c_uint64]
+        L.ora_op_splitmix64.restype = C.c_uint64
+        L.ora_num_threads.restype = C.c_int32
+        _lib = L
+    return _lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _u16(a) -> np.ndarray:
+    a = np.ascontiguousarray(a)
+    assert a.dtype == np.uint16, a.dtype
+    return a
+
+
+def _f32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+class Oracle:
+    """One oracle context.  `shape` is a spd_inputs.ModelShape (or anything with the same fields);
+    `weights` is the dict spd_inputs.make_weights returns (uint16 bf16-bit arrays)."""
+
+    def __init__(self, shape, weights, max_seq: int | None = None):
+        self.shape = shape
+        self.max_seq = int(max_seq if max_seq is not None else shape.max_seq)
+        self._keep = []
+        cfg = _Cfg(shape.d_model, shape.n_layers, shape.n_stages, shape.n_q_heads, shape.n_kv_heads,
+                   shape.head_dim, shape.d_ffn, shape.vocab, self.max_seq, shape.rms_eps, shape.rope_base)
+        w = _Weights()
+        for name in ("embed", "final_norm", "pdm_proj", "pdm_norm"):
+            arr = _u16(weights[name])
+            self._keep.append(arr)
+            setattr(w, name, arr.ctypes.data)
+        for name in _LAYER_NAMES:
+            arrs = [_u16(x) for x in weights[name]]
+            self._keep.extend(arrs)
+            tab = (C.c_void_p * len(arrs))(*[x.ctypes.data for x in arrs])
+            self._keep.append(tab)
+            setattr(w, name, C.cast(tab, _PP))
+        self._h = lib().ora_create(C.byref(cfg), C.byref(w))
+        if not self._h:
+            raise ValueError("ora_create rejected the configuration")
+
+    def close(self):
+        if self._h:
+            lib().ora_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- path ------------------------------------------------------------------------------
+    def prefill(self, tokens, block: int = 1) -> int:
+        t = np.ascontiguousarray(tokens, dtype=np.int32)
+        first = C.c_int32(-1)
+        rc = lib().ora_prefill(self._h, _p(t), len(t), block, C.byref(first))
+        if rc:
+            raise RuntimeError(f"ora_prefill rc={rc}")
+        return first.value
+
+    def step(self, draft_override: int = -1) -> StepResult:
+        r = _Res()
+        rc = lib().ora_step(self._h, draft_override, C.byref(r))
+        if rc:
+            raise RuntimeError(f"ora_step rc={rc}")
+        return StepResult(*[getattr(r, k) for k, _ in _Res._fields_])
+
+    def rollback(self, new_len: int, reseed_token: int) -> int:
+        return lib().ora_rollback(self._h, new_len, reseed_token)
+
+    def set_forced(self, truth, p: float, seed: int):
+        if truth is None:
+            rc = lib().ora_set_forced(self._h, None, 0, p, seed)
+        else:
+            t = np.ascontiguousarray(truth, dtype=np.int32)
+            self._keep.append(t)
+            rc = lib().ora_set_forced(self._h, _p(t), len(t), p, seed)
+        if rc:
+            raise ValueError("ora_set_forced")
+
+    def ar_step(self) -> int:
+        nxt = C.c_int32(-1)
+        rc = lib().ora_ar_step(self._h, C.byref(nxt))
+        if rc:
+            raise RuntimeError(f"ora_ar_step rc={rc}")
+        return nxt.value
+
+    def ar_set_trace(self, enable: bool = True):
+        if enable:
+            self._trace = np.zeros((self.shape.n_layers + 1, self.shape.d_model), dtype=np.float32)
+            lib().ora_ar_set_trace(self._h, _p(self._trace))
+        else:
+            self._trace = None
+            lib().ora_ar_set_trace(self._h, None)
+        return self._trace
+
+    def set_forward_order(self, reverse: bool):
+        lib().ora_set_forward_order(self._h, int(reverse))
+
+    def generate_spd(self, n_tokens: int, draft_fn=None, max_steps: int | None = None):
+        """Run cycles until n_tokens tokens are emitted (the prefill's first token counts).
+        Returns (emitted tokens excluding the first, list of StepResult)."""
+        out, log = [], []
+        limit = max_steps if max_steps is not None else 10 ** 9
+        while lib().ora_emitted(self._h) < n_tokens and len(log) < limit:
+            ov = -1 if draft_fn is None else int(draft_fn(self))
+            r = self.step(ov)
+            log.append(r)
+            if r.exited:
+                out.append(r.emitted_token)
+        return out, log
+
+    # -- readers ---------------------------------------------------------------------------
+    @property
+    def committed_len(self) -> int:
+        return lib().ora_committed_len(self._h)
+
+    @property
+    def fill(self) -> int:
+        return lib().ora_fill(self._h)
+
+    @property
+    def steps(self) -> int:
+        return lib().ora_steps(self._h)
+
+    @property
+    def emitted(self) -> int:
+        return lib().ora_emitted(self._h)
+
+    def kv_len(self) -> np.ndarray:
+        out = np.zeros(self.shape.n_layers, dtype=np.int32)
+        lib().ora_get_kv_len(self._h, _p(out))
+        return out
+
+    def kv(self, layer: int, which: int, rows: int) -> np.ndarray:
+        out = np.zeros((rows, self.shape.n_kv_heads * self.shape.head_dim), dtype=np.uint16)
+        if rows:
+            lib().ora_get_kv(self._h, layer, which, rows, _p(out))
+        return out
+
+    def ring(self, i: int):
+        pos, tok, k = C.c_int32(), C.c_int32(), C.c_int32()
+        h = np.zeros(self.shape.d_model, dtype=np.float32)
+        rc = lib().ora_get_ring(self._h, i, C.byref(pos), C.byref(tok), C.byref(k), _p(h))
+        if rc:
+            raise IndexError(i)
+        return pos.value, tok.value, k.value, h
+
+    def hfin(self, pos: int) -> np.ndarray:
+        out = np.zeros(self.shape.d_model, dtype=np.float32)
+        lib().ora_get_hfin(self._h, pos, _p(out))
+        return out
+
+    def last(self, what: str) -> np.ndarray:
+        idx = {"exit_logits": 0, "pdm_logits": 1, "pdm_prenorm": 2, "pdm_feat": 3}[what]
+        n = {0: self.shape.vocab, 1: self.shape.vocab, 2: self.shape.d_model,
+             3: self.shape.d_model * self.shape.n_stages}[idx]
+        out = np.zeros(n, dtype=np.float32)
+        lib().ora_get_last(self._h, idx, _p(out))
+        return out
+
+    def margin(self, which: int):
+        g, m = C.c_float(), C.c_float()
+        lib().ora_get_margin(self._h, which, C.byref(g), C.byref(m))
+        return g.value, m.value
+
+    # -- timing-only -----------------------------------------------------------------------
+    def load_kv(self, layer: int, k: np.ndarray, v: np.ndarray):
+        k, v = _u16(k), _u16(v)
+        lib().ora_load_kv(self._h, layer, _p(k), _p(v), k.shape[0])
+
+    def assume_prefilled(self, committed_len: int, first_token: int):
+        if lib().ora_assume_prefilled(self._h, committed_len, first_token):
+            raise ValueError("ora_assume_prefilled")
+
+
+# -- single operations (per-kernel parity) -----------------------------------------------------
+
+def op_rmsnorm(x, gain, eps: float) -> np.ndarray:
+    x, gain = _f32(x), _u16(gain)
+    out = np.empty_like(x)
+    lib().ora_op_rmsnorm(_p(x), _p(gain), x.size, eps, _p(out))
+    return out
+
+
+def op_gemv(w, x) -> np.ndarray:
+    w, x = _u16(w), _f32(x)
+    rows, k = w.shape
+    assert x.size == k
+    out = np.empty(rows, dtype=np.float32)
+    lib().ora_op_gemv(_p(w), rows, k, _p(x), _p(out))
+    return out
+
+
+def op_rope(vec, n_heads: int, head_dim: int, pos: int, base: float) -> np.ndarray:
+    v = _f32(vec).copy()
+    lib().ora_op_rope(_p(v), n_heads, head_dim, pos, base)
+    return v
+
+
+def op_attention(q, kc, vc, n_q_heads: int, n_kv_heads: int, head_dim: int) -> np.ndarray:
+    q, kc, vc = _f32(q), _u16(kc), _u16(vc)
+    out = np.empty(n_q_heads * head_dim, dtype=np.float32)
+    lib().ora_op_attention(_p(q), _p(kc), _p(vc), kc.shape[0], n_q_heads, n_kv_heads, head_dim, _p(out))
+    return out
+
+
+def op_silu_mul(gate, up) -> np.ndarray:
+    g, u = _f32(gate), _f32(up)
+    out = np.empty_like(g)
+    lib().ora_op_silu_mul(_p(g), _p(u), g.size, _p(out))
+    return out
+
+
+def op_argmax(x) -> int:
+    x = _f32(x)
+    return lib().ora_op_argmax(_p(x), x.size)
+
+
+def op_f32_to_bf16(x: float) -> int:
+    return lib().ora_op_f32_to_bf16(x)
+
+
+def op_splitmix64(x: int) -> int:
+    return lib().ora_op_splitmix64(x & 0xFFFFFFFFFFFFFFFF)
+
+
+def num_threads() -> int:
+    return lib().ora_num_threads()

@@ -1,0 +1,564 @@
+/* spd_oracle.c — CPU oracle for the SPD step.  TEST INFRASTRUCTURE ONLY; see spd_oracle.h.
+ *
+ * Written from /root/reference/PAPER.md (cited as PAPER.md:<line>) and the readings C-1 / C-2.x of
+ * SURVEY.md §8(c) (also listed in DESIGN.md).  Plain loops, fp32 tensors, fp64 accumulation,
+ * OpenMP only over independent output rows.  No blocking/fusion except ora_prefill(block>1), which
+ * only interchanges the (token, row) loops.
+ */
+#include "spd_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ------------------------------------------------------------------ scalars and bf16 ---------- */
+
+static inline float bf16_to_f32(uint16_t b) {
+  uint32_t u = (uint32_t)b << 16;
+  float f;
+  memcpy(&f, &u, 4);
+  return f;
+}
+
+/* fp32 -> bf16, round to nearest even (C-2.17: the only rounding below fp32 on the path). */
+uint16_t ora_op_f32_to_bf16(float x) {
+  uint32_t u;
+  memcpy(&u, &x, 4);
+  if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x40); /* NaN stays NaN */
+  u += 0x7fffu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+
+/* C-2.19: the forced-acceptance draw is a pure integer function of (seed, step counter). */
+uint64_t ora_op_splitmix64(uint64_t x) {
+  uint64_t z = x + 0x9e3779b97f4a7c15ull;
+  z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull;
+  z = (z ^ (z >> 27)) * 0x94d049bb133111ebull;
+  return z ^ (z >> 31);
+}
+
+int32_t ora_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/* Dot product of a bf16 weight row with an fp32 vector, accumulated in fp64.  Sixteen interleaved
+ * partial sums (element i goes to partial i mod 16) are added in index order at the end, so the
+ * value does not depend on how the compiler vectorises the loop. */
+static inline double dot_row(const uint16_t *w, const float *x, int k) {
+  double acc[16];
+  for (int j = 0; j < 16; ++j) acc[j] = 0.0;
+  int i = 0;
+  for (; i + 16 <= k; i += 16)
+    for (int j = 0; j < 16; ++j) acc[j] += (double)bf16_to_f32(w[i + j]) * (double)x[i + j];
+  for (int j = 0; i < k; ++i, ++j) acc[j] += (double)bf16_to_f32(w[i]) * (double)x[i];
+  double s = 0.0;
+  for (int j = 0; j < 16; ++j) s += acc[j];
+  return s;
+}
+
+/* ------------------------------------------------------------------ single operations --------- */
+
+/* RMSNorm(x, g) = x * (mean(x^2) + eps)^(-1/2) * g   (C-1; eps from BASELINE.json). */
+void ora_op_rmsnorm(const float *x, const uint16_t *gain, int32_t d, float eps, float *out) {
+  double ss = 0.0;
+  for (int i = 0; i < d; ++i) ss += (double)x[i] * (double)x[i];
+  double r = 1.0 / sqrt(ss / (double)d + (double)eps);
+  for (int i = 0; i < d; ++i) out[i] = (float)((double)x[i] * r * (double)bf16_to_f32(gain[i]));
+}
+
+/* out = W x, W bf16 [rows, k] row-major. */
+void ora_op_gemv(const uint16_t *w, int32_t rows, int32_t k, const float *x, float *out) {
+#pragma omp parallel for schedule(static)
+  for (int r = 0; r < rows; ++r) out[r] = (float)dot_row(w + (size_t)r * k, x, k);
+}
+
+/* Same product for a block of vectors: Y[t][r] = W[r] . X[t].  Rows outside, tokens inside, so a
+ * weight row is read once per block; each (t, r) value is the same dot_row call as in ora_op_gemv. */
+static void gemv_block(const uint16_t *w, int rows, int k, const float *x, int ldx, float *y, int ldy,
+                       int nt) {
+#pragma omp parallel for schedule(static)
+  for (int r = 0; r < rows; ++r)
+    for (int t = 0; t < nt; ++t) y[(size_t)t * ldy + r] = (float)dot_row(w + (size_t)r * k, x + (size_t)t * ldx, k);
+}
+
+/* RoPE, rotate-half pairing (C-2.14): pair (i, i+hd/2), theta_i = base^(-2i/hd), angle = pos*theta_i,
+ * cos/sin evaluated in double and rounded to fp32. */
+void ora_op_rope(float *vec, int32_t n_heads, int32_t head_dim, int32_t pos, float base) {
+  int half = head_dim / 2;
+  for (int i = 0; i < half; ++i) {
+    double theta = pow((double)base, -2.0 * (double)i / (double)head_dim);
+    double ang = (double)pos * theta;
+    float c = (float)cos(ang), s = (float)sin(ang);
+    for (int h = 0; h < n_heads; ++h) {
+      float *v = vec + (size_t)h * head_dim;
+      double a = v[i], b = v[i + half];
+      v[i] = (float)(a * (double)c - b * (double)s);
+      v[i + half] = (float)(b * (double)c + a * (double)s);
+    }
+  }
+}
+
+/* GQA decode attention for one token (C-1): for q-head hq, kv-head kvh = hq / (Hq/Hkv),
+ * s_t = q_hq . K[t][kvh] / sqrt(hd) for t = 0..t_len-1, w = softmax(s), o_hq = sum_t w_t V[t][kvh].
+ * kc, vc: bf16 [t_len, Hkv*hd] (row t = position t). */
+void ora_op_attention(const float *q, const uint16_t *kc, const uint16_t *vc, int32_t t_len,
+                      int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, float *out) {
+  int group = n_q_heads / n_kv_heads;
+  size_t row = (size_t)n_kv_heads * head_dim;
+#pragma omp parallel for schedule(static)
+  for (int hq = 0; hq < n_q_heads; ++hq) {
+    int kvh = hq / group;
+    const float *qh = q + (size_t)hq * head_dim;
+    float *s = (float *)malloc(sizeof(float) * (size_t)t_len);
+    float m = -INFINITY;
+    for (int t = 0; t < t_len; ++t) {
+      double dot = dot_row(kc + (size_t)t * row + (size_t)kvh * head_dim, qh, head_dim);
+      s[t] = (float)(dot / sqrt((double)head_dim));
+      if (s[t] > m) m = s[t];
+    }
+    double *w = (double *)malloc(sizeof(double) * (size_t)t_len);
+    double denom = 0.0;
+    for (int t = 0; t < t_len; ++t) { w[t] = exp((double)s[t] - (double)m); denom += w[t]; }
+    for (int e = 0; e < head_dim; ++e) {
+      double acc = 0.0;
+      for (int t = 0; t < t_len; ++t)
+        acc += w[t] * (double)bf16_to_f32(vc[(size_t)t * row + (size_t)kvh * head_dim + e]);
+      out[(size_t)hq * head_dim + e] = (float)(acc / denom);
+    }
+    free(w);
+    free(s);
+  }
+}
+
+/* a = silu(gate) * up, silu(z) = z / (1 + exp(-z))  (C-1). */
+void ora_op_silu_mul(const float *gate, const float *up, int32_t n, float *out) {
+  for (int i = 0; i < n; ++i) {
+    double z = gate[i];
+    out[i] = (float)(z / (1.0 + exp(-z)) * (double)up[i]);
+  }
+}
+
+/* Greedy argmax: maximum value, lowest index among exact ties (C-2.8). */
+int32_t ora_op_argmax(const float *x, int32_t n) {
+  int best = 0;
+  for (int i = 1; i < n; ++i)
+    if (x[i] > x[best]) best = i;
+  return best;
+}
+
+static void top2_margin(const float *x, int n, float *gap, float *maxabs) {
+  float a = -INFINITY, b = -INFINITY, mx = 0.f;
+  for (int i = 0; i < n; ++i) {
+    float v = x[i];
+    if (v > a) { b = a; a = v; } else if (v > b) b = v;
+    if (fabsf(v) > mx) mx = fabsf(v);
+  }
+  *gap = a - b;
+  *maxabs = mx;
+}
+
+/* ------------------------------------------------------------------ context ------------------- */
+
+struct ora_ctx {
+  ora_config cfg;
+  ora_weights w;
+  uint16_t *kc, *vc; /* [L][max_seq][Hkv*hd] bf16 */
+  int32_t *len;      /* [L] valid KV rows (C-2.11) */
+  float *hfin;       /* [max_seq][d] final (pre-norm) hidden state of committed positions (C-2.4) */
+  int32_t c;         /* committed length */
+  int32_t a;         /* in-flight tokens, oldest first */
+  int32_t *r_pos, *r_tok, *r_k;
+  float *r_h;        /* [n][d] */
+  int64_t steps;     /* K */
+  int32_t emitted;   /* N */
+  int32_t prompt_len, prefilled;
+  const int32_t *truth;
+  int32_t n_truth;
+  int32_t forced_on;
+  uint64_t forced_thresh, forced_seed;
+  /* last-step records */
+  float *exit_logits, *pdm_logits, *pdm_u, *pdm_feat;
+  float gap[2], maxabs[2];
+  float *ar_trace;
+  int32_t reverse_forward;
+  /* scratch */
+  float *x, *q, *kk, *vv, *att, *o, *g, *u, *act, *dn, *z;
+};
+
+static size_t kv_row(const ora_config *c) { return (size_t)c->n_kv_heads * c->head_dim; }
+
+ora_ctx *ora_create(const ora_config *cfg, const ora_weights *w) {
+  if (!cfg || !w) return NULL;
+  if (cfg->n_stages < 1 || cfg->n_layers % cfg->n_stages != 0) return NULL;      /* C-2.7 */
+  if (cfg->n_kv_heads < 1 || cfg->n_q_heads % cfg->n_kv_heads != 0 || cfg->head_dim % 2 != 0) return NULL;
+  ora_ctx *o = (ora_ctx *)calloc(1, sizeof(ora_ctx));
+  o->cfg = *cfg;
+  o->w = *w;
+  int d = cfg->d_model, n = cfg->n_stages, L = cfg->n_layers, F = cfg->d_ffn, V = cfg->vocab;
+  size_t row = kv_row(cfg);
+  o->kc = (uint16_t *)calloc((size_t)L * cfg->max_seq * row, 2);
+  o->vc = (uint16_t *)calloc((size_t)L * cfg->max_seq * row, 2);
+  o->len = (int32_t *)calloc(L, 4);
+  o->hfin = (float *)calloc((size_t)cfg->max_seq * d, 4);
+  o->r_pos = (int32_t *)calloc(n, 4);
+  o->r_tok = (int32_t *)calloc(n, 4);
+  o->r_k = (int32_t *)calloc(n, 4);
+  o->r_h = (float *)calloc((size_t)n * d, 4);
+  o->exit_logits = (float *)calloc(V, 4);
+  o->pdm_logits = (float *)calloc(V, 4);
+  o->pdm_u = (float *)calloc(d, 4);
+  o->pdm_feat = (float *)calloc((size_t)n * d, 4);
+  int qd = cfg->n_q_heads * cfg->head_dim;
+  o->x = (float *)calloc(d, 4);
+  o->q = (float *)calloc(qd, 4);
+  o->kk = (float *)calloc(row, 4);
+  o->vv = (float *)calloc(row, 4);
+  o->att = (float *)calloc(qd, 4);
+  o->o = (float *)calloc(d, 4);
+  o->g = (float *)calloc(F, 4);
+  o->u = (float *)calloc(F, 4);
+  o->act = (float *)calloc(F, 4);
+  o->dn = (float *)calloc(d, 4);
+  o->z = (float *)calloc(d, 4);
+  return o;
+}
+
+void ora_destroy(ora_ctx *o) {
+  if (!o) return;
+  free(o->kc); free(o->vc); free(o->len); free(o->hfin); free(o->r_pos); free(o->r_tok); free(o->r_k);
+  free(o->r_h); free(o->exit_logits); free(o->pdm_logits); free(o->pdm_u); free(o->pdm_feat);
+  free(o->x); free(o->q); free(o->kk); free(o->vv); free(o->att); free(o->o); free(o->g); free(o->u);
+  free(o->act); free(o->dn); free(o->z);
+  free(o);
+}
+
+static void embed_row(const ora_ctx *o, int tok, float *h) {
+  const uint16_t *e = o->w.embed + (size_t)tok * o->cfg.d_model;
+  for (int i = 0; i < o->cfg.d_model; ++i) h[i] = bf16_to_f32(e[i]);
+}
+
+/* The per-token attention sub-step of Layer: RoPE(q,k,pos); require len[l]==pos; append bf16(k),
+ * bf16(v) as row pos; attend over rows 0..pos (causal incl. self).  Returns -1 if the causality
+ * precondition of north_star ("every earlier-position token already deeper") is violated. */
+static int attend_token(ora_ctx *o, int l, int pos, float *q, float *kk, const float *vv, float *att) {
+  const ora_config *c = &o->cfg;
+  size_t row = kv_row(c);
+  ora_op_rope(q, c->n_q_heads, c->head_dim, pos, c->rope_base);
+  ora_op_rope(kk, c->n_kv_heads, c->head_dim, pos, c->rope_base);
+  if (o->len[l] != pos || pos >= c->max_seq) return -1;
+  uint16_t *kd = o->kc + ((size_t)l * c->max_seq + pos) * row;
+  uint16_t *vd = o->vc + ((size_t)l * c->max_seq + pos) * row;
+  for (size_t i = 0; i < row; ++i) { kd[i] = ora_op_f32_to_bf16(kk[i]); vd[i] = ora_op_f32_to_bf16(vv[i]); }
+  o->len[l] = pos + 1;
+  ora_op_attention(q, o->kc + (size_t)l * c->max_seq * row, o->vc + (size_t)l * c->max_seq * row, pos + 1,
+                   c->n_q_heads, c->n_kv_heads, c->head_dim, att);
+  return 0;
+}
+
+/* Layer(l, h, pos) of C-1: pre-norm attention block then pre-norm SwiGLU block, residual stream h. */
+static int layer_forward(ora_ctx *o, int l, float *h, int pos) {
+  const ora_config *c = &o->cfg;
+  int d = c->d_model, qd = c->n_q_heads * c->head_dim, kd = c->n_kv_heads * c->head_dim, F = c->d_ffn;
+  ora_op_rmsnorm(h, o->w.attn_norm[l], d, c->rms_eps, o->x);
+  ora_op_gemv(o->w.wq[l], qd, d, o->x, o->q);
+  ora_op_gemv(o->w.wk[l], kd, d, o->x, o->kk);
+  ora_op_gemv(o->w.wv[l], kd, d, o->x, o->vv);
+  if (attend_token(o, l, pos, o->q, o->kk, o->vv, o->att)) return -1;
+  ora_op_gemv(o->w.wo[l], d, qd, o->att, o->o);
+  for (int i = 0; i < d; ++i) h[i] += o->o[i];
+  ora_op_rmsnorm(h, o->w.mlp_norm[l], d, c->rms_eps, o->x);
+  ora_op_gemv(o->w.w_gate[l], F, d, o->x, o->g);
+  ora_op_gemv(o->w.w_up[l], F, d, o->x, o->u);
+  ora_op_silu_mul(o->g, o->u, F, o->act);
+  ora_op_gemv(o->w.w_down[l], d, F, o->act, o->dn);
+  for (int i = 0; i < d; ++i) h[i] += o->dn[i];
+  return 0;
+}
+
+/* logits = E . RMSNorm(h, gain); returns argmax and records the margin. */
+static int head_argmax(ora_ctx *o, const float *h, const uint16_t *gain, float *logits, int which) {
+  const ora_config *c = &o->cfg;
+  ora_op_rmsnorm(h, gain, c->d_model, c->rms_eps, o->z);
+  ora_op_gemv(o->w.embed, c->vocab, c->d_model, o->z, logits);
+  top2_margin(logits, c->vocab, &o->gap[which], &o->maxabs[which]);
+  return ora_op_argmax(logits, c->vocab);
+}
+
+static void ring_set_single(ora_ctx *o, int pos, int tok) {
+  o->a = 1;
+  o->r_pos[0] = pos; o->r_tok[0] = tok; o->r_k[0] = 0;
+  embed_row(o, tok, o->r_h);
+}
+
+/* Blocked variant of "for every prompt token: Layer(l, h, pos)" for one layer and tokens t0..t1-1. */
+static int layer_forward_block(ora_ctx *o, int l, float *H, int t0, int t1) {
+  const ora_config *c = &o->cfg;
+  int d = c->d_model, qd = c->n_q_heads * c->head_dim, kd = c->n_kv_heads * c->head_dim, F = c->d_ffn;
+  int nt = t1 - t0;
+  float *X = (float *)malloc(sizeof(float) * (size_t)nt * (F > qd ? F : qd));
+  float *Q = (float *)malloc(sizeof(float) * (size_t)nt * qd);
+  float *Kb = (float *)malloc(sizeof(float) * (size_t)nt * kd);
+  float *Vb = (float *)malloc(sizeof(float) * (size_t)nt * kd);
+  float *A = (float *)malloc(sizeof(float) * (size_t)nt * qd);
+  float *O = (float *)malloc(sizeof(float) * (size_t)nt * d);
+  float *G = (float *)malloc(sizeof(float) * (size_t)nt * F);
+  float *U = (float *)malloc(sizeof(float) * (size_t)nt * F);
+  int rc = 0;
+  for (int t = 0; t < nt; ++t) ora_op_rmsnorm(H + (size_t)(t0 + t) * d, o->w.attn_norm[l], d, c->rms_eps, X + (size_t)t * d);
+  gemv_block(o->w.wq[l], qd, d, X, d, Q, qd, nt);
+  gemv_block(o->w.wk[l], kd, d, X, d, Kb, kd, nt);
+  gemv_block(o->w.wv[l], kd, d, X, d, Vb, kd, nt);
+  for (int t = 0; t < nt && !rc; ++t)
+    rc = attend_token(o, l, t0 + t, Q + (size_t)t * qd, Kb + (size_t)t * kd, Vb + (size_t)t * kd, A + (size_t)t * qd);
+  if (!rc) {
+    gemv_block(o->w.wo[l], d, qd, A, qd, O, d, nt);
+    for (int t = 0; t < nt; ++t)
+      for (int i = 0; i < d; ++i) H[(size_t)(t0 + t) * d + i] += O[(size_t)t * d + i];
+    for (int t = 0; t < nt; ++t) ora_op_rmsnorm(H + (size_t)(t0 + t) * d, o->w.mlp_norm[l], d, c->rms_eps, X + (size_t)t * d);
+    gemv_block(o->w.w_gate[l], F, d, X, d, G, F, nt);
+    gemv_block(o->w.w_up[l], F, d, X, d, U, F, nt);
+    for (int t = 0; t < nt; ++t) ora_op_silu_mul(G + (size_t)t * F, U + (size_t)t * F, F, X + (size_t)t * F);
+    gemv_block(o->w.w_down[l], d, F, X, F, O, d, nt);
+    for (int t = 0; t < nt; ++t)
+      for (int i = 0; i < d; ++i) H[(size_t)(t0 + t) * d + i] += O[(size_t)t * d + i];
+  }
+  free(X); free(Q); free(Kb); free(Vb); free(A); free(O); free(G); free(U);
+  return rc;
+}
+
+/* Prefill (C-1): for pos in order: h = E[tok]; for l: h = Layer(l, h, pos); Hfin[pos] = h.
+ * y_P = argmax(E . RMSNorm(Hfin[P-1], g_final)).  State: c = P, len[l] = P, ring = {(P, y_P, k=0, E[y_P])},
+ * emitted = [y_P], K = 0.  ("the prefill prefix ... fully processed"; prefill is outside
+ * the paper's timed region.) */
+int ora_prefill(ora_ctx *o, const int32_t *tokens, int32_t P, int32_t block, int32_t *first_token) {
+  const ora_config *c = &o->cfg;
+  int d = c->d_model, L = c->n_layers;
+  if (P < 1 || P >= c->max_seq) return -1;
+  for (int i = 0; i < P; ++i)
+    if (tokens[i] < 0 || tokens[i] >= c->vocab) return -1;
+  for (int l = 0; l < L; ++l) o->len[l] = 0;
+  if (block <= 1) {
+    for (int pos = 0; pos < P; ++pos) {
+      float *h = o->hfin + (size_t)pos * d;
+      embed_row(o, tokens[pos], h);
+      for (int l = 0; l < L; ++l)
+        if (layer_forward(o, l, h, pos)) return -2;
+    }
+  } else {
+    for (int pos = 0; pos < P; ++pos) embed_row(o, tokens[pos], o->hfin + (size_t)pos * d);
+    for (int l = 0; l < L; ++l)
+      for (int t0 = 0; t0 < P; t0 += block) {
+        int t1 = t0 + block < P ? t0 + block : P;
+        if (layer_forward_block(o, l, o->hfin, t0, t1)) return -2;
+      }
+  }
+  int y = head_argmax(o, o->hfin + (size_t)(P - 1) * d, o->w.final_norm, o->exit_logits, 0);
+  o->c = P;
+  o->prompt_len = P;
+  o->steps = 0;
+  o->emitted = 1;
+  o->prefilled = 1;
+  ring_set_single(o, P, y);
+  if (first_token) *first_token = y;
+  return 0;
+}
+
+int ora_set_forced(ora_ctx *o, const int32_t *truth, int32_t n_truth, float p, uint64_t seed) {
+  if (p < 0.f) { o->forced_on = 0; return 0; }
+  if (p > 1.f || (!truth && n_truth > 0)) return -1;
+  o->truth = truth; o->n_truth = n_truth; o->forced_on = 1; o->forced_seed = seed;
+  o->forced_thresh = (uint64_t)floor((double)p * 9007199254740992.0); /* floor(p * 2^53) */
+  return 0;
+}
+
+/* One SPD cycle — "Step" of C-1, in the paper's order: (1) read the ring, (2) PDM on PRE-step
+ * features, (3) every in-flight token runs its own stage's layer slice
+ * (PAPER.md:67-69), (4) the oldest token exits, its logits judge its successor,
+ * accept -> the draft enters stage 1; reject -> truncate KV, flush, reseed,
+ * (5) no exit (warm-up): the draft simply enters. */
+int ora_step(ora_ctx *o, int32_t draft_override, ora_step_result *out) {
+  const ora_config *c = &o->cfg;
+  int d = c->d_model, n = c->n_stages, L = c->n_layers, per = L / n;
+  if (!o->prefilled) return -1;
+  /* 1 */
+  int a = o->a;
+  int p_new = o->r_pos[a - 1];
+  if (p_new + 1 >= c->max_seq) return -3; /* capacity: the draft would need row p_new+1 next step */
+  o->steps += 1;
+  ora_step_result r;
+  memset(&r, 0, sizeof r);
+  r.step_index = (int32_t)o->steps;
+  r.fill = a;
+  r.emitted_token = -1;
+
+  /* 2: slot j <-> position p_new - j <-> depth j (C-2.2).  In-flight token: its state before this
+   * step's forward (C-2.5; depth 0 = the bare embedding row).  Committed token: Hfin (Eq. 5, C-2.4).
+   * Negative position: zero vector. */
+  for (int j = 0; j < n; ++j) {
+    float *f = o->pdm_feat + (size_t)j * d;
+    int q = p_new - j;
+    if (j < a) memcpy(f, o->r_h + (size_t)(a - 1 - j) * d, sizeof(float) * d);
+    else if (q >= 0) memcpy(f, o->hfin + (size_t)q * d, sizeof(float) * d);
+    else memset(f, 0, sizeof(float) * d);
+  }
+  ora_op_gemv(o->w.pdm_proj, d, n * d, o->pdm_feat, o->pdm_u);
+  int draft = head_argmax(o, o->pdm_u, o->w.pdm_norm, o->pdm_logits, 1);
+  if (o->forced_on) {
+    uint64_t draw = ora_op_splitmix64(o->forced_seed + (uint64_t)o->steps) >> 11;
+    int ti = p_new + 1 - o->prompt_len;
+    if (draw < o->forced_thresh && ti >= 0 && ti < o->n_truth) { draft = o->truth[ti]; r.draft_forced = 1; }
+  }
+  if (draft_override >= 0) draft = draft_override;
+  r.draft_token = draft;
+
+  /* 3: the in-flight tokens touch disjoint layer slices, so their order is irrelevant. */
+  for (int ii = 0; ii < a; ++ii) {
+    int i = o->reverse_forward ? a - 1 - ii : ii;
+    int k = o->r_k[i];
+    for (int l = k * per; l < (k + 1) * per; ++l)
+      if (layer_forward(o, l, o->r_h + (size_t)i * d, o->r_pos[i])) return -2;
+    o->r_k[i] = k + 1;
+  }
+
+  /* 4 */
+  if (o->r_k[0] == n) {
+    int e_pos = o->r_pos[0];
+    memcpy(o->hfin + (size_t)e_pos * d, o->r_h, sizeof(float) * d);
+    o->c = e_pos + 1;
+    int y = head_argmax(o, o->r_h, o->w.final_norm, o->exit_logits, 0);
+    o->emitted += 1;
+    r.exited = 1;
+    r.emitted_token = y;
+    /* pop the oldest */
+    for (int i = 1; i < a; ++i) {
+      o->r_pos[i - 1] = o->r_pos[i]; o->r_tok[i - 1] = o->r_tok[i]; o->r_k[i - 1] = o->r_k[i];
+      memcpy(o->r_h + (size_t)(i - 1) * d, o->r_h + (size_t)i * d, sizeof(float) * d);
+    }
+    a -= 1;
+    int succ = a > 0 ? o->r_tok[0] : draft; /* n = 1: the successor is the draft itself (C-2.12) */
+    if (succ == y) {
+      r.accepted = 1;
+      o->r_pos[a] = p_new + 1; o->r_tok[a] = draft; o->r_k[a] = 0;
+      embed_row(o, draft, o->r_h + (size_t)a * d);
+      o->a = a + 1;
+    } else {
+      r.accepted = 0;
+      r.discarded = a;
+      for (int l = 0; l < L; ++l)
+        if (o->len[l] > o->c) o->len[l] = o->c;
+      ring_set_single(o, o->c, y); /* the draft is dropped (C-2.10) */
+    }
+  } else {
+    /* 5 */
+    o->r_pos[a] = p_new + 1; o->r_tok[a] = draft; o->r_k[a] = 0;
+    embed_row(o, draft, o->r_h + (size_t)a * d);
+    o->a = a + 1;
+  }
+  r.committed_len = o->c;
+  if (out) *out = r;
+  return 0;
+}
+
+int ora_rollback(ora_ctx *o, int32_t new_len, int32_t reseed_token) {
+  if (!o->prefilled) return -1;
+  if (new_len < 0 || new_len > o->c || reseed_token < 0 || reseed_token >= o->cfg.vocab) return -1;
+  o->c = new_len;
+  for (int l = 0; l < o->cfg.n_layers; ++l)
+    if (o->len[l] > new_len) o->len[l] = new_len;
+  ring_set_single(o, new_len, reseed_token);
+  return 0;
+}
+
+/* O-AR: plain greedy decode, one token through all L layers (the single-GPU autoregressive
+ * baseline of PAPER.md:145).  The pending token is ring entry 0 left by ora_prefill. */
+int ora_ar_step(ora_ctx *o, int32_t *next_token) {
+  const ora_config *c = &o->cfg;
+  int d = c->d_model;
+  if (!o->prefilled || o->a != 1 || o->r_k[0] != 0) return -1;
+  int pos = o->r_pos[0];
+  if (pos + 1 >= c->max_seq) return -3;
+  float *h = o->r_h;
+  if (o->ar_trace) memcpy(o->ar_trace, h, sizeof(float) * d);
+  for (int l = 0; l < c->n_layers; ++l) {
+    if (layer_forward(o, l, h, pos)) return -2;
+    if (o->ar_trace) memcpy(o->ar_trace + (size_t)(l + 1) * d, h, sizeof(float) * d);
+  }
+  memcpy(o->hfin + (size_t)pos * d, h, sizeof(float) * d);
+  o->c = pos + 1;
+  int y = head_argmax(o, h, o->w.final_norm, o->exit_logits, 0);
+  o->steps += 1;
+  o->emitted += 1;
+  ring_set_single(o, pos + 1, y);
+  if (next_token) *next_token = y;
+  return 0;
+}
+
+void ora_ar_set_trace(ora_ctx *o, float *trace) { o->ar_trace = trace; }
+void ora_set_forward_order(ora_ctx *o, int32_t reverse) { o->reverse_forward = reverse; }
+
+/* ------------------------------------------------------------------ readers ------------------- */
+
+int32_t ora_committed_len(const ora_ctx *o) { return o->c; }
+int32_t ora_fill(const ora_ctx *o) { return o->a; }
+int64_t ora_steps(const ora_ctx *o) { return o->steps; }
+int32_t ora_emitted(const ora_ctx *o) { return o->emitted; }
+void ora_get_kv_len(const ora_ctx *o, int32_t *len) { memcpy(len, o->len, 4 * (size_t)o->cfg.n_layers); }
+
+void ora_get_kv(const ora_ctx *o, int32_t layer, int32_t which, int32_t rows, uint16_t *out) {
+  size_t row = kv_row(&o->cfg);
+  const uint16_t *src = (which ? o->vc : o->kc) + (size_t)layer * o->cfg.max_seq * row;
+  memcpy(out, src, 2 * row * (size_t)rows);
+}
+
+int ora_get_ring(const ora_ctx *o, int32_t i, int32_t *pos, int32_t *tok, int32_t *k, float *hidden) {
+  if (i < 0 || i >= o->a) return -1;
+  if (pos) *pos = o->r_pos[i];
+  if (tok) *tok = o->r_tok[i];
+  if (k) *k = o->r_k[i];
+  if (hidden) memcpy(hidden, o->r_h + (size_t)i * o->cfg.d_model, 4 * (size_t)o->cfg.d_model);
+  return 0;
+}
+
+void ora_get_hfin(const ora_ctx *o, int32_t pos, float *out) {
+  memcpy(out, o->hfin + (size_t)pos * o->cfg.d_model, 4 * (size_t)o->cfg.d_model);
+}
+
+void ora_get_last(const ora_ctx *o, int32_t what, float *out) {
+  const ora_config *c = &o->cfg;
+  if (what == 0) memcpy(out, o->exit_logits, 4 * (size_t)c->vocab);
+  else if (what == 1) memcpy(out, o->pdm_logits, 4 * (size_t)c->vocab);
+  else if (what == 2) memcpy(out, o->pdm_u, 4 * (size_t)c->d_model);
+  else if (what == 3) memcpy(out, o->pdm_feat, 4 * (size_t)c->d_model * c->n_stages);
+}
+
+void ora_get_margin(const ora_ctx *o, int32_t which, float *gap, float *maxabs) {
+  *gap = o->gap[which & 1];
+  *maxabs = o->maxabs[which & 1];
+}
+
+/* ------------------------------------------------------------------ timing-only helpers ------- */
+
+void ora_load_kv(ora_ctx *o, int32_t layer, const uint16_t *k, const uint16_t *v, int32_t rows) {
+  size_t row = kv_row(&o->cfg);
+  memcpy(o->kc + (size_t)layer * o->cfg.max_seq * row, k, 2 * row * (size_t)rows);
+  memcpy(o->vc + (size_t)layer * o->cfg.max_seq * row, v, 2 * row * (size_t)rows);
+}
+
+int ora_assume_prefilled(ora_ctx *o, int32_t committed_len, int32_t first_token) {
+  if (committed_len < 1 || committed_len >= o->cfg.max_seq) return -1;
+  for (int l = 0; l < o->cfg.n_layers; ++l) o->len[l] = committed_len;
+  o->c = committed_len;
+  o->prompt_len = committed_len;
+  o->steps = 0;
+  o->emitted = 1;
+  o->prefilled = 1;
+  ring_set_single(o, committed_len, first_token);
+  return 0;
+}
