@@ -1,0 +1,192 @@
+/* spd.h — C ABI of the B200-native Speculative Pipeline Decoding (SPD) step library.
+ *
+ * One SPD pipeline step of a batch-1 sequence on one GPU (sm_100a).  Every step of the path runs in
+ * this library's CUDA kernels; callers hand in plain pointers and sizes.  Citations "PAPER.md:<line>"
+ * are lines of /root/reference/PAPER.md (arxiv/paper_2605_30852); "C-2.x" are the readings listed in
+ * DESIGN.md ("Readings of the paper").
+ *
+ * The operation (PAPER.md:67-69 §3.1, :115 §3.3, :125-131 §3.4):
+ *   The target decoder's L layers are split into n contiguous stages; up to n tokens of ONE sequence
+ *   are in flight, the token that has completed k stages runs stage k this cycle.  A cycle
+ *     1. drafts the next token with the Pipeline Draft Module (PDM) from PRE-step hidden states of
+ *        the n most recent positions (slot j = position p_new - j at depth j; committed positions give
+ *        their final hidden state, Eq. 5),
+ *     2. runs every in-flight token through its stage's L/n layers (RMSNorm, QKV GEMV, RoPE, KV append,
+ *        GQA attention over that layer's cache, O GEMV, RMSNorm, SwiGLU GEMVs),
+ *     3. if the oldest token finished stage n: commits it, y = argmax(E . RMSNorm(h)) judges its
+ *        in-flight successor; equal -> the draft enters stage 0; different -> every layer's KV length
+ *        is truncated to the committed length, the pipeline is flushed and reseeded with y.
+ *   Greedy only; the emitted tokens equal plain greedy decoding ("lossless").
+ *
+ * Numeric contract (C-2.17): weights bf16, every activation fp32 with fp32 accumulation, K/V cache
+ * rows rounded to bf16 (round-to-nearest-even) when appended.  argmax = max value, lowest index (C-2.8).
+ *
+ * Memory and ownership: the library never allocates device memory.  The caller allocates three
+ * device buffers of the sizes spd_query_sizes reports (any 256-byte aligned allocation, e.g.
+ * torch.empty) plus two CUDA streams, and keeps them and all weight tensors alive until spd_destroy.
+ * The ctx owns only host metadata, CUDA events/graphs and one small pinned host buffer.
+ * Threading: one ctx is used from one host thread at a time.
+ * Errors: every call returns spd_status; out-parameters are written only on SPD_OK; no exception or
+ * foreign object crosses the ABI.  After SPD_ECUDA the ctx is unusable except for spd_last_error and
+ * spd_destroy.  There is NO CPU fallback: without a CUDA device spd_create returns SPD_ECUDA.
+ */
+#ifndef SPD_H
+#define SPD_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct spd_ctx spd_ctx; /* opaque */
+
+typedef enum {
+  SPD_OK = 0,
+  SPD_EINVAL = 1,    /* bad argument or unsupported configuration; state unchanged              */
+  SPD_ESTATE = 2,    /* call out of order (e.g. spd_step before spd_prefill); state unchanged   */
+  SPD_ECAPACITY = 3, /* the step would need a KV row >= max_seq; state unchanged                */
+  SPD_ECUDA = 4,     /* a CUDA call failed or a device-side check fired; see spd_last_error     */
+  SPD_ENOMEM = 5     /* a caller buffer is missing or too small                                 */
+} spd_status;
+
+/* Decoder shape (BASELINE.json configs; C-2.13: pre-norm, no biases, no QK-norm, GQA, SwiGLU, RoPE
+ * rotate-half on all head dims, scale 1/sqrt(head_dim)).  Requirements (else SPD_EINVAL):
+ * n_layers % n_stages == 0 (C-2.7), n_q_heads % n_kv_heads == 0, head_dim in {64, 128},
+ * d_model, d_ffn, n_q_heads*head_dim multiples of 8, 1 <= n_stages <= 32, vocab >= 2, max_seq >= 2. */
+typedef struct {
+  int32_t d_model, n_layers, n_stages, n_q_heads, n_kv_heads, head_dim, d_ffn, vocab, max_seq;
+  float rms_eps, rope_base;
+  int32_t device; /* CUDA device ordinal */
+} spd_config;
+
+/* Weights: DEVICE pointers to bf16 bit patterns, row-major [out, in].  The nine per-layer members
+ * are HOST arrays of n_layers DEVICE pointers (the arrays themselves are only read during
+ * spd_create).  All tensors are borrowed until spd_destroy. */
+typedef struct {
+  const uint16_t *embed;            /* [vocab, d]  tied: input embedding = LM head = PDM head (C-2.3) */
+  const uint16_t *const *attn_norm; /* [L] -> [d]                */
+  const uint16_t *const *wq;        /* [L] -> [n_q_heads*hd, d]  */
+  const uint16_t *const *wk;        /* [L] -> [n_kv_heads*hd, d] */
+  const uint16_t *const *wv;        /* [L] -> [n_kv_heads*hd, d] */
+  const uint16_t *const *wo;        /* [L] -> [d, n_q_heads*hd]  */
+  const uint16_t *const *mlp_norm;  /* [L] -> [d]                */
+  const uint16_t *const *w_gate;    /* [L] -> [d_ffn, d]         */
+  const uint16_t *const *w_up;      /* [L] -> [d_ffn, d]         */
+  const uint16_t *const *w_down;    /* [L] -> [d, d_ffn]         */
+  const uint16_t *final_norm;       /* [d]                       */
+  const uint16_t *pdm_proj;         /* [d, n*d]; column block j multiplies the depth-j slot (C-2.2) */
+  const uint16_t *pdm_norm;         /* [d]                       */
+} spd_weights;
+
+typedef struct {
+  size_t repack_bytes; /* streaming layout of the layer weights, written once by spd_create */
+  size_t kv_bytes;     /* K/V cache, bf16, [layer][K|V][kv_head][max_seq][head_dim]          */
+  size_t work_bytes;   /* step state, activations, hidden-state history, result ring         */
+} spd_sizes;
+
+typedef struct {
+  void *repack, *kv, *work;        /* DEVICE, >= the sizes above, 256-byte aligned            */
+  void *stream_main, *stream_pdm;  /* cudaStream_t handles (e.g. torch.cuda.Stream.cuda_stream) */
+} spd_buffers;
+
+/* What one cycle did.  step_index = K after the step (K counts cycles since prefill);
+ * fill = tokens in flight when the step began; exited/accepted are 0/1; emitted_token is the verified
+ * token y of an exit step (-1 otherwise); draft_token is what the PDM (or the forced rule) proposed;
+ * discarded = in-flight tokens dropped by a reject (n-1 in saturation); committed_len = c after it. */
+typedef struct {
+  int32_t step_index, fill, exited, accepted, emitted_token, draft_token, draft_forced, discarded,
+      committed_len;
+} spd_step_result;
+
+/* Engine options (spd_set_option). */
+enum {
+  SPD_OPT_ENGINE = 0,      /* 0 = one kernel per operation (reference engine), 1 = persistent fused
+                              step kernel (default when available)                               */
+  SPD_OPT_DEBUG_LOGITS = 1 /* 1 = also write full verify/PDM logit vectors (for parity tests)    */
+};
+
+/* spd_debug_read selectors.  `index` meaning in brackets. */
+enum {
+  SPD_DBG_SLOT_HIDDEN = 0, /* [depth k] fp32[d]: hidden state of the in-flight token at depth k     */
+  SPD_DBG_EXIT_LOGITS = 1, /* fp32[vocab] of the last verify (needs SPD_OPT_DEBUG_LOGITS)           */
+  SPD_DBG_PDM_LOGITS = 2,  /* fp32[vocab] of the last PDM   (needs SPD_OPT_DEBUG_LOGITS)           */
+  SPD_DBG_PDM_PRENORM = 3, /* fp32[d]: u = W_p . concat(slots) of the last PDM                     */
+  SPD_DBG_PDM_FEAT = 4,    /* fp32[n*d]: the slot vectors the last PDM read (slot j = depth j)     */
+  SPD_DBG_KV_K = 5,        /* [layer] bf16 [rows, n_kv_heads*hd], rows = bytes / row size          */
+  SPD_DBG_KV_V = 6,        /* [layer] same for V                                                   */
+  SPD_DBG_KV_LEN = 7,      /* int32[L]: valid KV rows per layer (C-2.11)                           */
+  SPD_DBG_RING = 8,        /* int32[2 + 3n]: fill a, committed c, then per depth k: occupied, pos, tok */
+  SPD_DBG_HFIN = 9         /* [position] fp32[d]: final hidden state of a committed position        */
+};
+
+/* Buffer sizes for a configuration.  SPD_EINVAL if the configuration is unsupported. */
+int spd_query_sizes(const spd_config *cfg, spd_sizes *out);
+
+/* Creates a context: validates, repacks the layer weights into `bufs->repack` (streaming layout of
+ * the fused step kernel), zeroes the state.  Blocks until done. */
+int spd_create(const spd_config *cfg, const spd_weights *w, const spd_buffers *bufs, spd_ctx **out);
+int spd_destroy(spd_ctx *ctx);
+
+/* Prefill (outside the paper's timed region): runs the prompt (HOST int32 ids,
+ * 1 <= n_tokens < max_seq - 1) through all layers with the same kernels as the step, n tokens
+ * pipelined over the n stages.  Afterwards: committed length = n_tokens, every layer holds n_tokens
+ * KV rows, *first_token = argmax of the last position's logits is the single in-flight token, K = 0.
+ * May be called again to start a new sequence. */
+int spd_prefill(spd_ctx *ctx, const int32_t *tokens, int32_t n_tokens, int32_t *first_token);
+
+/* One SPD cycle including verification and, on reject, the internal rollback.  Returns after the
+ * result is on the host (one small D2H copy + stream sync). */
+int spd_step(spd_ctx *ctx, spd_step_result *out);
+/* n_steps cycles enqueued back to back (the state lives on the device), one sync at the end;
+ * results[0..n_steps) in order.  SPD_ECAPACITY (nothing run) unless all n_steps are guaranteed to fit. */
+int spd_step_many(spd_ctx *ctx, int32_t n_steps, spd_step_result *results);
+
+/* External truncate + flush + reseed (PAPER.md:131 with c := new_len): every layer's KV length becomes
+ * min(len, new_len), in-flight tokens are dropped, reseed_token becomes the single in-flight token at
+ * position new_len.  0 <= new_len <= committed length, 0 <= reseed_token < vocab, else SPD_EINVAL.
+ * O(L) integers; no KV data moves. */
+int spd_rollback(spd_ctx *ctx, int32_t new_len, int32_t reseed_token);
+
+/* Bench mode (north_star: controlled acceptance from random-init weights; C-2.19): at cycle K the
+ * PDM's token is replaced by truth[p_new + 1 - prompt_len] iff
+ * (splitmix64(seed + K) >> 11) < floor(p * 2^53) and that entry exists.  truth: HOST int32[n_truth],
+ * copied.  p < 0 disables; p > 1 or n_truth > max_seq -> SPD_EINVAL. */
+int spd_set_forced(spd_ctx *ctx, const int32_t *truth, int32_t n_truth, float p, uint64_t seed);
+
+int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value);
+
+/* Copies internal state to HOST memory (parity tests).  bytes must match the selector's size
+ * (KV selectors: a multiple of the row size, at most max_seq rows). */
+int spd_debug_read(spd_ctx *ctx, int32_t what, int32_t index, void *host_out, size_t bytes);
+
+/* Counters since the last spd_prefill: cycles K, emitted tokens N (alpha = N/K), and the
+ * number of this library's kernel launches since spd_create. */
+int spd_get_counters(spd_ctx *ctx, int64_t *steps, int64_t *emitted, int64_t *kernel_launches);
+
+/* Last error text of the ctx (never NULL; static string if ctx is NULL). */
+const char *spd_last_error(const spd_ctx *ctx);
+
+/* ---- single operations, for per-kernel parity tests (DEVICE pointers, launched on `stream`,
+ *      asynchronous; the kernels are the reference engine's).  Return SPD_OK / SPD_EINVAL / SPD_ECUDA. */
+/* out[i] = x[i] * rsqrt(mean(x^2) + eps) * gain[i] */
+int spd_op_rmsnorm(const float *x, const uint16_t *gain, int32_t d, float eps, float *out, void *stream);
+/* out = W x, W bf16 [rows, k] row-major, k % 8 == 0 */
+int spd_op_gemv(const uint16_t *w, int32_t rows, int32_t k, const float *x, float *out, void *stream);
+/* RoPE (C-2.14) in place on vec = n_heads heads of head_dim at position pos */
+int spd_op_rope(float *vec, int32_t n_heads, int32_t head_dim, int32_t pos, float base, void *stream);
+/* GQA decode attention of one token over t_len rows.  kc, vc: bf16 [n_kv_heads][t_stride][head_dim]
+ * (the cache's head-major layout); scratch: fp32, >= spd_op_attention_scratch(...) bytes. */
+int spd_op_attention(const float *q, const uint16_t *kc, const uint16_t *vc, int32_t t_len, int32_t t_stride,
+                     int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, float *out, float *scratch,
+                     void *stream);
+size_t spd_op_attention_scratch(int32_t t_len, int32_t n_q_heads, int32_t head_dim);
+/* out[i] = silu(gate[i]) * up[i] */
+int spd_op_silu_mul(const float *gate, const float *up, int32_t n, float *out, void *stream);
+/* argmax with lowest-index ties of x[0..n); result int32 on the device */
+int spd_op_argmax(const float *x, int32_t n, int32_t *out_index, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

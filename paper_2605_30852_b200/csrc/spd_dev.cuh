@@ -1,0 +1,118 @@
+// spd_dev.cuh — device-side state, buffer map and small helpers shared by the library's kernels.
+// (CUDA path only; nothing here is used by, or taken from, oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace spd {
+
+constexpr int kMaxStages = 32;
+constexpr int kAttnSplit = 128;     // KV rows per attention split — fixed, so a token's result never
+                                    // depends on n, slot, fill or history (batch invariance)
+constexpr int kResultRing = 1024;   // device ring of step results (spd_step_many batch limit)
+constexpr int kMaxCand = 256;       // per-CTA argmax candidates of the LM-head pass
+
+enum Mode : int32_t { MODE_IDLE = 0, MODE_SPD = 1, MODE_PREFILL = 2, MODE_PREFILL_FINAL = 3 };
+
+struct StepResult {
+  int32_t step_index, fill, exited, accepted, emitted_token, draft_token, draft_forced, discarded,
+      committed_len;
+};
+
+// Device-resident controller state: the in-flight pipeline indexed by depth k (= stage), the
+// committed length, counters and the forced-acceptance rule.  Updated only by the step's last kernel,
+// so steps can be enqueued back to back without the host.
+struct StepState {
+  int32_t mode;
+  int32_t c;                         // committed length
+  int32_t occ[kMaxStages];           // stage k holds a token
+  int32_t pos[kMaxStages];
+  int32_t tok[kMaxStages];
+  int32_t hbuf[kMaxStages];          // which hidden-state buffer that token lives in
+  long long K, N;                    // cycles / emitted tokens since prefill
+  int32_t prompt_len;
+  int32_t forced_on, n_truth;
+  unsigned long long forced_thresh, forced_seed;
+  int32_t pf_next, pf_n;             // prefill progress
+  int32_t err;                       // sticky device-side check (causality / capacity)
+  // per-step scratch written by the step's first kernel
+  int32_t run_pdm, run_verify, fill, p_new, forced_now;
+  int32_t pad_;
+};
+
+struct Dims {
+  int32_t d, L, n, Hq, Hkv, hd, F, V, max_seq, per;   // per = L / n
+  float eps;
+};
+
+// Everything a kernel needs, passed by value.
+struct DevPtrs {
+  Dims dim;
+  StepState *st;
+  int32_t *len;                      // [L] valid KV rows
+  float *h;                          // [n][d]   hidden state buffers (indexed by hbuf)
+  float *x;                          // [n][d]   normed activations
+  float *act;                        // [n][F]   SwiGLU output silu(gate)*up
+  float *q;                          // [n][Hq*hd]
+  float *kvtmp;                      // [n][2*Hkv*hd] fp32 k, v before RoPE/rounding (reference engine)
+  float *att;                        // [n][Hq*hd]
+  float *part_o;                     // [n][Hq][nsplit][hd]
+  float2 *part_ml;                   // [n][Hq][nsplit]
+  int32_t *att_cnt;                  // [n][Hkv] split-completion counters (fused engine)
+  float *feat;                       // [n][d]   PDM slot vectors
+  float *pdm_part;                   // [n][d]   per-slot partial products of W_p (fused engine)
+  float *pdm_u;                      // [d]
+  float *xv, *xp;                    // [d] verify / PDM head inputs
+  float *logits_v, *logits_p;        // [V]
+  float *cand_val;                   // [2][kMaxCand]
+  int32_t *cand_idx;                 // [2][kMaxCand]
+  float2 *rope;                      // [n][hd/2] (cos, sin) for this step's positions
+  double *inv_freq;                  // [hd/2] base^(-2i/hd), computed on the host in double
+  float *hfin;                       // [max_seq][d]
+  int32_t *truth;                    // [max_seq]
+  int32_t *pf_tokens;                // [max_seq]
+  StepResult *results;               // [kResultRing]
+  unsigned int *bar;                 // grid-barrier words (fused engine)
+  uint16_t *kv;                      // K/V cache
+  const uint16_t *embed, *final_norm, *pdm_proj, *pdm_norm;
+  const uint16_t *const *attn_norm, *const *wq, *const *wk, *const *wv, *const *wo, *const *mlp_norm,
+      *const *w_gate, *const *w_up, *const *w_down;   // device arrays of [L] device pointers
+  int32_t debug_logits;
+  int32_t nsplit_max;
+};
+
+__host__ __device__ inline size_t kv_head_stride(const Dims &d) { return (size_t)d.max_seq * d.hd; }
+// K (which=0) or V (which=1) rows of (layer, kv head): [max_seq][hd] bf16
+__host__ __device__ inline size_t kv_offset(const Dims &d, int layer, int which, int kvh) {
+  return (((size_t)layer * 2 + which) * d.Hkv + kvh) * kv_head_stride(d);
+}
+
+__device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+__device__ __forceinline__ float bf16_to_f32(uint16_t b) { return __uint_as_float((uint32_t)b << 16); }
+// fp32 -> bf16 round-to-nearest-even (finite values)
+__device__ __forceinline__ uint16_t f32_to_bf16(float f) {
+  uint32_t u = __float_as_uint(f);
+  u += 0x7fffu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+__device__ __forceinline__ unsigned long long splitmix64(unsigned long long x) {
+  unsigned long long z = x + 0x9e3779b97f4a7c15ull;
+  z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull;
+  z = (z ^ (z >> 27)) * 0x94d049bb133111ebull;
+  return z ^ (z >> 31);
+}
+
+// (value, index) ordering of the greedy argmax: larger value wins, equal values -> lower index.
+__device__ __forceinline__ bool cand_better(float v, int i, float bv, int bi) {
+  return v > bv || (v == bv && i < bi);
+}
+
+}  // namespace spd

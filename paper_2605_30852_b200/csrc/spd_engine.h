@@ -1,0 +1,24 @@
+// spd_engine.h — host-side entry points of the two engines (internal to the library).
+#pragma once
+#include "spd_dev.cuh"
+
+namespace spd {
+
+// Reference engine: enqueue all kernels of one cycle (main stream + PDM branch on `sp`).
+int ref_enqueue_step(const DevPtrs &P, cudaStream_t sm, cudaStream_t sp, cudaEvent_t ev_fork, cudaEvent_t ev_join,
+                     long long *launches);
+
+// Fused persistent engine (spd_mega.cu).
+struct MegaPlan {
+  const uint16_t *repack;   // streaming layout of all layer weights + W_p (device)
+  int n_cta;                // persistent grid size (one CTA per SM)
+  int smem_bytes;
+  int available;
+};
+size_t mega_repack_bytes(const Dims &D);
+// src: the nine host tables of per-layer device pointers in spd_weights order.  Returns 0 on success.
+int mega_create(const DevPtrs &P, const uint16_t *const *const *src, void *repack, size_t repack_bytes,
+                cudaStream_t stream, MegaPlan *plan);
+int mega_enqueue_step(const DevPtrs &P, const MegaPlan &plan, cudaStream_t sm, long long *launches);
+
+}  // namespace spd

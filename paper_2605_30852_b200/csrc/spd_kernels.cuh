@@ -1,0 +1,276 @@
+// spd_kernels.cuh — device functions of the individual operations (plain pointers) and the
+// controller kernels (step begin / end) used by both engines.
+#pragma once
+#include "spd_dev.cuh"
+
+namespace spd {
+
+// ---------------------------------------------------------------------------------------------
+// RMSNorm, block-wide: out[i] = x[i] * (1/sqrt(mean(x^2)+eps)) * gain[i].  Fixed reduction tree
+// (per-thread strided sum -> warp xor-tree -> warp partials added in order) so the value depends
+// only on (x, blockDim).  `red` is >= 33 floats of shared memory.
+__device__ __forceinline__ float block_rms_scale(const float *x, int d, float eps, float *red) {
+  float ss = 0.f;
+  for (int i = threadIdx.x; i < d; i += blockDim.x) { float v = x[i]; ss = fmaf(v, v, ss); }
+  ss = warp_sum(ss);
+  int nw = (blockDim.x + 31) >> 5;
+  __syncthreads();                      // protect `red` against a previous use
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    float t = 0.f;
+    for (int w = 0; w < nw; ++w) t += red[w];
+    red[32] = 1.0f / sqrtf(t / (float)d + eps);
+  }
+  __syncthreads();
+  return red[32];
+}
+
+__device__ __forceinline__ void block_rmsnorm(const float *x, const uint16_t *gain, int d, float eps,
+                                              float *out, float *red) {
+  float r = block_rms_scale(x, d, eps, red);
+  for (int i = threadIdx.x; i < d; i += blockDim.x) out[i] = x[i] * r * bf16_to_f32(gain[i]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// One weight row (bf16, k % 8 == 0) dotted with an fp32 vector by one warp.  Lane l takes the
+// 8-element chunks l, l+32, ...; fp32 FMA chain per lane, then the xor-tree.  All lanes return the sum.
+__device__ __forceinline__ float warp_dot_row(const uint16_t *__restrict__ w, const float *__restrict__ x, int k) {
+  const uint4 *wp = reinterpret_cast<const uint4 *>(w);
+  const float4 *xp = reinterpret_cast<const float4 *>(x);
+  int lane = threadIdx.x & 31;
+  int nchunk = k >> 3;
+  float a0 = 0.f, a1 = 0.f;
+  int c = lane;
+  for (; c + 32 < nchunk; c += 64) {
+    uint4 w0 = __ldg(wp + c), w1 = __ldg(wp + c + 32);
+    float4 x0 = xp[2 * c], x1 = xp[2 * c + 1], y0 = xp[2 * (c + 32)], y1 = xp[2 * (c + 32) + 1];
+    a0 = fmaf(bf16_lo(w0.x), x0.x, a0); a0 = fmaf(bf16_hi(w0.x), x0.y, a0);
+    a0 = fmaf(bf16_lo(w0.y), x0.z, a0); a0 = fmaf(bf16_hi(w0.y), x0.w, a0);
+    a0 = fmaf(bf16_lo(w0.z), x1.x, a0); a0 = fmaf(bf16_hi(w0.z), x1.y, a0);
+    a0 = fmaf(bf16_lo(w0.w), x1.z, a0); a0 = fmaf(bf16_hi(w0.w), x1.w, a0);
+    a1 = fmaf(bf16_lo(w1.x), y0.x, a1); a1 = fmaf(bf16_hi(w1.x), y0.y, a1);
+    a1 = fmaf(bf16_lo(w1.y), y0.z, a1); a1 = fmaf(bf16_hi(w1.y), y0.w, a1);
+    a1 = fmaf(bf16_lo(w1.z), y1.x, a1); a1 = fmaf(bf16_hi(w1.z), y1.y, a1);
+    a1 = fmaf(bf16_lo(w1.w), y1.z, a1); a1 = fmaf(bf16_hi(w1.w), y1.w, a1);
+  }
+  for (; c < nchunk; c += 32) {
+    uint4 w0 = __ldg(wp + c);
+    float4 x0 = xp[2 * c], x1 = xp[2 * c + 1];
+    a0 = fmaf(bf16_lo(w0.x), x0.x, a0); a0 = fmaf(bf16_hi(w0.x), x0.y, a0);
+    a0 = fmaf(bf16_lo(w0.y), x0.z, a0); a0 = fmaf(bf16_hi(w0.y), x0.w, a0);
+    a0 = fmaf(bf16_lo(w0.z), x1.x, a0); a0 = fmaf(bf16_hi(w0.z), x1.y, a0);
+    a0 = fmaf(bf16_lo(w0.w), x1.z, a0); a0 = fmaf(bf16_hi(w0.w), x1.w, a0);
+  }
+  return warp_sum(a0 + a1);
+}
+
+__device__ __forceinline__ float silu_mul(float g, float u) { return g / (1.0f + expf(-g)) * u; }
+
+// ---------------------------------------------------------------------------------------------
+// Attention partial for one (kv head, split): the `group` q heads that share the kv head, one warp
+// each.  Lane l holds head-dim elements [l*EPL, (l+1)*EPL), EPL = HD/32.  Rows [t0, t1) of K/V
+// ([rows][HD] bf16).  Online softmax in fp32; writes unnormalised o, running max m and sum l.
+template <int HD>
+__device__ __forceinline__ void attn_partial_warp(const float *__restrict__ qh, const uint16_t *__restrict__ kc,
+                                                  const uint16_t *__restrict__ vc, int t0, int t1,
+                                                  float *__restrict__ o_out, float2 *__restrict__ ml_out) {
+  constexpr int EPL = HD / 32;
+  int lane = threadIdx.x & 31;
+  const float scale = 1.0f / sqrtf((float)HD);
+  float qv[EPL], acc[EPL];
+#pragma unroll
+  for (int e = 0; e < EPL; ++e) { qv[e] = qh[lane * EPL + e]; acc[e] = 0.f; }
+  float m = -INFINITY, l = 0.f;
+  for (int t = t0; t < t1; t += 4) {
+    float s[4];
+    float kv_[4][EPL];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      float part = 0.f;
+      if (t + r < t1) {
+        const uint16_t *kr = kc + (size_t)(t + r) * HD + lane * EPL;
+        if constexpr (EPL == 4) {
+          uint2 w = *reinterpret_cast<const uint2 *>(kr);
+          part = fmaf(bf16_lo(w.x), qv[0], part); part = fmaf(bf16_hi(w.x), qv[1], part);
+          part = fmaf(bf16_lo(w.y), qv[2], part); part = fmaf(bf16_hi(w.y), qv[3], part);
+        } else {
+          uint32_t w = *reinterpret_cast<const uint32_t *>(kr);
+          part = fmaf(bf16_lo(w), qv[0], part); part = fmaf(bf16_hi(w), qv[1], part);
+        }
+        const uint16_t *vr = vc + (size_t)(t + r) * HD + lane * EPL;
+        if constexpr (EPL == 4) {
+          uint2 w = *reinterpret_cast<const uint2 *>(vr);
+          kv_[r][0] = bf16_lo(w.x); kv_[r][1] = bf16_hi(w.x); kv_[r][2] = bf16_lo(w.y); kv_[r][3] = bf16_hi(w.y);
+        } else {
+          uint32_t w = *reinterpret_cast<const uint32_t *>(vr);
+          kv_[r][0] = bf16_lo(w); kv_[r][1] = bf16_hi(w);
+        }
+      } else {
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) kv_[r][e] = 0.f;
+      }
+      s[r] = part;
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) s[r] = warp_sum(s[r]) * scale;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      if (t + r < t1) {
+        float mn = fmaxf(m, s[r]);
+        float corr = expf(m - mn);       // exp(-inf) = 0 on the first row
+        float p = expf(s[r] - mn);
+        l = fmaf(l, corr, p);
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) acc[e] = fmaf(acc[e], corr, p * kv_[r][e]);
+        m = mn;
+      }
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < EPL; ++e) o_out[lane * EPL + e] = acc[e];
+  if (lane == 0) *ml_out = make_float2(m, l);
+}
+
+// Merge of the splits of one q head, in split order (fixed): out = sum_j o_j e^(m_j-M) / sum_j l_j e^(m_j-M).
+// Called by HD threads (thread e owns element e) or strided.
+__device__ __forceinline__ float attn_merge_elem(const float *__restrict__ part_o, const float2 *__restrict__ part_ml,
+                                                 int nsplit, int hd, int e) {
+  float M = -INFINITY;
+  for (int j = 0; j < nsplit; ++j) M = fmaxf(M, part_ml[j].x);
+  float L = 0.f, o = 0.f;
+  for (int j = 0; j < nsplit; ++j) {
+    float w = expf(part_ml[j].x - M);
+    L = fmaf(part_ml[j].y, w, L);
+    o = fmaf(part_o[(size_t)j * hd + e], w, o);
+  }
+  return o / L;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Controller, first part of a cycle (one thread): fill / p_new, what runs, cycle counter, the
+// forced-acceptance draw (C-2.19).
+__device__ __forceinline__ void controller_begin(const DevPtrs &P) {
+  StepState *st = P.st;
+  int n = P.dim.n, fill = 0;
+  for (int k = 0; k < n; ++k) fill += st->occ[k];
+  st->fill = fill;
+  st->p_new = st->occ[0] ? st->pos[0] : -1;
+  st->run_pdm = st->mode == MODE_SPD;
+  st->run_verify = (st->mode == MODE_SPD && st->occ[n - 1]) || st->mode == MODE_PREFILL_FINAL;
+  st->forced_now = 0;
+  if (st->mode == MODE_SPD) {
+    st->K += 1;
+    if (st->forced_on) {
+      unsigned long long draw = splitmix64(st->forced_seed + (unsigned long long)st->K) >> 11;
+      int ti = st->p_new + 1 - st->prompt_len;
+      if (draw < st->forced_thresh && ti >= 0 && ti < st->n_truth) st->forced_now = 1;
+    }
+  }
+}
+
+// RoPE table of this cycle: (cos, sin)(pos_k * theta_i) in double, rounded to fp32 (C-2.14).
+__device__ __forceinline__ void rope_table_fill(const DevPtrs &P, int tid, int nthreads) {
+  int half = P.dim.hd / 2;
+  for (int i = tid; i < P.dim.n * half; i += nthreads) {
+    int k = i / half, j = i - k * half;
+    if (!P.st->occ[k]) continue;
+    double ang = (double)P.st->pos[k] * P.inv_freq[j];
+    double s, c;
+    sincos(ang, &s, &c);
+    P.rope[i] = make_float2((float)c, (float)s);
+  }
+}
+
+// Controller, last part of a cycle (one CTA, >= 32 threads): reduce the argmax candidates, verify,
+// accept / reject + rollback, shift the pipeline, enter the next token, record.
+// `ncand` candidates per head (verify = row 0, PDM = row 1 of cand_val/cand_idx).
+__device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand) {
+  __shared__ int s_y, s_draft, s_exit_buf, s_exit_pos, s_enter_tok, s_enter_buf, s_do_exit, s_do_enter;
+  StepState *st = P.st;
+  const Dims &D = P.dim;
+  int n = D.n;
+  if (threadIdx.x < 2) {
+    // head 0 = verify, head 1 = PDM; lowest index among equal maxima
+    int which = threadIdx.x;
+    float bv = -INFINITY;
+    int bi = 0x7fffffff;
+    for (int i = 0; i < ncand; ++i) {
+      float v = P.cand_val[which * kMaxCand + i];
+      int ix = P.cand_idx[which * kMaxCand + i];
+      if (ix >= 0 && cand_better(v, ix, bv, bi)) { bv = v; bi = ix; }
+    }
+    if (which == 0) s_y = bi; else s_draft = bi;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int mode = st->mode;
+    int exited = st->occ[n - 1];
+    int y = s_y, draft = s_draft;
+    StepResult r;
+    r.step_index = (int)st->K; r.fill = st->fill; r.exited = 0; r.accepted = 0; r.emitted_token = -1;
+    r.draft_token = -1; r.draft_forced = 0; r.discarded = 0;
+    s_do_exit = 0; s_do_enter = 0;
+    s_exit_buf = st->hbuf[n - 1]; s_exit_pos = st->pos[n - 1];
+    int enter_tok = -1, enter_pos = -1;
+    bool flush = false;
+    if (mode == MODE_SPD) {
+      if (st->forced_now) { draft = P.truth[st->p_new + 1 - st->prompt_len]; r.draft_forced = 1; }
+      r.draft_token = draft;
+      if (exited) {
+        s_do_exit = 1;
+        st->c = st->pos[n - 1] + 1;
+        st->N += 1;
+        r.exited = 1; r.emitted_token = y;
+        int succ = n > 1 ? st->tok[n - 2] : draft;   // the token one stage behind (C-2.12 for n = 1)
+        if (succ == y) {
+          r.accepted = 1;
+          enter_tok = draft; enter_pos = st->p_new + 1;
+        } else {
+          r.discarded = st->fill - 1;
+          for (int l = 0; l < D.L; ++l) if (P.len[l] > st->c) P.len[l] = st->c;   // truncate
+          flush = true;
+          enter_tok = y; enter_pos = st->c;                                       // reseed; draft dropped
+        }
+      } else {
+        enter_tok = draft; enter_pos = st->p_new + 1;
+      }
+    } else if (mode == MODE_PREFILL) {
+      if (exited) { s_do_exit = 1; st->c = st->pos[n - 1] + 1; }
+      if (st->pf_next < st->pf_n) { enter_tok = P.pf_tokens[st->pf_next]; enter_pos = st->pf_next; st->pf_next += 1; }
+    } else if (mode == MODE_PREFILL_FINAL) {
+      flush = true;
+      enter_tok = y; enter_pos = st->c;
+      st->mode = MODE_SPD; st->K = 0; st->N = 1;
+      r.emitted_token = y;
+    }
+    // shift depth k -> k+1; the buffer ids rotate so the exiting token's buffer receives the entrant
+    int freebuf = st->hbuf[n - 1];
+    for (int k = n - 1; k > 0; --k) {
+      st->occ[k] = flush ? 0 : st->occ[k - 1];
+      st->pos[k] = st->pos[k - 1]; st->tok[k] = st->tok[k - 1]; st->hbuf[k] = st->hbuf[k - 1];
+    }
+    st->hbuf[0] = freebuf;
+    st->occ[0] = enter_tok >= 0;
+    st->pos[0] = enter_pos; st->tok[0] = enter_tok;
+    s_do_enter = enter_tok >= 0; s_enter_tok = enter_tok; s_enter_buf = freebuf;
+    r.committed_len = st->c;
+    if (mode == MODE_SPD) P.results[(r.step_index - 1) % kResultRing] = r;
+    else if (mode == MODE_PREFILL_FINAL) P.results[0] = r;
+  }
+  __syncthreads();
+  int d = D.d;
+  if (s_do_exit) {     // Hfin[e.pos] = e.h  (C-2.4) — read before the buffer is reused below
+    const float *src = P.h + (size_t)s_exit_buf * d;
+    float *dst = P.hfin + (size_t)s_exit_pos * d;
+    for (int i = threadIdx.x; i < d; i += blockDim.x) dst[i] = src[i];
+  }
+  __syncthreads();
+  if (s_do_enter) {    // token entry: h = E[tok] (k = 0 is the embedding-level input)
+    const uint16_t *e = P.embed + (size_t)s_enter_tok * d;
+    float *dst = P.h + (size_t)s_enter_buf * d;
+    for (int i = threadIdx.x; i < d; i += blockDim.x) dst[i] = bf16_to_f32(e[i]);
+  }
+}
+
+}  // namespace spd
