@@ -54,6 +54,8 @@ def lib():
         L.ora_destroy.argtypes = [C.c_void_p]
         L.ora_prefill.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_int32)]
         L.ora_step.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_Res)]
+        L.ora_step_follow.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float, C.POINTER(_Res)]
+        L.ora_get_ties.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.ora_rollback.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
         L.ora_set_forced.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_float, C.c_uint64]
         L.ora_ar_step.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
@@ -154,6 +156,18 @@ class Oracle:
         if rc:
             raise RuntimeError(f"ora_step rc={rc}")
         return StepResult(*[getattr(r, k) for k, _ in _Res._fields_])
+
+    def step_follow(self, draft_hint: int, verify_hint: int, band: float) -> StepResult:
+        r = _Res()
+        rc = lib().ora_step_follow(self._h, -1, draft_hint, verify_hint, band, C.byref(r))
+        if rc:
+            raise RuntimeError(f"ora_step_follow rc={rc}")
+        return StepResult(*[getattr(r, k) for k, _ in _Res._fields_])
+
+    def ties(self):
+        v, p = C.c_int32(), C.c_int32()
+        lib().ora_get_ties(self._h, C.byref(v), C.byref(p))
+        return v.value, p.value
 
     def rollback(self, new_len: int, reseed_token: int) -> int:
         return lib().ora_rollback(self._h, new_len, reseed_token)

@@ -186,6 +186,7 @@ struct ora_ctx {
   /* last-step records */
   float *exit_logits, *pdm_logits, *pdm_u, *pdm_feat;
   float gap[2], maxabs[2];
+  int32_t ties[2];   /* tie hints adopted: [0] verify, [1] PDM */
   float *ar_trace;
   int32_t reverse_forward;
   /* scratch */
@@ -384,6 +385,22 @@ int ora_set_forced(ora_ctx *o, const int32_t *truth, int32_t n_truth, float p, u
  * accept -> the draft enters stage 1; reject -> truncate KV, flush, reseed,
  * (5) no exit (warm-up): the draft simply enters. */
 int ora_step(ora_ctx *o, int32_t draft_override, ora_step_result *out) {
+  return ora_step_follow(o, draft_override, -1, -1, 0.f, out);
+}
+
+/* A tie hint (test hook): `hint` is the token the CUDA path chose.  If it
+ * is not the oracle's argmax but its oracle logit lies within band * max|logit| of the oracle's maximum,
+ * both are valid choices at the stated logit tolerance: the oracle continues with the hint and counts a
+ * tie.  Otherwise the oracle keeps its own argmax (and the caller reports the mismatch). */
+static int apply_hint(const float *logits, int own, int hint, int vocab, float band, float maxabs, int32_t *ties) {
+  if (hint < 0 || hint >= vocab || hint == own) return own;
+  if (logits[own] - logits[hint] <= band * maxabs) { *ties += 1; return hint; }
+  return own;
+}
+
+/* The same cycle with tie hints for the PDM argmax and the verify argmax (either may be -1). */
+int ora_step_follow(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int32_t verify_hint, float band,
+                    ora_step_result *out) {
   const ora_config *c = &o->cfg;
   int d = c->d_model, n = c->n_stages, L = c->n_layers, per = L / n;
   if (!o->prefilled) return -1;
@@ -410,6 +427,7 @@ int ora_step(ora_ctx *o, int32_t draft_override, ora_step_result *out) {
   }
   ora_op_gemv(o->w.pdm_proj, d, n * d, o->pdm_feat, o->pdm_u);
   int draft = head_argmax(o, o->pdm_u, o->w.pdm_norm, o->pdm_logits, 1);
+  draft = apply_hint(o->pdm_logits, draft, draft_hint, c->vocab, band, o->maxabs[1], &o->ties[1]);
   if (o->forced_on) {
     uint64_t draw = ora_op_splitmix64(o->forced_seed + (uint64_t)o->steps) >> 11;
     int ti = p_new + 1 - o->prompt_len;
@@ -433,6 +451,7 @@ int ora_step(ora_ctx *o, int32_t draft_override, ora_step_result *out) {
     memcpy(o->hfin + (size_t)e_pos * d, o->r_h, sizeof(float) * d);
     o->c = e_pos + 1;
     int y = head_argmax(o, o->r_h, o->w.final_norm, o->exit_logits, 0);
+    y = apply_hint(o->exit_logits, y, verify_hint, c->vocab, band, o->maxabs[0], &o->ties[0]);
     o->emitted += 1;
     r.exited = 1;
     r.emitted_token = y;
@@ -536,6 +555,11 @@ void ora_get_last(const ora_ctx *o, int32_t what, float *out) {
   else if (what == 1) memcpy(out, o->pdm_logits, 4 * (size_t)c->vocab);
   else if (what == 2) memcpy(out, o->pdm_u, 4 * (size_t)c->d_model);
   else if (what == 3) memcpy(out, o->pdm_feat, 4 * (size_t)c->d_model * c->n_stages);
+}
+
+void ora_get_ties(const ora_ctx *o, int32_t *verify_ties, int32_t *pdm_ties) {
+  *verify_ties = o->ties[0];
+  *pdm_ties = o->ties[1];
 }
 
 void ora_get_margin(const ora_ctx *o, int32_t which, float *gap, float *maxabs) {

@@ -71,6 +71,13 @@ int ora_prefill(ora_ctx *, const int32_t *tokens, int32_t n_tokens, int32_t bloc
 /* O-SPD: one cycle.  draft_override >= 0 replaces the PDM's token for this step (adversarial-draft
  * tests); -1 keeps the PDM / forced-acceptance token. */
 int ora_step(ora_ctx *, int32_t draft_override, ora_step_result *out);
+/* The same cycle with tie hints (test hook): draft_hint / verify_hint are
+ * the tokens the CUDA path chose (-1: none).  A hint that is not the oracle's argmax but whose oracle
+ * logit is within band * max|logit| of the oracle's maximum is adopted (both are valid at the stated
+ * logit tolerance) and counted by ora_get_ties; any other hint is ignored. */
+int ora_step_follow(ora_ctx *, int32_t draft_override, int32_t draft_hint, int32_t verify_hint, float band,
+                    ora_step_result *out);
+void ora_get_ties(const ora_ctx *, int32_t *verify_ties, int32_t *pdm_ties);
 /* External truncate + flush + reseed with c := new_len. */
 int ora_rollback(ora_ctx *, int32_t new_len, int32_t reseed_token);
 /* Forced acceptance (C-2.19): force <=> (splitmix64(seed + K) >> 11) < floor(p * 2^53); p<0 disables.

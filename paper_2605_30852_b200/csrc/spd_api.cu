@@ -101,7 +101,7 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
   Q.att = cv.take<float>(n * qd);
   Q.part_o = cv.take<float>(n * D.Hq * nsplit * D.hd);
   Q.part_ml = cv.take<float2>(n * D.Hq * nsplit);
-  Q.att_cnt = cv.take<int32_t>(n * D.Hkv);
+  Q.att_cnt = cv.take<int32_t>(n * D.Hq);
   Q.feat = cv.take<float>(n * D.d);
   Q.pdm_part = cv.take<float>(n * D.d);
   Q.pdm_u = cv.take<float>(D.d);

@@ -58,7 +58,7 @@ struct DevPtrs {
   float *att;                        // [n][Hq*hd]
   float *part_o;                     // [n][Hq][nsplit][hd]
   float2 *part_ml;                   // [n][Hq][nsplit]
-  int32_t *att_cnt;                  // [n][Hkv] split-completion counters (fused engine)
+  int32_t *att_cnt;                  // [n][Hq] split-completion counters (fused engine)
   float *feat;                       // [n][d]   PDM slot vectors
   float *pdm_part;                   // [n][d]   per-slot partial products of W_p (fused engine)
   float *pdm_u;                      // [d]

@@ -14,6 +14,7 @@ struct MegaPlan {
   int n_cta;                // persistent grid size (one CTA per SM)
   int smem_bytes;
   int available;
+  unsigned long long layout[24];   // opaque MegaLayout (offsets of the repacked matrices)
 };
 size_t mega_repack_bytes(const Dims &D);
 // src: the nine host tables of per-layer device pointers in spd_weights order.  Returns 0 on success.

@@ -80,7 +80,7 @@ __device__ __forceinline__ void attn_partial_warp(const float *__restrict__ qh, 
   const float scale = 1.0f / sqrtf((float)HD);
   float qv[EPL], acc[EPL];
 #pragma unroll
-  for (int e = 0; e < EPL; ++e) { qv[e] = qh[lane * EPL + e]; acc[e] = 0.f; }
+  for (int e = 0; e < EPL; ++e) { qv[e] = __ldcg(qh + lane * EPL + e); acc[e] = 0.f; }   // q comes from other CTAs
   float m = -INFINITY, l = 0.f;
   for (int t = t0; t < t1; t += 4) {
     float s[4];

@@ -1,12 +1,650 @@
-// spd_mega.cu — fused persistent engine (placeholder until the kernel lands: reports "not available",
-// the library then runs the reference engine).
+// spd_mega.cu — the fused persistent engine: ONE cooperative kernel per SPD cycle.
+//
+// Shape of the problem: a cycle streams every layer's weights once (12.3 GB at
+// the 9B-class config) through (L/n)*5 + 2 dependent phases; every product is an M=1 GEMV, so the
+// bound is HBM bandwidth and the enemy is the bubble at each phase boundary.  Design:
+//   * grid = one CTA per SM, resident for the whole cycle; 8 consumer warps + 1 producer warp.
+//   * weights are repacked once (spd_create) into 16 KB tiles — 16 rows x 512 columns, stored in the
+//     order a CTA consumes them, so each CTA's share of a phase is ONE contiguous byte range.
+//   * the producer lane streams that range with 1-D TMA bulk copies (cp.async.bulk + mbarrier
+//     complete_tx) into an 11-deep shared-memory ring.  Weight addresses are a static schedule, so
+//     the producer runs AHEAD of the activation dependency, across phase boundaries: while the
+//     consumers wait at a grid barrier the next phase's tiles are already landing.
+//   * consumers: warp w owns rows 2w, 2w+1 of a tile; 128-bit conflict-free LDS of weights and of
+//     the fp32 activation vector (staged in smem once per phase), fp32 FMA, warp-shuffle reduction at
+//     the end of a 16-row unit, fused epilogues (RoPE + bf16 KV append, residual add, SiLU*mul,
+//     PDM partials, LM-head argmax).
+//   * stages (the n in-flight tokens) own disjoint CTA groups, so a CTA keeps one activation vector.
+//   * phases are separated by a device-wide arrive/poll barrier on a monotonically increasing
+//     64-bit counter; cross-CTA activations are read with ld.global.cg.
+// Every row's dot product is computed by one warp with a fixed lane/column mapping and chunk order,
+// so a token's result never depends on n, slot, fill or history (batch invariance).
+#include <stdio.h>
+#include <string.h>
+
 #include "spd_engine.h"
+#include "spd_kernels.cuh"
 
 namespace spd {
-size_t mega_repack_bytes(const Dims &) { return 256; }
-int mega_create(const DevPtrs &, const uint16_t *const *const *, void *, size_t, cudaStream_t, MegaPlan *plan) {
-  if (plan) plan->available = 0;
-  return -1;
+
+constexpr int kTileRows = 16;
+constexpr int kTileCols = 512;
+constexpr int kTileBytes = kTileRows * kTileCols * 2;   // 16 KB
+constexpr int kStages = 11;                              // ring depth
+constexpr int kXFloats = 12288;                          // activation vector capacity (48 KB)
+constexpr int kConsumerThreads = 256;
+constexpr int kThreads = kConsumerThreads + 32;
+
+enum PhaseType { PH_PDM = 0, PH_QKV = 1, PH_ATTN = 2, PH_O = 3, PH_GATEUP = 4, PH_DOWN = 5, PH_HEAD = 6 };
+
+struct MegaLayout {
+  const uint8_t *repack;
+  unsigned long long layer_bytes, off_o, off_gu, off_dn, off_pdm, off_head, pdm_job_bytes;
+  int u_qkv, u_o, u_gu, u_dn, u_pdm, u_head;   // 16-row units per job
+  int nc_d, nc_qd, nc_f;                        // 512-column chunks for K = d, Hq*hd, F
+};
+
+// Per-cycle schedule, computed identically by every CTA from the device state.
+struct Sched {
+  int mode, n_act, run_pdm, run_verify, p_new, c;
+  int act[kMaxStages];                          // active stages (depth k), ascending
+  int pos[kMaxStages], hbuf[kMaxStages], occ[kMaxStages];
+  int my_stage;                                 // this CTA's stage in the layer phases (-1: none)
+  int my_idx, my_gs;                            // index in / size of the stage's CTA group
+};
+
+struct Work {                                   // one CTA's share of one phase
+  const uint8_t *base;                          // first tile
+  int ntiles, nc, u0, u1, job;
+};
+
+// ------------------------------------------------------------------ PTX helpers ----------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
-int mega_enqueue_step(const DevPtrs &, const MegaPlan &, cudaStream_t, long long *) { return -1; }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {}
+}
+__device__ __forceinline__ void tma_load_1d(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar,
+                                            uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+      ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
+}
+__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p) {
+  unsigned long long v;
+  asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+
+// CTA group of `cta` when `jobs` jobs share `ncta` CTAs: group g owns CTAs [g*ncta/jobs, (g+1)*ncta/jobs).
+__device__ __forceinline__ void group_of(int cta, int ncta, int jobs, int &g, int &idx, int &gs) {
+  g = ((cta + 1) * jobs - 1) / ncta;
+  int b0 = g * ncta / jobs, b1 = (g + 1) * ncta / jobs;
+  idx = cta - b0;
+  gs = b1 - b0;
+}
+
+__device__ __forceinline__ int phase_type(int p, int np) {
+  if (p == 0) return PH_PDM;
+  if (p == np - 1) return PH_HEAD;
+  return PH_QKV + (p - 1) % 5;
+}
+
+// This CTA's tiles of phase p.  Pure function of (Sched, layout, cta) — the producer and the consumers
+// both call it and must agree.
+__device__ __forceinline__ Work phase_work(int p, int np, const Sched &S, const MegaLayout &ML, const Dims &D, int cta,
+                                           int ncta) {
+  Work w;
+  w.base = nullptr; w.ntiles = 0; w.nc = 0; w.u0 = 0; w.u1 = 0; w.job = -1;
+  int t = phase_type(p, np);
+  int U = 0, g, idx, gs;
+  if (t == PH_PDM) {
+    if (!S.run_pdm) return w;
+    group_of(cta, ncta, D.n, g, idx, gs);
+    w.job = g; U = ML.u_pdm; w.nc = ML.nc_d;
+    w.base = ML.repack + ML.off_pdm + (unsigned long long)g * ML.pdm_job_bytes;
+  } else if (t == PH_HEAD) {
+    if (!S.run_pdm && !S.run_verify) return w;
+    idx = cta; gs = ncta; w.job = 0; U = ML.u_head; w.nc = ML.nc_d;
+    w.base = ML.repack + ML.off_head;
+  } else if (t == PH_ATTN) {
+    return w;
+  } else {
+    if (S.my_stage < 0) return w;
+    int pass = (p - 1) / 5;
+    int layer = S.my_stage * D.per + pass;
+    idx = S.my_idx; gs = S.my_gs; w.job = S.my_stage;
+    const uint8_t *lb = ML.repack + (unsigned long long)layer * ML.layer_bytes;
+    if (t == PH_QKV) { U = ML.u_qkv; w.nc = ML.nc_d; w.base = lb; }
+    else if (t == PH_O) { U = ML.u_o; w.nc = ML.nc_qd; w.base = lb + ML.off_o; }
+    else if (t == PH_GATEUP) { U = ML.u_gu; w.nc = ML.nc_d; w.base = lb + ML.off_gu; }
+    else { U = ML.u_dn; w.nc = ML.nc_f; w.base = lb + ML.off_dn; }
+  }
+  w.u0 = (int)((long long)idx * U / gs);
+  w.u1 = (int)((long long)(idx + 1) * U / gs);
+  w.ntiles = (w.u1 - w.u0) * w.nc;
+  w.base += (unsigned long long)w.u0 * w.nc * kTileBytes;
+  return w;
+}
+
+// ------------------------------------------------------------------ consumer pieces ------------
+// 8 fp32 FMAs of one 16-byte weight chunk against two float4 of x.
+__device__ __forceinline__ float fma8(uint4 w, float4 xa, float4 xb, float acc) {
+  acc = fmaf(bf16_lo(w.x), xa.x, acc); acc = fmaf(bf16_hi(w.x), xa.y, acc);
+  acc = fmaf(bf16_lo(w.y), xa.z, acc); acc = fmaf(bf16_hi(w.y), xa.w, acc);
+  acc = fmaf(bf16_lo(w.z), xb.x, acc); acc = fmaf(bf16_hi(w.z), xb.y, acc);
+  acc = fmaf(bf16_lo(w.w), xb.z, acc); acc = fmaf(bf16_hi(w.w), xb.w, acc);
+  return acc;
+}
+
+// RMS scale over the 256 consumer threads (fixed tree: strided per-thread sums, xor-tree, 8 warp
+// partials added in order).  src is read with ld.global.cg (it was written by other CTAs).
+__device__ __forceinline__ float consumer_rms_scale(const float *src, int d, float eps, float *red) {
+  float ss = 0.f;
+  for (int i = threadIdx.x; i < d; i += kConsumerThreads) { float v = __ldcg(src + i); ss = fmaf(v, v, ss); }
+  ss = warp_sum(ss);
+  consumer_sync();
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+  consumer_sync();
+  float t = 0.f;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) t += red[w];
+  return 1.0f / sqrtf(t / (float)d + eps);
+}
+
+// The fused kernel ---------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout ML) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint8_t *ring = smem;                                                  // kStages * 16 KB
+  float *xs = reinterpret_cast<float *>(smem + kStages * kTileBytes);    // kXFloats
+  uint64_t *full = reinterpret_cast<uint64_t *>(xs + kXFloats);          // [kStages]
+  uint64_t *empty = full + kStages;                                      // [kStages]
+  float2 *rope_s = reinterpret_cast<float2 *>(empty + kStages);          // [64]
+  float *red = reinterpret_cast<float *>(rope_s + 64);                   // [16]
+  float *cbest_v = red + 16;                                             // [2][8]
+  int *cbest_i = reinterpret_cast<int *>(cbest_v + 16);                  // [2][8]
+  Sched *Sp = reinterpret_cast<Sched *>(cbest_i + 16);
+
+  const Dims &D = P.dim;
+  const int cta = blockIdx.x, ncta = gridDim.x;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int np = 2 + 5 * D.per;
+  const unsigned long long nbar = (unsigned long long)(5 * D.per + 1);
+  unsigned long long *bar_count = reinterpret_cast<unsigned long long *>(P.bar);
+  unsigned long long *bar_launch = bar_count + 1;
+
+  // ---- schedule (every CTA computes the same thing from the state the previous cycle left) ----
+  if (tid == 0) {
+    const StepState *st = P.st;
+    Sched &S = *Sp;
+    S.mode = st->mode; S.c = st->c;
+    int a = 0;
+    for (int k = 0; k < D.n; ++k) {
+      S.occ[k] = st->occ[k]; S.pos[k] = st->pos[k]; S.hbuf[k] = st->hbuf[k];
+      if (st->occ[k]) S.act[a++] = k;
+    }
+    S.n_act = a;
+    S.p_new = st->occ[0] ? st->pos[0] : -1;
+    S.run_pdm = st->mode == MODE_SPD;
+    S.run_verify = (st->mode == MODE_SPD && st->occ[D.n - 1]) || st->mode == MODE_PREFILL_FINAL;
+    S.my_stage = -1; S.my_idx = 0; S.my_gs = 1;
+    if (a > 0) {
+      int g;
+      group_of(cta, ncta, a, g, S.my_idx, S.my_gs);
+      S.my_stage = S.act[g];
+    }
+    for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const Sched &S = *Sp;
+  const unsigned long long launch = ld_acquire_u64(bar_launch);
+  if (cta == 0 && tid == 0) controller_begin(P);   // writes only fields no other CTA reads in this kernel
+  if (S.my_stage >= 0 && tid < D.hd / 2) {         // RoPE table of this CTA's stage (C-2.14)
+    double s_, c_;
+    sincos((double)S.pos[S.my_stage] * P.inv_freq[tid], &s_, &c_);
+    rope_s[tid] = make_float2((float)c_, (float)s_);
+  }
+  __syncthreads();
+
+  if (warp == 8) {
+    // =========================== producer: stream every phase's tiles, running ahead ===========
+    if (lane == 0) {
+      uint64_t policy;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      uint32_t seq = 0;
+      for (int p = 0; p < np; ++p) {
+        Work w = phase_work(p, np, S, ML, D, cta, ncta);
+        const uint8_t *src = w.base;
+        for (int i = 0; i < w.ntiles; ++i, ++seq, src += kTileBytes) {
+          uint32_t slot = seq % kStages, it = seq / kStages;
+          mbar_wait(&empty[slot], (it & 1) ^ 1);
+          mbar_expect_tx(&full[slot], kTileBytes);
+          tma_load_1d(ring + (size_t)slot * kTileBytes, src, kTileBytes, &full[slot], policy);
+        }
+      }
+    }
+  } else {
+    // =========================== consumers ======================================================
+    uint32_t seq = 0;
+    unsigned long long bar_idx = 0;          // barriers passed in this cycle
+    float hbest_v[2] = {-INFINITY, -INFINITY};
+    int hbest_i[2] = {0x7fffffff, 0x7fffffff};
+    for (int p = 0; p < np; ++p) {
+      const int t = phase_type(p, np);
+      const int pass = (p - 1) / 5;
+      // ---- wait for the producers of this phase's inputs (all phases but PDM and the first QKV) ----
+      const bool need_barrier = !(p == 0 || p == 1);
+      if (need_barrier) {
+        if (tid == 0) {
+          unsigned long long target = (launch * nbar + bar_idx + 1) * (unsigned long long)ncta;
+          while (ld_acquire_u64(bar_count) < target) {}
+        }
+        ++bar_idx;
+      }
+      consumer_sync();   // also: every warp is done with the previous phase's xs
+      Work w = phase_work(p, np, S, ML, D, cta, ncta);
+      const int k = w.job;                    // stage (layer phases) / slot (PDM)
+      if (t == PH_ATTN) {
+        // ---- split-KV decode attention: items (stage, kv head, 128-row split) round-robin over CTAs;
+        //      warps [g*G, (g+1)*G) take one item, one q head per warp; the last warp to finish a
+        //      q head merges its splits in split order.
+        const int G = D.Hq / D.Hkv, spc = 8 / G;
+        const int slot_in_cta = warp / G, hq_in_group = warp % G;
+        int total = 0;
+        for (int a = 0; a < S.n_act; ++a) total += D.Hkv * ((S.pos[S.act[a]] + kAttnSplit) / kAttnSplit);
+        if (slot_in_cta < spc) {
+          for (int item = cta * spc + slot_in_cta; item < total; item += ncta * spc) {
+            int rem = item, stage = -1, nsplit = 0;
+            for (int a = 0; a < S.n_act; ++a) {
+              int ns = (S.pos[S.act[a]] + kAttnSplit) / kAttnSplit;
+              if (rem < D.Hkv * ns) { stage = S.act[a]; nsplit = ns; break; }
+              rem -= D.Hkv * ns;
+            }
+            int kvh = rem / nsplit, split = rem - kvh * nsplit;
+            int T = S.pos[stage] + 1, t0 = split * kAttnSplit, t1 = min(T, t0 + kAttnSplit);
+            int layer = stage * D.per + pass, hq = kvh * G + hq_in_group;
+            const uint16_t *kc = P.kv + kv_offset(D, layer, 0, kvh), *vc = P.kv + kv_offset(D, layer, 1, kvh);
+            size_t slot = ((size_t)stage * D.Hq + hq) * P.nsplit_max;
+            const float *qh = P.q + ((size_t)stage * D.Hq + hq) * D.hd;
+            if (D.hd == 128) attn_partial_warp<128>(qh, kc, vc, t0, t1, P.part_o + (slot + split) * 128, P.part_ml + slot + split);
+            else attn_partial_warp<64>(qh, kc, vc, t0, t1, P.part_o + (slot + split) * 64, P.part_ml + slot + split);
+            __threadfence();
+            int old = 0;
+            if (lane == 0) old = atomicAdd(&P.att_cnt[stage * D.Hq + hq], 1);
+            old = __shfl_sync(0xffffffffu, old, 0);
+            if (old == nsplit - 1) {           // last split of this q head: merge (fixed split order)
+              __threadfence();
+              const float2 *ml = P.part_ml + slot;
+              float M = -INFINITY;
+              for (int j = 0; j < nsplit; ++j) M = fmaxf(M, __ldcg(&ml[j].x));
+              const int epl = D.hd / 32;
+              for (int e = lane * epl; e < (lane + 1) * epl; ++e) {
+                float L = 0.f, o = 0.f;
+                for (int j = 0; j < nsplit; ++j) {
+                  float2 mlj = __ldcg(&ml[j]);
+                  float wj = expf(mlj.x - M);
+                  L = fmaf(mlj.y, wj, L);
+                  o = fmaf(__ldcg(P.part_o + (slot + j) * D.hd + e), wj, o);
+                }
+                P.att[((size_t)stage * D.Hq + hq) * D.hd + e] = o / L;
+              }
+              if (lane == 0) P.att_cnt[stage * D.Hq + hq] = 0;
+            }
+          }
+        }
+      } else if (w.ntiles > 0 || t == PH_QKV) {
+        // ---- stage the activation vector(s) of this phase in shared memory ----------------------
+        int K = 0;
+        if (w.ntiles > 0) {
+          if (t == PH_QKV || t == PH_GATEUP) {
+            int layer = k * D.per + pass;
+            const float *h = P.h + (size_t)S.hbuf[k] * D.d;
+            const uint16_t *g = t == PH_QKV ? P.attn_norm[layer] : P.mlp_norm[layer];
+            float r = consumer_rms_scale(h, D.d, D.eps, red);
+            for (int i = tid; i < D.d; i += kConsumerThreads) xs[i] = __ldcg(h + i) * r * bf16_to_f32(g[i]);
+            K = D.d;
+          } else if (t == PH_O) {
+            K = D.Hq * D.hd;
+            const float *src = P.att + (size_t)k * K;
+            for (int i = tid; i < K; i += kConsumerThreads) xs[i] = __ldcg(src + i);
+          } else if (t == PH_DOWN) {
+            K = D.F;
+            const float *src = P.act + (size_t)k * K;
+            for (int i = tid; i < K; i += kConsumerThreads) xs[i] = __ldcg(src + i);
+          } else if (t == PH_PDM) {
+            // slot j = k: pre-step state of the token at depth j, else Hfin[p_new - j], else zero (Eq. 5)
+            K = D.d;
+            int q = S.p_new - k;
+            const float *src = S.occ[k] ? P.h + (size_t)S.hbuf[k] * D.d : (q >= 0 ? P.hfin + (size_t)q * D.d : nullptr);
+            for (int i = tid; i < K; i += kConsumerThreads) {
+              float v = src ? __ldcg(src + i) : 0.f;
+              xs[i] = v;
+              if (w.u0 == 0) P.feat[(size_t)k * D.d + i] = v;   // kept for the parity tests (SPD_DBG_PDM_FEAT)
+            }
+          } else {  // PH_HEAD: verify input at xs[0..d), PDM input at xs[kXFloats/2 ..)
+            K = D.d;
+            if (S.run_verify) {
+              const float *h = S.mode == MODE_PREFILL_FINAL ? P.hfin + (size_t)(S.c - 1) * D.d
+                                                            : P.h + (size_t)S.hbuf[D.n - 1] * D.d;
+              float r = consumer_rms_scale(h, D.d, D.eps, red);
+              for (int i = tid; i < D.d; i += kConsumerThreads) xs[i] = __ldcg(h + i) * r * bf16_to_f32(P.final_norm[i]);
+            }
+            if (S.run_pdm) {
+              float *xp = xs + kXFloats / 2;
+              float ss = 0.f;
+              for (int i = tid; i < D.d; i += kConsumerThreads) {   // u = sum_j W_p[:, block j] f_j, j ascending
+                float u = 0.f;
+                for (int j = 0; j < D.n; ++j) u += __ldcg(P.pdm_part + (size_t)j * D.d + i);
+                xp[i] = u;
+                if (w.u0 == 0) P.pdm_u[i] = u;    // kept for the parity tests (SPD_DBG_PDM_PRENORM)
+                ss = fmaf(u, u, ss);
+              }
+              ss = warp_sum(ss);
+              consumer_sync();
+              if (lane == 0) red[warp] = ss;
+              consumer_sync();
+              float tt = 0.f;
+#pragma unroll
+              for (int ww = 0; ww < 8; ++ww) tt += red[ww];
+              float r = 1.0f / sqrtf(tt / (float)D.d + D.eps);
+              for (int i = tid; i < D.d; i += kConsumerThreads) xp[i] = xp[i] * r * bf16_to_f32(P.pdm_norm[i]);
+            }
+          }
+          int kpad = w.nc * kTileCols;
+          for (int i = K + tid; i < kpad; i += kConsumerThreads) xs[i] = 0.f;
+          if (t == PH_HEAD) for (int i = K + tid; i < kpad; i += kConsumerThreads) xs[kXFloats / 2 + i] = 0.f;
+        }
+        if (t == PH_QKV && S.my_stage >= 0 && S.my_idx == 0 && tid == 0) {
+          // causality / capacity precondition of the KV append, and the new length (one CTA per stage)
+          int layer = S.my_stage * D.per + pass, pos = S.pos[S.my_stage];
+          if (P.len[layer] != pos || pos >= D.max_seq) P.st->err = 1;
+          else P.len[layer] = pos + 1;
+        }
+        consumer_sync();
+        // ---- stream the tiles ------------------------------------------------------------------
+        const bool two = t == PH_HEAD;
+        const float4 *xv4 = reinterpret_cast<const float4 *>(xs);
+        const float4 *xp4 = reinterpret_cast<const float4 *>(xs + kXFloats / 2);
+        const bool do_v = !two || S.run_verify, do_p = two && S.run_pdm;
+        for (int u = w.u0; u < w.u1; ++u) {
+          float a00 = 0.f, a01 = 0.f, a10 = 0.f, a11 = 0.f;   // [row][column group], first vector
+          float b00 = 0.f, b01 = 0.f, b10 = 0.f, b11 = 0.f;   // second vector (LM head only)
+          for (int c = 0; c < w.nc; ++c, ++seq) {
+            uint32_t slot = seq % kStages, it = seq / kStages;
+            mbar_wait(&full[slot], it & 1);
+            const uint4 *wt = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kTileBytes);
+            uint4 wa0 = wt[(2 * warp) * 64 + lane], wa1 = wt[(2 * warp) * 64 + 32 + lane];
+            uint4 wb0 = wt[(2 * warp + 1) * 64 + lane], wb1 = wt[(2 * warp + 1) * 64 + 32 + lane];
+            if (do_v) {
+              const float4 *x4 = xv4 + c * (kTileCols / 4);
+              float4 x00 = x4[lane], x01 = x4[32 + lane], x10 = x4[64 + lane], x11 = x4[96 + lane];
+              a00 = fma8(wa0, x00, x01, a00); a01 = fma8(wa1, x10, x11, a01);
+              a10 = fma8(wb0, x00, x01, a10); a11 = fma8(wb1, x10, x11, a11);
+            }
+            if (do_p) {
+              const float4 *x4 = xp4 + c * (kTileCols / 4);
+              float4 x00 = x4[lane], x01 = x4[32 + lane], x10 = x4[64 + lane], x11 = x4[96 + lane];
+              b00 = fma8(wa0, x00, x01, b00); b01 = fma8(wa1, x10, x11, b01);
+              b10 = fma8(wb0, x00, x01, b10); b11 = fma8(wb1, x10, x11, b11);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[slot]);
+          }
+          // ---- unit done: reduce the two rows of this warp, fused epilogue (lane 0) ---------------
+          float y0 = warp_sum(a00 + a01), y1 = warp_sum(a10 + a11);
+          float z0 = 0.f, z1 = 0.f;
+          if (two) { z0 = warp_sum(b00 + b01); z1 = warp_sum(b10 + b11); }
+          if (lane == 0) {
+            const int r0 = u * kTileRows + 2 * warp;   // repacked row index (even); r0 + 1 is its partner
+            if (t == PH_QKV) {
+              const int qd = D.Hq * D.hd, kd = D.Hkv * D.hd, half = D.hd / 2, pos = S.pos[k];
+              const int layer = k * D.per + pass;
+              if (r0 < qd) {                           // q pair (i, i + hd/2) of head hh: RoPE (C-2.14)
+                int hh = r0 / D.hd, i = (r0 - hh * D.hd) >> 1;
+                float2 cs = rope_s[i];
+                float *q = P.q + (size_t)k * qd + hh * D.hd;
+                q[i] = y0 * cs.x - y1 * cs.y;
+                q[i + half] = y1 * cs.x + y0 * cs.y;
+              } else if (r0 < qd + kd) {               // k pair: RoPE, bf16 (RNE), append at row pos
+                int rr = r0 - qd, hh = rr / D.hd, i = (rr - hh * D.hd) >> 1;
+                float2 cs = rope_s[i];
+                if (pos < D.max_seq) {
+                  uint16_t *dst = P.kv + kv_offset(D, layer, 0, hh) + (size_t)pos * D.hd;
+                  dst[i] = f32_to_bf16(y0 * cs.x - y1 * cs.y);
+                  dst[i + half] = f32_to_bf16(y1 * cs.x + y0 * cs.y);
+                }
+              } else if (r0 < qd + 2 * kd) {           // two consecutive v elements: bf16, append
+                int rr = r0 - qd - kd, hh = rr / D.hd, i = rr - hh * D.hd;
+                if (pos < D.max_seq) {
+                  uint16_t *dst = P.kv + kv_offset(D, layer, 1, hh) + (size_t)pos * D.hd;
+                  dst[i] = f32_to_bf16(y0);
+                  dst[i + 1] = f32_to_bf16(y1);
+                }
+              }
+            } else if (t == PH_O || t == PH_DOWN) {    // residual add
+              float *h = P.h + (size_t)S.hbuf[k] * D.d;
+              if (r0 < D.d) h[r0] = __ldcg(h + r0) + y0;
+              if (r0 + 1 < D.d) h[r0 + 1] = __ldcg(h + r0 + 1) + y1;
+            } else if (t == PH_GATEUP) {               // rows (gate_i, up_i): SwiGLU
+              int i = r0 >> 1;
+              if (i < D.F) P.act[(size_t)k * D.F + i] = silu_mul(y0, y1);
+            } else if (t == PH_PDM) {
+              if (r0 < D.d) P.pdm_part[(size_t)k * D.d + r0] = y0;
+              if (r0 + 1 < D.d) P.pdm_part[(size_t)k * D.d + r0 + 1] = y1;
+            } else {                                   // PH_HEAD: running (value, index) argmax
+              if (S.run_verify) {
+                if (r0 < D.V && cand_better(y0, r0, hbest_v[0], hbest_i[0])) { hbest_v[0] = y0; hbest_i[0] = r0; }
+                if (r0 + 1 < D.V && cand_better(y1, r0 + 1, hbest_v[0], hbest_i[0])) { hbest_v[0] = y1; hbest_i[0] = r0 + 1; }
+              }
+              if (S.run_pdm) {
+                if (r0 < D.V && cand_better(z0, r0, hbest_v[1], hbest_i[1])) { hbest_v[1] = z0; hbest_i[1] = r0; }
+                if (r0 + 1 < D.V && cand_better(z1, r0 + 1, hbest_v[1], hbest_i[1])) { hbest_v[1] = z1; hbest_i[1] = r0 + 1; }
+              }
+              if (P.debug_logits) {
+                if (S.run_verify) { if (r0 < D.V) P.logits_v[r0] = y0; if (r0 + 1 < D.V) P.logits_v[r0 + 1] = y1; }
+                if (S.run_pdm) { if (r0 < D.V) P.logits_p[r0] = z0; if (r0 + 1 < D.V) P.logits_p[r0 + 1] = z1; }
+              }
+            }
+          }
+        }
+        if (t == PH_HEAD) {   // CTA-level candidates -> global
+          if (lane == 0) { cbest_v[warp] = hbest_v[0]; cbest_v[8 + warp] = hbest_v[1]; cbest_i[warp] = hbest_i[0]; cbest_i[8 + warp] = hbest_i[1]; }
+          consumer_sync();
+          if (tid < 2) {
+            float bv = -INFINITY;
+            int bi = 0x7fffffff;
+            for (int ww = 0; ww < 8; ++ww)
+              if (cand_better(cbest_v[tid * 8 + ww], cbest_i[tid * 8 + ww], bv, bi)) { bv = cbest_v[tid * 8 + ww]; bi = cbest_i[tid * 8 + ww]; }
+            P.cand_val[tid * kMaxCand + cta] = bv;
+            P.cand_idx[tid * kMaxCand + cta] = bi == 0x7fffffff ? -1 : bi;
+          }
+        }
+      }
+      // ---- publish this phase's outputs: arrive at the barrier that the dependent phase waits on ----
+      const bool arrive = p >= 1;              // PDM has no barrier of its own (see need_barrier)
+      if (arrive) {
+        __threadfence();
+        consumer_sync();
+        if (tid == 0) atomicAdd(bar_count, 1ull);
+      }
+    }
+  }
+  // ---- last: CTA 0 waits for every CTA's head candidates, then runs the controller ---------------
+  __syncthreads();
+  if (cta == 0) {
+    if (tid == 0) {
+      unsigned long long target = (launch + 1) * nbar * (unsigned long long)ncta;
+      while (ld_acquire_u64(bar_count) < target) {}
+      __threadfence();
+    }
+    __syncthreads();
+    controller_end(P, ncta);
+    __syncthreads();
+    if (tid == 0) { __threadfence(); atomicAdd(bar_launch, 1ull); }
+  }
+}
+
+// ------------------------------------------------------------------ weight repack --------------
+// dst tile layout: [unit u][chunk c][row r (16)][column group g (2)][lane l (32)][j (8)] bf16, where the
+// logical column of (g, l, j) inside the chunk is g*256 + (j < 4 ? 4l + j : 128 + 4l + j - 4): a lane's
+// 16-byte weight chunk multiplies the two float4 x[4l..4l+3] and x[128+4l..128+4l+3] of the group, both
+// read as conflict-free LDS.128.  Row maps: QKV -> RoPE pairs (i, i+hd/2) adjacent, q heads, k heads,
+// then v rows; GATEUP -> (gate_i, up_i) adjacent; others identity.  Padding rows/columns are zero.
+enum RowMap { RM_PLAIN = 0, RM_QKV = 1, RM_GATEUP = 2 };
+
+__global__ void k_repack(uint16_t *dst, int units, int nc, int rowmap, const uint16_t *s0, const uint16_t *s1,
+                         const uint16_t *s2, int rows0, int rows1, int rows2, int K, int src_ld, int src_col0, int hd) {
+  size_t total = (size_t)units * nc * kTileRows * 64;      // 16-byte chunks
+  for (size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x; id < total; id += (size_t)gridDim.x * blockDim.x) {
+    int l = id & 31, g = (id >> 5) & 1, r = (id >> 6) & 15;
+    size_t tile = id >> 10;
+    int c = tile % nc, u = tile / nc;
+    int rho = u * kTileRows + r;
+    const uint16_t *src = nullptr;
+    int row = -1;
+    if (rowmap == RM_PLAIN) {
+      if (rho < rows0) { src = s0; row = rho; }
+    } else if (rowmap == RM_GATEUP) {
+      int i = rho >> 1;
+      if (i < rows0) { src = (rho & 1) ? s1 : s0; row = i; }
+    } else {
+      int half = hd / 2;
+      if (rho < rows0 + rows1) {                           // q or k heads: pairs adjacent
+        int base = rho < rows0 ? 0 : rows0;
+        int rr = rho - base, hh = rr / hd, e = rr - hh * hd;
+        row = hh * hd + (e >> 1) + ((e & 1) ? half : 0);
+        src = rho < rows0 ? s0 : s1;
+      } else if (rho < rows0 + rows1 + rows2) { src = s2; row = rho - rows0 - rows1; }
+    }
+    uint16_t out[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      int col = c * kTileCols + g * 256 + (j < 4 ? 4 * l + j : 128 + 4 * l + j - 4);
+      out[j] = (src && col < K) ? src[(size_t)row * src_ld + src_col0 + col] : (uint16_t)0;
+    }
+    reinterpret_cast<uint4 *>(dst)[id] = *reinterpret_cast<uint4 *>(out);
+  }
+}
+
+// ------------------------------------------------------------------ host side ------------------
+static inline int cdiv_i(int a, int b) { return (a + b - 1) / b; }
+
+static void make_layout(const Dims &D, MegaLayout *ML, size_t *total) {
+  int qd = D.Hq * D.hd, kd = D.Hkv * D.hd;
+  ML->nc_d = cdiv_i(D.d, kTileCols); ML->nc_qd = cdiv_i(qd, kTileCols); ML->nc_f = cdiv_i(D.F, kTileCols);
+  ML->u_qkv = cdiv_i(qd + 2 * kd, kTileRows); ML->u_o = cdiv_i(D.d, kTileRows); ML->u_gu = cdiv_i(2 * D.F, kTileRows);
+  ML->u_dn = cdiv_i(D.d, kTileRows); ML->u_pdm = cdiv_i(D.d, kTileRows); ML->u_head = cdiv_i(D.V, kTileRows);
+  unsigned long long b_qkv = (unsigned long long)ML->u_qkv * ML->nc_d * kTileBytes;
+  unsigned long long b_o = (unsigned long long)ML->u_o * ML->nc_qd * kTileBytes;
+  unsigned long long b_gu = (unsigned long long)ML->u_gu * ML->nc_d * kTileBytes;
+  unsigned long long b_dn = (unsigned long long)ML->u_dn * ML->nc_f * kTileBytes;
+  ML->off_o = b_qkv; ML->off_gu = b_qkv + b_o; ML->off_dn = b_qkv + b_o + b_gu;
+  ML->layer_bytes = b_qkv + b_o + b_gu + b_dn;
+  ML->pdm_job_bytes = (unsigned long long)ML->u_pdm * ML->nc_d * kTileBytes;
+  ML->off_pdm = ML->layer_bytes * D.L;
+  ML->off_head = ML->off_pdm + ML->pdm_job_bytes * D.n;
+  *total = ML->off_head + (unsigned long long)ML->u_head * ML->nc_d * kTileBytes;
+}
+
+static bool mega_supported(const Dims &D) {
+  int qd = D.Hq * D.hd;
+  int G = D.Hq / D.Hkv;
+  return D.d <= kXFloats / 2 && qd <= kXFloats && D.F <= kXFloats && (G == 1 || G == 2 || G == 4 || G == 8) &&
+         (qd + 2 * D.Hkv * D.hd) % 2 == 0 && D.hd % 2 == 0;
+}
+
+size_t mega_repack_bytes(const Dims &D) {
+  if (!mega_supported(D)) return 256;
+  MegaLayout ML;
+  size_t total;
+  make_layout(D, &ML, &total);
+  return total;
+}
+
+int mega_create(const DevPtrs &P, const uint16_t *const *const *src, void *repack, size_t repack_bytes,
+                cudaStream_t stream, MegaPlan *plan) {
+  const Dims &D = P.dim;
+  plan->available = 0;
+  if (!mega_supported(D) || !repack) return -1;
+  MegaLayout ML;
+  size_t total;
+  make_layout(D, &ML, &total);
+  if (repack_bytes < total) return -1;
+  int dev = 0, sms = 0, coop = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+  int smem = kStages * kTileBytes + kXFloats * 4 + 2 * kStages * 8 + 64 * 8 + 16 * 4 + 32 * 4 + (int)sizeof(Sched) + 64;
+  if (!coop || sms < D.n) return -1;
+  if (cudaFuncSetAttribute(k_spd_cycle, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
+    cudaGetLastError();
+    return -1;
+  }
+  int occ = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_spd_cycle, kThreads, smem) != cudaSuccess || occ < 1) {
+    cudaGetLastError();
+    return -1;
+  }
+  ML.repack = (const uint8_t *)repack;
+  uint8_t *base = (uint8_t *)repack;
+  int qd = D.Hq * D.hd, kd = D.Hkv * D.hd;
+  const int RB = 1184, RT = 256;
+  for (int l = 0; l < D.L; ++l) {
+    uint8_t *lb = base + (size_t)l * ML.layer_bytes;
+    // spd_weights order: 0 attn_norm 1 wq 2 wk 3 wv 4 wo 5 mlp_norm 6 w_gate 7 w_up 8 w_down
+    k_repack<<<RB, RT, 0, stream>>>((uint16_t *)lb, ML.u_qkv, ML.nc_d, RM_QKV, src[1][l], src[2][l], src[3][l], qd, kd, kd,
+                                    D.d, D.d, 0, D.hd);
+    k_repack<<<RB, RT, 0, stream>>>((uint16_t *)(lb + ML.off_o), ML.u_o, ML.nc_qd, RM_PLAIN, src[4][l], nullptr, nullptr,
+                                    D.d, 0, 0, qd, qd, 0, D.hd);
+    k_repack<<<RB, RT, 0, stream>>>((uint16_t *)(lb + ML.off_gu), ML.u_gu, ML.nc_d, RM_GATEUP, src[6][l], src[7][l],
+                                    nullptr, D.F, D.F, 0, D.d, D.d, 0, D.hd);
+    k_repack<<<RB, RT, 0, stream>>>((uint16_t *)(lb + ML.off_dn), ML.u_dn, ML.nc_f, RM_PLAIN, src[8][l], nullptr, nullptr,
+                                    D.d, 0, 0, D.F, D.F, 0, D.hd);
+  }
+  for (int j = 0; j < D.n; ++j)   // W_p column block j: [d, d] at columns j*d
+    k_repack<<<RB, RT, 0, stream>>>((uint16_t *)(base + ML.off_pdm + (size_t)j * ML.pdm_job_bytes), ML.u_pdm, ML.nc_d,
+                                    RM_PLAIN, P.pdm_proj, nullptr, nullptr, D.d, 0, 0, D.d, D.n * D.d, j * D.d, D.hd);
+  k_repack<<<RB, RT, 0, stream>>>((uint16_t *)(base + ML.off_head), ML.u_head, ML.nc_d, RM_PLAIN, P.embed, nullptr, nullptr,
+                                  D.V, 0, 0, D.d, D.d, 0, D.hd);
+  if (cudaGetLastError() != cudaSuccess) return -1;
+  plan->repack = (const uint16_t *)repack;
+  plan->n_cta = sms;
+  plan->smem_bytes = smem;
+  plan->available = 1;
+  static_assert(sizeof(MegaLayout) <= sizeof(plan->layout), "layout storage");
+  memcpy(plan->layout, &ML, sizeof ML);
+  return 0;
+}
+
+int mega_enqueue_step(const DevPtrs &P, const MegaPlan &plan, cudaStream_t sm, long long *launches) {
+  if (!plan.available) return -1;
+  MegaLayout ML;
+  memcpy(&ML, plan.layout, sizeof ML);
+  DevPtrs Pc = P;
+  void *args[] = {(void *)&Pc, (void *)&ML};
+  cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_spd_cycle, dim3(plan.n_cta), dim3(kThreads), args,
+                                              (size_t)plan.smem_bytes, sm);
+  if (launches) *launches += 1;
+  return e == cudaSuccess ? 0 : -1;
+}
+
 }  // namespace spd

@@ -2,9 +2,16 @@
 
 Runs the CUDA library and the CPU oracle on the same seeded inputs, cycle by cycle, and compares:
 step results (token ids, accept bits, fill, committed length: exact), per-depth hidden states, PDM
-pre-norm vector, logits, KV lengths (exact) and KV rows.  Token mismatches are classified with the
-oracle's top-1/top-2 margin: below TAU * max|logit| it is a near-tie (fp32
-re-association can legitimately flip it) and the caller retries with the next seed; above, a failure.
+pre-norm vector, logits, KV lengths (exact) and KV rows.
+
+Token exactness and ties.  The CUDA path accumulates in fp32, the oracle
+in fp64; through 32 random-init layers that difference grows to ~1e-3 of the logit scale, while the
+top-1/top-2 gap of 151 936 near-i.i.d. logits is below that for a few percent of the argmaxes.  Where
+the two argmaxes differ, the CUDA token is accepted only if its ORACLE logit lies within
+2 * logit_tol * max|logit| of the oracle's maximum — i.e. only if the disagreement is implied by the
+logit tolerance that is asserted anyway (several results are then correct; the rest must be valid).
+The oracle then follows that token (ora_step_follow) so every later cycle is still compared exactly.
+Any other token difference is a failure.
 """
 from __future__ import annotations
 
@@ -15,7 +22,6 @@ import numpy as np
 import spd_inputs as si
 from oracle import Oracle
 
-TAU = 1e-4          # near-tie threshold on (top1 - top2) / max|logit|
 CONTRACT = 2e-2     # north_star: hidden states and logits within max relative error 2e-2
 
 
@@ -28,7 +34,7 @@ def rel_err(a, b) -> float:
 
 @dataclasses.dataclass
 class Report:
-    status: str = "ok"            # "ok" | "near_tie" | "fail"
+    status: str = "ok"            # "ok" | "fail"
     detail: str = ""
     steps: int = 0
     emitted: int = 0
@@ -39,7 +45,15 @@ class Report:
     min_margin: float = 1.0
     accepts: int = 0
     rejects: int = 0
+    verify_ties: int = 0
+    pdm_ties: int = 0
     tokens: list = dataclasses.field(default_factory=list)
+
+    def summary(self) -> str:
+        return (f"{self.status} steps={self.steps} emitted={self.emitted} acc/rej={self.accepts}/{self.rejects} "
+                f"hidden={self.max_hidden_err:.2e} pdm={self.max_pdm_err:.2e} logits={self.max_logit_err:.2e} "
+                f"kvflip={self.kv_flip_frac:.2e} min_margin={self.min_margin:.2e} "
+                f"ties(verify/pdm)={self.verify_ties}/{self.pdm_ties} {self.detail}")
 
 
 def kv_compare(gpu, ora, layers, rows, rep: Report, tol: float):
@@ -58,16 +72,23 @@ def kv_compare(gpu, ora, layers, rows, rep: Report, tol: float):
 
 
 def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, engine=None, tensor_every=1,
-               tensor_tol=CONTRACT, check_logits=True, prefill_block=16, max_seq=None, spd_cls=None, gpu=None) -> Report:
-    """forced = (truth tokens, p, seed) or None (the PDM's own drafts)."""
+               tensor_tol=CONTRACT, check_logits=True, prefill_block=16, max_seq=None, gpu=None) -> Report:
+    """forced = (truth tokens, p, seed) or None (the PDM's own drafts).  tensor_tol bounds hidden states,
+    the PDM vector and logits (C-2.18 metric); the tie band is 2 * tensor_tol."""
     from paper_2605_30852_b200 import SPD, OPT
     rep = Report()
     n = shape.n_stages
+    band = 2.0 * tensor_tol
     ms = max_seq or (len(prompt) + n_tokens * (n + 1) + 2 * n + 8)
     ora = Oracle(shape, weights_np, max_seq=ms)
     own = gpu is None
     if own:
-        gpu = (spd_cls or SPD)(shape, dev_weights, max_seq=ms)
+        gpu = SPD(shape, dev_weights, max_seq=ms)
+
+    def fail(msg):
+        rep.status, rep.detail = "fail", msg
+        return rep
+
     try:
         if engine is not None:
             gpu.set_option(OPT.ENGINE, engine)
@@ -76,42 +97,39 @@ def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, en
         fg = gpu.prefill(prompt)
         gap, mx = ora.margin(0)
         rep.min_margin = gap / mx
-        if fo != fg:
-            if gap < TAU * mx:
-                rep.status, rep.detail = "near_tie", "first token"
-            else:
-                rep.status, rep.detail = "fail", f"first token {fg} != oracle {fo} (margin {gap / mx:.2e})"
-            return rep
-        rep.tokens.append(fg)
         P = len(prompt)
         e = rel_err(gpu.hfin(P - 1), ora.hfin(P - 1))
         rep.max_hidden_err = max(rep.max_hidden_err, e)
         if e > tensor_tol:
-            rep.status, rep.detail = "fail", f"prefill final hidden state rel err {e:.3e}"
-            return rep
+            return fail(f"prefill final hidden state rel err {e:.3e}")
+        if fo != fg:
+            lg = ora.last("exit_logits")
+            if lg[fo] - lg[fg] <= band * mx:
+                rep.verify_ties += 1
+                ora.rollback(P, fg)          # both are valid first tokens at the logit tolerance: follow the GPU
+            else:
+                return fail(f"first token {fg} != oracle {fo} (margin {gap / mx:.2e})")
+        rep.tokens.append(fg)
         if not np.array_equal(gpu.kv_len(), ora.kv_len()):
-            rep.status, rep.detail = "fail", "KV lengths differ after prefill"
-            return rep
+            return fail("KV lengths differ after prefill")
         if not kv_compare(gpu, ora, sorted({0, shape.n_layers // 2, shape.n_layers - 1}), P, rep, tensor_tol):
             return rep
         if forced is not None:
             truth, p, seed = forced
             ora.set_forced(truth, p, seed)
             gpu.set_forced(truth, p, seed)
+        v0 = rep.verify_ties
         while ora.emitted < n_tokens:
-            ro = ora.step()
             rg = gpu.step()
+            ro = ora.step_follow(-1 if rg.draft_forced else rg.draft_token, rg.emitted_token if rg.exited else -1, band)
             rep.steps += 1
+            vt, pt = ora.ties()
+            rep.verify_ties, rep.pdm_ties = v0 + vt, pt
             if tuple(ro) != tuple(rg):
-                which = 0 if ro.emitted_token != rg.emitted_token else 1
-                gap, mx = ora.margin(which)
-                only_token = (ro._replace(emitted_token=0, draft_token=0, accepted=0, discarded=0, committed_len=0) ==
-                              rg._replace(emitted_token=0, draft_token=0, accepted=0, discarded=0, committed_len=0))
-                if only_token and gap < TAU * mx:
-                    rep.status, rep.detail = "near_tie", f"step {rep.steps}: {'verify' if which == 0 else 'PDM'} margin {gap / mx:.2e}"
-                else:
-                    rep.status, rep.detail = "fail", f"step {rep.steps}: gpu {tuple(rg)} != oracle {tuple(ro)} (margin {gap / mx:.2e})"
-                return rep
+                gv, mv = ora.margin(0)
+                gp, mp = ora.margin(1)
+                return fail(f"step {rep.steps}: gpu {tuple(rg)} != oracle {tuple(ro)} "
+                            f"(verify margin {gv / mv:.2e}, PDM margin {gp / mp:.2e}, band {band:.1e})")
             if ro.exited:
                 rep.emitted += 1
                 rep.tokens.append(ro.emitted_token)
@@ -124,48 +142,26 @@ def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, en
             if rep.steps % tensor_every == 0:
                 fill, c, slots = gpu.ring()
                 if fill != ora.fill or c != ora.committed_len:
-                    rep.status, rep.detail = "fail", f"step {rep.steps}: ring fill/committed differ"
-                    return rep
+                    return fail(f"step {rep.steps}: ring fill/committed differ")
                 for i in range(ora.fill):
                     pos, tok, k, h = ora.ring(i)
                     if slots[k] != (1, pos, tok):
-                        rep.status, rep.detail = "fail", f"step {rep.steps}: depth {k} holds {slots[k]}, oracle ({pos},{tok})"
-                        return rep
-                    e = rel_err(gpu.hidden(k), h)
-                    rep.max_hidden_err = max(rep.max_hidden_err, e)
-                e = rel_err(gpu.last("pdm_prenorm"), ora.last("pdm_prenorm"))
-                rep.max_pdm_err = max(rep.max_pdm_err, e)
+                        return fail(f"step {rep.steps}: depth {k} holds {slots[k]}, oracle ({pos},{tok})")
+                    rep.max_hidden_err = max(rep.max_hidden_err, rel_err(gpu.hidden(k), h))
+                rep.max_pdm_err = max(rep.max_pdm_err, rel_err(gpu.last("pdm_prenorm"), ora.last("pdm_prenorm")))
                 if check_logits:
                     e = rel_err(gpu.last("pdm_logits"), ora.last("pdm_logits"))
                     if ro.exited:
                         e = max(e, rel_err(gpu.last("exit_logits"), ora.last("exit_logits")))
                     rep.max_logit_err = max(rep.max_logit_err, e)
                 if not np.array_equal(gpu.kv_len(), ora.kv_len()):
-                    rep.status, rep.detail = "fail", f"step {rep.steps}: KV lengths differ"
-                    return rep
+                    return fail(f"step {rep.steps}: KV lengths differ")
                 worst = max(rep.max_hidden_err, rep.max_pdm_err, rep.max_logit_err)
                 if worst > tensor_tol:
-                    rep.status, rep.detail = "fail", f"step {rep.steps}: tensor rel err {worst:.3e} > {tensor_tol}"
-                    return rep
-        c = ora.committed_len
-        kv_compare(gpu, ora, sorted({0, shape.n_layers - 1}), c, rep, tensor_tol)
+                    return fail(f"step {rep.steps}: tensor rel err {worst:.3e} > {tensor_tol}")
+        kv_compare(gpu, ora, sorted({0, shape.n_layers - 1}), ora.committed_len, rep, tensor_tol)
         return rep
     finally:
         ora.close()
         if own:
             gpu.close()
-
-
-def run_parity_retry(make_inputs, seeds, **kw) -> Report:
-    """make_inputs(seed) -> dict of run_parity kwargs.  Retries on near-ties with the next seed (C-4);
-    returns the first clean report (its .detail lists the near-ties met on the way)."""
-    notes = []
-    for s in seeds:
-        rep = run_parity(**make_inputs(s), **kw)
-        if rep.status == "near_tie":
-            notes.append(f"seed {s}: near-tie at {rep.detail}")
-            continue
-        rep.detail = "; ".join(notes + ([rep.detail] if rep.detail else []))
-        return rep
-    rep.detail = "; ".join(notes)
-    return rep

@@ -1,58 +1,64 @@
-"""GPU-vs-oracle parity of the whole SPD path (-m gpu), through the C ABI.
+"""GPU-vs-oracle parity of the whole SPD path (-m gpu), through the C ABI, for both engines
+(0 = one kernel per op, 1 = the fused persistent kernel).
 
-Token ids, accept bits, fills, committed lengths and KV lengths: exact.  Hidden states, PDM vector and
-logits: max relative error (C-2.18) within the north_star contract 2e-2 — and, at the BASELINE init,
-within the much tighter bound the arithmetic allows (fp32 re-association only, ~1e-5).
+Token ids, accept bits, fills, committed lengths and KV lengths: exact (ties within the logit tolerance
+follow tests/_parity.py's protocol and are counted).  Hidden states, PDM vector and logits: max relative
+error (C-2.18) within the north_star contract 2e-2, and within the tighter per-config bound DESIGN.md
+derives from fp32 accumulation (1e-3 tiny, 1e-2 at the 4B/9B-class shapes).
 """
 import numpy as np
 import pytest
 
 import spd_inputs as si
-from tests._parity import run_parity, run_parity_retry, CONTRACT
+from tests._parity import run_parity, CONTRACT
 from tests._util import TINY, shape_of
 
 pytestmark = pytest.mark.gpu
 
 ENGINES = [0, 1]
+_HAS_MEGA = None
 
 
-def _engines_available():
-    return ENGINES
-
-
-def _inputs(shape, prompt_len, std=0.02, random_gains=False, attention_heavy=False):
-    def make(seed):
+def _need_engine(engine):
+    global _HAS_MEGA
+    if engine == 0:
+        return
+    if _HAS_MEGA is None:
         import paper_2605_30852_b200 as spd
-        w = si.make_weights(shape, seed=seed, std=std, random_gains=random_gains, attention_heavy=attention_heavy)
-        return dict(shape=shape, weights_np=w, dev_weights=spd.upload_weights(w),
-                    prompt=si.make_prompt(shape, seed, prompt_len))
-    return make
-
-
-def _skip_if_engine_missing(engine):
-    import paper_2605_30852_b200 as spd
-    if engine == 1:
-        shape = TINY
-        w = spd.upload_weights(si.make_weights(shape))
-        g = spd.SPD(shape, w)
+        g = spd.SPD(TINY, spd.upload_weights(si.make_weights(TINY)))
         try:
             g.set_option(spd.OPT.ENGINE, 1)
+            _HAS_MEGA = True
         except spd.SpdError:
-            pytest.skip("fused engine not built")
+            _HAS_MEGA = False
         finally:
             g.close()
+    assert _HAS_MEGA, "the fused engine must be available on a B200 (spd_create could not set it up)"
+
+
+def _inputs(shape, prompt_len, seed=1234, std=0.02, random_gains=False, attention_heavy=False):
+    import paper_2605_30852_b200 as spd
+    w = si.make_weights(shape, seed=seed, std=std, random_gains=random_gains, attention_heavy=attention_heavy)
+    return dict(shape=shape, weights_np=w, dev_weights=spd.upload_weights(w), prompt=si.make_prompt(shape, seed, prompt_len))
+
+
+def _truth(shape, inp, n, block=16):
+    from oracle import Oracle
+    o = Oracle(shape, inp["weights_np"], max_seq=len(inp["prompt"]) + n + 8)
+    t = [o.prefill(inp["prompt"], block=block)] + [o.ar_step() for _ in range(n)]
+    o.close()
+    return np.array(t, np.int32)
 
 
 @pytest.mark.parametrize("engine", ENGINES)
 def test_tiny_baseline_config_pdm_drafts(engine):
     """BASELINE.json configs[0] exactly: d256 L8 n2, std 0.02, gains 1, prompt 32, 64 greedy tokens,
     the PDM's own drafts."""
-    _skip_if_engine_missing(engine)
-    rep = run_parity_retry(_inputs(TINY, TINY.prompt_len), seeds=[1234, 1235, 1236], n_tokens=TINY.gen_len,
-                           engine=engine, tensor_tol=1e-3)
+    _need_engine(engine)
+    rep = run_parity(**_inputs(TINY, TINY.prompt_len), n_tokens=TINY.gen_len, engine=engine, tensor_tol=1e-3)
+    print("tiny baseline:", rep.summary())
     assert rep.status == "ok", rep.detail
-    assert rep.emitted == TINY.gen_len - 1
-    print("tiny baseline", rep)
+    assert rep.emitted == TINY.gen_len - 1 and rep.verify_ties + rep.pdm_ties == 0
 
 
 @pytest.mark.parametrize("engine", ENGINES)
@@ -60,54 +66,38 @@ def test_tiny_baseline_config_pdm_drafts(engine):
 @pytest.mark.parametrize("p", [0.0, 0.6, 1.0])
 def test_tiny_hot_forced_acceptance(engine, n, p):
     """Diverse tokens (test-only init std 0.08, random gains), every pipeline width, accept/reject mixes."""
-    _skip_if_engine_missing(engine)
-    from tests._util import ar_tokens
+    _need_engine(engine)
     shape = shape_of("tiny", n)
     G = 40
-
-    def make(seed):
-        d = _inputs(shape, 32, std=0.08, random_gains=True)(seed)
-        from oracle import Oracle
-        o = Oracle(shape, d["weights_np"], max_seq=512)
-        truth = [o.prefill(d["prompt"])] + [o.ar_step() for _ in range(G + 8)]
-        o.close()
-        d["forced"] = (np.array(truth, np.int32), p, 7)
-        return d
-    rep = run_parity_retry(make, seeds=[1234, 1235, 1236], n_tokens=G, engine=engine, tensor_tol=CONTRACT)
+    inp = _inputs(shape, 32, std=0.08, random_gains=True)
+    rep = run_parity(**inp, n_tokens=G, forced=(_truth(shape, inp, G + 8), p, 7), engine=engine, tensor_tol=5e-3)
+    print(f"tiny hot n={n} p={p}:", rep.summary())
     assert rep.status == "ok", rep.detail
     if p == 1.0:
         assert rep.rejects == 0 and rep.steps == G + n - 2
     if p == 0.0 and n > 1:
         assert rep.rejects > 0
-    print(f"tiny hot n={n} p={p}", rep.steps, rep.max_hidden_err, rep.max_logit_err, rep.detail)
 
 
 @pytest.mark.parametrize("engine", ENGINES)
 def test_tiny_attention_heavy(engine):
     """W_o, W_v x8 and W_d /8 make attention errors visible in the hidden state (C-4)."""
-    _skip_if_engine_missing(engine)
-    rep = run_parity_retry(_inputs(TINY, 32, std=0.04, attention_heavy=True), seeds=[1234, 1235, 1236],
-                           n_tokens=48, engine=engine, tensor_tol=CONTRACT)
+    _need_engine(engine)
+    rep = run_parity(**_inputs(TINY, 32, std=0.04, attention_heavy=True), n_tokens=48, engine=engine, tensor_tol=5e-3)
+    print("attention heavy:", rep.summary())
     assert rep.status == "ok", rep.detail
-    print("attention heavy", rep.max_hidden_err, rep.max_logit_err)
 
 
 @pytest.mark.parametrize("engine", ENGINES)
 @pytest.mark.parametrize("name,prompt_len,gen", [("4b_n4", 40, 20), ("4b_n8", 24, 14), ("9b_n4", 24, 12), ("9b_n16", 20, 10)])
 def test_full_model_dims_short_prompt(engine, name, prompt_len, gen):
     """The 4B/9B-class shapes of BASELINE.json at every n, with a prompt short enough for the oracle:
-    spans all tile shapes of the big configs (d 2560/4096, F 9728/12288, V 151936)."""
-    _skip_if_engine_missing(engine)
+    spans all tile shapes of the big configs (d 2560/4096, F 9728/12288, V 151936, ragged fills)."""
+    _need_engine(engine)
     shape = si.CONFIGS[name]
-    from oracle import Oracle
-
-    def make(seed):
-        d = _inputs(shape, prompt_len)(seed)
-        o = Oracle(shape, d["weights_np"], max_seq=prompt_len + gen + 8)
-        truth = [o.prefill(d["prompt"], block=16)] + [o.ar_step() for _ in range(gen + 2)]
-        o.close()
-        d["forced"] = (np.array(truth, np.int32), 0.7, 3)
-        return d
-    rep = run_parity_retry(make, seeds=[1234, 1235], n_tokens=gen, engine=engine, tensor_tol=1e-3, tensor_every=3)
+    inp = _inputs(shape, prompt_len)
+    rep = run_parity(**inp, n_tokens=gen, forced=(_truth(shape, inp, gen + 2), 0.7, 3), engine=engine,
+                     tensor_tol=1e-2, tensor_every=3)
+    print(name, rep.summary())
     assert rep.status == "ok", rep.detail
-    print(name, rep.steps, rep.accepts, rep.rejects, rep.max_hidden_err, rep.max_logit_err, rep.min_margin, rep.detail)
+    assert rep.max_hidden_err < CONTRACT and rep.max_logit_err < CONTRACT
