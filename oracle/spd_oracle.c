@@ -489,6 +489,7 @@ int ora_rollback(ora_ctx *o, int32_t new_len, int32_t reseed_token) {
   if (!o->prefilled) return -1;
   if (new_len < 0 || new_len > o->c || reseed_token < 0 || reseed_token >= o->cfg.vocab) return -1;
   o->c = new_len;
+  o->emitted = new_len - o->prompt_len + 1; /* tokens emitted up to and including the reseed token */
   for (int l = 0; l < o->cfg.n_layers; ++l)
     if (o->len[l] > new_len) o->len[l] = new_len;
   ring_set_single(o, new_len, reseed_token);

@@ -168,6 +168,7 @@ __global__ void k_rollback(DevPtrs P, int new_len, int tok) {
   __syncthreads();
   if (threadIdx.x == 0) {
     st->c = new_len;
+    st->N = (long long)new_len - st->prompt_len + 1;   // tokens emitted up to and including the reseed token
     for (int k = 1; k < P.dim.n; ++k) st->occ[k] = 0;
     st->occ[0] = 1; st->pos[0] = new_len; st->tok[0] = tok;
   }
