@@ -103,7 +103,8 @@ typedef struct {
 enum {
   SPD_OPT_ENGINE = 0,      /* 0 = one kernel per operation (reference engine), 1 = persistent fused
                               step kernel (default when available)                               */
-  SPD_OPT_DEBUG_LOGITS = 1 /* 1 = also write full verify/PDM logit vectors (for parity tests)    */
+  SPD_OPT_DEBUG_LOGITS = 1,/* 1 = also write full verify/PDM logit vectors (for parity tests)    */
+  SPD_OPT_PHASE_PROFILE = 2/* 1 = the fused kernel records per-phase clock stamps (SPD_DBG_PHASE_PROFILE) */
 };
 
 /* spd_debug_read selectors.  `index` meaning in brackets. */
@@ -117,7 +118,11 @@ enum {
   SPD_DBG_KV_V = 6,        /* [layer] same for V                                                   */
   SPD_DBG_KV_LEN = 7,      /* int32[L]: valid KV rows per layer (C-2.11)                           */
   SPD_DBG_RING = 8,        /* int32[2 + 3n]: fill a, committed c, then per depth k: occupied, pos, tok */
-  SPD_DBG_HFIN = 9         /* [position] fp32[d]: final hidden state of a committed position        */
+  SPD_DBG_HFIN = 9,        /* [position] fp32[d]: final hidden state of a committed position        */
+  SPD_DBG_PHASE_PROFILE = 10 /* uint64[160][168][6]: per (CTA, phase) clock stamps of the last fused cycle:
+                              0 inputs ready, 1 activations staged, 2 tiles consumed, 3/4 producer issued the
+                              phase's first/last tile (SM clock); 5 = %globaltimer at stamp 0; phase 167 holds
+                              (clock, %globaltimer) at kernel start (needs SPD_OPT_PHASE_PROFILE)            */
 };
 
 /* Buffer sizes for a configuration.  SPD_EINVAL if the configuration is unsupported. */

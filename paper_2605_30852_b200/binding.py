@@ -29,10 +29,11 @@ _STATUS = {0: "SPD_OK", 1: "SPD_EINVAL", 2: "SPD_ESTATE", 3: "SPD_ECAPACITY", 4:
 class OPT:
     ENGINE = 0
     DEBUG_LOGITS = 1
+    PHASE_PROFILE = 2
 
 
 class DBG:
-    SLOT_HIDDEN, EXIT_LOGITS, PDM_LOGITS, PDM_PRENORM, PDM_FEAT, KV_K, KV_V, KV_LEN, RING, HFIN = range(10)
+    SLOT_HIDDEN, EXIT_LOGITS, PDM_LOGITS, PDM_PRENORM, PDM_FEAT, KV_K, KV_V, KV_LEN, RING, HFIN, PHASE_PROFILE = range(11)
 
 
 class _Cfg(C.Structure):
@@ -275,6 +276,10 @@ class SPD:
         if rows == 0:
             return np.zeros((0, w), dtype=np.uint16)
         return self.debug_read(DBG.KV_V if which else DBG.KV_K, layer, np.uint16, rows * w).reshape(rows, w)
+
+    def phase_profile(self) -> np.ndarray:
+        """uint64[160, 168, 6] clock stamps of the last fused cycle (see SPD_DBG_PHASE_PROFILE in spd.h)."""
+        return self.debug_read(DBG.PHASE_PROFILE, 0, np.uint64, 160 * 168 * 6).reshape(160, 168, 6)
 
     def last(self, what: str) -> np.ndarray:
         sel, cnt = {"exit_logits": (DBG.EXIT_LOGITS, self.shape.vocab), "pdm_logits": (DBG.PDM_LOGITS, self.shape.vocab),

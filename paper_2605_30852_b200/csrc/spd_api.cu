@@ -118,6 +118,7 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
   Q.pf_tokens = cv.take<int32_t>(D.max_seq);
   Q.results = cv.take<StepResult>(kResultRing);
   Q.bar = cv.take<unsigned int>(64);
+  Q.prof = cv.take<unsigned long long>((size_t)kProfCtas * kProfPhases * kProfStamps);
   const uint16_t **tabs[9];
   for (int i = 0; i < 9; ++i) tabs[i] = cv.take<const uint16_t *>(D.L);
   Q.attn_norm = tabs[0]; Q.wq = tabs[1]; Q.wk = tabs[2]; Q.wv = tabs[3]; Q.wo = tabs[4];
@@ -388,10 +389,11 @@ extern "C" int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value) {
     if (value == 0 || (value == 1 && ctx->has_mega)) { ctx->engine = value; return SPD_OK; }
     return fail(ctx, SPD_EINVAL, "engine not available%s");
   }
-  if (option == SPD_OPT_DEBUG_LOGITS) {
+  if (option == SPD_OPT_DEBUG_LOGITS || option == SPD_OPT_PHASE_PROFILE) {
     int v = value ? 1 : 0;
-    if (v != ctx->P.debug_logits) {
-      ctx->P.debug_logits = v;   // kernel parameter: captured graphs must be rebuilt
+    int32_t *field = option == SPD_OPT_DEBUG_LOGITS ? &ctx->P.debug_logits : &ctx->P.prof_on;
+    if (v != *field) {
+      *field = v;                // kernel parameter: captured graphs must be rebuilt
       cudaStreamSynchronize(ctx->sm);
       for (int e = 0; e < 2; ++e) {
         if (ctx->graph[e]) cudaGraphExecDestroy(ctx->graph[e]);
@@ -436,6 +438,8 @@ extern "C" int spd_debug_read(spd_ctx *ctx, int32_t what, int32_t index, void *h
     case SPD_DBG_HFIN:
       if (index < 0 || index >= D.max_seq) return fail(ctx, SPD_EINVAL, "debug_read: position out of range%s");
       src = P.hfin + (size_t)index * D.d; want = sizeof(float) * D.d; break;
+    case SPD_DBG_PHASE_PROFILE:
+      src = P.prof; want = sizeof(unsigned long long) * kProfCtas * kProfPhases * kProfStamps; break;
     case SPD_DBG_RING: {
       want = sizeof(int32_t) * (2 + 3 * D.n);
       if (bytes != want) return fail(ctx, SPD_EINVAL, "debug_read: size mismatch%s");

@@ -11,6 +11,8 @@ constexpr int kAttnSplit = 128;     // KV rows per attention split — fixed, so
                                     // depends on n, slot, fill or history (batch invariance)
 constexpr int kResultRing = 1024;   // device ring of step results (spd_step_many batch limit)
 constexpr int kMaxCand = 256;       // per-CTA argmax candidates of the LM-head pass
+// Optional per-phase clock stamps of the fused kernel (SPD_OPT_PHASE_PROFILE): [cta][phase][stamp]
+constexpr int kProfCtas = 160, kProfPhases = 168, kProfStamps = 6;
 
 enum Mode : int32_t { MODE_IDLE = 0, MODE_SPD = 1, MODE_PREFILL = 2, MODE_PREFILL_FINAL = 3 };
 
@@ -79,6 +81,8 @@ struct DevPtrs {
       *const *w_gate, *const *w_up, *const *w_down;   // device arrays of [L] device pointers
   int32_t debug_logits;
   int32_t nsplit_max;
+  unsigned long long *prof;          // [kProfCtas][kProfPhases][kProfStamps] clock stamps (fused engine)
+  int32_t prof_on;
 };
 
 __host__ __device__ inline size_t kv_head_stride(const Dims &d) { return (size_t)d.max_seq * d.hd; }

@@ -88,6 +88,15 @@ __device__ __forceinline__ void tma_load_1d(void *dst_smem, const void *src_gmem
       ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
 }
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ void prof_stamp(const DevPtrs &P, int cta, int phase, int stamp) {
+  if (P.prof_on && cta < kProfCtas && phase < kProfPhases)
+    P.prof[((size_t)cta * kProfPhases + phase) * kProfStamps + stamp] = (unsigned long long)clock64();
+}
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p) {
   unsigned long long v;
   asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
@@ -218,6 +227,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
   const Sched &S = *Sp;
   const unsigned long long launch = ld_acquire_u64(bar_launch);
   if (cta == 0 && tid == 0) controller_begin(P);   // writes only fields no other CTA reads in this kernel
+  if (P.prof_on && tid == 0 && cta < kProfCtas) {
+    unsigned long long *pr = P.prof + ((size_t)cta * kProfPhases + (kProfPhases - 1)) * kProfStamps;
+    pr[0] = (unsigned long long)clock64(); pr[1] = globaltimer_ns();
+  }
   if (S.my_stage >= 0 && tid < D.hd / 2) {         // RoPE table of this CTA's stage (C-2.14)
     double s_, c_;
     sincos((double)S.pos[S.my_stage] * P.inv_freq[tid], &s_, &c_);
@@ -239,6 +252,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
           mbar_wait(&empty[slot], (it & 1) ^ 1);
           mbar_expect_tx(&full[slot], kTileBytes);
           tma_load_1d(ring + (size_t)slot * kTileBytes, src, kTileBytes, &full[slot], policy);
+          if (i == 0) prof_stamp(P, cta, p, 3);
+          if (i == w.ntiles - 1) prof_stamp(P, cta, p, 4);
         }
       }
     }
@@ -261,6 +276,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
         ++bar_idx;
       }
       consumer_sync();   // also: every warp is done with the previous phase's xs
+      if (tid == 0) {
+        prof_stamp(P, cta, p, 0);
+        if (P.prof_on && cta < kProfCtas && p < kProfPhases) P.prof[((size_t)cta * kProfPhases + p) * kProfStamps + 5] = globaltimer_ns();
+      }
       Work w = phase_work(p, np, S, ML, D, cta, ncta);
       const int k = w.job;                    // stage (layer phases) / slot (PDM)
       if (t == PH_ATTN) {
@@ -380,6 +399,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
           else P.len[layer] = pos + 1;
         }
         consumer_sync();
+        if (tid == 0) prof_stamp(P, cta, p, 1);
         // ---- stream the tiles ------------------------------------------------------------------
         const bool two = t == PH_HEAD;
         const float4 *xv4 = reinterpret_cast<const float4 *>(xs);
@@ -481,6 +501,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
       }
       // ---- publish this phase's outputs: arrive at the barrier that the dependent phase waits on ----
       const bool arrive = p >= 1;              // PDM has no barrier of its own (see need_barrier)
+      if (tid == 0) prof_stamp(P, cta, p, 2);
       if (arrive) {
         __threadfence();
         consumer_sync();
