@@ -118,6 +118,7 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
   Q.pf_tokens = cv.take<int32_t>(D.max_seq);
   Q.results = cv.take<StepResult>(kResultRing);
   Q.bar = cv.take<unsigned int>(64);
+  Q.claim = cv.take<unsigned int>((size_t)kProfPhases * kMaxStages);
   Q.prof = cv.take<unsigned long long>((size_t)kProfCtas * kProfPhases * kProfStamps);
   const uint16_t **tabs[9];
   for (int i = 0; i < 9; ++i) tabs[i] = cv.take<const uint16_t *>(D.L);

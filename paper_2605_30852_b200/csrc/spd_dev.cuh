@@ -75,6 +75,7 @@ struct DevPtrs {
   int32_t *pf_tokens;                // [max_seq]
   StepResult *results;               // [kResultRing]
   unsigned int *bar;                 // grid-barrier words (fused engine)
+  unsigned int *claim;               // [kProfPhases][kMaxStages] work-claim counters of one cycle (fused engine)
   uint16_t *kv;                      // K/V cache
   const uint16_t *embed, *final_norm, *pdm_proj, *pdm_norm;
   const uint16_t *const *attn_norm, *const *wq, *const *wk, *const *wv, *const *wo, *const *mlp_norm,

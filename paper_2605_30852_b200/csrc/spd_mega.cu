@@ -2,23 +2,32 @@
 //
 // Shape of the problem: a cycle streams every layer's weights once (12.3 GB at
 // the 9B-class config) through (L/n)*5 + 2 dependent phases; every product is an M=1 GEMV, so the
-// bound is HBM bandwidth and the enemy is the bubble at each phase boundary.  Design:
+// bound is HBM bandwidth and the enemy is the idle time at each phase boundary.  Design:
 //   * grid = one CTA per SM, resident for the whole cycle; 8 consumer warps + 1 producer warp.
-//   * weights are repacked once (spd_create) into 16 KB tiles — 16 rows x 512 columns, stored in the
-//     order a CTA consumes them, so each CTA's share of a phase is ONE contiguous byte range.
-//   * the producer lane streams that range with 1-D TMA bulk copies (cp.async.bulk + mbarrier
-//     complete_tx) into an 11-deep shared-memory ring.  Weight addresses are a static schedule, so
-//     the producer runs AHEAD of the activation dependency, across phase boundaries: while the
-//     consumers wait at a grid barrier the next phase's tiles are already landing.
+//   * weights are repacked once (spd_create) into 16 KB tiles — 16 rows x 512 columns; a "unit" is the
+//     nc tiles of 16 output rows, contiguous in memory.
+//   * the stages (the n in-flight tokens) own disjoint CTA groups (CTA c -> active stage c mod a), so a
+//     CTA keeps one activation vector per phase; inside a group the units of a phase are CLAIMED
+//     dynamically from a per-(phase, stage) counter, so SMs with less bandwidth simply take fewer units
+//     and every CTA reaches the phase barrier at about the same time.
+//   * the producer lane streams the claimed units with 1-D TMA bulk copies (cp.async.bulk + mbarrier
+//     complete_tx) into an 11-deep shared-memory ring, tagging each slot with its unit index and closing
+//     each phase with an END slot.  Unit claims do not depend on activations, so the producer runs
+//     AHEAD of the activation dependency, across phase boundaries: while the consumers wait at a grid
+//     barrier the next phase's tiles are already landing.
 //   * consumers: warp w owns rows 2w, 2w+1 of a tile; 128-bit conflict-free LDS of weights and of
-//     the fp32 activation vector (staged in smem once per phase), fp32 FMA, warp-shuffle reduction at
-//     the end of a 16-row unit, fused epilogues (RoPE + bf16 KV append, residual add, SiLU*mul,
-//     PDM partials, LM-head argmax).
-//   * stages (the n in-flight tokens) own disjoint CTA groups, so a CTA keeps one activation vector.
+//     the fp32 activation vector (staged in smem once per phase with 128-bit L2 loads), fp32 FMA,
+//     warp-shuffle reduction at the end of a unit, fused epilogues (RoPE + bf16 KV append, residual add,
+//     SiLU*mul, PDM partials, LM-head argmax).
+//   * attention: items (stage, kv head, 128-row split) are claimed dynamically by all CTAs; the
+//     producer brings the K and V rows of an item through the same ring (TMA), the 8 consumer warps
+//     compute the G q heads of the kv group together (scores with a transposed butterfly reduction,
+//     softmax per head, P.V with a fixed cross-warp reduction); the last split of a head merges.
 //   * phases are separated by a device-wide arrive/poll barrier on a monotonically increasing
 //     64-bit counter; cross-CTA activations are read with ld.global.cg.
 // Every row's dot product is computed by one warp with a fixed lane/column mapping and chunk order,
-// so a token's result never depends on n, slot, fill or history (batch invariance).
+// attention splits are fixed 128-row blocks merged in split order, so a token's result never depends
+// on n, slot, fill, history or on which CTA happened to claim the work (batch invariance).
 #include <stdio.h>
 #include <string.h>
 
@@ -34,6 +43,7 @@ constexpr int kStages = 11;                              // ring depth
 constexpr int kXFloats = 12288;                          // activation vector capacity (48 KB)
 constexpr int kConsumerThreads = 256;
 constexpr int kThreads = kConsumerThreads + 32;
+constexpr int kEndMark = -1;                             // slot tag: no more work in this phase
 
 enum PhaseType { PH_PDM = 0, PH_QKV = 1, PH_ATTN = 2, PH_O = 3, PH_GATEUP = 4, PH_DOWN = 5, PH_HEAD = 6 };
 
@@ -50,13 +60,18 @@ struct Sched {
   int act[kMaxStages];                          // active stages (depth k), ascending
   int pos[kMaxStages], hbuf[kMaxStages], occ[kMaxStages];
   int my_stage;                                 // this CTA's stage in the layer phases (-1: none)
-  int my_idx, my_gs;                            // index in / size of the stage's CTA group
+  int my_idx;                                   // index inside the stage's CTA group
+  int pdm_slot, pdm_idx;                        // this CTA's slot (column block of W_p) in the PDM phase
+  int attn_total;                               // attention items of one pass
 };
 
-struct Work {                                   // one CTA's share of one phase
-  const uint8_t *base;                          // first tile
-  int ntiles, nc, u0, u1, job;
+struct PhaseDesc {                              // what one phase means for this CTA
+  int type, job, U, nc;                         // job < 0: nothing to stream
+  const uint8_t *base;                          // unit 0 of the job
+  unsigned int *ctr;                            // claim counter
 };
+
+struct AttnItem { int stage, kvh, split, nsplit, t0, rows; };
 
 // ------------------------------------------------------------------ PTX helpers ----------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -87,6 +102,8 @@ __device__ __forceinline__ void tma_load_1d(void *dst_smem, const void *src_gmem
       "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
       ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
 }
+// Orders generic-proxy accesses (st.global of the KV append) against async-proxy accesses (TMA reads).
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;
@@ -103,55 +120,57 @@ __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long
   return v;
 }
 
-// CTA group of `cta` when `jobs` jobs share `ncta` CTAs: group g owns CTAs [g*ncta/jobs, (g+1)*ncta/jobs).
-__device__ __forceinline__ void group_of(int cta, int ncta, int jobs, int &g, int &idx, int &gs) {
-  g = ((cta + 1) * jobs - 1) / ncta;
-  int b0 = g * ncta / jobs, b1 = (g + 1) * ncta / jobs;
-  idx = cta - b0;
-  gs = b1 - b0;
-}
-
 __device__ __forceinline__ int phase_type(int p, int np) {
   if (p == 0) return PH_PDM;
   if (p == np - 1) return PH_HEAD;
   return PH_QKV + (p - 1) % 5;
 }
 
-// This CTA's tiles of phase p.  Pure function of (Sched, layout, cta) — the producer and the consumers
-// both call it and must agree.
-__device__ __forceinline__ Work phase_work(int p, int np, const Sched &S, const MegaLayout &ML, const Dims &D, int cta,
-                                           int ncta) {
-  Work w;
-  w.base = nullptr; w.ntiles = 0; w.nc = 0; w.u0 = 0; w.u1 = 0; w.job = -1;
-  int t = phase_type(p, np);
-  int U = 0, g, idx, gs;
-  if (t == PH_PDM) {
+// Pure function of (Sched, layout, phase) — the producer and the consumers both call it and must agree.
+__device__ __forceinline__ PhaseDesc phase_desc(int p, int np, const Sched &S, const MegaLayout &ML, const Dims &D,
+                                                unsigned int *claim) {
+  PhaseDesc w;
+  w.type = phase_type(p, np);
+  w.job = -1; w.U = 0; w.nc = 0; w.base = nullptr; w.ctr = claim + (size_t)p * kMaxStages;
+  if (w.type == PH_PDM) {
     if (!S.run_pdm) return w;
-    group_of(cta, ncta, D.n, g, idx, gs);
-    w.job = g; U = ML.u_pdm; w.nc = ML.nc_d;
-    w.base = ML.repack + ML.off_pdm + (unsigned long long)g * ML.pdm_job_bytes;
-  } else if (t == PH_HEAD) {
+    w.job = S.pdm_slot; w.U = ML.u_pdm; w.nc = ML.nc_d;
+    w.base = ML.repack + ML.off_pdm + (unsigned long long)w.job * ML.pdm_job_bytes;
+  } else if (w.type == PH_HEAD) {
     if (!S.run_pdm && !S.run_verify) return w;
-    idx = cta; gs = ncta; w.job = 0; U = ML.u_head; w.nc = ML.nc_d;
+    w.job = 0; w.U = ML.u_head; w.nc = ML.nc_d;
     w.base = ML.repack + ML.off_head;
-  } else if (t == PH_ATTN) {
-    return w;
+  } else if (w.type == PH_ATTN) {
+    if (S.n_act > 0) { w.job = 0; w.U = S.attn_total; }
   } else {
     if (S.my_stage < 0) return w;
     int pass = (p - 1) / 5;
     int layer = S.my_stage * D.per + pass;
-    idx = S.my_idx; gs = S.my_gs; w.job = S.my_stage;
+    w.job = S.my_stage;
     const uint8_t *lb = ML.repack + (unsigned long long)layer * ML.layer_bytes;
-    if (t == PH_QKV) { U = ML.u_qkv; w.nc = ML.nc_d; w.base = lb; }
-    else if (t == PH_O) { U = ML.u_o; w.nc = ML.nc_qd; w.base = lb + ML.off_o; }
-    else if (t == PH_GATEUP) { U = ML.u_gu; w.nc = ML.nc_d; w.base = lb + ML.off_gu; }
-    else { U = ML.u_dn; w.nc = ML.nc_f; w.base = lb + ML.off_dn; }
+    if (w.type == PH_QKV) { w.U = ML.u_qkv; w.nc = ML.nc_d; w.base = lb; }
+    else if (w.type == PH_O) { w.U = ML.u_o; w.nc = ML.nc_qd; w.base = lb + ML.off_o; }
+    else if (w.type == PH_GATEUP) { w.U = ML.u_gu; w.nc = ML.nc_d; w.base = lb + ML.off_gu; }
+    else { w.U = ML.u_dn; w.nc = ML.nc_f; w.base = lb + ML.off_dn; }
   }
-  w.u0 = (int)((long long)idx * U / gs);
-  w.u1 = (int)((long long)(idx + 1) * U / gs);
-  w.ntiles = (w.u1 - w.u0) * w.nc;
-  w.base += (unsigned long long)w.u0 * w.nc * kTileBytes;
+  if (w.job >= 0) w.ctr += w.job;
   return w;
+}
+
+// Attention item -> (stage, kv head, split).  Items are ordered stage-major, then kv head, then split.
+__device__ __forceinline__ void attn_decode(const Sched &S, const Dims &D, int item, AttnItem &it) {
+  int rem = item;
+  it.stage = -1; it.nsplit = 0;
+  for (int a = 0; a < S.n_act; ++a) {
+    int ns = (S.pos[S.act[a]] + kAttnSplit) / kAttnSplit;     // ceil((pos + 1) / split)
+    if (rem < D.Hkv * ns) { it.stage = S.act[a]; it.nsplit = ns; break; }
+    rem -= D.Hkv * ns;
+  }
+  it.kvh = rem / it.nsplit;
+  it.split = rem - it.kvh * it.nsplit;
+  it.t0 = it.split * kAttnSplit;
+  int T = S.pos[it.stage] + 1;
+  it.rows = min(T - it.t0, kAttnSplit);
 }
 
 // ------------------------------------------------------------------ consumer pieces ------------
@@ -164,19 +183,302 @@ __device__ __forceinline__ float fma8(uint4 w, float4 xa, float4 xb, float acc) 
   return acc;
 }
 
-// RMS scale over the 256 consumer threads (fixed tree: strided per-thread sums, xor-tree, 8 warp
-// partials added in order).  src is read with ld.global.cg (it was written by other CTAs).
-__device__ __forceinline__ float consumer_rms_scale(const float *src, int d, float eps, float *red) {
-  float ss = 0.f;
-  for (int i = threadIdx.x; i < d; i += kConsumerThreads) { float v = __ldcg(src + i); ss = fmaf(v, v, ss); }
-  ss = warp_sum(ss);
-  consumer_sync();
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+// Sum over the 256 consumer threads with a fixed tree: warp xor-tree, then the 8 warp partials in order.
+__device__ __forceinline__ float consumer_sum(float v, float *red) {
+  v = warp_sum(v);
+  consumer_sync();                      // protect `red` against a previous use
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
   consumer_sync();
   float t = 0.f;
 #pragma unroll
   for (int w = 0; w < 8; ++w) t += red[w];
-  return 1.0f / sqrtf(t / (float)d + eps);
+  return t;
+}
+
+// Copies K fp32 values (K % 4 == 0) written by other CTAs (ld.global.cg, 128-bit) into shared memory;
+// returns this thread's sum of squares.  Thread t owns float4 t, t + 256, ...
+__device__ __forceinline__ float stage_copy(const float *src, float *dst, int K) {
+  const float4 *s4 = reinterpret_cast<const float4 *>(src);
+  float4 *d4 = reinterpret_cast<float4 *>(dst);
+  const int n4 = K >> 2;
+  float ss = 0.f;
+#pragma unroll 4
+  for (int i = threadIdx.x; i < n4; i += kConsumerThreads) {
+    float4 v = __ldcg(s4 + i);
+    d4[i] = v;
+    ss = fmaf(v.x, v.x, ss); ss = fmaf(v.y, v.y, ss); ss = fmaf(v.z, v.z, ss); ss = fmaf(v.w, v.w, ss);
+  }
+  return ss;
+}
+
+// xs[i] *= r * gain[i] for the float4s this thread wrote in stage_copy.
+__device__ __forceinline__ void stage_scale(float *xs, const uint16_t *gain, int K, float r) {
+  float4 *d4 = reinterpret_cast<float4 *>(xs);
+  const uint2 *g2 = reinterpret_cast<const uint2 *>(gain);
+  const int n4 = K >> 2;
+  for (int i = threadIdx.x; i < n4; i += kConsumerThreads) {
+    float4 v = d4[i];
+    uint2 g = __ldg(g2 + i);
+    v.x = v.x * r * bf16_lo(g.x); v.y = v.y * r * bf16_hi(g.x);
+    v.z = v.z * r * bf16_lo(g.y); v.w = v.w * r * bf16_hi(g.y);
+    d4[i] = v;
+  }
+}
+
+// Transposed butterfly reduction.  Every lane holds N partial sums v[0..N); the lanes that differ in the
+// bits below 2*OFF hold partials of the same N quantities.  Each level halves the values a lane keeps
+// (lane bit set: the upper half) and adds the partner's partials of the kept half; when one value is
+// left the remaining levels are plain xor-sums.  Afterwards v[0..max(N/W,1)) are complete sums of the
+// quantities base * max(N/W,1) + i, where `base` collects the lane bits of the halving levels (first
+// level = most significant).  N - 1 shuffles instead of N * log2(W).
+template <int N, int OFF>
+struct XReduce {
+  static __device__ __forceinline__ void run(float *v, int lane, int &base) {
+    if constexpr (OFF >= 1) {
+      if constexpr (N > 1) {
+        constexpr int H = N / 2;
+        const bool up = (lane & OFF) != 0;
+#pragma unroll
+        for (int i = 0; i < H; ++i) {
+          float send = up ? v[i] : v[i + H];
+          float keep = up ? v[i + H] : v[i];
+          v[i] = keep + __shfl_xor_sync(0xffffffffu, send, OFF);
+        }
+        base = base * 2 + (up ? 1 : 0);
+        XReduce<H, OFF / 2>::run(v, lane, base);
+      } else {
+        v[0] += __shfl_xor_sync(0xffffffffu, v[0], OFF);
+        XReduce<1, OFF / 2>::run(v, lane, base);
+      }
+    }
+  }
+};
+
+// One attention item: the G q heads of kv head `kvh` of the token at stage `stage`, over K/V rows
+// [t0, t0 + rows) that the producer placed in ring slots seq0.. (K: nk slots, then V: nk slots).
+// Writes the unnormalised partial output and (max, sum) of every head; the caller merges.
+// scratch (the activation buffer, free during attention): sc[G][128] scores, ps[128][G] probabilities,
+// red[8][G][HD] per-warp partial outputs.
+template <int HD, int G>
+__device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, const uint8_t *ring, uint32_t seq0, int nk,
+                                          float *scratch) {
+  constexpr int CH = HD / 8;            // 16-byte chunks (= lanes) per K row
+  constexpr int RPI = 32 / CH;          // rows covered by one warp-wide LDS.128
+  constexpr int NI = 16 / RPI;          // iterations for a warp's 16 rows
+  constexpr int NV = NI * G;            // partial scores per lane
+  constexpr int NF = NV >= CH ? NV / CH : 1;
+  constexpr int RPS = kTileBytes / (HD * 2);   // rows per ring slot
+  constexpr int EPL = HD / 32;          // head-dim elements per lane in P.V
+  const Dims &D = P.dim;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  float *sc = scratch, *ps = scratch + G * kAttnSplit, *red = scratch + 2 * G * kAttnSplit;
+  const int hq0 = it.kvh * G;
+  const int rows = it.rows;
+
+  // ---- scores: lane (rsel, c) owns chunk c of rows 16*warp + i*RPI + rsel ----
+  {
+    const int c = lane % CH, rsel = lane / CH;
+    float qv[G][8];
+#pragma unroll
+    for (int h = 0; h < G; ++h) {
+      const float4 *q4 = reinterpret_cast<const float4 *>(P.q + ((size_t)it.stage * D.Hq + hq0 + h) * HD + c * 8);
+      float4 a = __ldcg(q4), b = __ldcg(q4 + 1);
+      qv[h][0] = a.x; qv[h][1] = a.y; qv[h][2] = a.z; qv[h][3] = a.w;
+      qv[h][4] = b.x; qv[h][5] = b.y; qv[h][6] = b.z; qv[h][7] = b.w;
+    }
+    float v[NV];
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+      const int row = 16 * warp + i * RPI + rsel;
+      uint4 kw = make_uint4(0u, 0u, 0u, 0u);
+      if (row < rows) {
+        const uint8_t *tile = ring + (size_t)((seq0 + row / RPS) % kStages) * kTileBytes;
+        kw = *reinterpret_cast<const uint4 *>(tile + (size_t)(row % RPS) * (HD * 2) + c * 16);
+      }
+      const float k0 = bf16_lo(kw.x), k1 = bf16_hi(kw.x), k2 = bf16_lo(kw.y), k3 = bf16_hi(kw.y);
+      const float k4 = bf16_lo(kw.z), k5 = bf16_hi(kw.z), k6 = bf16_lo(kw.w), k7 = bf16_hi(kw.w);
+#pragma unroll
+      for (int h = 0; h < G; ++h) {
+        float a = k0 * qv[h][0];
+        a = fmaf(k1, qv[h][1], a); a = fmaf(k2, qv[h][2], a); a = fmaf(k3, qv[h][3], a);
+        a = fmaf(k4, qv[h][4], a); a = fmaf(k5, qv[h][5], a); a = fmaf(k6, qv[h][6], a); a = fmaf(k7, qv[h][7], a);
+        v[i * G + h] = a;
+      }
+    }
+    int base = 0;
+    XReduce<NV, CH / 2>::run(v, lane, base);
+    const float scale = 1.0f / sqrtf((float)HD);
+#pragma unroll
+    for (int i = 0; i < NF; ++i) {
+      const int idx = base * NF + i, itn = idx / G, h = idx % G;
+      sc[h * kAttnSplit + 16 * warp + itn * RPI + rsel] = v[i] * scale;
+    }
+  }
+  consumer_sync();
+  // ---- softmax of the split, one warp per head: m = max, p = exp(s - m), l = sum p ----
+  if (warp < G) {
+    float s[kAttnSplit / 32], m = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < kAttnSplit / 32; ++j) {
+      int r = lane + 32 * j;
+      s[j] = r < rows ? sc[warp * kAttnSplit + r] : -INFINITY;
+      m = fmaxf(m, s[j]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    float l = 0.f;
+#pragma unroll
+    for (int j = 0; j < kAttnSplit / 32; ++j) {
+      int r = lane + 32 * j;
+      float p = r < rows ? expf(s[j] - m) : 0.f;
+      ps[r * G + warp] = p;
+      l += p;
+    }
+    l = warp_sum(l);
+    if (lane == 0) {
+      size_t slot = ((size_t)it.stage * D.Hq + hq0 + warp) * P.nsplit_max + it.split;
+      P.part_ml[slot] = make_float2(m, l);
+    }
+  }
+  consumer_sync();
+  // ---- P.V: warp w sums its 16 rows for all G heads; lane owns EPL consecutive head-dim elements ----
+  {
+    float acc[G][EPL];
+#pragma unroll
+    for (int h = 0; h < G; ++h)
+#pragma unroll
+      for (int e = 0; e < EPL; ++e) acc[h][e] = 0.f;
+    const int r_end = min(rows, 16 * warp + 16);
+    for (int row = 16 * warp; row < r_end; ++row) {
+      const uint8_t *tile = ring + (size_t)((seq0 + nk + row / RPS) % kStages) * kTileBytes;
+      const uint8_t *vr = tile + (size_t)(row % RPS) * (HD * 2) + lane * (EPL * 2);
+      float vv[EPL];
+      if constexpr (EPL == 4) {
+        uint2 w = *reinterpret_cast<const uint2 *>(vr);
+        vv[0] = bf16_lo(w.x); vv[1] = bf16_hi(w.x); vv[2] = bf16_lo(w.y); vv[3] = bf16_hi(w.y);
+      } else {
+        uint32_t w = *reinterpret_cast<const uint32_t *>(vr);
+        vv[0] = bf16_lo(w); vv[1] = bf16_hi(w);
+      }
+      float pr[G];
+      if constexpr (G == 4) {
+        float4 t = *reinterpret_cast<const float4 *>(ps + row * G);
+        pr[0] = t.x; pr[1] = t.y; pr[2] = t.z; pr[3] = t.w;
+      } else if constexpr (G == 8) {
+        float4 t = *reinterpret_cast<const float4 *>(ps + row * G), u = *reinterpret_cast<const float4 *>(ps + row * G + 4);
+        pr[0] = t.x; pr[1] = t.y; pr[2] = t.z; pr[3] = t.w; pr[4] = u.x; pr[5] = u.y; pr[6] = u.z; pr[7] = u.w;
+      } else {
+#pragma unroll
+        for (int h = 0; h < G; ++h) pr[h] = ps[row * G + h];
+      }
+#pragma unroll
+      for (int h = 0; h < G; ++h)
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) acc[h][e] = fmaf(pr[h], vv[e], acc[h][e]);
+    }
+#pragma unroll
+    for (int h = 0; h < G; ++h)
+#pragma unroll
+      for (int e = 0; e < EPL; ++e) red[((size_t)warp * G + h) * HD + lane * EPL + e] = acc[h][e];
+  }
+  consumer_sync();
+  // ---- cross-warp sum in warp order (fixed), unnormalised partial output of the split ----
+  for (int o = tid; o < G * HD; o += kConsumerThreads) {
+    const int h = o / HD, e = o - h * HD;
+    float t = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) t += red[((size_t)w * G + h) * HD + e];
+    size_t slot = ((size_t)it.stage * D.Hq + hq0 + h) * P.nsplit_max + it.split;
+    P.part_o[slot * HD + e] = t;
+  }
+}
+
+// Merge of the splits of one q head by one warp, in split order (fixed): out = sum_j o_j e^(m_j-M) / sum_j l_j e^(m_j-M).
+__device__ __forceinline__ void attn_merge_warp(const DevPtrs &P, int stage, int hq, int nsplit, int lane) {
+  const Dims &D = P.dim;
+  size_t slot = ((size_t)stage * D.Hq + hq) * P.nsplit_max;
+  const float2 *ml = P.part_ml + slot;
+  float M = -INFINITY;
+  for (int j = 0; j < nsplit; ++j) M = fmaxf(M, __ldcg(&ml[j].x));
+  const int epl = D.hd / 32;
+  for (int e = lane * epl; e < (lane + 1) * epl; ++e) {
+    float L = 0.f, o = 0.f;
+    for (int j = 0; j < nsplit; ++j) {
+      float2 mlj = __ldcg(&ml[j]);
+      float wj = expf(mlj.x - M);
+      L = fmaf(mlj.y, wj, L);
+      o = fmaf(__ldcg(P.part_o + (slot + j) * D.hd + e), wj, o);
+    }
+    P.att[((size_t)stage * D.Hq + hq) * D.hd + e] = o / L;
+  }
+}
+
+// Fused epilogue of one 16-row unit (lane 0 of every warp; rows r0, r0 + 1 of the repacked matrix).
+__device__ __forceinline__ void unit_epilogue(const DevPtrs &P, const Sched &S, int t, int k, int pass, int r0, float y0,
+                                              float y1, float z0, float z1, const float2 *rope_s, float *hbest_v,
+                                              int *hbest_i) {
+  const Dims &D = P.dim;
+  if (t == PH_QKV) {
+    const int qd = D.Hq * D.hd, kd = D.Hkv * D.hd, half = D.hd / 2, pos = S.pos[k];
+    const int layer = k * D.per + pass;
+    if (r0 < qd) {                           // q pair (i, i + hd/2) of head hh: RoPE (C-2.14)
+      int hh = r0 / D.hd, i = (r0 - hh * D.hd) >> 1;
+      float2 cs = rope_s[i];
+      float *q = P.q + (size_t)k * qd + hh * D.hd;
+      q[i] = y0 * cs.x - y1 * cs.y;
+      q[i + half] = y1 * cs.x + y0 * cs.y;
+    } else if (r0 < qd + kd) {               // k pair: RoPE, bf16 (RNE), append at row pos
+      int rr = r0 - qd, hh = rr / D.hd, i = (rr - hh * D.hd) >> 1;
+      float2 cs = rope_s[i];
+      if (pos < D.max_seq) {
+        uint16_t *dst = P.kv + kv_offset(D, layer, 0, hh) + (size_t)pos * D.hd;
+        dst[i] = f32_to_bf16(y0 * cs.x - y1 * cs.y);
+        dst[i + half] = f32_to_bf16(y1 * cs.x + y0 * cs.y);
+      }
+    } else if (r0 < qd + 2 * kd) {           // two consecutive v elements: bf16, append
+      int rr = r0 - qd - kd, hh = rr / D.hd, i = rr - hh * D.hd;
+      if (pos < D.max_seq) {
+        uint16_t *dst = P.kv + kv_offset(D, layer, 1, hh) + (size_t)pos * D.hd;
+        *reinterpret_cast<uint32_t *>(dst + i) = (uint32_t)f32_to_bf16(y0) | ((uint32_t)f32_to_bf16(y1) << 16);
+      }
+    }
+  } else if (t == PH_O || t == PH_DOWN) {    // residual add
+    float *h = P.h + (size_t)S.hbuf[k] * D.d;
+    if (r0 + 1 < D.d) {
+      float2 v = __ldcg(reinterpret_cast<const float2 *>(h + r0));
+      *reinterpret_cast<float2 *>(h + r0) = make_float2(v.x + y0, v.y + y1);
+    } else if (r0 < D.d) {
+      h[r0] = __ldcg(h + r0) + y0;
+    }
+  } else if (t == PH_GATEUP) {               // rows (gate_i, up_i): SwiGLU
+    int i = r0 >> 1;
+    if (i < D.F) P.act[(size_t)k * D.F + i] = silu_mul(y0, y1);
+  } else if (t == PH_PDM) {
+    if (r0 < D.d) P.pdm_part[(size_t)k * D.d + r0] = y0;
+    if (r0 + 1 < D.d) P.pdm_part[(size_t)k * D.d + r0 + 1] = y1;
+  } else {                                   // PH_HEAD: running (value, index) argmax
+    if (S.run_verify) {
+      if (r0 < D.V && cand_better(y0, r0, hbest_v[0], hbest_i[0])) { hbest_v[0] = y0; hbest_i[0] = r0; }
+      if (r0 + 1 < D.V && cand_better(y1, r0 + 1, hbest_v[0], hbest_i[0])) { hbest_v[0] = y1; hbest_i[0] = r0 + 1; }
+    }
+    if (S.run_pdm) {
+      if (r0 < D.V && cand_better(z0, r0, hbest_v[1], hbest_i[1])) { hbest_v[1] = z0; hbest_i[1] = r0; }
+      if (r0 + 1 < D.V && cand_better(z1, r0 + 1, hbest_v[1], hbest_i[1])) { hbest_v[1] = z1; hbest_i[1] = r0 + 1; }
+    }
+    if (P.debug_logits) {
+      if (S.run_verify) { if (r0 < D.V) P.logits_v[r0] = y0; if (r0 + 1 < D.V) P.logits_v[r0 + 1] = y1; }
+      if (S.run_pdm) { if (r0 < D.V) P.logits_p[r0] = z0; if (r0 + 1 < D.V) P.logits_p[r0 + 1] = z1; }
+    }
+  }
+}
+
+template <int HD>
+__device__ __forceinline__ void attn_item_g(const DevPtrs &P, const AttnItem &it, const uint8_t *ring, uint32_t seq0, int nk,
+                                            float *scratch, int G) {
+  if (G == 4) attn_item<HD, 4>(P, it, ring, seq0, nk, scratch);
+  else if (G == 2) attn_item<HD, 2>(P, it, ring, seq0, nk, scratch);
+  else if (G == 8) attn_item<HD, 8>(P, it, ring, seq0, nk, scratch);
+  else attn_item<HD, 1>(P, it, ring, seq0, nk, scratch);
 }
 
 // The fused kernel ---------------------------------------------------------------------------------
@@ -190,7 +492,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
   float *red = reinterpret_cast<float *>(rope_s + 64);                   // [16]
   float *cbest_v = red + 16;                                             // [2][8]
   int *cbest_i = reinterpret_cast<int *>(cbest_v + 16);                  // [2][8]
-  Sched *Sp = reinterpret_cast<Sched *>(cbest_i + 16);
+  int *meta = cbest_i + 16;                                              // [kStages] slot tags (+ padding to 16)
+  Sched *Sp = reinterpret_cast<Sched *>(meta + 16);
 
   const Dims &D = P.dim;
   const int cta = blockIdx.x, ncta = gridDim.x;
@@ -205,21 +508,21 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
     const StepState *st = P.st;
     Sched &S = *Sp;
     S.mode = st->mode; S.c = st->c;
-    int a = 0;
+    int a = 0, items = 0;
     for (int k = 0; k < D.n; ++k) {
       S.occ[k] = st->occ[k]; S.pos[k] = st->pos[k]; S.hbuf[k] = st->hbuf[k];
-      if (st->occ[k]) S.act[a++] = k;
+      if (st->occ[k]) { S.act[a++] = k; items += D.Hkv * ((st->pos[k] + kAttnSplit) / kAttnSplit); }
     }
     S.n_act = a;
+    S.attn_total = items;
     S.p_new = st->occ[0] ? st->pos[0] : -1;
     S.run_pdm = st->mode == MODE_SPD;
     S.run_verify = (st->mode == MODE_SPD && st->occ[D.n - 1]) || st->mode == MODE_PREFILL_FINAL;
-    S.my_stage = -1; S.my_idx = 0; S.my_gs = 1;
-    if (a > 0) {
-      int g;
-      group_of(cta, ncta, a, g, S.my_idx, S.my_gs);
-      S.my_stage = S.act[g];
-    }
+    // CTA c serves active stage c mod a (every group gets the same mix of SMs); PDM slot c mod n
+    S.my_stage = a > 0 ? S.act[cta % a] : -1;
+    S.my_idx = a > 0 ? cta / a : 0;
+    S.pdm_slot = cta % D.n;
+    S.pdm_idx = cta / D.n;
     for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -237,24 +540,71 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
     rope_s[tid] = make_float2((float)c_, (float)s_);
   }
   __syncthreads();
+  const int RPS = kTileBytes / (D.hd * 2);         // K/V rows per ring slot
 
   if (warp == 8) {
-    // =========================== producer: stream every phase's tiles, running ahead ===========
+    // =========================== producer: claim and stream every phase's work, running ahead =====
     if (lane == 0) {
-      uint64_t policy;
-      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      uint64_t pol_w, pol_kv;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_w));
+      asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol_kv));
       uint32_t seq = 0;
       for (int p = 0; p < np; ++p) {
-        Work w = phase_work(p, np, S, ML, D, cta, ncta);
-        const uint8_t *src = w.base;
-        for (int i = 0; i < w.ntiles; ++i, ++seq, src += kTileBytes) {
-          uint32_t slot = seq % kStages, it = seq / kStages;
-          mbar_wait(&empty[slot], (it & 1) ^ 1);
-          mbar_expect_tx(&full[slot], kTileBytes);
-          tma_load_1d(ring + (size_t)slot * kTileBytes, src, kTileBytes, &full[slot], policy);
-          if (i == 0) prof_stamp(P, cta, p, 3);
-          if (i == w.ntiles - 1) prof_stamp(P, cta, p, 4);
+        PhaseDesc w = phase_desc(p, np, S, ML, D, P.claim);
+        if (w.job >= 0) {
+          unsigned int next = atomicAdd(w.ctr, 1u);
+          if (w.type == PH_ATTN) {
+            // K/V rows of this pass were appended by other CTAs in the QKV phase: wait for its barrier
+            unsigned long long target = (launch * nbar + (unsigned long long)(p - 2) + 1) * (unsigned long long)ncta;
+            while (ld_acquire_u64(bar_count) < target) {}
+            fence_proxy_async();
+            const int pass = (p - 1) / 5;
+            bool first = true;
+            while (next < (unsigned int)w.U) {
+              AttnItem it;
+              attn_decode(S, D, (int)next, it);
+              const int item = (int)next;
+              next = atomicAdd(w.ctr, 1u);
+              const int layer = it.stage * D.per + pass;
+              const int nk = (it.rows + RPS - 1) / RPS;
+              for (int kvsel = 0; kvsel < 2; ++kvsel) {
+                const uint16_t *src = P.kv + kv_offset(D, layer, kvsel, it.kvh) + (size_t)it.t0 * D.hd;
+                for (int j = 0; j < nk; ++j, ++seq) {
+                  uint32_t slot = seq % kStages, itn = seq / kStages;
+                  int r = min(RPS, it.rows - j * RPS);
+                  uint32_t bytes = (uint32_t)r * D.hd * 2;
+                  mbar_wait(&empty[slot], (itn & 1) ^ 1);
+                  meta[slot] = item;
+                  mbar_expect_tx(&full[slot], bytes);
+                  tma_load_1d(ring + (size_t)slot * kTileBytes, src + (size_t)j * RPS * D.hd, bytes, &full[slot], pol_kv);
+                  if (first) { prof_stamp(P, cta, p, 3); first = false; }
+                }
+              }
+            }
+          } else {
+            bool first = true;
+            while (next < (unsigned int)w.U) {
+              const int u = (int)next;
+              next = atomicAdd(w.ctr, 1u);         // claim ahead: its latency hides behind this unit's tiles
+              const uint8_t *src = w.base + (unsigned long long)u * w.nc * kTileBytes;
+              for (int i = 0; i < w.nc; ++i, ++seq, src += kTileBytes) {
+                uint32_t slot = seq % kStages, itn = seq / kStages;
+                mbar_wait(&empty[slot], (itn & 1) ^ 1);
+                meta[slot] = u;
+                mbar_expect_tx(&full[slot], kTileBytes);
+                tma_load_1d(ring + (size_t)slot * kTileBytes, src, kTileBytes, &full[slot], pol_w);
+                if (first) { prof_stamp(P, cta, p, 3); first = false; }
+              }
+            }
+          }
+          prof_stamp(P, cta, p, 4);
         }
+        // END slot: closes the phase for the consumers
+        uint32_t slot = seq % kStages, itn = seq / kStages;
+        mbar_wait(&empty[slot], (itn & 1) ^ 1);
+        meta[slot] = kEndMark;
+        mbar_arrive(&full[slot]);
+        ++seq;
       }
     }
   } else {
@@ -263,8 +613,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
     unsigned long long bar_idx = 0;          // barriers passed in this cycle
     float hbest_v[2] = {-INFINITY, -INFINITY};
     int hbest_i[2] = {0x7fffffff, 0x7fffffff};
+    const int G = D.Hq / D.Hkv;
     for (int p = 0; p < np; ++p) {
-      const int t = phase_type(p, np);
       const int pass = (p - 1) / 5;
       // ---- wait for the producers of this phase's inputs (all phases but PDM and the first QKV) ----
       const bool need_barrier = !(p == 0 || p == 1);
@@ -280,112 +630,98 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
         prof_stamp(P, cta, p, 0);
         if (P.prof_on && cta < kProfCtas && p < kProfPhases) P.prof[((size_t)cta * kProfPhases + p) * kProfStamps + 5] = globaltimer_ns();
       }
-      Work w = phase_work(p, np, S, ML, D, cta, ncta);
+      PhaseDesc w = phase_desc(p, np, S, ML, D, P.claim);
+      const int t = w.type;
       const int k = w.job;                    // stage (layer phases) / slot (PDM)
       if (t == PH_ATTN) {
-        // ---- split-KV decode attention: items (stage, kv head, 128-row split) round-robin over CTAs;
-        //      warps [g*G, (g+1)*G) take one item, one q head per warp; the last warp to finish a
-        //      q head merges its splits in split order.
-        const int G = D.Hq / D.Hkv, spc = 8 / G;
-        const int slot_in_cta = warp / G, hq_in_group = warp % G;
-        int total = 0;
-        for (int a = 0; a < S.n_act; ++a) total += D.Hkv * ((S.pos[S.act[a]] + kAttnSplit) / kAttnSplit);
-        if (slot_in_cta < spc) {
-          for (int item = cta * spc + slot_in_cta; item < total; item += ncta * spc) {
-            int rem = item, stage = -1, nsplit = 0;
-            for (int a = 0; a < S.n_act; ++a) {
-              int ns = (S.pos[S.act[a]] + kAttnSplit) / kAttnSplit;
-              if (rem < D.Hkv * ns) { stage = S.act[a]; nsplit = ns; break; }
-              rem -= D.Hkv * ns;
-            }
-            int kvh = rem / nsplit, split = rem - kvh * nsplit;
-            int T = S.pos[stage] + 1, t0 = split * kAttnSplit, t1 = min(T, t0 + kAttnSplit);
-            int layer = stage * D.per + pass, hq = kvh * G + hq_in_group;
-            const uint16_t *kc = P.kv + kv_offset(D, layer, 0, kvh), *vc = P.kv + kv_offset(D, layer, 1, kvh);
-            size_t slot = ((size_t)stage * D.Hq + hq) * P.nsplit_max;
-            const float *qh = P.q + ((size_t)stage * D.Hq + hq) * D.hd;
-            if (D.hd == 128) attn_partial_warp<128>(qh, kc, vc, t0, t1, P.part_o + (slot + split) * 128, P.part_ml + slot + split);
-            else attn_partial_warp<64>(qh, kc, vc, t0, t1, P.part_o + (slot + split) * 64, P.part_ml + slot + split);
-            __threadfence();
+        if (tid == 0) prof_stamp(P, cta, p, 1);
+        // ---- split-KV decode attention: items claimed by the producer arrive through the ring ----
+        while (true) {
+          uint32_t slot = seq % kStages, itn = seq / kStages;
+          mbar_wait(&full[slot], itn & 1);
+          const int item = meta[slot];
+          if (item == kEndMark) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[slot]);
+            ++seq;
+            break;
+          }
+          AttnItem it;
+          attn_decode(S, D, item, it);
+          const int nk = (it.rows + RPS - 1) / RPS;
+          for (int j = 1; j < 2 * nk; ++j) mbar_wait(&full[(seq + j) % kStages], ((seq + j) / kStages) & 1);
+          if (D.hd == 128) attn_item_g<128>(P, it, ring, seq, nk, xs, G);
+          else attn_item_g<64>(P, it, ring, seq, nk, xs, G);
+          __syncwarp();
+          if (lane == 0) for (int j = 0; j < 2 * nk; ++j) mbar_arrive(&empty[(seq + j) % kStages]);
+          seq += 2 * nk;
+          // the last split of a q head to finish merges them (fixed split order)
+          __threadfence();
+          consumer_sync();
+          if (warp < G) {
+            const int hq = it.kvh * G + warp;
             int old = 0;
-            if (lane == 0) old = atomicAdd(&P.att_cnt[stage * D.Hq + hq], 1);
+            if (lane == 0) old = atomicAdd(&P.att_cnt[it.stage * D.Hq + hq], 1);
             old = __shfl_sync(0xffffffffu, old, 0);
-            if (old == nsplit - 1) {           // last split of this q head: merge (fixed split order)
+            if (old == it.nsplit - 1) {
               __threadfence();
-              const float2 *ml = P.part_ml + slot;
-              float M = -INFINITY;
-              for (int j = 0; j < nsplit; ++j) M = fmaxf(M, __ldcg(&ml[j].x));
-              const int epl = D.hd / 32;
-              for (int e = lane * epl; e < (lane + 1) * epl; ++e) {
-                float L = 0.f, o = 0.f;
-                for (int j = 0; j < nsplit; ++j) {
-                  float2 mlj = __ldcg(&ml[j]);
-                  float wj = expf(mlj.x - M);
-                  L = fmaf(mlj.y, wj, L);
-                  o = fmaf(__ldcg(P.part_o + (slot + j) * D.hd + e), wj, o);
-                }
-                P.att[((size_t)stage * D.Hq + hq) * D.hd + e] = o / L;
-              }
-              if (lane == 0) P.att_cnt[stage * D.Hq + hq] = 0;
+              attn_merge_warp(P, it.stage, hq, it.nsplit, lane);
+              if (lane == 0) P.att_cnt[it.stage * D.Hq + hq] = 0;
             }
           }
         }
-      } else if (w.ntiles > 0 || t == PH_QKV) {
+      } else {
         // ---- stage the activation vector(s) of this phase in shared memory ----------------------
-        int K = 0;
-        if (w.ntiles > 0) {
+        if (k >= 0) {
+          int K = 0;
           if (t == PH_QKV || t == PH_GATEUP) {
             int layer = k * D.per + pass;
             const float *h = P.h + (size_t)S.hbuf[k] * D.d;
             const uint16_t *g = t == PH_QKV ? P.attn_norm[layer] : P.mlp_norm[layer];
-            float r = consumer_rms_scale(h, D.d, D.eps, red);
-            for (int i = tid; i < D.d; i += kConsumerThreads) xs[i] = __ldcg(h + i) * r * bf16_to_f32(g[i]);
+            float ss = consumer_sum(stage_copy(h, xs, D.d), red);
+            stage_scale(xs, g, D.d, 1.0f / sqrtf(ss / (float)D.d + D.eps));
             K = D.d;
           } else if (t == PH_O) {
             K = D.Hq * D.hd;
-            const float *src = P.att + (size_t)k * K;
-            for (int i = tid; i < K; i += kConsumerThreads) xs[i] = __ldcg(src + i);
+            stage_copy(P.att + (size_t)k * K, xs, K);
           } else if (t == PH_DOWN) {
             K = D.F;
-            const float *src = P.act + (size_t)k * K;
-            for (int i = tid; i < K; i += kConsumerThreads) xs[i] = __ldcg(src + i);
+            stage_copy(P.act + (size_t)k * K, xs, K);
           } else if (t == PH_PDM) {
             // slot j = k: pre-step state of the token at depth j, else Hfin[p_new - j], else zero (Eq. 5)
             K = D.d;
             int q = S.p_new - k;
             const float *src = S.occ[k] ? P.h + (size_t)S.hbuf[k] * D.d : (q >= 0 ? P.hfin + (size_t)q * D.d : nullptr);
-            for (int i = tid; i < K; i += kConsumerThreads) {
-              float v = src ? __ldcg(src + i) : 0.f;
-              xs[i] = v;
-              if (w.u0 == 0) P.feat[(size_t)k * D.d + i] = v;   // kept for the parity tests (SPD_DBG_PDM_FEAT)
+            if (src) stage_copy(src, xs, K);
+            else for (int i = tid; i < K; i += kConsumerThreads) xs[i] = 0.f;
+            if (S.pdm_idx == 0) {             // kept for the parity tests (SPD_DBG_PDM_FEAT)
+              consumer_sync();
+              for (int i = tid; i < K; i += kConsumerThreads) P.feat[(size_t)k * D.d + i] = xs[i];
             }
           } else {  // PH_HEAD: verify input at xs[0..d), PDM input at xs[kXFloats/2 ..)
             K = D.d;
             if (S.run_verify) {
               const float *h = S.mode == MODE_PREFILL_FINAL ? P.hfin + (size_t)(S.c - 1) * D.d
                                                             : P.h + (size_t)S.hbuf[D.n - 1] * D.d;
-              float r = consumer_rms_scale(h, D.d, D.eps, red);
-              for (int i = tid; i < D.d; i += kConsumerThreads) xs[i] = __ldcg(h + i) * r * bf16_to_f32(P.final_norm[i]);
+              float ss = consumer_sum(stage_copy(h, xs, D.d), red);
+              stage_scale(xs, P.final_norm, D.d, 1.0f / sqrtf(ss / (float)D.d + D.eps));
             }
             if (S.run_pdm) {
               float *xp = xs + kXFloats / 2;
+              float4 *xp4w = reinterpret_cast<float4 *>(xp);
               float ss = 0.f;
-              for (int i = tid; i < D.d; i += kConsumerThreads) {   // u = sum_j W_p[:, block j] f_j, j ascending
-                float u = 0.f;
-                for (int j = 0; j < D.n; ++j) u += __ldcg(P.pdm_part + (size_t)j * D.d + i);
-                xp[i] = u;
-                if (w.u0 == 0) P.pdm_u[i] = u;    // kept for the parity tests (SPD_DBG_PDM_PRENORM)
-                ss = fmaf(u, u, ss);
+              for (int i = tid; i < (D.d >> 2); i += kConsumerThreads) {   // u = sum_j W_p[:, block j] f_j, j ascending
+                float4 u = make_float4(0.f, 0.f, 0.f, 0.f);
+                for (int j = 0; j < D.n; ++j) {
+                  float4 v = __ldcg(reinterpret_cast<const float4 *>(P.pdm_part + (size_t)j * D.d) + i);
+                  u.x += v.x; u.y += v.y; u.z += v.z; u.w += v.w;
+                }
+                xp4w[i] = u;
+                if (cta == 0) reinterpret_cast<float4 *>(P.pdm_u)[i] = u;    // kept for the parity tests (SPD_DBG_PDM_PRENORM)
+                ss = fmaf(u.x, u.x, ss); ss = fmaf(u.y, u.y, ss); ss = fmaf(u.z, u.z, ss); ss = fmaf(u.w, u.w, ss);
               }
-              ss = warp_sum(ss);
-              consumer_sync();
-              if (lane == 0) red[warp] = ss;
-              consumer_sync();
-              float tt = 0.f;
-#pragma unroll
-              for (int ww = 0; ww < 8; ++ww) tt += red[ww];
-              float r = 1.0f / sqrtf(tt / (float)D.d + D.eps);
-              for (int i = tid; i < D.d; i += kConsumerThreads) xp[i] = xp[i] * r * bf16_to_f32(P.pdm_norm[i]);
+              ss = consumer_sum(ss, red);
+              stage_scale(xp, P.pdm_norm, D.d, 1.0f / sqrtf(ss / (float)D.d + D.eps));
             }
           }
           int kpad = w.nc * kTileCols;
@@ -400,17 +736,29 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
         }
         consumer_sync();
         if (tid == 0) prof_stamp(P, cta, p, 1);
-        // ---- stream the tiles ------------------------------------------------------------------
+        // ---- stream the claimed units ------------------------------------------------------------
         const bool two = t == PH_HEAD;
         const float4 *xv4 = reinterpret_cast<const float4 *>(xs);
         const float4 *xp4 = reinterpret_cast<const float4 *>(xs + kXFloats / 2);
         const bool do_v = !two || S.run_verify, do_p = two && S.run_pdm;
-        for (int u = w.u0; u < w.u1; ++u) {
+        while (true) {
+          int u = 0;
           float a00 = 0.f, a01 = 0.f, a10 = 0.f, a11 = 0.f;   // [row][column group], first vector
           float b00 = 0.f, b01 = 0.f, b10 = 0.f, b11 = 0.f;   // second vector (LM head only)
-          for (int c = 0; c < w.nc; ++c, ++seq) {
-            uint32_t slot = seq % kStages, it = seq / kStages;
-            mbar_wait(&full[slot], it & 1);
+          bool end = false;
+          for (int c = 0; c < w.nc || c == 0; ++c, ++seq) {
+            uint32_t slot = seq % kStages, itn = seq / kStages;
+            mbar_wait(&full[slot], itn & 1);
+            if (c == 0) {
+              u = meta[slot];
+              if (u == kEndMark) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[slot]);
+                ++seq;
+                end = true;
+                break;
+              }
+            }
             const uint4 *wt = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kTileBytes);
             uint4 wa0 = wt[(2 * warp) * 64 + lane], wa1 = wt[(2 * warp) * 64 + 32 + lane];
             uint4 wb0 = wt[(2 * warp + 1) * 64 + lane], wb1 = wt[(2 * warp + 1) * 64 + 32 + lane];
@@ -429,62 +777,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[slot]);
           }
+          if (end) break;
           // ---- unit done: reduce the two rows of this warp, fused epilogue (lane 0) ---------------
           float y0 = warp_sum(a00 + a01), y1 = warp_sum(a10 + a11);
           float z0 = 0.f, z1 = 0.f;
           if (two) { z0 = warp_sum(b00 + b01); z1 = warp_sum(b10 + b11); }
-          if (lane == 0) {
-            const int r0 = u * kTileRows + 2 * warp;   // repacked row index (even); r0 + 1 is its partner
-            if (t == PH_QKV) {
-              const int qd = D.Hq * D.hd, kd = D.Hkv * D.hd, half = D.hd / 2, pos = S.pos[k];
-              const int layer = k * D.per + pass;
-              if (r0 < qd) {                           // q pair (i, i + hd/2) of head hh: RoPE (C-2.14)
-                int hh = r0 / D.hd, i = (r0 - hh * D.hd) >> 1;
-                float2 cs = rope_s[i];
-                float *q = P.q + (size_t)k * qd + hh * D.hd;
-                q[i] = y0 * cs.x - y1 * cs.y;
-                q[i + half] = y1 * cs.x + y0 * cs.y;
-              } else if (r0 < qd + kd) {               // k pair: RoPE, bf16 (RNE), append at row pos
-                int rr = r0 - qd, hh = rr / D.hd, i = (rr - hh * D.hd) >> 1;
-                float2 cs = rope_s[i];
-                if (pos < D.max_seq) {
-                  uint16_t *dst = P.kv + kv_offset(D, layer, 0, hh) + (size_t)pos * D.hd;
-                  dst[i] = f32_to_bf16(y0 * cs.x - y1 * cs.y);
-                  dst[i + half] = f32_to_bf16(y1 * cs.x + y0 * cs.y);
-                }
-              } else if (r0 < qd + 2 * kd) {           // two consecutive v elements: bf16, append
-                int rr = r0 - qd - kd, hh = rr / D.hd, i = rr - hh * D.hd;
-                if (pos < D.max_seq) {
-                  uint16_t *dst = P.kv + kv_offset(D, layer, 1, hh) + (size_t)pos * D.hd;
-                  dst[i] = f32_to_bf16(y0);
-                  dst[i + 1] = f32_to_bf16(y1);
-                }
-              }
-            } else if (t == PH_O || t == PH_DOWN) {    // residual add
-              float *h = P.h + (size_t)S.hbuf[k] * D.d;
-              if (r0 < D.d) h[r0] = __ldcg(h + r0) + y0;
-              if (r0 + 1 < D.d) h[r0 + 1] = __ldcg(h + r0 + 1) + y1;
-            } else if (t == PH_GATEUP) {               // rows (gate_i, up_i): SwiGLU
-              int i = r0 >> 1;
-              if (i < D.F) P.act[(size_t)k * D.F + i] = silu_mul(y0, y1);
-            } else if (t == PH_PDM) {
-              if (r0 < D.d) P.pdm_part[(size_t)k * D.d + r0] = y0;
-              if (r0 + 1 < D.d) P.pdm_part[(size_t)k * D.d + r0 + 1] = y1;
-            } else {                                   // PH_HEAD: running (value, index) argmax
-              if (S.run_verify) {
-                if (r0 < D.V && cand_better(y0, r0, hbest_v[0], hbest_i[0])) { hbest_v[0] = y0; hbest_i[0] = r0; }
-                if (r0 + 1 < D.V && cand_better(y1, r0 + 1, hbest_v[0], hbest_i[0])) { hbest_v[0] = y1; hbest_i[0] = r0 + 1; }
-              }
-              if (S.run_pdm) {
-                if (r0 < D.V && cand_better(z0, r0, hbest_v[1], hbest_i[1])) { hbest_v[1] = z0; hbest_i[1] = r0; }
-                if (r0 + 1 < D.V && cand_better(z1, r0 + 1, hbest_v[1], hbest_i[1])) { hbest_v[1] = z1; hbest_i[1] = r0 + 1; }
-              }
-              if (P.debug_logits) {
-                if (S.run_verify) { if (r0 < D.V) P.logits_v[r0] = y0; if (r0 + 1 < D.V) P.logits_v[r0 + 1] = y1; }
-                if (S.run_pdm) { if (r0 < D.V) P.logits_p[r0] = z0; if (r0 + 1 < D.V) P.logits_p[r0 + 1] = z1; }
-              }
-            }
-          }
+          if (lane == 0) unit_epilogue(P, S, t, k, pass, u * kTileRows + 2 * warp, y0, y1, z0, z1, rope_s, hbest_v, hbest_i);
         }
         if (t == PH_HEAD) {   // CTA-level candidates -> global
           if (lane == 0) { cbest_v[warp] = hbest_v[0]; cbest_v[8 + warp] = hbest_v[1]; cbest_i[warp] = hbest_i[0]; cbest_i[8 + warp] = hbest_i[1]; }
@@ -498,6 +796,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
             P.cand_idx[tid * kMaxCand + cta] = bi == 0x7fffffff ? -1 : bi;
           }
         }
+        if (t == PH_QKV) fence_proxy_async();   // the appended K/V rows are read by TMA (async proxy) next
       }
       // ---- publish this phase's outputs: arrive at the barrier that the dependent phase waits on ----
       const bool arrive = p >= 1;              // PDM has no barrier of its own (see need_barrier)
@@ -519,6 +818,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
     }
     __syncthreads();
     controller_end(P, ncta);
+    for (int i = tid; i < np * kMaxStages; i += kThreads) P.claim[i] = 0u;   // every producer is done claiming
     __syncthreads();
     if (tid == 0) { __threadfence(); atomicAdd(bar_launch, 1ull); }
   }
@@ -614,7 +914,7 @@ int mega_create(const DevPtrs &P, const uint16_t *const *const *src, void *repac
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-  int smem = kStages * kTileBytes + kXFloats * 4 + 2 * kStages * 8 + 64 * 8 + 16 * 4 + 32 * 4 + (int)sizeof(Sched) + 64;
+  int smem = kStages * kTileBytes + kXFloats * 4 + 2 * kStages * 8 + 64 * 8 + 16 * 4 + 32 * 4 + 16 * 4 + (int)sizeof(Sched) + 64;
   if (!coop || sms < D.n) return -1;
   if (cudaFuncSetAttribute(k_spd_cycle, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
     cudaGetLastError();
