@@ -122,7 +122,8 @@ enum {
   SPD_DBG_PHASE_PROFILE = 10 /* uint64[160][168][6]: per (CTA, phase) clock stamps of the last fused cycle:
                               0 inputs ready, 1 activations staged, 2 tiles consumed, 3/4 producer issued the
                               phase's first/last tile (SM clock); 5 = %globaltimer at stamp 0; phase 167 holds
-                              (clock, %globaltimer) at kernel start (needs SPD_OPT_PHASE_PROFILE)            */
+                              (clock, %globaltimer) after the schedule [0,1] and at kernel entry [2,3]; CTA 0 also
+                              at the end of the controller [4,5] (needs SPD_OPT_PHASE_PROFILE)               */
 };
 
 /* Buffer sizes for a configuration.  SPD_EINVAL if the configuration is unsupported. */

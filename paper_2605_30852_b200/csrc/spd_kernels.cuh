@@ -184,23 +184,29 @@ __device__ __forceinline__ void rope_table_fill(const DevPtrs &P, int tid, int n
 
 // Controller, last part of a cycle (one CTA, >= 32 threads): reduce the argmax candidates, verify,
 // accept / reject + rollback, shift the pipeline, enter the next token, record.
-// `ncand` candidates per head (verify = row 0, PDM = row 1 of cand_val/cand_idx).
+// Needs >= 64 threads.  `ncand` candidates per head (verify = row 0, PDM = row 1 of cand_val/cand_idx).
 __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand) {
   __shared__ int s_y, s_draft, s_exit_buf, s_exit_pos, s_enter_tok, s_enter_buf, s_do_exit, s_do_enter;
   StepState *st = P.st;
   const Dims &D = P.dim;
   int n = D.n;
-  if (threadIdx.x < 2) {
-    // head 0 = verify, head 1 = PDM; lowest index among equal maxima
-    int which = threadIdx.x;
+  if (threadIdx.x < 64) {
+    // warp 0 = verify, warp 1 = PDM; lowest index among equal maxima ((value, index) is a total order,
+    // so the result does not depend on the reduction shape)
+    int which = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float bv = -INFINITY;
     int bi = 0x7fffffff;
-    for (int i = 0; i < ncand; ++i) {
+    for (int i = lane; i < ncand; i += 32) {
       float v = P.cand_val[which * kMaxCand + i];
       int ix = P.cand_idx[which * kMaxCand + i];
       if (ix >= 0 && cand_better(v, ix, bv, bi)) { bv = v; bi = ix; }
     }
-    if (which == 0) s_y = bi; else s_draft = bi;
+    for (int o = 16; o > 0; o >>= 1) {
+      float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+      int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+      if (cand_better(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+    }
+    if (lane == 0) { if (which == 0) s_y = bi; else s_draft = bi; }
   }
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -259,17 +265,20 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand) {
     else if (mode == MODE_PREFILL_FINAL) P.results[0] = r;
   }
   __syncthreads();
-  int d = D.d;
+  int d = D.d;   // d % 8 == 0
   if (s_do_exit) {     // Hfin[e.pos] = e.h  (C-2.4) — read before the buffer is reused below
-    const float *src = P.h + (size_t)s_exit_buf * d;
-    float *dst = P.hfin + (size_t)s_exit_pos * d;
-    for (int i = threadIdx.x; i < d; i += blockDim.x) dst[i] = src[i];
+    const float4 *src = reinterpret_cast<const float4 *>(P.h + (size_t)s_exit_buf * d);
+    float4 *dst = reinterpret_cast<float4 *>(P.hfin + (size_t)s_exit_pos * d);
+    for (int i = threadIdx.x; i < (d >> 2); i += blockDim.x) dst[i] = src[i];
   }
   __syncthreads();
   if (s_do_enter) {    // token entry: h = E[tok] (k = 0 is the embedding-level input)
-    const uint16_t *e = P.embed + (size_t)s_enter_tok * d;
-    float *dst = P.h + (size_t)s_enter_buf * d;
-    for (int i = threadIdx.x; i < d; i += blockDim.x) dst[i] = bf16_to_f32(e[i]);
+    const uint2 *e = reinterpret_cast<const uint2 *>(P.embed + (size_t)s_enter_tok * d);
+    float4 *dst = reinterpret_cast<float4 *>(P.h + (size_t)s_enter_buf * d);
+    for (int i = threadIdx.x; i < (d >> 2); i += blockDim.x) {
+      uint2 w = e[i];
+      dst[i] = make_float4(bf16_lo(w.x), bf16_hi(w.x), bf16_lo(w.y), bf16_hi(w.y));
+    }
   }
 }
 

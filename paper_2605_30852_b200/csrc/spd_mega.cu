@@ -394,22 +394,50 @@ __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, 
 }
 
 // Merge of the splits of one q head by one warp, in split order (fixed): out = sum_j o_j e^(m_j-M) / sum_j l_j e^(m_j-M).
+// Lane owns EPL consecutive elements; the loads of different splits are independent and batched.
+template <int HD>
 __device__ __forceinline__ void attn_merge_warp(const DevPtrs &P, int stage, int hq, int nsplit, int lane) {
+  constexpr int EPL = HD / 32;
   const Dims &D = P.dim;
-  size_t slot = ((size_t)stage * D.Hq + hq) * P.nsplit_max;
+  const size_t slot = ((size_t)stage * D.Hq + hq) * P.nsplit_max;
   const float2 *ml = P.part_ml + slot;
   float M = -INFINITY;
-  for (int j = 0; j < nsplit; ++j) M = fmaxf(M, __ldcg(&ml[j].x));
-  const int epl = D.hd / 32;
-  for (int e = lane * epl; e < (lane + 1) * epl; ++e) {
-    float L = 0.f, o = 0.f;
-    for (int j = 0; j < nsplit; ++j) {
-      float2 mlj = __ldcg(&ml[j]);
-      float wj = expf(mlj.x - M);
-      L = fmaf(mlj.y, wj, L);
-      o = fmaf(__ldcg(P.part_o + (slot + j) * D.hd + e), wj, o);
+  for (int j = lane; j < nsplit; j += 32) M = fmaxf(M, __ldcg(&ml[j].x));
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+  float L = 0.f, acc[EPL];
+#pragma unroll
+  for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
+  const float *po = P.part_o + slot * HD + lane * EPL;
+#pragma unroll 8
+  for (int j = 0; j < nsplit; ++j) {
+    float2 mlj = __ldcg(&ml[j]);
+    float v[EPL];
+    if constexpr (EPL == 4) {
+      float4 t = __ldcg(reinterpret_cast<const float4 *>(po + (size_t)j * HD));
+      v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+    } else {
+      float2 t = __ldcg(reinterpret_cast<const float2 *>(po + (size_t)j * HD));
+      v[0] = t.x; v[1] = t.y;
     }
-    P.att[((size_t)stage * D.Hq + hq) * D.hd + e] = o / L;
+    float wj = expf(mlj.x - M);
+    L = fmaf(mlj.y, wj, L);
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) acc[e] = fmaf(v[e], wj, acc[e]);
+  }
+  float *out = P.att + ((size_t)stage * D.Hq + hq) * HD + lane * EPL;
+#pragma unroll
+  for (int e = 0; e < EPL; ++e) out[e] = acc[e] / L;
+}
+
+// Resolves a pending split-completion count: the warp that completed the last split merges the head.
+__device__ __forceinline__ void attn_resolve(const DevPtrs &P, int old, int stage, int hq, int nsplit, int lane) {
+  old = __shfl_sync(0xffffffffu, old, 0);
+  if (old == nsplit - 1) {
+    __threadfence();
+    if (P.dim.hd == 128) attn_merge_warp<128>(P, stage, hq, nsplit, lane);
+    else attn_merge_warp<64>(P, stage, hq, nsplit, lane);
+    if (lane == 0) P.att_cnt[stage * P.dim.Hq + hq] = 0;
   }
 }
 
@@ -503,6 +531,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
   unsigned long long *bar_count = reinterpret_cast<unsigned long long *>(P.bar);
   unsigned long long *bar_launch = bar_count + 1;
 
+  if (P.prof_on && tid == 0 && cta < kProfCtas) {
+    unsigned long long *pr = P.prof + ((size_t)cta * kProfPhases + (kProfPhases - 1)) * kProfStamps;
+    pr[2] = (unsigned long long)clock64(); pr[3] = globaltimer_ns();
+  }
   // ---- schedule (every CTA computes the same thing from the state the previous cycle left) ----
   if (tid == 0) {
     const StepState *st = P.st;
@@ -635,6 +667,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
       const int k = w.job;                    // stage (layer phases) / slot (PDM)
       if (t == PH_ATTN) {
         if (tid == 0) prof_stamp(P, cta, p, 1);
+        int pend_old = 0, pend_stage = 0, pend_hq = 0, pend_cnt = -1;
         // ---- split-KV decode attention: items claimed by the producer arrive through the ring ----
         while (true) {
           uint32_t slot = seq % kStages, itn = seq / kStages;
@@ -655,21 +688,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
           __syncwarp();
           if (lane == 0) for (int j = 0; j < 2 * nk; ++j) mbar_arrive(&empty[(seq + j) % kStages]);
           seq += 2 * nk;
-          // the last split of a q head to finish merges them (fixed split order)
+          // the last split of a q head to finish merges them (fixed split order).  The completion count
+          // is fetched asynchronously: its latency hides behind the next item, where it is resolved.
           __threadfence();
           consumer_sync();
           if (warp < G) {
-            const int hq = it.kvh * G + warp;
-            int old = 0;
-            if (lane == 0) old = atomicAdd(&P.att_cnt[it.stage * D.Hq + hq], 1);
-            old = __shfl_sync(0xffffffffu, old, 0);
-            if (old == it.nsplit - 1) {
-              __threadfence();
-              attn_merge_warp(P, it.stage, hq, it.nsplit, lane);
-              if (lane == 0) P.att_cnt[it.stage * D.Hq + hq] = 0;
-            }
+            if (pend_cnt >= 0) attn_resolve(P, pend_old, pend_stage, pend_hq, pend_cnt, lane);
+            pend_stage = it.stage; pend_hq = it.kvh * G + warp; pend_cnt = it.nsplit;
+            if (lane == 0) pend_old = atomicAdd(&P.att_cnt[pend_stage * D.Hq + pend_hq], 1);
           }
         }
+        if (warp < G && pend_cnt >= 0) { attn_resolve(P, pend_old, pend_stage, pend_hq, pend_cnt, lane); pend_cnt = -1; }
       } else {
         // ---- stage the activation vector(s) of this phase in shared memory ----------------------
         if (k >= 0) {
@@ -820,7 +849,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
     controller_end(P, ncta);
     for (int i = tid; i < np * kMaxStages; i += kThreads) P.claim[i] = 0u;   // every producer is done claiming
     __syncthreads();
-    if (tid == 0) { __threadfence(); atomicAdd(bar_launch, 1ull); }
+    if (tid == 0) {
+      __threadfence();
+      atomicAdd(bar_launch, 1ull);
+      if (P.prof_on) {
+        unsigned long long *pr = P.prof + ((size_t)(kProfPhases - 1)) * kProfStamps;
+        pr[4] = (unsigned long long)clock64(); pr[5] = globaltimer_ns();
+      }
+    }
   }
 }
 
