@@ -44,6 +44,9 @@ constexpr int kXFloats = 12288;                          // activation vector ca
 constexpr int kConsumerThreads = 256;
 constexpr int kThreads = kConsumerThreads + 32;
 constexpr int kEndMark = -1;                             // slot tag: no more work in this phase
+constexpr int kAttnScratchFloats = 2 * 8 * kAttnSplit + 8 * 8 * 128;   // scores, probabilities, per-warp partial outputs (G <= 8, hd <= 128)
+constexpr int kAttnDoneMax = 32;                         // items whose completion counts are published together
+static_assert(kAttnScratchFloats + kAttnDoneMax * 9 + 1 <= kXFloats, "attention scratch must fit the activation buffer");
 
 enum PhaseType { PH_PDM = 0, PH_QKV = 1, PH_ATTN = 2, PH_O = 3, PH_GATEUP = 4, PH_DOWN = 5, PH_HEAD = 6 };
 
@@ -63,6 +66,7 @@ struct Sched {
   int my_idx;                                   // index inside the stage's CTA group
   int pdm_slot, pdm_idx;                        // this CTA's slot (column block of W_p) in the PDM phase
   int attn_total;                               // attention items of one pass
+  int attn_nonfinal;                            // ... of which do not contain the row appended in this pass
 };
 
 struct PhaseDesc {                              // what one phase means for this CTA
@@ -157,17 +161,28 @@ __device__ __forceinline__ PhaseDesc phase_desc(int p, int np, const Sched &S, c
   return w;
 }
 
-// Attention item -> (stage, kv head, split).  Items are ordered stage-major, then kv head, then split.
+// Attention item -> (stage, kv head, split).  Items [0, attn_nonfinal) are the splits that do not contain
+// the row appended in this pass (stage-major, kv head, split) — their K/V rows are old and can be fetched
+// before the QKV phase has finished; items [attn_nonfinal, attn_total) are the last split of every
+// (stage, kv head).
 __device__ __forceinline__ void attn_decode(const Sched &S, const Dims &D, int item, AttnItem &it) {
-  int rem = item;
-  it.stage = -1; it.nsplit = 0;
-  for (int a = 0; a < S.n_act; ++a) {
-    int ns = (S.pos[S.act[a]] + kAttnSplit) / kAttnSplit;     // ceil((pos + 1) / split)
-    if (rem < D.Hkv * ns) { it.stage = S.act[a]; it.nsplit = ns; break; }
-    rem -= D.Hkv * ns;
+  it.stage = S.act[0]; it.nsplit = 1; it.kvh = 0; it.split = 0;
+  if (item < S.attn_nonfinal) {
+    int rem = item;
+    for (int a = 0; a < S.n_act; ++a) {
+      int ns = (S.pos[S.act[a]] + kAttnSplit) / kAttnSplit;     // ceil((pos + 1) / split)
+      if (rem < D.Hkv * (ns - 1)) { it.stage = S.act[a]; it.nsplit = ns; break; }
+      rem -= D.Hkv * (ns - 1);
+    }
+    it.kvh = rem / (it.nsplit - 1);
+    it.split = rem - it.kvh * (it.nsplit - 1);
+  } else {
+    int f = item - S.attn_nonfinal;
+    it.stage = S.act[f / D.Hkv];
+    it.kvh = f % D.Hkv;
+    it.nsplit = (S.pos[it.stage] + kAttnSplit) / kAttnSplit;
+    it.split = it.nsplit - 1;
   }
-  it.kvh = rem / it.nsplit;
-  it.split = rem - it.kvh * it.nsplit;
   it.t0 = it.split * kAttnSplit;
   int T = S.pos[it.stage] + 1;
   it.rows = min(T - it.t0, kAttnSplit);
@@ -261,7 +276,7 @@ struct XReduce {
 // red[8][G][HD] per-warp partial outputs.
 template <int HD, int G>
 __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, const uint8_t *ring, uint32_t seq0, int nk,
-                                          float *scratch) {
+                                          float *scratch, uint64_t *empty) {
   constexpr int CH = HD / 8;            // 16-byte chunks (= lanes) per K row
   constexpr int RPI = 32 / CH;          // rows covered by one warp-wide LDS.128
   constexpr int NI = 16 / RPI;          // iterations for a warp's 16 rows
@@ -315,6 +330,7 @@ __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, 
     }
   }
   consumer_sync();
+  if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + j) % kStages]);   // K slots are free
   // ---- softmax of the split, one warp per head: m = max, p = exp(s - m), l = sum p ----
   if (warp < G) {
     float s[kAttnSplit / 32], m = -INFINITY;
@@ -348,34 +364,39 @@ __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, 
     for (int h = 0; h < G; ++h)
 #pragma unroll
       for (int e = 0; e < EPL; ++e) acc[h][e] = 0.f;
-    const int r_end = min(rows, 16 * warp + 16);
-    for (int row = 16 * warp; row < r_end; ++row) {
-      const uint8_t *tile = ring + (size_t)((seq0 + nk + row / RPS) % kStages) * kTileBytes;
-      const uint8_t *vr = tile + (size_t)(row % RPS) * (HD * 2) + lane * (EPL * 2);
-      float vv[EPL];
-      if constexpr (EPL == 4) {
-        uint2 w = *reinterpret_cast<const uint2 *>(vr);
-        vv[0] = bf16_lo(w.x); vv[1] = bf16_hi(w.x); vv[2] = bf16_lo(w.y); vv[3] = bf16_hi(w.y);
-      } else {
-        uint32_t w = *reinterpret_cast<const uint32_t *>(vr);
-        vv[0] = bf16_lo(w); vv[1] = bf16_hi(w);
+#pragma unroll 4
+    for (int i = 0; i < 16; ++i) {
+      const int row = 16 * warp + i;
+      if (row < rows) {
+        const uint8_t *tile = ring + (size_t)((seq0 + nk + row / RPS) % kStages) * kTileBytes;
+        const uint8_t *vr = tile + (size_t)(row % RPS) * (HD * 2) + lane * (EPL * 2);
+        float vv[EPL];
+        if constexpr (EPL == 4) {
+          uint2 w = *reinterpret_cast<const uint2 *>(vr);
+          vv[0] = bf16_lo(w.x); vv[1] = bf16_hi(w.x); vv[2] = bf16_lo(w.y); vv[3] = bf16_hi(w.y);
+        } else {
+          uint32_t w = *reinterpret_cast<const uint32_t *>(vr);
+          vv[0] = bf16_lo(w); vv[1] = bf16_hi(w);
+        }
+        float pr[G];
+        if constexpr (G == 4) {
+          float4 t = *reinterpret_cast<const float4 *>(ps + row * G);
+          pr[0] = t.x; pr[1] = t.y; pr[2] = t.z; pr[3] = t.w;
+        } else if constexpr (G == 8) {
+          float4 t = *reinterpret_cast<const float4 *>(ps + row * G), u = *reinterpret_cast<const float4 *>(ps + row * G + 4);
+          pr[0] = t.x; pr[1] = t.y; pr[2] = t.z; pr[3] = t.w; pr[4] = u.x; pr[5] = u.y; pr[6] = u.z; pr[7] = u.w;
+        } else {
+#pragma unroll
+          for (int h = 0; h < G; ++h) pr[h] = ps[row * G + h];
+        }
+#pragma unroll
+        for (int h = 0; h < G; ++h)
+#pragma unroll
+          for (int e = 0; e < EPL; ++e) acc[h][e] = fmaf(pr[h], vv[e], acc[h][e]);
       }
-      float pr[G];
-      if constexpr (G == 4) {
-        float4 t = *reinterpret_cast<const float4 *>(ps + row * G);
-        pr[0] = t.x; pr[1] = t.y; pr[2] = t.z; pr[3] = t.w;
-      } else if constexpr (G == 8) {
-        float4 t = *reinterpret_cast<const float4 *>(ps + row * G), u = *reinterpret_cast<const float4 *>(ps + row * G + 4);
-        pr[0] = t.x; pr[1] = t.y; pr[2] = t.z; pr[3] = t.w; pr[4] = u.x; pr[5] = u.y; pr[6] = u.z; pr[7] = u.w;
-      } else {
-#pragma unroll
-        for (int h = 0; h < G; ++h) pr[h] = ps[row * G + h];
-      }
-#pragma unroll
-      for (int h = 0; h < G; ++h)
-#pragma unroll
-        for (int e = 0; e < EPL; ++e) acc[h][e] = fmaf(pr[h], vv[e], acc[h][e]);
     }
+    __syncwarp();
+    if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + nk + j) % kStages]);   // V slots are free
 #pragma unroll
     for (int h = 0; h < G; ++h)
 #pragma unroll
@@ -428,17 +449,6 @@ __device__ __forceinline__ void attn_merge_warp(const DevPtrs &P, int stage, int
   float *out = P.att + ((size_t)stage * D.Hq + hq) * HD + lane * EPL;
 #pragma unroll
   for (int e = 0; e < EPL; ++e) out[e] = acc[e] / L;
-}
-
-// Resolves a pending split-completion count: the warp that completed the last split merges the head.
-__device__ __forceinline__ void attn_resolve(const DevPtrs &P, int old, int stage, int hq, int nsplit, int lane) {
-  old = __shfl_sync(0xffffffffu, old, 0);
-  if (old == nsplit - 1) {
-    __threadfence();
-    if (P.dim.hd == 128) attn_merge_warp<128>(P, stage, hq, nsplit, lane);
-    else attn_merge_warp<64>(P, stage, hq, nsplit, lane);
-    if (lane == 0) P.att_cnt[stage * P.dim.Hq + hq] = 0;
-  }
 }
 
 // Fused epilogue of one 16-row unit (lane 0 of every warp; rows r0, r0 + 1 of the repacked matrix).
@@ -502,11 +512,11 @@ __device__ __forceinline__ void unit_epilogue(const DevPtrs &P, const Sched &S, 
 
 template <int HD>
 __device__ __forceinline__ void attn_item_g(const DevPtrs &P, const AttnItem &it, const uint8_t *ring, uint32_t seq0, int nk,
-                                            float *scratch, int G) {
-  if (G == 4) attn_item<HD, 4>(P, it, ring, seq0, nk, scratch);
-  else if (G == 2) attn_item<HD, 2>(P, it, ring, seq0, nk, scratch);
-  else if (G == 8) attn_item<HD, 8>(P, it, ring, seq0, nk, scratch);
-  else attn_item<HD, 1>(P, it, ring, seq0, nk, scratch);
+                                            float *scratch, uint64_t *empty, int G) {
+  if (G == 4) attn_item<HD, 4>(P, it, ring, seq0, nk, scratch, empty);
+  else if (G == 2) attn_item<HD, 2>(P, it, ring, seq0, nk, scratch, empty);
+  else if (G == 8) attn_item<HD, 8>(P, it, ring, seq0, nk, scratch, empty);
+  else attn_item<HD, 1>(P, it, ring, seq0, nk, scratch, empty);
 }
 
 // The fused kernel ---------------------------------------------------------------------------------
@@ -540,13 +550,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
     const StepState *st = P.st;
     Sched &S = *Sp;
     S.mode = st->mode; S.c = st->c;
-    int a = 0, items = 0;
+    int a = 0, items = 0, nonfinal = 0;
     for (int k = 0; k < D.n; ++k) {
       S.occ[k] = st->occ[k]; S.pos[k] = st->pos[k]; S.hbuf[k] = st->hbuf[k];
-      if (st->occ[k]) { S.act[a++] = k; items += D.Hkv * ((st->pos[k] + kAttnSplit) / kAttnSplit); }
+      if (st->occ[k]) {
+        int ns = (st->pos[k] + kAttnSplit) / kAttnSplit;
+        S.act[a++] = k; items += D.Hkv * ns; nonfinal += D.Hkv * (ns - 1);
+      }
     }
     S.n_act = a;
     S.attn_total = items;
+    S.attn_nonfinal = nonfinal;
     S.p_new = st->occ[0] ? st->pos[0] : -1;
     S.run_pdm = st->mode == MODE_SPD;
     S.run_verify = (st->mode == MODE_SPD && st->occ[D.n - 1]) || st->mode == MODE_PREFILL_FINAL;
@@ -586,17 +600,20 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
         if (w.job >= 0) {
           unsigned int next = atomicAdd(w.ctr, 1u);
           if (w.type == PH_ATTN) {
-            // K/V rows of this pass were appended by other CTAs in the QKV phase: wait for its barrier
-            unsigned long long target = (launch * nbar + (unsigned long long)(p - 2) + 1) * (unsigned long long)ncta;
-            while (ld_acquire_u64(bar_count) < target) {}
-            fence_proxy_async();
             const int pass = (p - 1) / 5;
-            bool first = true;
+            bool first = true, kv_ready = false;
             while (next < (unsigned int)w.U) {
               AttnItem it;
               attn_decode(S, D, (int)next, it);
               const int item = (int)next;
               next = atomicAdd(w.ctr, 1u);
+              if (item >= S.attn_nonfinal && !kv_ready) {
+                // the last split holds the row appended by other CTAs in this pass's QKV phase: wait for its barrier
+                unsigned long long target = (launch * nbar + (unsigned long long)(p - 2) + 1) * (unsigned long long)ncta;
+                while (ld_acquire_u64(bar_count) < target) {}
+                fence_proxy_async();
+                kv_ready = true;
+              }
               const int layer = it.stage * D.per + pass;
               const int nk = (it.rows + RPS - 1) / RPS;
               for (int kvsel = 0; kvsel < 2; ++kvsel) {
@@ -667,9 +684,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
       const int k = w.job;                    // stage (layer phases) / slot (PDM)
       if (t == PH_ATTN) {
         if (tid == 0) prof_stamp(P, cta, p, 1);
-        int pend_old = 0, pend_stage = 0, pend_hq = 0, pend_cnt = -1;
-        // ---- split-KV decode attention: items claimed by the producer arrive through the ring ----
-        while (true) {
+        // ---- split-KV decode attention: items claimed by the producer arrive through the ring; the
+        //      split-completion counts of the items this CTA processed are published together at the end
+        //      of the phase (one fence), and whoever completes a q head merges its splits ------------------
+        int *done_list = reinterpret_cast<int *>(xs + kAttnScratchFloats);   // [kAttnDoneMax] item ids
+        int *merge_cnt = done_list + kAttnDoneMax;                           // [1]
+        int *merge_list = merge_cnt + 1;                                     // [kAttnDoneMax * 8] (item slot, head)
+        int n_done = 0;
+        bool more = true;
+        while (more) {
           uint32_t slot = seq % kStages, itn = seq / kStages;
           mbar_wait(&full[slot], itn & 1);
           const int item = meta[slot];
@@ -677,28 +700,46 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[slot]);
             ++seq;
-            break;
+            more = false;
+          } else {
+            AttnItem it;
+            attn_decode(S, D, item, it);
+            const int nk = (it.rows + RPS - 1) / RPS;
+            for (int j = 1; j < 2 * nk; ++j) mbar_wait(&full[(seq + j) % kStages], ((seq + j) / kStages) & 1);
+            if (D.hd == 128) attn_item_g<128>(P, it, ring, seq, nk, xs, empty, G);
+            else attn_item_g<64>(P, it, ring, seq, nk, xs, empty, G);
+            seq += 2 * nk;
+            if (tid == 0) done_list[n_done] = item;
+            ++n_done;
           }
-          AttnItem it;
-          attn_decode(S, D, item, it);
-          const int nk = (it.rows + RPS - 1) / RPS;
-          for (int j = 1; j < 2 * nk; ++j) mbar_wait(&full[(seq + j) % kStages], ((seq + j) / kStages) & 1);
-          if (D.hd == 128) attn_item_g<128>(P, it, ring, seq, nk, xs, G);
-          else attn_item_g<64>(P, it, ring, seq, nk, xs, G);
-          __syncwarp();
-          if (lane == 0) for (int j = 0; j < 2 * nk; ++j) mbar_arrive(&empty[(seq + j) % kStages]);
-          seq += 2 * nk;
-          // the last split of a q head to finish merges them (fixed split order).  The completion count
-          // is fetched asynchronously: its latency hides behind the next item, where it is resolved.
-          __threadfence();
-          consumer_sync();
-          if (warp < G) {
-            if (pend_cnt >= 0) attn_resolve(P, pend_old, pend_stage, pend_hq, pend_cnt, lane);
-            pend_stage = it.stage; pend_hq = it.kvh * G + warp; pend_cnt = it.nsplit;
-            if (lane == 0) pend_old = atomicAdd(&P.att_cnt[pend_stage * D.Hq + pend_hq], 1);
+          if (n_done == kAttnDoneMax || (!more && n_done > 0)) {
+            if (tid == 0) *merge_cnt = 0;
+            __threadfence();                       // this CTA's partial outputs, before their completion counts
+            consumer_sync();
+            for (int e = tid; e < n_done * G; e += kConsumerThreads) {
+              AttnItem it;
+              attn_decode(S, D, done_list[e / G], it);
+              const int hq = it.kvh * G + e % G;
+              if (atomicAdd(&P.att_cnt[it.stage * D.Hq + hq], 1) == it.nsplit - 1) merge_list[atomicAdd(merge_cnt, 1)] = e;
+            }
+            consumer_sync();
+            const int nm = *merge_cnt;
+            if (nm > 0) {
+              __threadfence();
+              for (int m = warp; m < nm; m += 8) {   // the last split of a q head to finish merges them (fixed split order)
+                const int e = merge_list[m];
+                AttnItem it;
+                attn_decode(S, D, done_list[e / G], it);
+                const int hq = it.kvh * G + e % G;
+                if (D.hd == 128) attn_merge_warp<128>(P, it.stage, hq, it.nsplit, lane);
+                else attn_merge_warp<64>(P, it.stage, hq, it.nsplit, lane);
+                if (lane == 0) P.att_cnt[it.stage * D.Hq + hq] = 0;
+              }
+            }
+            consumer_sync();                         // done_list / merge_list are reused
+            n_done = 0;
           }
         }
-        if (warp < G && pend_cnt >= 0) { attn_resolve(P, pend_old, pend_stage, pend_hq, pend_cnt, lane); pend_cnt = -1; }
       } else {
         // ---- stage the activation vector(s) of this phase in shared memory ----------------------
         if (k >= 0) {
