@@ -117,7 +117,7 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
   Q.truth = cv.take<int32_t>(D.max_seq);
   Q.pf_tokens = cv.take<int32_t>(D.max_seq);
   Q.results = cv.take<StepResult>(kResultRing);
-  Q.bar = cv.take<unsigned int>(64);
+  Q.bar = cv.take<unsigned int>(kBarWords);
   Q.claim = cv.take<unsigned int>((size_t)kProfPhases * kMaxStages);
   Q.prof = cv.take<unsigned long long>((size_t)kProfCtas * kProfPhases * kProfStamps);
   const uint16_t **tabs[9];

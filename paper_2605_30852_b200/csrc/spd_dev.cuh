@@ -11,6 +11,10 @@ constexpr int kAttnSplit = 128;     // KV rows per attention split — fixed, so
                                     // depends on n, slot, fill or history (batch invariance)
 constexpr int kResultRing = 1024;   // device ring of step results (spd_step_many batch limit)
 constexpr int kMaxCand = 256;       // per-CTA argmax candidates of the LM-head pass
+// Synchronisation words of the fused engine (DevPtrs::bar), one 128-byte line each: [0] finished-CTA count,
+// [32] launch count, [kBarGroup0 + 32 k] arrivals of stage k's CTA group, then two PDM counters.
+constexpr int kBarGroup0 = 64;
+constexpr int kBarWords = kBarGroup0 + 32 * (kMaxStages + 2);
 // Optional per-phase clock stamps of the fused kernel (SPD_OPT_PHASE_PROFILE): [cta][phase][stamp]
 constexpr int kProfCtas = 160, kProfPhases = 168, kProfStamps = 6;
 

@@ -64,8 +64,11 @@ struct Sched {
   int pos[kMaxStages], hbuf[kMaxStages], occ[kMaxStages];
   int my_stage;                                 // this CTA's stage in the layer phases (-1: none)
   int my_idx;                                   // index inside the stage's CTA group
+  int my_gsize;                                 // CTAs in this CTA's stage group
+  int exit_gsize;                               // CTAs in the group of stage n - 1 (0: that stage is empty)
   int pdm_slot, pdm_idx;                        // this CTA's slot (column block of W_p) in the PDM phase
-  int attn_total;                               // attention items of one pass
+  int attn_ns;                                  // 128-row splits of this CTA's stage in this cycle
+  int attn_total;                               // attention items (kv head, split) of this CTA's stage in one pass
   int attn_nonfinal;                            // ... of which do not contain the row appended in this pass
 };
 
@@ -124,6 +127,12 @@ __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long
   return v;
 }
 
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int *p) {
+  unsigned int v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
 __device__ __forceinline__ int phase_type(int p, int np) {
   if (p == 0) return PH_PDM;
   if (p == np - 1) return PH_HEAD;
@@ -145,7 +154,7 @@ __device__ __forceinline__ PhaseDesc phase_desc(int p, int np, const Sched &S, c
     w.job = 0; w.U = ML.u_head; w.nc = ML.nc_d;
     w.base = ML.repack + ML.off_head;
   } else if (w.type == PH_ATTN) {
-    if (S.n_act > 0) { w.job = 0; w.U = S.attn_total; }
+    if (S.my_stage >= 0) { w.job = S.my_stage; w.U = S.attn_total; }
   } else {
     if (S.my_stage < 0) return w;
     int pass = (p - 1) / 5;
@@ -161,26 +170,16 @@ __device__ __forceinline__ PhaseDesc phase_desc(int p, int np, const Sched &S, c
   return w;
 }
 
-// Attention item -> (stage, kv head, split).  Items [0, attn_nonfinal) are the splits that do not contain
-// the row appended in this pass (stage-major, kv head, split) — their K/V rows are old and can be fetched
-// before the QKV phase has finished; items [attn_nonfinal, attn_total) are the last split of every
-// (stage, kv head).
+// Attention item of this CTA's stage -> (kv head, split).  Items [0, attn_nonfinal) are the splits that do
+// not contain the row appended in this pass (kv head major) — their K/V rows are old and can be fetched
+// before the QKV phase has finished; items [attn_nonfinal, attn_total) are the last split of every kv head.
 __device__ __forceinline__ void attn_decode(const Sched &S, const Dims &D, int item, AttnItem &it) {
-  it.stage = S.act[0]; it.nsplit = 1; it.kvh = 0; it.split = 0;
+  it.stage = S.my_stage; it.nsplit = S.attn_ns;
   if (item < S.attn_nonfinal) {
-    int rem = item;
-    for (int a = 0; a < S.n_act; ++a) {
-      int ns = (S.pos[S.act[a]] + kAttnSplit) / kAttnSplit;     // ceil((pos + 1) / split)
-      if (rem < D.Hkv * (ns - 1)) { it.stage = S.act[a]; it.nsplit = ns; break; }
-      rem -= D.Hkv * (ns - 1);
-    }
-    it.kvh = rem / (it.nsplit - 1);
-    it.split = rem - it.kvh * (it.nsplit - 1);
+    it.kvh = item / (it.nsplit - 1);
+    it.split = item - it.kvh * (it.nsplit - 1);
   } else {
-    int f = item - S.attn_nonfinal;
-    it.stage = S.act[f / D.Hkv];
-    it.kvh = f % D.Hkv;
-    it.nsplit = (S.pos[it.stage] + kAttnSplit) / kAttnSplit;
+    it.kvh = item - S.attn_nonfinal;
     it.split = it.nsplit - 1;
   }
   it.t0 = it.split * kAttnSplit;
@@ -537,9 +536,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
   const int cta = blockIdx.x, ncta = gridDim.x;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int np = 2 + 5 * D.per;
-  const unsigned long long nbar = (unsigned long long)(5 * D.per + 1);
+  // Synchronisation words (each on its own 128-byte line): bar_count = CTAs that finished the cycle (monotonic over
+  // launches), bar_launch = cycles completed; per cycle (zeroed by CTA 0 at the end): gbar[k] = phase arrivals of the
+  // CTA group of stage k, pdm_staged = CTAs that have read their PDM slot vector, pdm_done = CTAs past the PDM phase.
   unsigned long long *bar_count = reinterpret_cast<unsigned long long *>(P.bar);
-  unsigned long long *bar_launch = bar_count + 1;
+  unsigned long long *bar_launch = reinterpret_cast<unsigned long long *>(P.bar + 32);
+  unsigned int *gbar = P.bar + kBarGroup0;
+  unsigned int *pdm_staged = gbar + 32 * kMaxStages, *pdm_done = pdm_staged + 32;
 
   if (P.prof_on && tid == 0 && cta < kProfCtas) {
     unsigned long long *pr = P.prof + ((size_t)cta * kProfPhases + (kProfPhases - 1)) * kProfStamps;
@@ -550,23 +553,23 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
     const StepState *st = P.st;
     Sched &S = *Sp;
     S.mode = st->mode; S.c = st->c;
-    int a = 0, items = 0, nonfinal = 0;
+    int a = 0;
     for (int k = 0; k < D.n; ++k) {
       S.occ[k] = st->occ[k]; S.pos[k] = st->pos[k]; S.hbuf[k] = st->hbuf[k];
-      if (st->occ[k]) {
-        int ns = (st->pos[k] + kAttnSplit) / kAttnSplit;
-        S.act[a++] = k; items += D.Hkv * ns; nonfinal += D.Hkv * (ns - 1);
-      }
+      if (st->occ[k]) S.act[a++] = k;
     }
     S.n_act = a;
-    S.attn_total = items;
-    S.attn_nonfinal = nonfinal;
     S.p_new = st->occ[0] ? st->pos[0] : -1;
     S.run_pdm = st->mode == MODE_SPD;
     S.run_verify = (st->mode == MODE_SPD && st->occ[D.n - 1]) || st->mode == MODE_PREFILL_FINAL;
     // CTA c serves active stage c mod a (every group gets the same mix of SMs); PDM slot c mod n
     S.my_stage = a > 0 ? S.act[cta % a] : -1;
     S.my_idx = a > 0 ? cta / a : 0;
+    S.my_gsize = a > 0 ? ncta / a + (cta % a < ncta % a ? 1 : 0) : 0;
+    S.exit_gsize = (a > 0 && st->occ[D.n - 1]) ? ncta / a + (a - 1 < ncta % a ? 1 : 0) : 0;   // stage n-1 = act[a-1]
+    S.attn_ns = a > 0 ? (S.pos[S.my_stage] + kAttnSplit) / kAttnSplit : 0;                      // ceil((pos + 1) / split)
+    S.attn_total = D.Hkv * S.attn_ns;
+    S.attn_nonfinal = D.Hkv * (S.attn_ns - 1);
     S.pdm_slot = cta % D.n;
     S.pdm_idx = cta / D.n;
     for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
@@ -608,9 +611,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
               const int item = (int)next;
               next = atomicAdd(w.ctr, 1u);
               if (item >= S.attn_nonfinal && !kv_ready) {
-                // the last split holds the row appended by other CTAs in this pass's QKV phase: wait for its barrier
-                unsigned long long target = (launch * nbar + (unsigned long long)(p - 2) + 1) * (unsigned long long)ncta;
-                while (ld_acquire_u64(bar_count) < target) {}
+                // the last split holds the row appended by the group's CTAs in this pass's QKV phase: wait for it
+                const unsigned int target = (unsigned int)(p - 1) * (unsigned int)S.my_gsize;
+                while (ld_acquire_u32(gbar + 32 * S.my_stage) < target) {}
                 fence_proxy_async();
                 kv_ready = true;
               }
@@ -659,20 +662,28 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
   } else {
     // =========================== consumers ======================================================
     uint32_t seq = 0;
-    unsigned long long bar_idx = 0;          // barriers passed in this cycle
     float hbest_v[2] = {-INFINITY, -INFINITY};
     int hbest_i[2] = {0x7fffffff, 0x7fffffff};
     const int G = D.Hq / D.Hkv;
     for (int p = 0; p < np; ++p) {
       const int pass = (p - 1) / 5;
-      // ---- wait for the producers of this phase's inputs (all phases but PDM and the first QKV) ----
-      const bool need_barrier = !(p == 0 || p == 1);
-      if (need_barrier) {
-        if (tid == 0) {
-          unsigned long long target = (launch * nbar + bar_idx + 1) * (unsigned long long)ncta;
-          while (ld_acquire_u64(bar_count) < target) {}
+      // ---- wait for the producers of this phase's inputs.  The n stages are independent chains, so a layer
+      //      phase waits only for its own stage's CTA group (the groups drift apart and one group's attention or
+      //      barrier wait is covered by the other groups' weight streams); the first O phase, the first to
+      //      overwrite a residual stream, also waits until every CTA has read its pre-step PDM slot vector;
+      //      the LM head waits for the exit stage's group and for the PDM partial products -----------------
+      if (tid == 0) {
+        if (p == np - 1) {
+          if (S.run_verify && S.exit_gsize > 0) {
+            const unsigned int target = (unsigned int)(np - 2) * (unsigned int)S.exit_gsize;
+            while (ld_acquire_u32(gbar + 32 * (D.n - 1)) < target) {}
+          }
+          if (S.run_pdm) while (ld_acquire_u32(pdm_done) < (unsigned int)ncta) {}
+        } else if (p >= 2 && S.my_stage >= 0) {
+          const unsigned int target = (unsigned int)(p - 1) * (unsigned int)S.my_gsize;
+          while (ld_acquire_u32(gbar + 32 * S.my_stage) < target) {}
+          if (p == 3 && S.run_pdm) while (ld_acquire_u32(pdm_staged) < (unsigned int)ncta) {}
         }
-        ++bar_idx;
       }
       consumer_sync();   // also: every warp is done with the previous phase's xs
       if (tid == 0) {
@@ -764,10 +775,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
             const float *src = S.occ[k] ? P.h + (size_t)S.hbuf[k] * D.d : (q >= 0 ? P.hfin + (size_t)q * D.d : nullptr);
             if (src) stage_copy(src, xs, K);
             else for (int i = tid; i < K; i += kConsumerThreads) xs[i] = 0.f;
-            if (S.pdm_idx == 0) {             // kept for the parity tests (SPD_DBG_PDM_FEAT)
-              consumer_sync();
+            consumer_sync();
+            if (tid == 0) { __threadfence(); atomicAdd(pdm_staged, 1u); }   // the pre-step state has been read
+            if (S.pdm_idx == 0)               // kept for the parity tests (SPD_DBG_PDM_FEAT)
               for (int i = tid; i < K; i += kConsumerThreads) P.feat[(size_t)k * D.d + i] = xs[i];
-            }
           } else {  // PH_HEAD: verify input at xs[0..d), PDM input at xs[kXFloats/2 ..)
             K = D.d;
             if (S.run_verify) {
@@ -868,13 +879,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
         }
         if (t == PH_QKV) fence_proxy_async();   // the appended K/V rows are read by TMA (async proxy) next
       }
-      // ---- publish this phase's outputs: arrive at the barrier that the dependent phase waits on ----
-      const bool arrive = p >= 1;              // PDM has no barrier of its own (see need_barrier)
+      // ---- publish this phase's outputs: arrive at the counter that the dependent phase waits on ----
       if (tid == 0) prof_stamp(P, cta, p, 2);
-      if (arrive) {
+      if (p == np - 1 || (p == 0 && S.run_pdm) || (p > 0 && S.my_stage >= 0)) {
         __threadfence();
         consumer_sync();
-        if (tid == 0) atomicAdd(bar_count, 1ull);
+        if (tid == 0) {
+          if (p == np - 1) atomicAdd(bar_count, 1ull);
+          else if (p == 0) atomicAdd(pdm_done, 1u);
+          else atomicAdd(gbar + 32 * S.my_stage, 1u);
+        }
       }
     }
   }
@@ -882,13 +896,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
   __syncthreads();
   if (cta == 0) {
     if (tid == 0) {
-      unsigned long long target = (launch + 1) * nbar * (unsigned long long)ncta;
+      unsigned long long target = (launch + 1) * (unsigned long long)ncta;
       while (ld_acquire_u64(bar_count) < target) {}
       __threadfence();
     }
     __syncthreads();
     controller_end(P, ncta);
     for (int i = tid; i < np * kMaxStages; i += kThreads) P.claim[i] = 0u;   // every producer is done claiming
+    if (tid < kMaxStages + 2) gbar[32 * tid] = 0u;                           // ... and every CTA with its group counters
     __syncthreads();
     if (tid == 0) {
       __threadfence();
