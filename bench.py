@@ -58,13 +58,16 @@ def measured_peak():
 
 
 def recorded_traffic(kernel: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture, or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(p):
-        try:
-            return json.load(open(p)).get(kernel)
-        except Exception:
-            return None
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/traffic.csv; the command that made it is in the .md named in its `source` column), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        for line in open(p).read().splitlines()[1:]:
+            name, nbytes = line.split(",")[:2]
+            if name == kernel:
+                return int(nbytes)
+    except Exception:
+        return None
     return None
 
 
