@@ -1,0 +1,169 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (-m gpu).
+
+The oracle cannot run a 2048-token 9B-class prefill in test time, so at full size the CUDA path is checked
+(a) on sampled outputs the oracle CAN compute one by one — K/V rows of layer 0 at any position (a function
+    of that position's token only) and the whole depth of the first prompt positions (causal: they do not
+    depend on the 2040 tokens after them);
+(b) via properties that hold at any size (north_star facts 1-3): SPD(n, p) emits exactly the tokens of the
+    n = 1 run (plain greedy decode), rollback leaves K/V rows below the committed length bit-identical to
+    never having run the rejected tokens, per-layer lengths equal the committed length after a reject,
+    step accounting K = G + n - 2 at p = 1; and the two independent CUDA engines agree.
+The 4B-class config runs against the live oracle at its full prompt length (SPD_FULL_GEN=1: full 256 tokens).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle as ora
+import spd_inputs as si
+from tests._parity import run_parity, rel_err, CONTRACT
+
+pytestmark = pytest.mark.gpu
+FULL = os.environ.get("SPD_FULL_GEN", "0") == "1"
+
+
+def _n1_view(shape, w):
+    """The same decoder with n = 1 (plain greedy decode through the same library): W_p's first column block."""
+    s1 = shape.replace(n_stages=1)
+    w1 = dict(w)
+    w1["pdm_proj"] = np.ascontiguousarray(w["pdm_proj"][:, :shape.d_model])
+    return s1, w1
+
+
+def _oracle_layer0_kv(shape, w, tok, pos):
+    """K and V rows of layer 0 for token `tok` at position `pos`, from the oracle's single operations
+    (C-1 Layer: x = RMSNorm(E[tok]); k = RoPE(W_k x, pos) -> bf16; v = W_v x -> bf16)."""
+    h = si.bf16_bits_to_f32(w["embed"][tok])
+    x = ora.op_rmsnorm(h, w["attn_norm"][0], shape.rms_eps)
+    k = ora.op_rope(ora.op_gemv(w["wk"][0], x), shape.n_kv_heads, shape.head_dim, pos, shape.rope_base)
+    v = ora.op_gemv(w["wv"][0], x)
+    return si.f32_to_bf16_bits(k), si.f32_to_bf16_bits(v)
+
+
+def _bf16_close(got_bits, want_bits, what, tol=1e-4, max_flip=0.02):
+    """bf16 rows: one bf16 ulp (a value at a rounding boundary) plus `tol` of the tensor's scale (the fp32-vs-
+    fp64 accumulation difference of the layers below, same bound as tests/_parity.kv_compare)."""
+    g = si.bf16_bits_to_f32(got_bits).astype(np.float64)
+    o = si.bf16_bits_to_f32(want_bits).astype(np.float64)
+    lim = 2.0 ** -7 * np.abs(o) + tol * np.max(np.abs(o))
+    assert np.all(np.abs(g - o) <= lim), what
+    assert np.mean(g != o) <= max_flip, what + ": too many rounding-boundary flips"
+
+
+@pytest.mark.timeout(1500)
+def test_9b_n4_full_prompt_sampled_oracle_outputs_and_invariants():
+    import paper_2605_30852_b200 as spd
+    shape = si.CONFIGS["9b_n4"]
+    n, P, L = shape.n_stages, shape.prompt_len, shape.n_layers
+    G = 40
+    w = si.make_weights(shape, seed=1234)
+    prompt = si.make_prompt(shape, 1234)
+    wd = spd.upload_weights(w)
+    max_seq = P + G * (n + 1) + 4 * n + 16
+    eng = spd.SPD(shape, wd, max_seq=max_seq)
+    first = eng.prefill(prompt)
+    assert np.all(eng.kv_len() == P)
+
+    # ---- (a) sampled outputs the oracle computes one by one -------------------------------------
+    k_gpu, v_gpu = eng.kv(0, 0, P), eng.kv(0, 1, P)
+    for pos in (0, 1, 127, 128, 129, 1000, 2047):
+        k_o, v_o = _oracle_layer0_kv(shape, w, int(prompt[pos]), pos)
+        _bf16_close(k_gpu[pos], k_o, f"layer-0 K row {pos}")
+        _bf16_close(v_gpu[pos], v_o, f"layer-0 V row {pos}")
+    head = 6                                                    # full depth of the first prompt positions
+    o = ora.Oracle(shape, w, max_seq=head + 8)
+    o.prefill(prompt[:head], block=head)
+    for pos in range(head):
+        assert rel_err(eng.hfin(pos), o.hfin(pos)) < 1e-2, f"final hidden state of position {pos}"
+    for layer in (0, L // 2, L - 1):
+        for which in (0, 1):
+            deep = layer > 0
+            _bf16_close(eng.kv(layer, which, head), o.kv(layer, which, head), f"layer {layer} KV rows 0..{head - 1}",
+                        tol=5e-3 if deep else 1e-4, max_flip=1.0 if deep else 0.02)
+    o.close()
+
+    # ---- (b) fact 1/2: SPD(n = 4) tokens == the n = 1 run's tokens (plain greedy decode) ----------
+    s1, w1 = _n1_view(shape, w)
+    wd1 = dict(wd)
+    wd1["pdm_proj"] = spd.upload_weights({"pdm_proj": w1["pdm_proj"]})["pdm_proj"]
+    ar = spd.SPD(s1, wd1, max_seq=P + G + 16)
+    first1 = ar.prefill(prompt)
+    assert first1 == first
+    toks1, log1 = ar.generate(G + n + 2)
+    truth = np.array([first1] + toks1, np.int32)
+    assert all(r.fill == 1 and r.exited for r in log1)
+    # bit-identical prefill state in both pipelines widths (batch invariance of every kernel)
+    for layer in (0, 11, L - 1):
+        for which in (0, 1):
+            assert np.array_equal(ar.kv(layer, which, P), eng.kv(layer, which, P))
+
+    def run(p, seed):
+        eng.rollback(P, first)
+        if p is None:
+            eng.set_forced(None, -1.0, 0)
+        else:
+            eng.set_forced(truth, p, seed)
+        return eng.generate(G, chunk=1)
+
+    for p, seed in ((None, 0), (0.6, 11), (1.0, 0)):
+        toks, log = run(p, seed)
+        assert ([first] + toks)[:G] == list(truth[:G]), f"p={p}: SPD tokens differ from greedy decode"
+        rejects = [r for r in log if r.exited and not r.accepted]
+        if p == 1.0:
+            assert not rejects and len(log) == G + n - 2                  # step accounting (C-3)
+        else:
+            assert rejects
+            assert all(r.discarded == r.fill - 1 for r in rejects)
+        # fact 3: after the run, lengths and rows below c equal the never-speculated n = 1 cache
+        fill, c, _ = eng.ring()
+        lens = eng.kv_len()
+        assert np.all(lens >= c) and np.all(lens <= c + n)
+        eng.rollback(c, int(truth[c - P]))
+        assert np.all(eng.kv_len() == c)
+        rows = min(c, P + len(toks1))
+        for layer in (0, 7, 8, L - 1):                                     # stage boundaries included
+            for which in (0, 1):
+                assert np.array_equal(eng.kv(layer, which, rows)[P:], ar.kv(layer, which, rows)[P:]), \
+                    f"p={p}: KV rows of layer {layer} differ from the never-speculated run"
+    ar.close()
+
+    # ---- the per-op reference engine (independent kernels) agrees with the fused engine -------------
+    # (p = 1: the forced rule is keyed on the cycle counter K, which a rollback does not reset, so only p = 1
+    # gives both engines the same drafts; reject handling of the reference engine is covered at short prompts)
+    eng.rollback(P, first)
+    eng.set_forced(truth, 1.0, 5)
+    a_toks, a_log = eng.generate(12, chunk=1)
+    h_fused = [eng.hidden(k) for k in range(n)]
+    ring_fused = eng.ring()
+    eng.rollback(P, first)
+    eng.set_option(spd.OPT.ENGINE, 0)
+    eng.set_forced(truth, 1.0, 5)
+    b_toks, b_log = eng.generate(12, chunk=1)
+    assert a_toks == b_toks == list(truth[1:12])
+    assert [tuple(r)[1:] for r in a_log] == [tuple(r)[1:] for r in b_log]          # all but step_index
+    assert eng.ring() == ring_fused
+    for k in range(n):
+        if ring_fused[2][k][0]:
+            assert rel_err(eng.hidden(k), h_fused[k]) < 1e-3
+    eng.close()
+
+
+@pytest.mark.timeout(1800)
+def test_4b_n4_full_prompt_against_the_live_oracle():
+    """BASELINE.json configs[1] at its full prompt length (512) against the oracle, cycle by cycle: tokens,
+    accept bits, fills, lengths exact; hidden states / PDM vector / logits within 1e-2 (contract 2e-2)."""
+    import paper_2605_30852_b200 as spd
+    shape = si.CONFIGS["4b_n4"]
+    G = shape.gen_len if FULL else 24
+    w = si.make_weights(shape, seed=1234)
+    prompt = si.make_prompt(shape, 1234)
+    o = ora.Oracle(shape, w, max_seq=shape.prompt_len + G + 16)
+    truth = np.array([o.prefill(prompt, block=16)] + [o.ar_step() for _ in range(G + 6)], np.int32)
+    o.close()
+    rep = run_parity(shape=shape, weights_np=w, dev_weights=spd.upload_weights(w), prompt=prompt, n_tokens=G,
+                     forced=(truth, 0.8, 3), engine=1, tensor_tol=1e-2, tensor_every=4)
+    print("4b_n4 full prompt:", rep.summary())
+    assert rep.status == "ok", rep.detail
+    assert rep.max_hidden_err < CONTRACT and rep.max_logit_err < CONTRACT
+    assert rep.rejects > 0 and rep.accepts > 0
