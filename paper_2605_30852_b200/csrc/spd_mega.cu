@@ -91,6 +91,9 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive_n(uint64_t *bar, uint32_t n) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(n) : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
   uint32_t ok;
   asm volatile(
@@ -452,8 +455,7 @@ __device__ __forceinline__ void attn_merge_warp(const DevPtrs &P, int stage, int
 
 // Fused epilogue of one 16-row unit (lane 0 of every warp; rows r0, r0 + 1 of the repacked matrix).
 __device__ __forceinline__ void unit_epilogue(const DevPtrs &P, const Sched &S, int t, int k, int pass, int r0, float y0,
-                                              float y1, float z0, float z1, const float2 *rope_s, float *hbest_v,
-                                              int *hbest_i) {
+                                              float y1, const float2 *rope_s) {
   const Dims &D = P.dim;
   if (t == PH_QKV) {
     const int qd = D.Hq * D.hd, kd = D.Hkv * D.hd, half = D.hd / 2, pos = S.pos[k];
@@ -493,20 +495,7 @@ __device__ __forceinline__ void unit_epilogue(const DevPtrs &P, const Sched &S, 
   } else if (t == PH_PDM) {
     if (r0 < D.d) P.pdm_part[(size_t)k * D.d + r0] = y0;
     if (r0 + 1 < D.d) P.pdm_part[(size_t)k * D.d + r0 + 1] = y1;
-  } else {                                   // PH_HEAD: running (value, index) argmax
-    if (S.run_verify) {
-      if (r0 < D.V && cand_better(y0, r0, hbest_v[0], hbest_i[0])) { hbest_v[0] = y0; hbest_i[0] = r0; }
-      if (r0 + 1 < D.V && cand_better(y1, r0 + 1, hbest_v[0], hbest_i[0])) { hbest_v[0] = y1; hbest_i[0] = r0 + 1; }
-    }
-    if (S.run_pdm) {
-      if (r0 < D.V && cand_better(z0, r0, hbest_v[1], hbest_i[1])) { hbest_v[1] = z0; hbest_i[1] = r0; }
-      if (r0 + 1 < D.V && cand_better(z1, r0 + 1, hbest_v[1], hbest_i[1])) { hbest_v[1] = z1; hbest_i[1] = r0 + 1; }
-    }
-    if (P.debug_logits) {
-      if (S.run_verify) { if (r0 < D.V) P.logits_v[r0] = y0; if (r0 + 1 < D.V) P.logits_v[r0 + 1] = y1; }
-      if (S.run_pdm) { if (r0 < D.V) P.logits_p[r0] = z0; if (r0 + 1 < D.V) P.logits_p[r0 + 1] = z1; }
-    }
-  }
+  }                                          // PH_HEAD: head_stream() has its own epilogue
 }
 
 template <int HD>
@@ -516,6 +505,101 @@ __device__ __forceinline__ void attn_item_g(const DevPtrs &P, const AttnItem &it
   else if (G == 2) attn_item<HD, 2>(P, it, ring, seq0, nk, scratch, empty);
   else if (G == 8) attn_item<HD, 8>(P, it, ring, seq0, nk, scratch, empty);
   else attn_item<HD, 1>(P, it, ring, seq0, nk, scratch, empty);
+}
+
+// LM-head pass (M = 2: the verify and the PDM vector against the tied matrix E, read once).  With both vectors
+// in shared memory the pass is bound by shared-memory bandwidth (16 KB of TMA writes + 16 KB of weight reads +
+// 32 KB of x reads per tile), not by HBM.  Here K is split across the consumer warps by whole tiles: the warp
+// pair p = warp >> 1 owns the chunks c = p, p + 4, ... of every unit (its two warps take rows 0..7 and 8..15 of
+// the tile), so the pair's 512-column slices of both vectors live in REGISTERS and a tile costs only its own
+// 16 KB of reads.  Per unit a lane accumulates 8 rows x 2 vectors over its columns, a transposed butterfly
+// leaves the warp's partial of quantity q (vector q >> 3, row q & 7 of the warp's half) in lanes 2q, 2q + 1, the
+// warp partials go through shared memory (double-buffered, one named barrier per unit) and are added in warp
+// order by warp (unit count mod 8), whose lanes keep a running (value, index) maximum.  Fixed mapping and
+// order: a logit never depends on which CTA claimed the unit.
+template <int NXS>
+__device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v, bool do_p, const uint8_t *ring,
+                                            uint64_t *full, uint64_t *empty, const int *meta, float *xs, uint32_t &seq,
+                                            float *cbest_v, int *cbest_i) {
+  const Dims &D = P.dim;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int pair = warp >> 1, half = warp & 1;
+  float4 xv[NXS][4], xp[NXS][4];
+#pragma unroll
+  for (int s = 0; s < NXS; ++s) {
+    const int c = pair + 4 * s;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      xv[s][i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      xp[s][i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (c < nc) {
+        if (do_v) xv[s][i] = reinterpret_cast<const float4 *>(xs)[c * (kTileCols / 4) + 32 * i + lane];
+        if (do_p) xp[s][i] = reinterpret_cast<const float4 *>(xs + kXFloats / 2)[c * (kTileCols / 4) + 32 * i + lane];
+      }
+    }
+  }
+  consumer_sync();                       // both vectors are in registers: xs is free for the warp partials
+  float *part = xs;                      // [2][8 warps][16 quantities]
+  float bv = -INFINITY;
+  int bi = 0x7fffffff;
+  int ucount = 0;
+  while (true) {
+    const uint32_t s0 = seq;
+    mbar_wait(&full[s0 % kStages], (s0 / kStages) & 1);
+    const int u = meta[s0 % kStages];
+    if (u == kEndMark) {
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[s0 % kStages]);
+      ++seq;
+      break;
+    }
+    float acc[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) acc[i] = 0.f;
+#pragma unroll
+    for (int s = 0; s < NXS; ++s) {
+      const int c = pair + 4 * s;
+      if (c < nc) {
+        const uint32_t sq = s0 + c, slot = sq % kStages;
+        mbar_wait(&full[slot], (sq / kStages) & 1);
+        const uint4 *wt = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kTileBytes) + half * (8 * 64);
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+          const uint4 w0 = wt[r * 64 + lane], w1 = wt[r * 64 + 32 + lane];
+          if (do_v) { acc[r] = fma8(w0, xv[s][0], xv[s][1], acc[r]); acc[r] = fma8(w1, xv[s][2], xv[s][3], acc[r]); }
+          if (do_p) { acc[8 + r] = fma8(w0, xp[s][0], xp[s][1], acc[8 + r]); acc[8 + r] = fma8(w1, xp[s][2], xp[s][3], acc[8 + r]); }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive_n(&empty[slot], 4);   // the pair's two warps are the tile's only readers
+      }
+    }
+    seq += nc;
+    int q = 0;
+    XReduce<16, 16>::run(acc, lane, q);                  // q == lane >> 1: quantity (vector q >> 3, row q & 7)
+    if ((lane & 1) == 0) part[(ucount & 1) * 128 + warp * 16 + q] = acc[0];
+    consumer_sync();
+    if (warp == (ucount & 7)) {
+      const int vec = lane >> 4, r16 = lane & 15;        // this lane's logit: row r16 of the unit, vector vec
+      const float *pp = part + (ucount & 1) * 128 + (r16 >> 3) * 16 + vec * 8 + (r16 & 7);
+      float y = 0.f;
+#pragma unroll
+      for (int pr = 0; pr < 4; ++pr) y += pp[pr * 32];   // warps 2 pr + (r16 >> 3), pr ascending
+      const int row = u * kTileRows + r16;
+      if ((vec ? do_p : do_v) && row < D.V) {
+        if (cand_better(y, row, bv, bi)) { bv = y; bi = row; }
+        if (P.debug_logits) (vec ? P.logits_p : P.logits_v)[row] = y;
+      }
+    }
+    ++ucount;
+  }
+  // lanes 0..15 hold verify candidates, lanes 16..31 PDM candidates: reduce inside each half
+#pragma unroll
+  for (int o = 8; o > 0; o >>= 1) {
+    const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+    if (cand_better(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+  }
+  if ((lane & 15) == 0) { cbest_v[(lane >> 4) * 8 + warp] = bv; cbest_i[(lane >> 4) * 8 + warp] = bi; }
 }
 
 // The fused kernel ---------------------------------------------------------------------------------
@@ -662,8 +746,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
   } else {
     // =========================== consumers ======================================================
     uint32_t seq = 0;
-    float hbest_v[2] = {-INFINITY, -INFINITY};
-    int hbest_i[2] = {0x7fffffff, 0x7fffffff};
     const int G = D.Hq / D.Hkv;
     for (int p = 0; p < np; ++p) {
       const int pass = (p - 1) / 5;
@@ -818,14 +900,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
         consumer_sync();
         if (tid == 0) prof_stamp(P, cta, p, 1);
         // ---- stream the claimed units ------------------------------------------------------------
-        const bool two = t == PH_HEAD;
         const float4 *xv4 = reinterpret_cast<const float4 *>(xs);
-        const float4 *xp4 = reinterpret_cast<const float4 *>(xs + kXFloats / 2);
-        const bool do_v = !two || S.run_verify, do_p = two && S.run_pdm;
-        while (true) {
+        if (t == PH_HEAD) {
+          const bool do_v = S.run_verify, do_p = S.run_pdm;
+          if (w.nc <= 4) head_stream<1>(P, w.nc, do_v, do_p, ring, full, empty, meta, xs, seq, cbest_v, cbest_i);
+          else if (w.nc <= 8) head_stream<2>(P, w.nc, do_v, do_p, ring, full, empty, meta, xs, seq, cbest_v, cbest_i);
+          else head_stream<3>(P, w.nc, do_v, do_p, ring, full, empty, meta, xs, seq, cbest_v, cbest_i);
+        } else while (true) {
           int u = 0;
-          float a00 = 0.f, a01 = 0.f, a10 = 0.f, a11 = 0.f;   // [row][column group], first vector
-          float b00 = 0.f, b01 = 0.f, b10 = 0.f, b11 = 0.f;   // second vector (LM head only)
+          float a00 = 0.f, a01 = 0.f, a10 = 0.f, a11 = 0.f;   // [row][column group]
           bool end = false;
           for (int c = 0; c < w.nc || c == 0; ++c, ++seq) {
             uint32_t slot = seq % kStages, itn = seq / kStages;
@@ -843,30 +926,19 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
             const uint4 *wt = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kTileBytes);
             uint4 wa0 = wt[(2 * warp) * 64 + lane], wa1 = wt[(2 * warp) * 64 + 32 + lane];
             uint4 wb0 = wt[(2 * warp + 1) * 64 + lane], wb1 = wt[(2 * warp + 1) * 64 + 32 + lane];
-            if (do_v) {
-              const float4 *x4 = xv4 + c * (kTileCols / 4);
-              float4 x00 = x4[lane], x01 = x4[32 + lane], x10 = x4[64 + lane], x11 = x4[96 + lane];
-              a00 = fma8(wa0, x00, x01, a00); a01 = fma8(wa1, x10, x11, a01);
-              a10 = fma8(wb0, x00, x01, a10); a11 = fma8(wb1, x10, x11, a11);
-            }
-            if (do_p) {
-              const float4 *x4 = xp4 + c * (kTileCols / 4);
-              float4 x00 = x4[lane], x01 = x4[32 + lane], x10 = x4[64 + lane], x11 = x4[96 + lane];
-              b00 = fma8(wa0, x00, x01, b00); b01 = fma8(wa1, x10, x11, b01);
-              b10 = fma8(wb0, x00, x01, b10); b11 = fma8(wb1, x10, x11, b11);
-            }
+            const float4 *x4 = xv4 + c * (kTileCols / 4);
+            float4 x00 = x4[lane], x01 = x4[32 + lane], x10 = x4[64 + lane], x11 = x4[96 + lane];
+            a00 = fma8(wa0, x00, x01, a00); a01 = fma8(wa1, x10, x11, a01);
+            a10 = fma8(wb0, x00, x01, a10); a11 = fma8(wb1, x10, x11, a11);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[slot]);
           }
           if (end) break;
           // ---- unit done: reduce the two rows of this warp, fused epilogue (lane 0) ---------------
           float y0 = warp_sum(a00 + a01), y1 = warp_sum(a10 + a11);
-          float z0 = 0.f, z1 = 0.f;
-          if (two) { z0 = warp_sum(b00 + b01); z1 = warp_sum(b10 + b11); }
-          if (lane == 0) unit_epilogue(P, S, t, k, pass, u * kTileRows + 2 * warp, y0, y1, z0, z1, rope_s, hbest_v, hbest_i);
+          if (lane == 0) unit_epilogue(P, S, t, k, pass, u * kTileRows + 2 * warp, y0, y1, rope_s);
         }
         if (t == PH_HEAD) {   // CTA-level candidates -> global
-          if (lane == 0) { cbest_v[warp] = hbest_v[0]; cbest_v[8 + warp] = hbest_v[1]; cbest_i[warp] = hbest_i[0]; cbest_i[8 + warp] = hbest_i[1]; }
           consumer_sync();
           if (tid < 2) {
             float bv = -INFINITY;
