@@ -507,6 +507,73 @@ __device__ __forceinline__ void attn_item_g(const DevPtrs &P, const AttnItem &it
   else attn_item<HD, 1>(P, it, ring, seq0, nk, scratch, empty);
 }
 
+// Slot protocol of the tile-per-warp-pair mapping.  Only the owner pair of a tile reads its data, but EVERY
+// consumer warp still waits on every slot's full barrier in ring order and arrives on its empty barrier (the
+// non-owners right away, without touching the tile).  A slot is therefore recycled only after all 8 warps have
+// passed it, exactly as when all warps read every tile: a parity wait can never observe a slot two phases late.
+// One GEMV phase (M = 1) over the units the producer claimed for this CTA.  A tile (16 rows x 512 columns) is
+// consumed by ONE warp pair: pair p = warp >> 1 owns the chunks c = p, p + 4, ... of every unit and its two
+// warps take rows 0..7 / 8..15 of the tile, so a tile's slice of x is read from shared memory by 2 warps
+// instead of 8 (the old row-per-warp mapping moved 48 KB of shared-memory traffic per 16 KB tile and capped an
+// SM at ~60 GB/s; this one moves 36 KB).  Per unit a lane accumulates 8 rows over its columns, a transposed
+// butterfly leaves the warp's partial of row q = lane >> 2 of its half in 4 lanes, the partials go through
+// shared memory (double-buffered, one named barrier per unit) and warp (unit count mod 8) adds the 4 pair
+// partials of every row in pair order and runs the fused epilogue on row pairs (even lanes 0..14).
+__device__ __forceinline__ void gemv_stream(const DevPtrs &P, const Sched &S, int t, int k, int pass, int nc,
+                                            const uint8_t *ring, uint64_t *full, uint64_t *empty, const int *meta,
+                                            const float *xs, float *part, uint32_t &seq, const float2 *rope_s) {
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int pair = warp >> 1, half = warp & 1;
+  const float4 *xv4 = reinterpret_cast<const float4 *>(xs);
+  int ucount = 0;
+  while (true) {
+    const uint32_t s0 = seq;
+    mbar_wait(&full[s0 % kStages], (s0 / kStages) & 1);
+    const int u = meta[s0 % kStages];
+    if (u == kEndMark) {
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[s0 % kStages]);
+      ++seq;
+      break;
+    }
+    float acc[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] = 0.f;
+    for (int c = 0; c < nc; ++c) {
+      const uint32_t sq = s0 + c, slot = sq % kStages;
+      if (c > 0) mbar_wait(&full[slot], (sq / kStages) & 1);
+      if ((c & 3) == pair) {
+        const uint4 *wt = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kTileBytes) + half * (8 * 64);
+        const float4 *x4 = xv4 + c * (kTileCols / 4);
+        const float4 x00 = x4[lane], x01 = x4[32 + lane], x10 = x4[64 + lane], x11 = x4[96 + lane];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+          const uint4 w0 = wt[r * 64 + lane], w1 = wt[r * 64 + 32 + lane];
+          acc[r] = fma8(w0, x00, x01, acc[r]);
+          acc[r] = fma8(w1, x10, x11, acc[r]);
+        }
+        __syncwarp();
+      }
+      if (lane == 0) mbar_arrive(&empty[slot]);
+    }
+    seq += nc;
+    int q = 0;
+    XReduce<8, 16>::run(acc, lane, q);                   // q == lane >> 2: row q of this warp's half
+    if ((lane & 3) == 0) part[(ucount & 1) * 64 + warp * 8 + q] = acc[0];
+    consumer_sync();
+    if (warp == (ucount & 7)) {
+      const int r16 = lane & 15;
+      const float *pp = part + (ucount & 1) * 64 + (r16 >> 3) * 8 + (r16 & 7);
+      float y = 0.f;
+#pragma unroll
+      for (int pr = 0; pr < 4; ++pr) y += pp[pr * 16];   // warps 2 pr + (r16 >> 3), pr ascending
+      const float y1 = __shfl_down_sync(0xffffffffu, y, 1);
+      if (lane < 16 && (lane & 1) == 0) unit_epilogue(P, S, t, k, pass, u * kTileRows + r16, y, y1, rope_s);
+    }
+    ++ucount;
+  }
+}
+
 // LM-head pass (M = 2: the verify and the PDM vector against the tied matrix E, read once).  With both vectors
 // in shared memory the pass is bound by shared-memory bandwidth (16 KB of TMA writes + 16 KB of weight reads +
 // 32 KB of x reads per tile), not by HBM.  Here K is split across the consumer warps by whole tiles: the warp
@@ -556,12 +623,17 @@ __device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v,
     float acc[16];
 #pragma unroll
     for (int i = 0; i < 16; ++i) acc[i] = 0.f;
+    if (pair != 0 && lane == 0) mbar_arrive(&empty[s0 % kStages]);   // first slot: the other warps right away
+    // The unit's first slot is passed by all 8 warps (it carries the unit tag); every other tile is waited on and
+    // released by its owner pair alone, so a tile is recycled as soon as its two readers are done.  An owner's
+    // slot last held a tile of the previous unit (or this unit's first tile, nc <= 12): consumed before the
+    // per-unit barrier this warp has passed, so the parity wait always targets the slot's next phase.
 #pragma unroll
     for (int s = 0; s < NXS; ++s) {
       const int c = pair + 4 * s;
       if (c < nc) {
         const uint32_t sq = s0 + c, slot = sq % kStages;
-        mbar_wait(&full[slot], (sq / kStages) & 1);
+        if (c > 0) mbar_wait(&full[slot], (sq / kStages) & 1);
         const uint4 *wt = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kTileBytes) + half * (8 * 64);
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
@@ -570,8 +642,9 @@ __device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v,
           if (do_p) { acc[8 + r] = fma8(w0, xp[s][0], xp[s][1], acc[8 + r]); acc[8 + r] = fma8(w1, xp[s][2], xp[s][3], acc[8 + r]); }
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive_n(&empty[slot], 4);   // the pair's two warps are the tile's only readers
+        if (c > 0 && lane == 0) mbar_arrive_n(&empty[slot], 4);
       }
+      if (s == 0 && pair == 0 && lane == 0) mbar_arrive(&empty[s0 % kStages]);   // first slot: pair 0 after reading it
     }
     seq += nc;
     int q = 0;
@@ -604,7 +677,7 @@ __device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v,
 
 // The fused kernel ---------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout ML) {
-  extern __shared__ __align__(1024) uint8_t smem[];
+  extern __shared__ __align__(128) uint8_t smem[];
   uint8_t *ring = smem;                                                  // kStages * 16 KB
   float *xs = reinterpret_cast<float *>(smem + kStages * kTileBytes);    // kXFloats
   uint64_t *full = reinterpret_cast<uint64_t *>(xs + kXFloats);          // [kStages]
@@ -614,7 +687,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
   float *cbest_v = red + 16;                                             // [2][8]
   int *cbest_i = reinterpret_cast<int *>(cbest_v + 16);                  // [2][8]
   int *meta = cbest_i + 16;                                              // [kStages] slot tags (+ padding to 16)
-  Sched *Sp = reinterpret_cast<Sched *>(meta + 16);
+  float *gpart = reinterpret_cast<float *>(meta + 16);                     // [2][8][8] warp partials of a unit
+  Sched *Sp = reinterpret_cast<Sched *>(gpart + 128);
 
   const Dims &D = P.dim;
   const int cta = blockIdx.x, ncta = gridDim.x;
@@ -900,43 +974,19 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
         consumer_sync();
         if (tid == 0) prof_stamp(P, cta, p, 1);
         // ---- stream the claimed units ------------------------------------------------------------
-        const float4 *xv4 = reinterpret_cast<const float4 *>(xs);
-        if (t == PH_HEAD) {
+        if (k < 0) {                               // nothing to stream: one END slot, read by every warp
+          const uint32_t slot = seq % kStages;
+          mbar_wait(&full[slot], (seq / kStages) & 1);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&empty[slot]);
+          ++seq;
+        } else if (t == PH_HEAD) {
           const bool do_v = S.run_verify, do_p = S.run_pdm;
           if (w.nc <= 4) head_stream<1>(P, w.nc, do_v, do_p, ring, full, empty, meta, xs, seq, cbest_v, cbest_i);
           else if (w.nc <= 8) head_stream<2>(P, w.nc, do_v, do_p, ring, full, empty, meta, xs, seq, cbest_v, cbest_i);
           else head_stream<3>(P, w.nc, do_v, do_p, ring, full, empty, meta, xs, seq, cbest_v, cbest_i);
-        } else while (true) {
-          int u = 0;
-          float a00 = 0.f, a01 = 0.f, a10 = 0.f, a11 = 0.f;   // [row][column group]
-          bool end = false;
-          for (int c = 0; c < w.nc || c == 0; ++c, ++seq) {
-            uint32_t slot = seq % kStages, itn = seq / kStages;
-            mbar_wait(&full[slot], itn & 1);
-            if (c == 0) {
-              u = meta[slot];
-              if (u == kEndMark) {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[slot]);
-                ++seq;
-                end = true;
-                break;
-              }
-            }
-            const uint4 *wt = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kTileBytes);
-            uint4 wa0 = wt[(2 * warp) * 64 + lane], wa1 = wt[(2 * warp) * 64 + 32 + lane];
-            uint4 wb0 = wt[(2 * warp + 1) * 64 + lane], wb1 = wt[(2 * warp + 1) * 64 + 32 + lane];
-            const float4 *x4 = xv4 + c * (kTileCols / 4);
-            float4 x00 = x4[lane], x01 = x4[32 + lane], x10 = x4[64 + lane], x11 = x4[96 + lane];
-            a00 = fma8(wa0, x00, x01, a00); a01 = fma8(wa1, x10, x11, a01);
-            a10 = fma8(wb0, x00, x01, a10); a11 = fma8(wb1, x10, x11, a11);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[slot]);
-          }
-          if (end) break;
-          // ---- unit done: reduce the two rows of this warp, fused epilogue (lane 0) ---------------
-          float y0 = warp_sum(a00 + a01), y1 = warp_sum(a10 + a11);
-          if (lane == 0) unit_epilogue(P, S, t, k, pass, u * kTileRows + 2 * warp, y0, y1, rope_s);
+        } else {
+          gemv_stream(P, S, t, k, pass, w.nc, ring, full, empty, meta, xs, gpart, seq, rope_s);
         }
         if (t == PH_HEAD) {   // CTA-level candidates -> global
           consumer_sync();
@@ -1078,7 +1128,7 @@ int mega_create(const DevPtrs &P, const uint16_t *const *const *src, void *repac
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-  int smem = kStages * kTileBytes + kXFloats * 4 + 2 * kStages * 8 + 64 * 8 + 16 * 4 + 32 * 4 + 16 * 4 + (int)sizeof(Sched) + 64;
+  int smem = kStages * kTileBytes + kXFloats * 4 + 2 * kStages * 8 + 64 * 8 + 16 * 4 + 32 * 4 + 16 * 4 + 128 * 4 + (int)sizeof(Sched);
   if (!coop || sms < D.n) return -1;
   if (cudaFuncSetAttribute(k_spd_cycle, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
     cudaGetLastError();
