@@ -52,11 +52,13 @@ def _bf16_close(got_bits, want_bits, what, tol=1e-4, max_flip=0.02):
 
 
 @pytest.mark.timeout(1500)
-def test_9b_n4_full_prompt_sampled_oracle_outputs_and_invariants():
+@pytest.mark.parametrize("name,G", [("9b_n4", 40), ("4b_n8", 28), ("9b_n16", 24)])
+def test_full_prompt_sampled_oracle_outputs_and_invariants(name, G):
+    """BASELINE.json configs[3] (the graded one), configs[2] (n = 8, prompt 1024) and configs[4] (n = 16,
+    prompt 4096) at their full prompt lengths."""
     import paper_2605_30852_b200 as spd
-    shape = si.CONFIGS["9b_n4"]
+    shape = si.CONFIGS[name]
     n, P, L = shape.n_stages, shape.prompt_len, shape.n_layers
-    G = 40
     w = si.make_weights(shape, seed=1234)
     prompt = si.make_prompt(shape, 1234)
     wd = spd.upload_weights(w)
@@ -67,7 +69,7 @@ def test_9b_n4_full_prompt_sampled_oracle_outputs_and_invariants():
 
     # ---- (a) sampled outputs the oracle computes one by one -------------------------------------
     k_gpu, v_gpu = eng.kv(0, 0, P), eng.kv(0, 1, P)
-    for pos in (0, 1, 127, 128, 129, 1000, 2047):
+    for pos in (0, 1, 127, 128, 129, P // 2 + 1, P - 1):
         k_o, v_o = _oracle_layer0_kv(shape, w, int(prompt[pos]), pos)
         _bf16_close(k_gpu[pos], k_o, f"layer-0 K row {pos}")
         _bf16_close(v_gpu[pos], v_o, f"layer-0 V row {pos}")
@@ -87,7 +89,7 @@ def test_9b_n4_full_prompt_sampled_oracle_outputs_and_invariants():
     s1, w1 = _n1_view(shape, w)
     wd1 = dict(wd)
     wd1["pdm_proj"] = spd.upload_weights({"pdm_proj": w1["pdm_proj"]})["pdm_proj"]
-    ar = spd.SPD(s1, wd1, max_seq=P + G + 16)
+    ar = spd.SPD(s1, wd1, max_seq=P + G + n + 24)
     first1 = ar.prefill(prompt)
     assert first1 == first
     toks1, log1 = ar.generate(G + n + 2)
@@ -106,7 +108,7 @@ def test_9b_n4_full_prompt_sampled_oracle_outputs_and_invariants():
             eng.set_forced(truth, p, seed)
         return eng.generate(G, chunk=1)
 
-    for p, seed in ((None, 0), (0.6, 11), (1.0, 0)):
+    for p, seed in ((None, 0), (0.6 if n <= 8 else 0.8, 11), (1.0, 0)):
         toks, log = run(p, seed)
         assert ([first] + toks)[:G] == list(truth[:G]), f"p={p}: SPD tokens differ from greedy decode"
         rejects = [r for r in log if r.exited and not r.accepted]
@@ -122,7 +124,7 @@ def test_9b_n4_full_prompt_sampled_oracle_outputs_and_invariants():
         eng.rollback(c, int(truth[c - P]))
         assert np.all(eng.kv_len() == c)
         rows = min(c, P + len(toks1))
-        for layer in (0, 7, 8, L - 1):                                     # stage boundaries included
+        for layer in (0, L // n - 1, L // n, L - 1):                       # a stage boundary included
             for which in (0, 1):
                 assert np.array_equal(eng.kv(layer, which, rows)[P:], ar.kv(layer, which, rows)[P:]), \
                     f"p={p}: KV rows of layer {layer} differ from the never-speculated run"
@@ -140,7 +142,7 @@ def test_9b_n4_full_prompt_sampled_oracle_outputs_and_invariants():
     eng.set_option(spd.OPT.ENGINE, 0)
     eng.set_forced(truth, 1.0, 5)
     b_toks, b_log = eng.generate(12, chunk=1)
-    assert a_toks == b_toks == list(truth[1:12])
+    assert a_toks[:11] == b_toks[:11] == list(truth[1:12])
     assert [tuple(r)[1:] for r in a_log] == [tuple(r)[1:] for r in b_log]          # all but step_index
     assert eng.ring() == ring_fused
     for k in range(n):
