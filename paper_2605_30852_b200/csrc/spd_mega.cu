@@ -15,17 +15,20 @@
 //     each phase with an END slot.  Unit claims do not depend on activations, so the producer runs
 //     AHEAD of the activation dependency, across phase boundaries: while the consumers wait at a grid
 //     barrier the next phase's tiles are already landing.
-//   * consumers: warp w owns rows 2w, 2w+1 of a tile; 128-bit conflict-free LDS of weights and of
-//     the fp32 activation vector (staged in smem once per phase with 128-bit L2 loads), fp32 FMA,
-//     warp-shuffle reduction at the end of a unit, fused epilogues (RoPE + bf16 KV append, residual add,
-//     SiLU*mul, PDM partials, LM-head argmax).
+//   * consumers: a tile is read by ONE warp pair (pair = chunk index mod 4; its two warps take rows 0..7 /
+//     8..15) with 128-bit conflict-free LDS of the weights and of the fp32 activation vector (staged in smem
+//     once per phase with 128-bit L2 loads), fp32 FMA, a transposed butterfly per warp, the 8 warp partials
+//     of a 16-row unit meet in shared memory under one named barrier, and one warp runs the fused epilogue
+//     (RoPE + bf16 KV append, residual add, SiLU*mul, PDM partials).  The LM head (two vectors against the
+//     tied matrix) keeps both vectors in registers.  Every warp still passes every slot's barriers in ring
+//     order (gemv_stream) or the unit's first slot (head_stream), which keeps slot recycling race-free.
 //   * attention: items (stage, kv head, 128-row split) are claimed dynamically by all CTAs; the
 //     producer brings the K and V rows of an item through the same ring (TMA), the 8 consumer warps
 //     compute the G q heads of the kv group together (scores with a transposed butterfly reduction,
 //     softmax per head, P.V with a fixed cross-warp reduction); the last split of a head merges.
-//   * phases are separated by a device-wide arrive/poll barrier on a monotonically increasing
-//     64-bit counter; cross-CTA activations are read with ld.global.cg.
-// Every row's dot product is computed by one warp with a fixed lane/column mapping and chunk order,
+//   * phases are separated by arrive/poll barriers per stage group (red.release / ld.acquire at gpu scope on
+//     per-cycle counters); cross-CTA activations are read with ld.global.cg.
+// Every row's dot product is computed with a fixed warp/lane/column mapping and a fixed order of partial sums,
 // attention splits are fixed 128-row blocks merged in split order, so a token's result never depends
 // on n, slot, fill, history or on which CTA happened to claim the work (batch invariance).
 #include <stdio.h>
@@ -130,6 +133,12 @@ __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long
   return v;
 }
 
+__device__ __forceinline__ void red_release_add_u32(unsigned int *p, unsigned int v) {
+  asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_release_add_u64(unsigned long long *p, unsigned long long v) {
+  asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
 __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int *p) {
   unsigned int v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -1004,12 +1013,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
       // ---- publish this phase's outputs: arrive at the counter that the dependent phase waits on ----
       if (tid == 0) prof_stamp(P, cta, p, 2);
       if (p == np - 1 || (p == 0 && S.run_pdm) || (p > 0 && S.my_stage >= 0)) {
-        __threadfence();
+        // one release at gpu scope by thread 0 after the CTA barrier publishes every consumer's writes of this
+        // phase (release is cumulative over what the barrier ordered before it); the waiters acquire
         consumer_sync();
         if (tid == 0) {
-          if (p == np - 1) atomicAdd(bar_count, 1ull);
-          else if (p == 0) atomicAdd(pdm_done, 1u);
-          else atomicAdd(gbar + 32 * S.my_stage, 1u);
+          if (p == np - 1) red_release_add_u64(bar_count, 1ull);
+          else if (p == 0) red_release_add_u32(pdm_done, 1u);
+          else red_release_add_u32(gbar + 32 * S.my_stage, 1u);
         }
       }
     }
