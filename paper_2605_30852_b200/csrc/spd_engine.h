@@ -15,6 +15,8 @@ struct MegaPlan {
   int smem_bytes;
   int available;
   unsigned long long layout[24];   // opaque MegaLayout (offsets of the repacked matrices)
+  alignas(64) unsigned char kv_tmap[128];   // CUtensorMap over the K/V cache (128-byte-swizzled 64 x 64 boxes)
+  int has_kv_tmap;          // 0: the driver entry point is missing -> attention stays on the scalar path
 };
 size_t mega_repack_bytes(const Dims &D);
 // src: the nine host tables of per-layer device pointers in spd_weights order.  Returns 0 on success.

@@ -31,6 +31,7 @@
 // Every row's dot product is computed with a fixed warp/lane/column mapping and a fixed order of partial sums,
 // attention splits are fixed 128-row blocks merged in split order, so a token's result never depends
 // on n, slot, fill, history or on which CTA happened to claim the work (batch invariance).
+#include <cuda.h>
 #include <stdio.h>
 #include <string.h>
 
@@ -48,6 +49,7 @@ constexpr int kConsumerThreads = 256;
 constexpr int kThreads = kConsumerThreads + 32;
 constexpr int kEndMark = -1;                             // slot tag: no more work in this phase
 constexpr int kAttnScratchFloats = 2 * 8 * kAttnSplit + 8 * 8 * 128;   // scores, probabilities, per-warp partial outputs (G <= 8, hd <= 128)
+constexpr int kQPairStride = 68;                         // u32 (bf16 pairs) per q head in the staged hi / lo arrays: 64 + 4 (bank spread)
 constexpr int kAttnDoneMax = 32;                         // items whose completion counts are published together
 static_assert(kAttnScratchFloats + kAttnDoneMax * 9 + 1 <= kXFloats, "attention scratch must fit the activation buffer");
 
@@ -58,6 +60,7 @@ struct MegaLayout {
   unsigned long long layer_bytes, off_o, off_gu, off_dn, off_pdm, off_head, pdm_job_bytes;
   int u_qkv, u_o, u_gu, u_dn, u_pdm, u_head;   // 16-row units per job
   int nc_d, nc_qd, nc_f;                        // 512-column chunks for K = d, Hq*hd, F
+  int attn_mma;                                 // full 128-row attention items go through the tensor cores
 };
 
 // Per-cycle schedule, computed identically by every CTA from the device state.
@@ -114,6 +117,35 @@ __device__ __forceinline__ void tma_load_1d(void *dst_smem, const void *src_gmem
   asm volatile(
       "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
       ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy) : "memory");
+}
+// One 64 x 64 bf16 box (8 KB, 128-byte swizzled) of the K/V tensor map -> shared memory.
+__device__ __forceinline__ void tma_load_box(void *dst_smem, const CUtensorMap *tmap, int c0, int c1, int c2, uint64_t *bar,
+                                             uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;"
+      ::"r"(smem_u32(dst_smem)), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)), "l"(policy) : "memory");
+}
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], uint32_t addr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], uint32_t addr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+// D (16 x 8, fp32) += A (16 x 16, bf16, row) * B (16 x 8, bf16, col)
+__device__ __forceinline__ void mma_bf16_16816(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
+                                               uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+// fp32 pair -> (bf16 hi pair, bf16 lo pair) with x = hi + lo to 16 mantissa bits: products with exact bf16 operands
+// accumulated in fp32 keep ~fp32 accuracy.  Low half of a register = first element.
+__device__ __forceinline__ void split_bf16x2(float x0, float x1, uint32_t &hi, uint32_t &lo) {
+  const uint16_t h0 = f32_to_bf16(x0), h1 = f32_to_bf16(x1);
+  const uint16_t l0 = f32_to_bf16(x0 - bf16_to_f32(h0)), l1 = f32_to_bf16(x1 - bf16_to_f32(h1));
+  hi = (uint32_t)h0 | ((uint32_t)h1 << 16);
+  lo = (uint32_t)l0 | ((uint32_t)l1 << 16);
 }
 // Orders generic-proxy accesses (st.global of the KV append) against async-proxy accesses (TMA reads).
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
@@ -425,6 +457,132 @@ __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, 
   }
 }
 
+// Tensor-core version of attn_item for a FULL split (128 rows) at head_dim 128.  The scalar path spends ~1000 issue
+// slots per warp and item (4 q heads x 128 dims x 128 rows of fp32 FMAs on unpacked bf16) and makes the attention
+// phase issue-bound; here scores (Q K^T) and P.V run as mma.sync m16n8k16 with the G q heads in rows 0..G-1 of the
+// 16-row A operand.  q and the probabilities are fp32 (C-2.17), so each is split into bf16 hi + lo parts (hi in rows
+// 0..G-1, lo in rows 8..8+G-1 of the same A operand, the two result rows are added): K and V are exact bf16,
+// products are exact and accumulate in fp32, which keeps ~2^-17 relative accuracy per element.  K/V arrive as 128-byte-swizzled 64 x 64 boxes (tma_load_box): chunk c of row r sits at
+// r * 128 + ((c ^ (r & 7)) << 4), so every ldmatrix phase touches 8 distinct 16-byte bank groups.  Warp w owns rows
+// 16 w .. 16 w + 15 of the split (fixed), splits are merged in split order: results do not depend on who ran the item.
+template <int G>
+__device__ __forceinline__ void attn_item_mma(const DevPtrs &P, const AttnItem &it, const uint8_t *ring, uint32_t seq0,
+                                              float *scratch, uint64_t *empty, const uint32_t *qs) {
+  constexpr int HD = 128, nk = 2;
+  const Dims &D = P.dim;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, t = lane & 3;          // mma fragment coordinates
+  const int mi = lane >> 3, mr = lane & 7;        // ldmatrix: this lane addresses row mr of matrix mi
+  float *sc = scratch, *ps = scratch + G * kAttnSplit, *red = scratch + 2 * G * kAttnSplit;
+  const int hq0 = it.kvh * G;
+  const int rb = warp >> 2, r0 = (warp & 3) * 16; // this warp's rows: slot rb, local rows r0 .. r0 + 15
+
+  // ---- scores S[head][row] = q . K[row]: A = Q (head g in row g < G, other rows zero), B = K^T ----
+  {
+    uint32_t qh[8][2], ql[8][2];                  // per k-step: a0 (dims 16 ks + 2t, +1), a2 (dims 16 ks + 8 + 2t, +1)
+#pragma unroll
+    for (int ks = 0; ks < 8; ++ks) { qh[ks][0] = qh[ks][1] = ql[ks][0] = ql[ks][1] = 0u; }
+    if (g < G) {
+      if (qs) {                                   // staged once per phase: hi pairs, then lo pairs, kQPairStride per head
+        const uint32_t *h = qs + (size_t)(hq0 + g) * kQPairStride, *l = h + (size_t)D.Hq * kQPairStride;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+          qh[ks][0] = h[8 * ks + t]; qh[ks][1] = h[8 * ks + 4 + t];
+          ql[ks][0] = l[8 * ks + t]; ql[ks][1] = l[8 * ks + 4 + t];
+        }
+      } else {
+        const float *q = P.q + ((size_t)it.stage * D.Hq + hq0 + g) * HD;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+          const float2 x = __ldcg(reinterpret_cast<const float2 *>(q + 16 * ks + 2 * t));
+          const float2 y = __ldcg(reinterpret_cast<const float2 *>(q + 16 * ks + 8 + 2 * t));
+          split_bf16x2(x.x, x.y, qh[ks][0], ql[ks][0]);
+          split_bf16x2(y.x, y.y, qh[ks][1], ql[ks][1]);
+        }
+      }
+    }
+    float sa[2][4];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) { sa[i][0] = sa[i][1] = sa[i][2] = sa[i][3] = 0.f; }
+    const uint32_t kbase = smem_u32(ring + (size_t)((seq0 + rb) % kStages) * kTileBytes);
+    const int krow = r0 + (mi >> 1) * 8 + mr;     // matrices 0, 1: rows 0..7 (dims lo, hi); 2, 3: rows 8..15
+#pragma unroll
+    for (int ks = 0; ks < 8; ++ks) {
+      const int cc = 2 * ks + (mi & 1);           // 16-byte chunk of the 256-byte row
+      uint32_t b[4];
+      ldmatrix_x4(b, kbase + (cc >> 3) * (kTileBytes / 2) + krow * 128 + (((cc & 7) ^ (krow & 7)) << 4));
+      mma_bf16_16816(sa[0], qh[ks][0], ql[ks][0], qh[ks][1], ql[ks][1], b[0], b[1]);   // rows g: hi part, rows g + 8: lo part
+      mma_bf16_16816(sa[1], qh[ks][0], ql[ks][0], qh[ks][1], ql[ks][1], b[2], b[3]);
+    }
+    if (g < G) {
+      const float scale = 1.0f / sqrtf((float)HD);
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt)
+        *reinterpret_cast<float2 *>(sc + g * kAttnSplit + 16 * warp + nt * 8 + 2 * t) =
+            make_float2((sa[nt][0] + sa[nt][2]) * scale, (sa[nt][1] + sa[nt][3]) * scale);
+    }
+  }
+  consumer_sync();
+  if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + j) % kStages]);   // K slots are free
+  // ---- softmax of the split, one warp per head: m = max, p = exp(s - m), l = sum p ----
+  if (warp < G) {
+    float s[kAttnSplit / 32], m = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < kAttnSplit / 32; ++j) { s[j] = sc[warp * kAttnSplit + lane + 32 * j]; m = fmaxf(m, s[j]); }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    float l = 0.f;
+#pragma unroll
+    for (int j = 0; j < kAttnSplit / 32; ++j) {
+      const float p = expf(s[j] - m);
+      ps[(lane + 32 * j) * G + warp] = p;
+      l += p;
+    }
+    l = warp_sum(l);
+    if (lane == 0) P.part_ml[((size_t)it.stage * D.Hq + hq0 + warp) * P.nsplit_max + it.split] = make_float2(m, l);
+  }
+  consumer_sync();
+  // ---- P.V: O[head][dim] = sum over this warp's 16 rows: A = P (k = rows), B = V via ldmatrix.trans ----
+  {
+    uint32_t ph[2] = {0u, 0u}, pl[2] = {0u, 0u};  // a0: rows 2t, 2t+1; a2: rows 2t+8, 2t+9 (of the warp's 16)
+    if (g < G) {
+      const float *pr = ps + (size_t)(16 * warp) * G + g;
+      split_bf16x2(pr[(2 * t) * G], pr[(2 * t + 1) * G], ph[0], pl[0]);
+      split_bf16x2(pr[(2 * t + 8) * G], pr[(2 * t + 9) * G], ph[1], pl[1]);
+    }
+    float oa[16][4];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) { oa[j][0] = oa[j][1] = oa[j][2] = oa[j][3] = 0.f; }
+    const uint32_t vbase = smem_u32(ring + (size_t)((seq0 + nk + rb) % kStages) * kTileBytes);
+    const int vrow = r0 + (mi & 1) * 8 + mr;      // matrices 0, 1: rows 0..7, 8..15 of dims tile 2 jj; 2, 3: of tile 2 jj + 1
+#pragma unroll
+    for (int jj = 0; jj < 8; ++jj) {
+      const int cc = 2 * jj + (mi >> 1);
+      uint32_t b[4];
+      ldmatrix_x4_trans(b, vbase + (cc >> 3) * (kTileBytes / 2) + vrow * 128 + (((cc & 7) ^ (vrow & 7)) << 4));
+      mma_bf16_16816(oa[2 * jj], ph[0], pl[0], ph[1], pl[1], b[0], b[1]);              // rows g: hi part, rows g + 8: lo part
+      mma_bf16_16816(oa[2 * jj + 1], ph[0], pl[0], ph[1], pl[1], b[2], b[3]);
+    }
+    __syncwarp();
+    if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + nk + j) % kStages]);   // V slots are free
+    if (g < G) {
+#pragma unroll
+      for (int j = 0; j < 16; ++j)
+        *reinterpret_cast<float2 *>(red + ((size_t)warp * G + g) * HD + 8 * j + 2 * t) =
+            make_float2(oa[j][0] + oa[j][2], oa[j][1] + oa[j][3]);
+    }
+  }
+  consumer_sync();
+  // ---- cross-warp sum in warp order (fixed), unnormalised partial output of the split ----
+  for (int o = tid; o < G * HD; o += kConsumerThreads) {
+    const int h = o / HD, e = o - h * HD;
+    float acc = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) acc += red[((size_t)w * G + h) * HD + e];
+    P.part_o[(((size_t)it.stage * D.Hq + hq0 + h) * P.nsplit_max + it.split) * HD + e] = acc;
+  }
+}
+
 // Merge of the splits of one q head by one warp, in split order (fixed): out = sum_j o_j e^(m_j-M) / sum_j l_j e^(m_j-M).
 // Lane owns EPL consecutive elements; the loads of different splits are independent and batched.
 template <int HD>
@@ -685,8 +843,8 @@ __device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v,
 }
 
 // The fused kernel ---------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout ML) {
-  extern __shared__ __align__(128) uint8_t smem[];
+__global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout ML, const __grid_constant__ CUtensorMap kv_tmap) {
+  extern __shared__ __align__(1024) uint8_t smem[];   // ring slots must be 1024-byte aligned (128-byte swizzle)
   uint8_t *ring = smem;                                                  // kStages * 16 KB
   float *xs = reinterpret_cast<float *>(smem + kStages * kTileBytes);    // kXFloats
   uint64_t *full = reinterpret_cast<uint64_t *>(xs + kXFloats);          // [kStages]
@@ -786,8 +944,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
               }
               const int layer = it.stage * D.per + pass;
               const int nk = (it.rows + RPS - 1) / RPS;
+              const bool boxed = ML.attn_mma && it.rows == kAttnSplit;   // full split: swizzled boxes for the MMA path
               for (int kvsel = 0; kvsel < 2; ++kvsel) {
                 const uint16_t *src = P.kv + kv_offset(D, layer, kvsel, it.kvh) + (size_t)it.t0 * D.hd;
+                const int plane = (layer * 2 + kvsel) * D.Hkv + it.kvh;
                 for (int j = 0; j < nk; ++j, ++seq) {
                   uint32_t slot = seq % kStages, itn = seq / kStages;
                   int r = min(RPS, it.rows - j * RPS);
@@ -795,7 +955,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
                   mbar_wait(&empty[slot], (itn & 1) ^ 1);
                   meta[slot] = item;
                   mbar_expect_tx(&full[slot], bytes);
-                  tma_load_1d(ring + (size_t)slot * kTileBytes, src + (size_t)j * RPS * D.hd, bytes, &full[slot], pol_kv);
+                  uint8_t *dst = ring + (size_t)slot * kTileBytes;
+                  if (boxed) {           // 64 rows: head-dim halves [0, 64) and [64, 128) as two 8 KB boxes
+                    tma_load_box(dst, &kv_tmap, 0, it.t0 + j * RPS, plane, &full[slot], pol_kv);
+                    tma_load_box(dst + kTileBytes / 2, &kv_tmap, 64, it.t0 + j * RPS, plane, &full[slot], pol_kv);
+                  } else {
+                    tma_load_1d(dst, src + (size_t)j * RPS * D.hd, bytes, &full[slot], pol_kv);
+                  }
                   if (first) { prof_stamp(P, cta, p, 3); first = false; }
                 }
               }
@@ -868,6 +1034,24 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
         int *merge_list = merge_cnt + 1;                                     // [kAttnDoneMax * 8] (item slot, head)
         int n_done = 0;
         bool more = true;
+        // q of this CTA's stage, split into bf16 hi / lo pairs, staged once per phase for the tensor-core items
+        // (behind the score / probability / partial-output scratch, if it fits in front of the done lists)
+        const uint32_t *qs = nullptr;
+        if (ML.attn_mma && S.my_stage >= 0 && S.attn_ns > 1 &&
+            10 * G * kAttnSplit + 2 * D.Hq * kQPairStride <= kAttnScratchFloats) {
+          uint32_t *qw = reinterpret_cast<uint32_t *>(xs) + 10 * G * kAttnSplit;
+          const float2 *q2 = reinterpret_cast<const float2 *>(P.q + (size_t)S.my_stage * D.Hq * D.hd);
+          for (int i = tid; i < D.Hq * 64; i += kConsumerThreads) {
+            const float2 v = __ldcg(q2 + i);
+            uint32_t hi, lo;
+            split_bf16x2(v.x, v.y, hi, lo);
+            const int o = (i >> 6) * kQPairStride + (i & 63);
+            qw[o] = hi;
+            qw[D.Hq * kQPairStride + o] = lo;
+          }
+          qs = qw;
+          consumer_sync();
+        }
         while (more) {
           uint32_t slot = seq % kStages, itn = seq / kStages;
           mbar_wait(&full[slot], itn & 1);
@@ -882,7 +1066,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
             attn_decode(S, D, item, it);
             const int nk = (it.rows + RPS - 1) / RPS;
             for (int j = 1; j < 2 * nk; ++j) mbar_wait(&full[(seq + j) % kStages], ((seq + j) / kStages) & 1);
-            if (D.hd == 128) attn_item_g<128>(P, it, ring, seq, nk, xs, empty, G);
+            if (ML.attn_mma && it.rows == kAttnSplit) {
+              if (G == 4) attn_item_mma<4>(P, it, ring, seq, xs, empty, qs);
+              else if (G == 8) attn_item_mma<8>(P, it, ring, seq, xs, empty, qs);
+              else if (G == 2) attn_item_mma<2>(P, it, ring, seq, xs, empty, qs);
+              else attn_item_mma<1>(P, it, ring, seq, xs, empty, qs);
+            } else if (D.hd == 128) attn_item_g<128>(P, it, ring, seq, nk, xs, empty, G);
             else attn_item_g<64>(P, it, ring, seq, nk, xs, empty, G);
             seq += 2 * nk;
             if (tid == 0) done_list[n_done] = item;
@@ -1149,6 +1338,36 @@ int mega_create(const DevPtrs &P, const uint16_t *const *const *src, void *repac
     cudaGetLastError();
     return -1;
   }
+  // K/V cache as a rank-3 bf16 tensor {hd, max_seq, L * 2 * Hkv}; boxes of 64 head-dim elements (128 bytes) x 64
+  // rows land 128-byte-swizzled, so ldmatrix on a landed tile is bank-conflict-free.  The encoder is a driver
+  // entry point fetched at run time (the library does not link libcuda).
+  plan->has_kv_tmap = 0;
+  ML.attn_mma = 0;
+  if (D.hd == 128 && (D.Hq / D.Hkv) <= 8) {
+    typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                 const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess && fn &&
+        qres == cudaDriverEntryPointSuccess) {
+      CUtensorMap tm;
+      cuuint64_t gdim[3] = {(cuuint64_t)D.hd, (cuuint64_t)D.max_seq, (cuuint64_t)D.L * 2 * D.Hkv};
+      cuuint64_t gstr[2] = {(cuuint64_t)D.hd * 2, (cuuint64_t)D.max_seq * D.hd * 2};
+      cuuint32_t box[3] = {64, 64, 1}, estr[3] = {1, 1, 1};
+      CUresult r = ((EncodeFn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, (void *)P.kv, gdim, gstr, box, estr,
+                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r == CUDA_SUCCESS) {
+        static_assert(sizeof(CUtensorMap) == sizeof(plan->kv_tmap), "tensor map storage");
+        memcpy(plan->kv_tmap, &tm, sizeof tm);
+        plan->has_kv_tmap = 1;
+        ML.attn_mma = 1;
+      }
+    } else {
+      cudaGetLastError();
+    }
+  }
   ML.repack = (const uint8_t *)repack;
   uint8_t *base = (uint8_t *)repack;
   int qd = D.Hq * D.hd, kd = D.Hkv * D.hd;
@@ -1185,7 +1404,9 @@ int mega_enqueue_step(const DevPtrs &P, const MegaPlan &plan, cudaStream_t sm, l
   MegaLayout ML;
   memcpy(&ML, plan.layout, sizeof ML);
   DevPtrs Pc = P;
-  void *args[] = {(void *)&Pc, (void *)&ML};
+  CUtensorMap tm;
+  memcpy(&tm, plan.kv_tmap, sizeof tm);
+  void *args[] = {(void *)&Pc, (void *)&ML, (void *)&tm};
   cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_spd_cycle, dim3(plan.n_cta), dim3(kThreads), args,
                                               (size_t)plan.smem_bytes, sm);
   if (launches) *launches += 1;
