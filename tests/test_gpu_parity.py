@@ -101,3 +101,18 @@ def test_full_model_dims_short_prompt(engine, name, prompt_len, gen):
     print(name, rep.summary())
     assert rep.status == "ok", rep.detail
     assert rep.max_hidden_err < CONTRACT and rep.max_logit_err < CONTRACT
+
+
+@pytest.mark.parametrize("hq,hkv", [(8, 2), (8, 1), (4, 2), (2, 2)])
+def test_tensor_core_attention_path_midsize(hq, hkv):
+    """head_dim 128 with a 300-token prompt: two full 128-row splits per head go through the fused engine's
+    mma.sync attention (swizzled K/V boxes, q and probabilities split into bf16 hi + lo), the ragged third
+    split through the scalar path; G = 4, 8 (q read from global), 2, 1.  Attention-heavy weights (C-4) make an
+    attention error visible in the hidden state; compared with the oracle cycle by cycle at 5e-4."""
+    _need_engine(1)
+    shape = si.ModelShape("mid", 512, 4, 2, hq, hkv, 128, 1024, 2048, 300, 24, ())
+    inp = _inputs(shape, 300, std=0.04, attention_heavy=True)
+    rep = run_parity(**inp, n_tokens=24, engine=1, tensor_tol=5e-4)
+    print(f"mid Hq={hq} Hkv={hkv}:", rep.summary())
+    assert rep.status == "ok", rep.detail
+    assert rep.max_hidden_err < 5e-4 and rep.max_logit_err < 5e-4
