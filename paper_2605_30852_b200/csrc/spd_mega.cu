@@ -464,7 +464,9 @@ __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, 
 // 0..G-1, lo in rows 8..8+G-1 of the same A operand, the two result rows are added): K and V are exact bf16,
 // products are exact and accumulate in fp32, which keeps ~2^-17 relative accuracy per element.  K/V arrive as 128-byte-swizzled 64 x 64 boxes (tma_load_box): chunk c of row r sits at
 // r * 128 + ((c ^ (r & 7)) << 4), so every ldmatrix phase touches 8 distinct 16-byte bank groups.  Warp w owns rows
-// 16 w .. 16 w + 15 of the split (fixed), splits are merged in split order: results do not depend on who ran the item.
+// 16 w .. 16 w + 15 of the split (fixed) and runs scores -> softmax over its 16 rows -> P.V entirely in registers (the
+// score fragment of thread (g, t) is the P.V A fragment); the 8 warps' (max, sum, output) are merged in warp order
+// after one CTA barrier, the splits in split order: results do not depend on who ran the item.
 template <int G>
 __device__ __forceinline__ void attn_item_mma(const DevPtrs &P, const AttnItem &it, const uint8_t *ring, uint32_t seq0,
                                               float *scratch, uint64_t *empty, const uint32_t *qs) {
@@ -473,9 +475,11 @@ __device__ __forceinline__ void attn_item_mma(const DevPtrs &P, const AttnItem &
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, t = lane & 3;          // mma fragment coordinates
   const int mi = lane >> 3, mr = lane & 7;        // ldmatrix: this lane addresses row mr of matrix mi
-  float *sc = scratch, *ps = scratch + G * kAttnSplit, *red = scratch + 2 * G * kAttnSplit;
+  float2 *wml = reinterpret_cast<float2 *>(scratch);   // [8 warps][G] (max, sum) of a warp's 16 rows
+  float *red = scratch + 2 * G * kAttnSplit;           // [8 warps][G][HD] unnormalised outputs (same place as attn_item)
   const int hq0 = it.kvh * G;
   const int rb = warp >> 2, r0 = (warp & 3) * 16; // this warp's rows: slot rb, local rows r0 .. r0 + 15
+  float p0, p1, p2, p3;                           // probabilities of head g at rows 2t, 2t+1, 8+2t, 9+2t
 
   // ---- scores S[head][row] = q . K[row]: A = Q (head g in row g < G, other rows zero), B = K^T ----
   {
@@ -514,41 +518,28 @@ __device__ __forceinline__ void attn_item_mma(const DevPtrs &P, const AttnItem &
       mma_bf16_16816(sa[0], qh[ks][0], ql[ks][0], qh[ks][1], ql[ks][1], b[0], b[1]);   // rows g: hi part, rows g + 8: lo part
       mma_bf16_16816(sa[1], qh[ks][0], ql[ks][0], qh[ks][1], ql[ks][1], b[2], b[3]);
     }
-    if (g < G) {
-      const float scale = 1.0f / sqrtf((float)HD);
-#pragma unroll
-      for (int nt = 0; nt < 2; ++nt)
-        *reinterpret_cast<float2 *>(sc + g * kAttnSplit + 16 * warp + nt * 8 + 2 * t) =
-            make_float2((sa[nt][0] + sa[nt][2]) * scale, (sa[nt][1] + sa[nt][3]) * scale);
-    }
+    // ---- softmax of this warp's 16 rows, in registers (flash-attention style): thread (g, t) holds the scores of
+    //      head g for rows 2t, 2t+1, 8+2t, 9+2t, which is exactly the A fragment P.V needs ----
+    const float scale = 1.0f / sqrtf((float)HD);
+    const float s0 = (sa[0][0] + sa[0][2]) * scale, s1 = (sa[0][1] + sa[0][3]) * scale;
+    const float s2 = (sa[1][0] + sa[1][2]) * scale, s3 = (sa[1][1] + sa[1][3]) * scale;
+    float m = fmaxf(fmaxf(s0, s1), fmaxf(s2, s3));
+    m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+    m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+    p0 = expf(s0 - m); p1 = expf(s1 - m); p2 = expf(s2 - m); p3 = expf(s3 - m);
+    float l = (p0 + p1) + (p2 + p3);
+    l += __shfl_xor_sync(0xffffffffu, l, 1);
+    l += __shfl_xor_sync(0xffffffffu, l, 2);
+    if (g < G && t == 0) wml[warp * G + g] = make_float2(m, l);
   }
-  consumer_sync();
-  if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + j) % kStages]);   // K slots are free
-  // ---- softmax of the split, one warp per head: m = max, p = exp(s - m), l = sum p ----
-  if (warp < G) {
-    float s[kAttnSplit / 32], m = -INFINITY;
-#pragma unroll
-    for (int j = 0; j < kAttnSplit / 32; ++j) { s[j] = sc[warp * kAttnSplit + lane + 32 * j]; m = fmaxf(m, s[j]); }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-    float l = 0.f;
-#pragma unroll
-    for (int j = 0; j < kAttnSplit / 32; ++j) {
-      const float p = expf(s[j] - m);
-      ps[(lane + 32 * j) * G + warp] = p;
-      l += p;
-    }
-    l = warp_sum(l);
-    if (lane == 0) P.part_ml[((size_t)it.stage * D.Hq + hq0 + warp) * P.nsplit_max + it.split] = make_float2(m, l);
-  }
-  consumer_sync();
+  __syncwarp();
+  if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + j) % kStages]);   // this warp is done with K
   // ---- P.V: O[head][dim] = sum over this warp's 16 rows: A = P (k = rows), B = V via ldmatrix.trans ----
   {
     uint32_t ph[2] = {0u, 0u}, pl[2] = {0u, 0u};  // a0: rows 2t, 2t+1; a2: rows 2t+8, 2t+9 (of the warp's 16)
     if (g < G) {
-      const float *pr = ps + (size_t)(16 * warp) * G + g;
-      split_bf16x2(pr[(2 * t) * G], pr[(2 * t + 1) * G], ph[0], pl[0]);
-      split_bf16x2(pr[(2 * t + 8) * G], pr[(2 * t + 9) * G], ph[1], pl[1]);
+      split_bf16x2(p0, p1, ph[0], pl[0]);
+      split_bf16x2(p2, p3, ph[1], pl[1]);
     }
     float oa[16][4];
 #pragma unroll
@@ -564,7 +555,7 @@ __device__ __forceinline__ void attn_item_mma(const DevPtrs &P, const AttnItem &
       mma_bf16_16816(oa[2 * jj + 1], ph[0], pl[0], ph[1], pl[1], b[2], b[3]);
     }
     __syncwarp();
-    if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + nk + j) % kStages]);   // V slots are free
+    if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + nk + j) % kStages]);   // ... and with V
     if (g < G) {
 #pragma unroll
       for (int j = 0; j < 16; ++j)
@@ -573,14 +564,26 @@ __device__ __forceinline__ void attn_item_mma(const DevPtrs &P, const AttnItem &
     }
   }
   consumer_sync();
-  // ---- cross-warp sum in warp order (fixed), unnormalised partial output of the split ----
+  // ---- the 8 warps' (max, sum, unnormalised output) of every head, merged in warp order (fixed):
+  //      M = max m_w, o = sum_w o_w e^(m_w - M), l = sum_w l_w e^(m_w - M) -> the split's partial ----
   for (int o = tid; o < G * HD; o += kConsumerThreads) {
     const int h = o / HD, e = o - h * HD;
-    float acc = 0.f;
+    float M = -INFINITY;
 #pragma unroll
-    for (int w = 0; w < 8; ++w) acc += red[((size_t)w * G + h) * HD + e];
-    P.part_o[(((size_t)it.stage * D.Hq + hq0 + h) * P.nsplit_max + it.split) * HD + e] = acc;
+    for (int w = 0; w < 8; ++w) M = fmaxf(M, wml[w * G + h].x);
+    float acc = 0.f, L = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+      const float2 ml = wml[w * G + h];
+      const float f = expf(ml.x - M);
+      acc = fmaf(red[((size_t)w * G + h) * HD + e], f, acc);
+      L = fmaf(ml.y, f, L);
+    }
+    const size_t slot = ((size_t)it.stage * D.Hq + hq0 + h) * P.nsplit_max + it.split;
+    P.part_o[slot * HD + e] = acc;
+    if (e == 0) P.part_ml[slot] = make_float2(M, L);
   }
+  consumer_sync();                                // red / wml are rewritten by the next item
 }
 
 // Merge of the splits of one q head by one warp, in split order (fixed): out = sum_j o_j e^(m_j-M) / sum_j l_j e^(m_j-M).
