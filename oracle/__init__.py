@@ -6,7 +6,9 @@ other.  `Oracle` is a thin ctypes wrapper over oracle/spd_oracle.c (all arithmet
 `nocache_ref` is a separately written float64 numpy full-sequence model used to pin the C oracle.
 """
 from .oracle import Oracle, StepResult, lib, op_rmsnorm, op_gemv, op_rope, op_attention, \
-    op_silu_mul, op_argmax, op_f32_to_bf16, op_splitmix64, num_threads
+    op_silu_mul, op_argmax, op_f32_to_bf16, op_splitmix64, num_threads, Dist, op_topk_softmax, op_uniform, \
+    op_sample_cdf, op_accept, op_sample_residual
 
 __all__ = ["Oracle", "StepResult", "lib", "op_rmsnorm", "op_gemv", "op_rope", "op_attention",
-           "op_silu_mul", "op_argmax", "op_f32_to_bf16", "op_splitmix64", "num_threads"]
+           "op_silu_mul", "op_argmax", "op_f32_to_bf16", "op_splitmix64", "num_threads", "Dist", "op_topk_softmax", "op_uniform", "op_sample_cdf",
+           "op_accept", "op_sample_residual"]

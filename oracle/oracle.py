@@ -30,6 +30,48 @@ class _Res(C.Structure):
                                           "draft_token", "draft_forced", "discarded", "committed_len")]
 
 
+MAX_TOPK = 64
+
+
+class _Dist(C.Structure):
+    _fields_ = [("k", C.c_int32), ("id", C.c_int32 * MAX_TOPK), ("p", C.c_float * MAX_TOPK)]
+
+
+class _Hints(C.Structure):
+    _fields_ = [("draft_k", C.c_int32), ("draft_ids", C.c_int32 * MAX_TOPK),
+                ("verify_k", C.c_int32), ("verify_ids", C.c_int32 * MAX_TOPK),
+                ("draft_token", C.c_int32), ("accepted", C.c_int32), ("emitted_token", C.c_int32),
+                ("logit_band", C.c_float), ("prob_eps", C.c_float)]
+
+
+class _SampleRec(C.Structure):
+    _fields_ = [("draft", _Dist), ("target", _Dist),
+                ("u_draft", C.c_double), ("u_accept", C.c_double), ("u_resid", C.c_double),
+                ("succ_token", C.c_int32), ("succ_q", C.c_float), ("succ_p", C.c_float),
+                ("ties_support", C.c_int32), ("ties_draft", C.c_int32), ("ties_accept", C.c_int32),
+                ("ties_resid", C.c_int32)]
+
+
+class Dist(NamedTuple):
+    """A filtered distribution: support in ascending token id, fp32 probabilities."""
+    ids: np.ndarray
+    p: np.ndarray
+
+
+def _dist_out(d: _Dist) -> Dist:
+    k = d.k
+    return Dist(np.array(d.id[:k], dtype=np.int32), np.array(d.p[:k], dtype=np.float32))
+
+
+def _dist_in(d: Dist) -> _Dist:
+    out = _Dist()
+    out.k = len(d.ids)
+    for i, (t, p) in enumerate(zip(d.ids, d.p)):
+        out.id[i] = int(t)
+        out.p[i] = float(p)
+    return out
+
+
 class StepResult(NamedTuple):
     step_index: int
     fill: int
@@ -87,6 +129,15 @@ def lib():
         L.ora_op_splitmix64.argtypes = [C.c_uint64]
         L.ora_op_splitmix64.restype = C.c_uint64
         L.ora_num_threads.restype = C.c_int32
+        L.ora_op_topk_softmax.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.POINTER(_Dist)]
+        L.ora_op_uniform.argtypes = [C.c_uint64, C.c_int64, C.c_int32]
+        L.ora_op_uniform.restype = C.c_double
+        L.ora_op_sample_cdf.argtypes = [C.POINTER(_Dist), C.c_double]
+        L.ora_op_accept.argtypes = [C.POINTER(_Dist), C.POINTER(_Dist), C.c_int32, C.c_double]
+        L.ora_op_sample_residual.argtypes = [C.POINTER(_Dist), C.POINTER(_Dist), C.c_double]
+        L.ora_set_sampling.argtypes = [C.c_void_p, C.c_float, C.c_int32, C.c_uint64]
+        L.ora_step_sample_follow.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_Hints), C.POINTER(_Res)]
+        L.ora_get_sample_record.argtypes = [C.c_void_p, C.POINTER(_SampleRec)]
         _lib = L
     return _lib
 
@@ -181,6 +232,34 @@ class Oracle:
             rc = lib().ora_set_forced(self._h, _p(t), len(t), p, seed)
         if rc:
             raise ValueError("ora_set_forced")
+
+    def set_sampling(self, temperature: float, top_k: int, seed: int):
+        if lib().ora_set_sampling(self._h, temperature, top_k, seed):
+            raise ValueError("ora_set_sampling")
+
+    def step_sample_follow(self, draft_ids=None, verify_ids=None, draft_token: int = -1, accepted: int = -1,
+                           emitted_token: int = -1, logit_band: float = 0.0, prob_eps: float = 0.0,
+                           draft_override: int = -1) -> StepResult:
+        h = _Hints()
+        for name, ids in (("draft", draft_ids), ("verify", verify_ids)):
+            n = 0 if ids is None else len(ids)
+            setattr(h, name + "_k", n)
+            for i in range(n):
+                getattr(h, name + "_ids")[i] = int(ids[i])
+        h.draft_token, h.accepted, h.emitted_token = draft_token, accepted, emitted_token
+        h.logit_band, h.prob_eps = logit_band, prob_eps
+        r = _Res()
+        rc = lib().ora_step_sample_follow(self._h, draft_override, C.byref(h), C.byref(r))
+        if rc:
+            raise RuntimeError(f"ora_step_sample_follow rc={rc}")
+        return StepResult(*[getattr(r, k) for k, _ in _Res._fields_])
+
+    def sample_record(self) -> dict:
+        r = _SampleRec()
+        lib().ora_get_sample_record(self._h, C.byref(r))
+        return dict(draft=_dist_out(r.draft), target=_dist_out(r.target), u_draft=r.u_draft, u_accept=r.u_accept,
+                    u_resid=r.u_resid, succ_token=r.succ_token, succ_q=r.succ_q, succ_p=r.succ_p,
+                    ties=(r.ties_support, r.ties_draft, r.ties_accept, r.ties_resid))
 
     def ar_step(self) -> int:
         nxt = C.c_int32(-1)
@@ -331,3 +410,29 @@ def op_splitmix64(x: int) -> int:
 
 def num_threads() -> int:
     return lib().ora_num_threads()
+
+
+# -- NEXT-2 sampling operations ------------------------------------------------------------------
+
+def op_topk_softmax(logits, top_k: int, temperature: float, support=None) -> Dist:
+    x = _f32(logits)
+    d = _Dist()
+    sup = None if support is None else np.ascontiguousarray(support, dtype=np.int32)
+    lib().ora_op_topk_softmax(_p(x), x.size, top_k, temperature, None if sup is None else _p(sup), C.byref(d))
+    return _dist_out(d)
+
+
+def op_uniform(seed: int, K: int, j: int) -> float:
+    return lib().ora_op_uniform(seed & 0xFFFFFFFFFFFFFFFF, K, j)
+
+
+def op_sample_cdf(dist: Dist, u: float) -> int:
+    return lib().ora_op_sample_cdf(C.byref(_dist_in(dist)), u)
+
+
+def op_accept(P: Dist, Q: Dist, token: int, u: float) -> int:
+    return lib().ora_op_accept(C.byref(_dist_in(P)), C.byref(_dist_in(Q)), token, u)
+
+
+def op_sample_residual(P: Dist, Q: Dist, u: float) -> int:
+    return lib().ora_op_sample_residual(C.byref(_dist_in(P)), C.byref(_dist_in(Q)), u)

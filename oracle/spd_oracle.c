@@ -75,7 +75,8 @@ void ora_op_rmsnorm(const float *x, const uint16_t *gain, int32_t d, float eps, 
 
 /* out = W x, W bf16 [rows, k] row-major. */
 void ora_op_gemv(const uint16_t *w, int32_t rows, int32_t k, const float *x, float *out) {
-#pragma omp parallel for schedule(static)
+  /* rows are independent, so threading never changes a value; tiny products stay on the calling thread */
+#pragma omp parallel for schedule(static) if ((size_t)rows * (size_t)k >= 32768)
   for (int r = 0; r < rows; ++r) out[r] = (float)dot_row(w + (size_t)r * k, x, k);
 }
 
@@ -83,7 +84,7 @@ void ora_op_gemv(const uint16_t *w, int32_t rows, int32_t k, const float *x, flo
  * weight row is read once per block; each (t, r) value is the same dot_row call as in ora_op_gemv. */
 static void gemv_block(const uint16_t *w, int rows, int k, const float *x, int ldx, float *y, int ldy,
                        int nt) {
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if ((size_t)rows * (size_t)k * (size_t)nt >= 32768)
   for (int r = 0; r < rows; ++r)
     for (int t = 0; t < nt; ++t) y[(size_t)t * ldy + r] = (float)dot_row(w + (size_t)r * k, x + (size_t)t * ldx, k);
 }
@@ -112,7 +113,7 @@ void ora_op_attention(const float *q, const uint16_t *kc, const uint16_t *vc, in
                       int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, float *out) {
   int group = n_q_heads / n_kv_heads;
   size_t row = (size_t)n_kv_heads * head_dim;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if ((size_t)n_q_heads * (size_t)t_len * (size_t)head_dim >= 32768)
   for (int hq = 0; hq < n_q_heads; ++hq) {
     int kvh = hq / group;
     const float *qh = q + (size_t)hq * head_dim;
@@ -189,11 +190,175 @@ struct ora_ctx {
   int32_t ties[2];   /* tie hints adopted: [0] verify, [1] PDM */
   float *ar_trace;
   int32_t reverse_forward;
+  /* NEXT-2 sampling verification */
+  int32_t sampling_on, top_k;
+  float temperature;
+  uint64_t samp_seed;
+  ora_dist *r_q;     /* [n] the draft distribution each in-flight token was drawn from */
+  ora_sample_record rec;
   /* scratch */
   float *x, *q, *kk, *vv, *att, *o, *g, *u, *act, *dn, *z;
 };
 
 static size_t kv_row(const ora_config *c) { return (size_t)c->n_kv_heads * c->head_dim; }
+
+/* ------------------------------------------------------------------ NEXT-2: sampling ops ------ */
+
+/* S-6: 24-bit uniform in [0, 1), exactly representable in fp32 and fp64. */
+double ora_op_uniform(uint64_t seed, int64_t K, int32_t j) {
+  uint64_t r = ora_op_splitmix64(seed + 3ull * (uint64_t)K + (uint64_t)j) >> 40;
+  return (double)r * (1.0 / 16777216.0);
+}
+
+/* S-2: top-k filter + temperature softmax ("top-k=50 and top-p=1.0", T = 1). */
+void ora_op_topk_softmax(const float *logits, int32_t vocab, int32_t top_k, float temperature,
+                         const int32_t *support, ora_dist *out) {
+  int k = top_k < vocab ? top_k : vocab;
+  if (k > ORA_MAX_TOPK) k = ORA_MAX_TOPK;
+  int ids[ORA_MAX_TOPK];
+  if (support) {
+    for (int i = 0; i < k; ++i) ids[i] = support[i];
+  } else {
+    /* k passes; pass r takes the best entry not taken yet: larger value first, lower index on ties */
+    for (int r = 0; r < k; ++r) {
+      int best = -1;
+      for (int i = 0; i < vocab; ++i) {
+        int taken = 0;
+        for (int t = 0; t < r; ++t) taken |= ids[t] == i;
+        if (taken) continue;
+        if (best < 0 || logits[i] > logits[best]) best = i;
+      }
+      ids[r] = best;
+    }
+  }
+  /* ascending token id */
+  for (int i = 1; i < k; ++i) {
+    int v = ids[i], j = i - 1;
+    while (j >= 0 && ids[j] > v) { ids[j + 1] = ids[j]; --j; }
+    ids[j + 1] = v;
+  }
+  double m = -INFINITY, e[ORA_MAX_TOPK], Z = 0.0;
+  for (int i = 0; i < k; ++i)
+    if ((double)logits[ids[i]] > m) m = (double)logits[ids[i]];
+  for (int i = 0; i < k; ++i) {
+    e[i] = exp(((double)logits[ids[i]] - m) / (double)temperature);
+    Z += e[i];
+  }
+  memset(out, 0, sizeof *out);
+  out->k = k;
+  for (int i = 0; i < k; ++i) { out->id[i] = ids[i]; out->p[i] = (float)(e[i] / Z); }
+}
+
+/* S-3: inverse CDF over weights w[0..k) in list order: the smallest i with u * W < w_0 + .. + w_i.
+ * lo/hi (may be NULL) receive that entry's interval [C_{i-1}, C_i) / W for every entry. */
+static int pick_index(const double *w, int k, double u, double *lo, double *hi) {
+  double W = 0.0;
+  for (int i = 0; i < k; ++i) W += w[i];
+  double c = 0.0;
+  int chosen = -1, last = -1;
+  for (int i = 0; i < k; ++i) {
+    if (lo) lo[i] = c / W;
+    c += w[i];
+    if (hi) hi[i] = c / W;
+    if (w[i] > 0.0) last = i;
+    if (chosen < 0 && u * W < c) chosen = i;
+  }
+  return chosen >= 0 ? chosen : last;
+}
+
+static double dist_prob(const ora_dist *D, int token) {
+  for (int i = 0; i < D->k; ++i)
+    if (D->id[i] == token) return (double)D->p[i];
+  return 0.0;
+}
+
+int32_t ora_op_sample_cdf(const ora_dist *D, double u) {
+  double w[ORA_MAX_TOPK];
+  for (int i = 0; i < D->k; ++i) w[i] = (double)D->p[i];
+  return D->id[pick_index(w, D->k, u, NULL, NULL)];
+}
+
+/* PAPER.md:129 "standard rejection sampling": accept x ~ Q with probability min(1, P(x)/Q(x)). */
+int32_t ora_op_accept(const ora_dist *P, const ora_dist *Q, int32_t token, double u) {
+  return u * dist_prob(Q, token) < dist_prob(P, token);
+}
+
+static void residual_weights(const ora_dist *P, const ora_dist *Q, double *w) {
+  double W = 0.0;
+  for (int i = 0; i < P->k; ++i) {
+    double r = (double)P->p[i] - dist_prob(Q, P->id[i]);
+    w[i] = r > 0.0 ? r : 0.0;
+    W += w[i];
+  }
+  if (!(W > 0.0))
+    for (int i = 0; i < P->k; ++i) w[i] = (double)P->p[i];
+}
+
+/* the replacement of a rejected token; standard rejection sampling draws it from
+ * norm(max(0, P - Q)) so that the emitted token is distributed as P. */
+int32_t ora_op_sample_residual(const ora_dist *P, const ora_dist *Q, double u) {
+  double w[ORA_MAX_TOPK];
+  residual_weights(P, Q, w);
+  return P->id[pick_index(w, P->k, u, NULL, NULL)];
+}
+
+int ora_set_sampling(ora_ctx *o, float temperature, int32_t top_k, uint64_t seed) {
+  if (top_k < 1) { o->sampling_on = 0; return 0; }
+  if (top_k > ORA_MAX_TOPK || !(temperature > 0.f) || o->forced_on) return -1;
+  o->sampling_on = 1; o->top_k = top_k; o->temperature = temperature; o->samp_seed = seed;
+  return 0;
+}
+
+void ora_get_sample_record(const ora_ctx *o, ora_sample_record *out) { *out = o->rec; }
+
+/* Test hook: is `ids` (k distinct entries) a top-k set of `logits` up to `band`? */
+static int support_hint_valid(const float *logits, int vocab, const int32_t *ids, int k, float band) {
+  float mn = INFINITY, mx = -INFINITY;
+  for (int i = 0; i < k; ++i) {
+    if (ids[i] < 0 || ids[i] >= vocab) return 0;
+    for (int j = 0; j < i; ++j)
+      if (ids[j] == ids[i]) return 0;
+    if (logits[ids[i]] < mn) mn = logits[ids[i]];
+  }
+  for (int i = 0; i < vocab; ++i) {
+    int in = 0;
+    for (int j = 0; j < k; ++j) in |= ids[j] == i;
+    if (!in && logits[i] > mx) mx = logits[i];
+  }
+  return mn >= mx - band;
+}
+
+/* Filtered distribution of a head's logits; a valid differing support hint is adopted (counted). */
+static void head_dist(ora_ctx *o, const float *logits, const int32_t *hint_ids, int hint_k, float band,
+                      ora_dist *out) {
+  int V = o->cfg.vocab;
+  ora_op_topk_softmax(logits, V, o->top_k, o->temperature, NULL, out);
+  if (hint_ids && hint_k == out->k) {
+    int same = 1;
+    for (int i = 0; i < hint_k; ++i) {
+      int found = 0;
+      for (int j = 0; j < out->k; ++j) found |= out->id[j] == hint_ids[i];
+      same &= found;
+    }
+    if (!same && support_hint_valid(logits, V, hint_ids, hint_k, band)) {
+      ora_op_topk_softmax(logits, V, o->top_k, o->temperature, hint_ids, out);
+      o->rec.ties_support += 1;
+    }
+  }
+}
+
+/* Own inverse-CDF draw over weights w on support ids; a differing hint token is adopted iff u lies within
+ * eps (in units of normalised mass) of the hint's interval. */
+static int draw_with_hint(const int32_t *ids, const double *w, int k, double u, int hint, double eps,
+                          int32_t *ties) {
+  double lo[ORA_MAX_TOPK], hi[ORA_MAX_TOPK];
+  int own = pick_index(w, k, u, lo, hi);
+  if (hint >= 0 && hint != ids[own])
+    for (int i = 0; i < k; ++i)
+      if (ids[i] == hint && u >= lo[i] - eps && u < hi[i] + eps) { *ties += 1; return hint; }
+  return ids[own];
+}
+
 
 ora_ctx *ora_create(const ora_config *cfg, const ora_weights *w) {
   if (!cfg || !w) return NULL;
@@ -212,6 +377,7 @@ ora_ctx *ora_create(const ora_config *cfg, const ora_weights *w) {
   o->r_tok = (int32_t *)calloc(n, 4);
   o->r_k = (int32_t *)calloc(n, 4);
   o->r_h = (float *)calloc((size_t)n * d, 4);
+  o->r_q = (ora_dist *)calloc(n, sizeof(ora_dist));
   o->exit_logits = (float *)calloc(V, 4);
   o->pdm_logits = (float *)calloc(V, 4);
   o->pdm_u = (float *)calloc(d, 4);
@@ -236,7 +402,7 @@ void ora_destroy(ora_ctx *o) {
   free(o->kc); free(o->vc); free(o->len); free(o->hfin); free(o->r_pos); free(o->r_tok); free(o->r_k);
   free(o->r_h); free(o->exit_logits); free(o->pdm_logits); free(o->pdm_u); free(o->pdm_feat);
   free(o->x); free(o->q); free(o->kk); free(o->vv); free(o->att); free(o->o); free(o->g); free(o->u);
-  free(o->act); free(o->dn); free(o->z);
+  free(o->act); free(o->dn); free(o->z); free(o->r_q);
   free(o);
 }
 
@@ -361,6 +527,12 @@ int ora_prefill(ora_ctx *o, const int32_t *tokens, int32_t P, int32_t block, int
       }
   }
   int y = head_argmax(o, o->hfin + (size_t)(P - 1) * d, o->w.final_norm, o->exit_logits, 0);
+  if (o->sampling_on) { /* the first token is drawn from P as well ("x ~ P"), u(seed, 0, 2) */
+    memset(&o->rec, 0, sizeof o->rec);
+    head_dist(o, o->exit_logits, NULL, 0, 0.f, &o->rec.target);
+    o->rec.u_resid = ora_op_uniform(o->samp_seed, 0, 2);
+    y = ora_op_sample_cdf(&o->rec.target, o->rec.u_resid);
+  }
   o->c = P;
   o->prompt_len = P;
   o->steps = 0;
@@ -373,7 +545,7 @@ int ora_prefill(ora_ctx *o, const int32_t *tokens, int32_t P, int32_t block, int
 
 int ora_set_forced(ora_ctx *o, const int32_t *truth, int32_t n_truth, float p, uint64_t seed) {
   if (p < 0.f) { o->forced_on = 0; return 0; }
-  if (p > 1.f || (!truth && n_truth > 0)) return -1;
+  if (p > 1.f || (!truth && n_truth > 0) || o->sampling_on) return -1;
   o->truth = truth; o->n_truth = n_truth; o->forced_on = 1; o->forced_seed = seed;
   o->forced_thresh = (uint64_t)floor((double)p * 9007199254740992.0); /* floor(p * 2^53) */
   return 0;
@@ -398,9 +570,23 @@ static int apply_hint(const float *logits, int own, int hint, int vocab, float b
   return own;
 }
 
+static int step_impl(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int32_t verify_hint, float band,
+                     const ora_sample_hints *sh, ora_step_result *out);
+
 /* The same cycle with tie hints for the PDM argmax and the verify argmax (either may be -1). */
 int ora_step_follow(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int32_t verify_hint, float band,
                     ora_step_result *out) {
+  return step_impl(o, draft_override, draft_hint, verify_hint, band, NULL, out);
+}
+
+/* Sampling mode with the CUDA path's decisions as hints (NULL: none). */
+int ora_step_sample_follow(ora_ctx *o, int32_t draft_override, const ora_sample_hints *hints, ora_step_result *out) {
+  if (!o->sampling_on) return -1;
+  return step_impl(o, draft_override, -1, -1, 0.f, hints, out);
+}
+
+static int step_impl(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int32_t verify_hint, float band,
+                     const ora_sample_hints *sh, ora_step_result *out) {
   const ora_config *c = &o->cfg;
   int d = c->d_model, n = c->n_stages, L = c->n_layers, per = L / n;
   if (!o->prefilled) return -1;
@@ -428,6 +614,25 @@ int ora_step_follow(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int3
   ora_op_gemv(o->w.pdm_proj, d, n * d, o->pdm_feat, o->pdm_u);
   int draft = head_argmax(o, o->pdm_u, o->w.pdm_norm, o->pdm_logits, 1);
   draft = apply_hint(o->pdm_logits, draft, draft_hint, c->vocab, band, o->maxabs[1], &o->ties[1]);
+  ora_dist Qd; /* the distribution the entering draft is drawn from (sampling mode) */
+  memset(&Qd, 0, sizeof Qd);
+  if (o->sampling_on) { /* x^ ~ Q_t = filtered PDM distribution (S-2, S-3; j = 0) */
+    double w[ORA_MAX_TOPK];
+    head_dist(o, o->pdm_logits, sh && sh->draft_k ? sh->draft_ids : NULL, sh ? sh->draft_k : 0,
+              sh ? sh->logit_band : 0.f, &Qd);
+    o->rec.draft = Qd;
+    memset(&o->rec.target, 0, sizeof o->rec.target);
+    o->rec.u_draft = ora_op_uniform(o->samp_seed, o->steps, 0);
+    o->rec.u_accept = o->rec.u_resid = -1.0;
+    o->rec.succ_token = -1; o->rec.succ_q = o->rec.succ_p = 0.f;
+    for (int i = 0; i < Qd.k; ++i) w[i] = (double)Qd.p[i];
+    draft = draw_with_hint(Qd.id, w, Qd.k, o->rec.u_draft, sh ? sh->draft_token : -1,
+                           sh ? (double)sh->prob_eps : 0.0, &o->rec.ties_draft);
+    if (draft_override >= 0) { /* a deterministic drafter: Q = one-hot on the override */
+      memset(&Qd, 0, sizeof Qd);
+      Qd.k = 1; Qd.id[0] = draft_override; Qd.p[0] = 1.f;
+    }
+  }
   if (o->forced_on) {
     uint64_t draw = ora_op_splitmix64(o->forced_seed + (uint64_t)o->steps) >> 11;
     int ti = p_new + 1 - o->prompt_len;
@@ -454,17 +659,45 @@ int ora_step_follow(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int3
     y = apply_hint(o->exit_logits, y, verify_hint, c->vocab, band, o->maxabs[0], &o->ties[0]);
     o->emitted += 1;
     r.exited = 1;
-    r.emitted_token = y;
     /* pop the oldest */
     for (int i = 1; i < a; ++i) {
       o->r_pos[i - 1] = o->r_pos[i]; o->r_tok[i - 1] = o->r_tok[i]; o->r_k[i - 1] = o->r_k[i];
+      o->r_q[i - 1] = o->r_q[i];
       memcpy(o->r_h + (size_t)(i - 1) * d, o->r_h + (size_t)i * d, sizeof(float) * d);
     }
     a -= 1;
     int succ = a > 0 ? o->r_tok[0] : draft; /* n = 1: the successor is the draft itself (C-2.12) */
-    if (succ == y) {
+    int ok = succ == y;                     /* greedy: exact argmax match */
+    if (o->sampling_on) {                   /* sampling: standard rejection sampling */
+      const ora_dist *Qs = a > 0 ? &o->r_q[0] : &Qd;
+      ora_dist *Pt = &o->rec.target;
+      head_dist(o, o->exit_logits, sh && sh->verify_k ? sh->verify_ids : NULL, sh ? sh->verify_k : 0,
+                sh ? sh->logit_band : 0.f, Pt);
+      double eps = sh ? (double)sh->prob_eps : 0.0;
+      double qx = dist_prob(Qs, succ), px = dist_prob(Pt, succ);
+      o->rec.succ_token = succ; o->rec.succ_q = (float)qx; o->rec.succ_p = (float)px;
+      o->rec.u_accept = ora_op_uniform(o->samp_seed, o->steps, 1);
+      ok = ora_op_accept(Pt, Qs, succ, o->rec.u_accept);
+      if (sh && sh->accepted >= 0 && sh->accepted != ok && fabs(o->rec.u_accept * qx - px) <= eps * qx) {
+        ok = sh->accepted;
+        o->rec.ties_accept += 1;
+      }
+      if (ok) {
+        y = succ;
+      } else {
+        double w[ORA_MAX_TOPK], W = 0.0;
+        residual_weights(Pt, Qs, w);
+        for (int i = 0; i < Pt->k; ++i) W += w[i];
+        o->rec.u_resid = ora_op_uniform(o->samp_seed, o->steps, 2);
+        y = draw_with_hint(Pt->id, w, Pt->k, o->rec.u_resid, sh ? sh->emitted_token : -1, eps / W,
+                           &o->rec.ties_resid);
+      }
+    }
+    r.emitted_token = y;
+    if (ok) {
       r.accepted = 1;
       o->r_pos[a] = p_new + 1; o->r_tok[a] = draft; o->r_k[a] = 0;
+      o->r_q[a] = Qd;
       embed_row(o, draft, o->r_h + (size_t)a * d);
       o->a = a + 1;
     } else {
@@ -477,6 +710,7 @@ int ora_step_follow(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int3
   } else {
     /* 5 */
     o->r_pos[a] = p_new + 1; o->r_tok[a] = draft; o->r_k[a] = 0;
+    o->r_q[a] = Qd;
     embed_row(o, draft, o->r_h + (size_t)a * d);
     o->a = a + 1;
   }

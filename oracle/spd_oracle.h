@@ -112,6 +112,70 @@ void ora_get_last(const ora_ctx *, int32_t what, float *out);
 /* top1-top2 gap and max|logit| of the last verify (which=0) / PDM (which=1) argmax (C-4). */
 void ora_get_margin(const ora_ctx *, int32_t which, float *gap, float *maxabs);
 
+/* ---- NEXT-2: sampling verification (readings S-1..S-9 of DESIGN.md §2) ----------
+ * PAPER.md:129 "under sampling we apply standard rejection sampling"; PAPER.md:131 on a reject the
+ * pipeline is reseeded "from x ~ P(x | x_1:t-n+1)"; "Sampling runs (T=1) use top-k=50 and
+ * top-p=1.0".  Standard rejection sampling of speculative decoding: a token x drafted from Q is accepted
+ * with probability min(1, P(x)/Q(x)); on a reject the replacement is drawn from norm(max(0, P - Q)), so
+ * the emitted token is distributed exactly as P (pinned by enumeration in tests/test_oracle_sampling.py).
+ *
+ * S-2  filtered distribution of a logit vector l: support S = the top_k entries in the order (value
+ *      descending, index ascending); p_i = exp((l_i - max l)/T) / Z on S (Z summed in fp64 in ascending
+ *      token id, p rounded to fp32), 0 elsewhere.  Distributions list their support in ASCENDING TOKEN ID.
+ * S-3  every draw is inverse-CDF over the support in ascending token id: the smallest i with
+ *      u * W < w_0 + .. + w_i (fp64), W the total weight.
+ * S-6  uniforms: u(seed, K, j) = (splitmix64(seed + 3 K + j) >> 40) * 2^-24, j = 0 draft, 1 accept,
+ *      2 residual / first token; K = the cycle counter after its increment (0 at the prefill's final head). */
+#define ORA_MAX_TOPK 64
+typedef struct {
+  int32_t k;
+  int32_t id[ORA_MAX_TOPK]; /* ascending */
+  float p[ORA_MAX_TOPK];
+} ora_dist;
+
+/* S-2.  support == NULL: the top_k set is selected here; otherwise `support` lists top_k distinct ids that
+ * are used as the support as given (test hook: the CUDA path's set, validated by the caller). */
+void ora_op_topk_softmax(const float *logits, int32_t vocab, int32_t top_k, float temperature,
+                         const int32_t *support, ora_dist *out);
+/* S-6 */
+double ora_op_uniform(uint64_t seed, int64_t K, int32_t j);
+/* S-3 on the distribution's own probabilities; returns the token id. */
+int32_t ora_op_sample_cdf(const ora_dist *dist, double u);
+/* Accept test of token x drafted from Q under target P: 1 iff u * Q(x) < P(x) (fp64 on the fp32
+ * probabilities; a token outside a support has probability 0). */
+int32_t ora_op_accept(const ora_dist *P, const ora_dist *Q, int32_t token, double u);
+/* Residual draw: weights w_i = max(0, P(i) - Q(i)) over P's support (all zero -> w = P), S-3 with u. */
+int32_t ora_op_sample_residual(const ora_dist *P, const ora_dist *Q, double u);
+
+/* Enables sampling for the ctx (top_k < 1 disables = greedy).  1 <= top_k <= ORA_MAX_TOPK, T > 0.
+ * Called before ora_prefill the first token is drawn from P as well (u(seed, 0, 2)); forced acceptance
+ * and sampling are mutually exclusive (-1).  In sampling mode a cycle drafts x ~ Q_t (S-3, j = 0) and
+ * keeps Q_t with the in-flight token; at the exit the successor is judged by ora_op_accept (j = 1) and
+ * on a reject replaced by ora_op_sample_residual (j = 2); emitted_token = the accepted successor or the
+ * replacement.  draft_override >= 0 acts as a deterministic drafter (Q = one-hot on the override). */
+int ora_set_sampling(ora_ctx *, float temperature, int32_t top_k, uint64_t seed);
+
+/* Test hook: what the CUDA path decided in this cycle.  A hint that differs
+ * from the oracle's own decision is adopted only when the difference is implied by the logit difference
+ * the test measured: a support is adopted iff min over it >= max over the rest - logit_band; a token /
+ * accept bit iff the uniform lies within prob_eps (probability mass) of the oracle's decision boundary. */
+typedef struct {
+  int32_t draft_k, draft_ids[ORA_MAX_TOPK];   /* draft_k = 0: no support hint */
+  int32_t verify_k, verify_ids[ORA_MAX_TOPK];
+  int32_t draft_token, accepted, emitted_token; /* -1: no hint */
+  float logit_band, prob_eps;
+} ora_sample_hints;
+typedef struct {
+  ora_dist draft;   /* Q_t of the last cycle */
+  ora_dist target;  /* P of the last exit (or of the prefill's final head) */
+  double u_draft, u_accept, u_resid;
+  int32_t succ_token;
+  float succ_q, succ_p;
+  int32_t ties_support, ties_draft, ties_accept, ties_resid; /* hints adopted so far */
+} ora_sample_record;
+int ora_step_sample_follow(ora_ctx *, int32_t draft_override, const ora_sample_hints *hints, ora_step_result *out);
+void ora_get_sample_record(const ora_ctx *, ora_sample_record *out);
+
 /* Timing-only helpers (bench cpu_baseline): load KV rows / declare a committed length without a
  * prefill.  Never used by a parity test. */
 void ora_load_kv(ora_ctx *, int32_t layer, const uint16_t *k, const uint16_t *v, int32_t rows);

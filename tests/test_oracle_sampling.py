@@ -1,0 +1,329 @@
+"""Pins for the oracle's sampling verification (readings S-1..S-9).  CPU only.
+
+What fixes the oracle here is not the oracle: library softmax / argsort (numpy, scipy), the defining
+property of standard rejection sampling — the emitted token is distributed exactly as the
+target's filtered distribution P whatever the draft distribution Q — checked (i) on the three decision
+functions by measuring the set of uniforms that leads to each outcome, (ii) end to end on a micro decoder
+against the exact autoregressive sampling distribution computed from whole-prefix recomputes, and the
+special case top_k = 1, where sampling must reduce to the greedy path bit for bit (PAPER.md:129
+"exact argmax match").
+"""
+import numpy as np
+import pytest
+import scipy.special
+import scipy.stats
+
+import spd_inputs as si
+from oracle import Dist, Oracle, op_accept, op_sample_cdf, op_sample_residual, op_splitmix64, op_topk_softmax, \
+    op_uniform
+from tests._util import TINY, shape_of, weights
+
+PROMPT = si.make_prompt(TINY, 1)
+
+
+def lib_filtered(logits, k, T):
+    """Top-k + temperature softmax with library routines: stable argsort of (-value) keeps the lower index
+    among equal values; returns a dense float64 probability vector."""
+    x = np.asarray(logits, dtype=np.float64)
+    order = np.argsort(-x, kind="stable")[:k]
+    p = np.zeros_like(x)
+    p[order] = scipy.special.softmax(x[order] / T)
+    return p
+
+
+def dense(d: Dist, V: int) -> np.ndarray:
+    p = np.zeros(V)
+    p[d.ids] = d.p
+    return p
+
+
+# ------------------------------------------------------------------ the filtered distribution ----
+
+@pytest.mark.parametrize("V,k,T", [(1000, 50, 1.0), (37, 5, 0.7), (64, 64, 1.0), (10, 50, 2.0), (151936, 50, 1.0)])
+def test_topk_softmax_matches_library(V, k, T):
+    rng = np.random.default_rng(V + k)
+    x = rng.standard_normal(V).astype(np.float32) * 1.3
+    d = op_topk_softmax(x, k, T)
+    assert len(d.ids) == min(k, V) and np.all(np.diff(d.ids) > 0)          # ascending token id (S-2)
+    np.testing.assert_allclose(dense(d, V), lib_filtered(x, k, T), rtol=0, atol=1e-7)
+    assert abs(float(np.sum(d.p.astype(np.float64))) - 1.0) < 1e-6
+
+
+def test_topk_ties_take_the_lower_index_and_k_ge_vocab_is_plain_softmax():
+    x = np.array([0.5, 2.0, 2.0, -1.0, 2.0, 0.5], dtype=np.float32)
+    assert list(op_topk_softmax(x, 2, 1.0).ids) == [1, 2]
+    assert list(op_topk_softmax(x, 4, 1.0).ids) == [0, 1, 2, 4]
+    d = op_topk_softmax(x, 64, 1.0)
+    np.testing.assert_allclose(d.p, scipy.special.softmax(x.astype(np.float64)), atol=1e-7)
+    # given support: used as given, listed ascending
+    g = op_topk_softmax(x, 2, 1.0, support=[5, 3])
+    assert list(g.ids) == [3, 5]
+    np.testing.assert_allclose(g.p, scipy.special.softmax(np.array([-1.0, 0.5])), atol=1e-7)
+
+
+def test_topk_one_is_the_greedy_argmax():
+    rng = np.random.default_rng(3)
+    for _ in range(20):
+        x = rng.standard_normal(300).astype(np.float32)
+        d = op_topk_softmax(x, 1, 1.0)
+        assert list(d.ids) == [int(np.argmax(x))] and d.p[0] == 1.0
+
+
+def test_temperature_limits():
+    x = np.array([1.0, 3.0, 2.0, 0.0], dtype=np.float32)
+    cold = op_topk_softmax(x, 4, 1e-3)
+    assert cold.p[1] == 1.0 and np.all(cold.p[[0, 2, 3]] == 0.0)            # T -> 0: argmax
+    hot = op_topk_softmax(x, 4, 1e6)
+    np.testing.assert_allclose(hot.p, 0.25, atol=1e-5)                      # T -> inf: uniform on the support
+
+
+# ------------------------------------------------------------------ uniforms ---------------------
+
+def test_uniform_is_24_bits_of_splitmix64():
+    """S-6; splitmix64 itself is pinned by tests/golden/splitmix64.txt (test_oracle_model.py)."""
+    for seed, K, j in [(0, 1, 0), (7, 5, 1), (2 ** 63 + 11, 123456, 2), (99, 0, 2)]:
+        u = op_uniform(seed, K, j)
+        want = (op_splitmix64((seed + 3 * K + j) % 2 ** 64) >> 40) / 2.0 ** 24
+        assert u == want and 0.0 <= u < 1.0
+        assert np.float32(u) == u                                            # exact in fp32
+    us = np.array([op_uniform(5, K, j) for K in range(2000) for j in range(3)])
+    assert abs(us.mean() - 0.5) < 0.02 and abs(np.mean(us < 0.1) - 0.1) < 0.02
+
+
+# ------------------------------------------------------------------ decisions: measured in u -----
+
+GRID = (np.arange(1 << 14) + 0.5) / (1 << 14)
+
+
+def measure(fn):
+    """Lebesgue measure of the u-set mapped to each outcome, on a midpoint grid (resolution 2^-14)."""
+    out = {}
+    for u in GRID:
+        t = fn(float(u))
+        out[t] = out.get(t, 0) + 1
+    return {t: c / len(GRID) for t, c in out.items()}
+
+
+def random_pair(rng, V=12, k=5):
+    lp = rng.standard_normal(V).astype(np.float32) * 1.5
+    lq = (0.6 * lp + 0.8 * rng.standard_normal(V) * 1.5).astype(np.float32)   # correlated: supports overlap partly
+    return op_topk_softmax(lp, k, 1.0), op_topk_softmax(lq, k, 1.0)
+
+
+def test_inverse_cdf_measure_equals_probability_and_order_is_ascending_token_id():
+    rng = np.random.default_rng(0)
+    P, _ = random_pair(rng)
+    m = measure(lambda u: op_sample_cdf(P, u))
+    for t, p in zip(P.ids, P.p):
+        assert abs(m.get(int(t), 0.0) - p) < 2e-4
+    picks = [op_sample_cdf(P, float(u)) for u in GRID[::64]]
+    assert picks == sorted(picks)                                           # S-3: CDF runs in ascending id
+    assert op_sample_cdf(P, 0.0) == P.ids[0] and op_sample_cdf(P, 1.0 - 2.0 ** -24) == P.ids[-1]
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_rejection_sampling_emits_exactly_P(seed):
+    """Enumeration over the drafted token x and measurement over (u_accept, u_resid):
+    sum_x Q(x) [acc(x) 1{x=y} + (1-acc(x)) R_x(y)] == P(y) for every y — the lossless property of
+    standard rejection sampling.  A wrong sign or a missing normalisation in the residual,
+    an inverted ratio in the accept test, or P and Q exchanged all break it."""
+    rng = np.random.default_rng(100 + seed)
+    P, Q = random_pair(rng)
+    V = 12
+    out = np.zeros(V)
+    total_acc = 0.0
+    res = measure(lambda u: op_sample_residual(P, Q, u))          # the residual does not depend on x
+    for x, qx in zip(Q.ids, Q.p):
+        acc = measure(lambda u: op_accept(P, Q, int(x), u)).get(1, 0.0)
+        px = dense(P, V)[x]
+        assert abs(acc - min(1.0, px / qx)) < 2e-4
+        total_acc += qx * acc
+        out[x] += qx * acc
+        for y, r in res.items():
+            out[y] += qx * (1.0 - acc) * r
+    np.testing.assert_allclose(out, dense(P, V), atol=1e-3)
+    assert abs(total_acc - np.minimum(dense(P, V), dense(Q, V)).sum()) < 1e-3
+    # the residual never returns a token outside P's support, nor one with P <= Q
+    for y in res:
+        assert dense(P, V)[y] > dense(Q, V)[y]
+
+
+def test_decision_special_cases():
+    P = Dist(np.array([2, 5, 9], dtype=np.int32), np.array([0.5, 0.25, 0.25], dtype=np.float32))
+    # Q == P: always accepted; residual falls back to P (never used)
+    assert all(op_accept(P, P, 5, u) == 1 for u in (0.0, 0.5, 0.999999))
+    assert measure(lambda u: op_sample_residual(P, P, u)).keys() == {2, 5, 9}
+    # one-hot drafter on x: accepted with probability P(x); replaced by P restricted to the others
+    Q = Dist(np.array([5], dtype=np.int32), np.array([1.0], dtype=np.float32))
+    assert op_accept(P, Q, 5, 0.2499) == 1 and op_accept(P, Q, 5, 0.2501) == 0
+    r = measure(lambda u: op_sample_residual(P, Q, u))
+    assert abs(r[2] - 2 / 3) < 2e-4 and abs(r[9] - 1 / 3) < 2e-4 and 5 not in r
+    # a drafted token outside P's support is always rejected
+    Q7 = Dist(np.array([7], dtype=np.int32), np.array([1.0], dtype=np.float32))
+    assert op_accept(P, Q7, 7, 0.0) == 0
+
+
+# ------------------------------------------------------------------ the cycle in sampling mode ---
+
+def run_spd_sampled(o, prompt, n_tokens, draft_fn=None):
+    toks = [o.prefill(prompt)]
+    log = []
+    while o.emitted < n_tokens:
+        r = o.step_sample_follow(draft_override=-1 if draft_fn is None else int(draft_fn(o)))
+        log.append(r)
+        if r.exited:
+            toks.append(r.emitted_token)
+    return toks, log
+
+
+@pytest.mark.parametrize("n", [1, 2, 4])
+def test_top_k_one_reduces_to_the_greedy_cycle_bitwise(n):
+    """top_k = 1: P and Q are one-hot, accept <=> successor == argmax, the residual is the argmax:
+    every step result, KV length and KV row must equal the greedy cycle's."""
+    shape = shape_of("tiny", n)
+    w = weights("tiny", n)
+    g = Oracle(shape, w, max_seq=512)
+    s = Oracle(shape, w, max_seq=512)
+    s.set_sampling(1.0, 1, 12345)
+    assert g.prefill(PROMPT) == s.prefill(PROMPT)
+    for _ in range(60):
+        rg, rs = g.step(), s.step_sample_follow()
+        assert tuple(rg) == tuple(rs)
+        assert np.array_equal(g.kv_len(), s.kv_len())
+    for l in (0, shape.n_layers - 1):
+        assert np.array_equal(g.kv(l, 0, g.committed_len), s.kv(l, 0, s.committed_len))
+    g.close(); s.close()
+
+
+def test_sampling_and_forcing_exclude_each_other():
+    o = Oracle(shape_of("tiny", 2), weights("tiny", 2), max_seq=128)
+    o.set_sampling(1.0, 50, 1)
+    with pytest.raises(ValueError):
+        o.set_forced(np.zeros(4, dtype=np.int32), 0.5, 1)
+    o.set_sampling(1.0, 0, 1)           # off again
+    o.set_forced(np.zeros(4, dtype=np.int32), 0.5, 1)
+    with pytest.raises(ValueError):
+        o.set_sampling(1.0, 50, 1)
+    with pytest.raises(ValueError):
+        Oracle(shape_of("tiny", 2), weights("tiny", 2), max_seq=128).set_sampling(0.0, 50, 1)
+    o.close()
+
+
+def test_cycle_bookkeeping_in_sampling_mode():
+    """Every accepted token was in flight with the distribution it was drawn from; rollback identity and
+    fill pattern as in the greedy cycle; the record exposes P, Q and the uniforms of S-6."""
+    n = 4
+    shape = shape_of("tiny", n, vocab=64)      # a 64-token vocabulary so that top-50 supports overlap (acceptance ~1/3)
+    o = Oracle(shape, si.make_weights(shape, seed=1234, std=0.08, random_gains=True), max_seq=1024)
+    o.set_sampling(1.0, 50, 77)
+    first = o.prefill(si.make_prompt(shape, 1))
+    rec = o.sample_record()
+    assert rec["u_resid"] == op_uniform(77, 0, 2)
+    assert first == op_sample_cdf(rec["target"], rec["u_resid"])
+    np.testing.assert_allclose(dense(rec["target"], shape.vocab), lib_filtered(o.last("exit_logits"), 50, 1.0), atol=1e-6)
+    in_flight = {}                      # position -> (token, Q)
+    prev_fill = 1
+    acc = rej = 0
+    for _ in range(150):
+        p_new = o.ring(o.fill - 1)[0]
+        r = o.step_sample_follow()
+        rec = o.sample_record()
+        K = r.step_index
+        Q = rec["draft"]
+        np.testing.assert_allclose(dense(Q, shape.vocab), lib_filtered(o.last("pdm_logits"), 50, 1.0), atol=1e-6)
+        assert rec["u_draft"] == op_uniform(77, K, 0)
+        assert r.draft_token == op_sample_cdf(Q, rec["u_draft"])
+        assert r.fill == prev_fill
+        if r.exited:
+            c = r.committed_len
+            x, Qx = in_flight[c]
+            P = rec["target"]
+            np.testing.assert_allclose(dense(P, shape.vocab), lib_filtered(o.last("exit_logits"), 50, 1.0), atol=1e-6)
+            assert rec["succ_token"] == x and rec["u_accept"] == op_uniform(77, K, 1)
+            assert r.accepted == op_accept(P, Qx, x, rec["u_accept"])
+            if r.accepted:
+                acc += 1
+                assert r.emitted_token == x
+                in_flight[p_new + 1] = (r.draft_token, Q)
+                prev_fill = r.fill
+            else:
+                rej += 1
+                assert rec["u_resid"] == op_uniform(77, K, 2)
+                assert r.emitted_token == op_sample_residual(P, Qx, rec["u_resid"])
+                assert np.all(o.kv_len() == c) and o.fill == 1 and r.discarded == r.fill - 1
+                in_flight = {}
+                prev_fill = 1
+        else:
+            in_flight[p_new + 1] = (r.draft_token, Q)
+            prev_fill = r.fill + 1
+    assert acc > 5 and rej > 5, (acc, rej)
+    o.close()
+
+
+# ------------------------------------------------------------------ lossless in distribution ------
+
+MICRO = TINY.replace(name="micro", d_model=64, n_layers=4, n_stages=2, n_q_heads=2, n_kv_heads=1, head_dim=32,
+                     d_ffn=96, vocab=24, prompt_len=6, gen_len=8)
+MK, MT = 3, 1.0     # top-k 3, T = 1 on a 24-token vocabulary
+
+
+def micro_weights(n):
+    return si.make_weights(MICRO.replace(n_stages=n), seed=4321, std=0.25, random_gains=True)
+
+
+def exact_ar_distribution(n, prompt, depth):
+    """P(t_1..t_depth) of autoregressive sampling from the filtered target distribution, by whole-prefix
+    recompute: each factor is library top-k softmax of the logits the oracle's prefill gives for
+    prompt + prefix (the PDM and the pipeline play no part)."""
+    shape = MICRO.replace(n_stages=n)
+    o = Oracle(shape, micro_weights(n), max_seq=64)
+    dist = {(): 1.0}
+    for _ in range(depth):
+        nxt = {}
+        for prefix, pr in dist.items():
+            o.prefill(np.concatenate([prompt, np.array(prefix, dtype=np.int32)]).astype(np.int32))
+            p = lib_filtered(o.last("exit_logits"), MK, MT)
+            for t in np.nonzero(p)[0]:
+                nxt[prefix + (int(t),)] = pr * p[t]
+        dist = nxt
+    o.close()
+    return dist
+
+
+@pytest.mark.parametrize("n,drafter", [(2, "pdm"), (4, "pdm"), (1, "pdm"), (2, "fixed"), (4, "random")])
+def test_sampled_spd_is_distributed_as_autoregressive_sampling(n, drafter):
+    """The defining property under sampling: SPD with rejection-sampling verification
+    emits tokens distributed exactly as autoregressive sampling from the target.  3000 seeds, the joint
+    distribution of the first three tokens against the exact one (chi-square; seeds are fixed, so the
+    test is deterministic).  Drafters: the PDM (Q = its filtered distribution), a fixed token and a
+    random token (deterministic drafters, Q one-hot) — acceptance differs widely, the output law may not."""
+    depth, runs = 3, 3000
+    prompt = si.make_prompt(MICRO, 3)
+    want = exact_ar_distribution(n, prompt, depth)
+    assert abs(sum(want.values()) - 1.0) < 1e-9
+    shape = MICRO.replace(n_stages=n)
+    o = Oracle(shape, micro_weights(n), max_seq=256)
+    rng = np.random.default_rng(9)
+    fn = {"pdm": None, "fixed": lambda _o: 5, "random": lambda _o: rng.integers(0, MICRO.vocab)}[drafter]
+    counts = {k: 0 for k in want}
+    accepted = exits = 0
+    for seed in range(runs):
+        o.set_sampling(MT, MK, 1000 + seed)
+        toks, log = run_spd_sampled(o, prompt, depth, fn)
+        counts[tuple(toks[:depth])] += 1        # KeyError: a token outside the target's support was emitted
+        accepted += sum(r.accepted for r in log)
+        exits += sum(r.exited for r in log)
+    o.close()
+    keys = sorted(want, key=lambda k: -want[k])
+    exp = np.array([want[k] * runs for k in keys])
+    obs = np.array([counts[k] for k in keys], dtype=np.float64)
+    big = exp >= 8.0                                        # pool the rare outcomes into one cell
+    e = np.append(exp[big], exp[~big].sum())
+    c = np.append(obs[big], obs[~big].sum())
+    if e[-1] < 8.0:
+        e[-2] += e[-1]; c[-2] += c[-1]; e, c = e[:-1], c[:-1]
+    chi2 = float(((c - e) ** 2 / e).sum())
+    pval = float(scipy.stats.chi2.sf(chi2, len(e) - 1))
+    assert pval > 1e-3, f"chi2 {chi2:.1f} over {len(e)} cells, p = {pval:.2e}, acceptance {accepted}/{exits}"
+    if drafter == "pdm" and n > 1:
+        assert 0 < accepted < exits                          # both branches of the verifier were exercised
