@@ -16,7 +16,9 @@
  *     3. if the oldest token finished stage n: commits it, y = argmax(E . RMSNorm(h)) judges its
  *        in-flight successor; equal -> the draft enters stage 0; different -> every layer's KV length
  *        is truncated to the committed length, the pipeline is flushed and reseeded with y.
- *   Greedy only; the emitted tokens equal plain greedy decoding ("lossless").
+ *   Greedy by default: the emitted tokens equal plain greedy decoding ("lossless").
+ *   spd_set_sampling switches step 3 to sampling verification ("under sampling we apply
+ *   standard rejection sampling"): the emitted tokens are then distributed as sampling from the target.
  *
  * Numeric contract (C-2.17): weights bf16, every activation fp32 with fp32 accumulation, K/V cache
  * rows rounded to bf16 (round-to-nearest-even) when appended.  argmax = max value, lowest index (C-2.8).
@@ -119,6 +121,7 @@ enum {
   SPD_DBG_KV_LEN = 7,      /* int32[L]: valid KV rows per layer (C-2.11)                           */
   SPD_DBG_RING = 8,        /* int32[2 + 3n]: fill a, committed c, then per depth k: occupied, pos, tok */
   SPD_DBG_HFIN = 9,        /* [position] fp32[d]: final hidden state of a committed position        */
+  SPD_DBG_SAMPLE = 11,     /* spd_sample_record of the last cycle (needs spd_set_sampling)                */
   SPD_DBG_PHASE_PROFILE = 10 /* uint64[160][168][6]: per (CTA, phase) clock stamps of the last fused cycle:
                               0 inputs ready, 1 activations staged, 2 tiles consumed, 3/4 producer issued the
                               phase's first/last tile (SM clock); 5 = %globaltimer at stamp 0; phase 167 holds
@@ -160,6 +163,42 @@ int spd_rollback(spd_ctx *ctx, int32_t new_len, int32_t reseed_token);
  * copied.  p < 0 disables; p > 1 or n_truth > max_seq -> SPD_EINVAL. */
 int spd_set_forced(spd_ctx *ctx, const int32_t *truth, int32_t n_truth, float p, uint64_t seed);
 
+/* Sampling verification.  PAPER.md:129: "under sampling we apply standard rejection
+ * sampling"; on a reject the pipeline is reseeded "from x ~ P(x | x_1:t-n+1)"; PAPER.md:141:
+ * "Sampling runs (T=1) use top-k=50 and top-p=1.0".  With sampling on (1 <= top_k <= SPD_MAX_TOPK,
+ * temperature > 0):
+ *   - a logit vector l is filtered to its top_k entries (value descending, index ascending) with
+ *     p = softmax(l / temperature) over them (sum in fp64, p in fp32); supports are listed in ascending token id;
+ *   - the PDM's token is DRAWN from its filtered distribution Q_t, which stays with the in-flight token;
+ *   - at the exit the successor x (drafted from Q) is accepted iff u * Q(x) < P(x), P the filtered exit
+ *     distribution; a rejected x is replaced by a draw from norm(max(0, P - Q)) and the pipeline is flushed and
+ *     reseeded with it (KV truncation as in the greedy path); emitted_token = x or the replacement;
+ *   - spd_prefill draws first_token from P;
+ *   - every draw is the inverse CDF in ascending token id in fp64 with the uniform
+ *     u(seed, K, j) = (splitmix64(seed + 3 K + j) >> 40) * 2^-24, j = 0 draft, 1 accept, 2 replacement / first
+ *     token, K = step_index of the cycle (0 in spd_prefill).
+ * The emitted tokens are distributed exactly as autoregressive sampling from the filtered target (not
+ * token-identical to any other run).  top_k < 1 switches back to greedy.  top_k = 1 is the greedy path.
+ * SPD_EINVAL: top_k > SPD_MAX_TOPK or temperature <= 0.  SPD_ESTATE: forced acceptance is on (and
+ * spd_set_forced while sampling is on).  Logits must be finite.  May be called before or after spd_prefill. */
+#define SPD_MAX_TOPK 64
+typedef struct {
+  int32_t k;
+  int32_t id[SPD_MAX_TOPK]; /* ascending token id */
+  float p[SPD_MAX_TOPK];
+} spd_sample_dist;
+/* What the sampler of the last cycle saw and decided (spd_debug_read(SPD_DBG_SAMPLE), parity tests). */
+typedef struct {
+  spd_sample_dist draft;   /* Q_t of this cycle's PDM (k = 0: the PDM did not run)                      */
+  spd_sample_dist target;  /* P of this cycle's exit or of spd_prefill's final head (k = 0: no exit)    */
+  float u_draft, u_accept, u_resid; /* -1: not drawn                                                    */
+  int32_t succ_token;      /* the judged token (-1: none), its stored draft probability, its target probability */
+  float succ_q, succ_p;
+  int32_t exact_rounds;    /* selections of this cycle that took the exact k-round path (0..2)          */
+  int32_t pad_;
+} spd_sample_record;
+int spd_set_sampling(spd_ctx *ctx, float temperature, int32_t top_k, uint64_t seed);
+
 int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value);
 
 /* Copies internal state to HOST memory (parity tests).  bytes must match the selector's size
@@ -191,6 +230,12 @@ size_t spd_op_attention_scratch(int32_t t_len, int32_t n_q_heads, int32_t head_d
 int spd_op_silu_mul(const float *gate, const float *up, int32_t n, float *out, void *stream);
 /* argmax with lowest-index ties of x[0..n); result int32 on the device */
 int spd_op_argmax(const float *x, int32_t n, int32_t *out_index, void *stream);
+/* The filtered distribution of spd_set_sampling: top_k + temperature softmax of x[0..n) into *out (DEVICE
+ * spd_sample_dist).  use_candidates != 0: threshold scan seeded by 128 chunk maxima (the step's path);
+ * 0: no candidates (the exact k-round selection when n > 2048).  scratch: DEVICE, >= spd_op_topk_scratch() bytes. */
+int spd_op_topk_softmax(const float *x, int32_t n, int32_t top_k, float temperature, int32_t use_candidates,
+                        spd_sample_dist *out, void *scratch, void *stream);
+size_t spd_op_topk_scratch(void);
 
 #ifdef __cplusplus
 }

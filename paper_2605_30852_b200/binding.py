@@ -33,7 +33,26 @@ class OPT:
 
 
 class DBG:
-    SLOT_HIDDEN, EXIT_LOGITS, PDM_LOGITS, PDM_PRENORM, PDM_FEAT, KV_K, KV_V, KV_LEN, RING, HFIN, PHASE_PROFILE = range(11)
+    SLOT_HIDDEN, EXIT_LOGITS, PDM_LOGITS, PDM_PRENORM, PDM_FEAT, KV_K, KV_V, KV_LEN, RING, HFIN, PHASE_PROFILE, \
+        SAMPLE = range(12)
+
+
+MAX_TOPK = 64
+
+
+class _Dist(C.Structure):
+    _fields_ = [("k", C.c_int32), ("id", C.c_int32 * MAX_TOPK), ("p", C.c_float * MAX_TOPK)]
+
+
+class _SampleRec(C.Structure):
+    _fields_ = [("draft", _Dist), ("target", _Dist), ("u_draft", C.c_float), ("u_accept", C.c_float),
+                ("u_resid", C.c_float), ("succ_token", C.c_int32), ("succ_q", C.c_float), ("succ_p", C.c_float),
+                ("exact_rounds", C.c_int32), ("pad_", C.c_int32)]
+
+
+def _dist_out(d: _Dist):
+    k = d.k
+    return np.array(d.id[:k], dtype=np.int32), np.array(d.p[:k], dtype=np.float32)
 
 
 class _Cfg(C.Structure):
@@ -98,6 +117,10 @@ def lib():
         L.spd_rollback.argtypes = [vp, i32, i32]
         L.spd_set_forced.argtypes = [vp, vp, i32, f32, u64]
         L.spd_set_option.argtypes = [vp, i32, i32]
+        L.spd_set_sampling.argtypes = [vp, f32, i32, u64]
+        L.spd_op_topk_softmax.argtypes = [vp, i32, i32, f32, i32, vp, vp, vp]
+        L.spd_op_topk_scratch.argtypes = []
+        L.spd_op_topk_scratch.restype = C.c_size_t
         L.spd_debug_read.argtypes = [vp, i32, i32, vp, C.c_size_t]
         L.spd_get_counters.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.spd_last_error.argtypes = [vp]
@@ -228,6 +251,19 @@ class SPD:
             t = np.ascontiguousarray(truth, dtype=np.int32)
             self._check(lib().spd_set_forced(self._h, t.ctypes.data, len(t), p, seed))
 
+    def set_sampling(self, temperature: float, top_k: int, seed: int):
+        """Sampling verification (include/spd.h spd_set_sampling); top_k < 1 switches back to greedy."""
+        self._check(lib().spd_set_sampling(self._h, temperature, top_k, seed))
+
+    def sample_record(self) -> dict:
+        """spd_sample_record of the last cycle: (ids, p) of the draft and target distributions, the uniforms,
+        the judged token with its two probabilities."""
+        r = _SampleRec()
+        self._check(lib().spd_debug_read(self._h, DBG.SAMPLE, 0, C.addressof(r), C.sizeof(r)))
+        return dict(draft=_dist_out(r.draft), target=_dist_out(r.target), u_draft=r.u_draft, u_accept=r.u_accept,
+                    u_resid=r.u_resid, succ_token=r.succ_token, succ_q=r.succ_q, succ_p=r.succ_p,
+                    exact_rounds=r.exact_rounds)
+
     def set_option(self, option: int, value: int):
         self._check(lib().spd_set_option(self._h, option, value))
 
@@ -340,3 +376,13 @@ def op_argmax(x: torch.Tensor, stream=None) -> int:
     out = torch.empty(1, dtype=torch.int32, device=x.device)
     _chk(lib().spd_op_argmax(x.data_ptr(), x.numel(), out.data_ptr(), _s(stream)), "spd_op_argmax")
     return int(out.item())
+
+
+def op_topk_softmax(x: torch.Tensor, top_k: int, temperature: float, use_candidates: bool = True, stream=None):
+    """(ids ascending, p) of the filtered distribution of spd_set_sampling."""
+    out = torch.zeros(C.sizeof(_Dist), dtype=torch.uint8, device=x.device)
+    scratch = torch.empty(lib().spd_op_topk_scratch(), dtype=torch.uint8, device=x.device)
+    _chk(lib().spd_op_topk_softmax(x.data_ptr(), x.numel(), top_k, temperature, int(use_candidates), out.data_ptr(),
+                                   scratch.data_ptr(), _s(stream)), "spd_op_topk_softmax")
+    d = _Dist.from_buffer_copy(out.cpu().numpy().tobytes())
+    return _dist_out(d)

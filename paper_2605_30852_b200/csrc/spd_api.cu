@@ -27,6 +27,7 @@ struct spd_ctx {
   StepResult *h_results;   // pinned
   StepState *h_state;      // pinned mirror
   int prefilled, dead;
+  int forced_on, sampling_on;   // host mirrors (the two modes exclude each other)
   long long launches;
   long long launches_per_step[2];
   char err[512];
@@ -120,6 +121,9 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
   Q.bar = cv.take<unsigned int>(kBarWords);
   Q.claim = cv.take<unsigned int>((size_t)kProfPhases * kMaxStages);
   Q.prof = cv.take<unsigned long long>((size_t)kProfCtas * kProfPhases * kProfStamps);
+  Q.samp = cv.take<SampleState>(1);
+  Q.samp_val = cv.take<float>(kSampCap);
+  Q.samp_idx = cv.take<int32_t>(kSampCap);
   const uint16_t **tabs[9];
   for (int i = 0; i < 9; ++i) tabs[i] = cv.take<const uint16_t *>(D.L);
   Q.attn_norm = tabs[0]; Q.wq = tabs[1]; Q.wk = tabs[2]; Q.wv = tabs[3]; Q.wo = tabs[4];
@@ -161,6 +165,9 @@ __global__ void k_state_init(DevPtrs P, int mode, int pf_n) {
 __global__ void k_set_mode(DevPtrs P, int mode) { P.st->mode = mode; }
 __global__ void k_set_forced(DevPtrs P, int on, int n_truth, unsigned long long thresh, unsigned long long seed) {
   P.st->forced_on = on; P.st->n_truth = n_truth; P.st->forced_thresh = thresh; P.st->forced_seed = seed;
+}
+__global__ void k_set_sampling(DevPtrs P, int on, int top_k, float temperature, unsigned long long seed) {
+  P.samp->on = on; P.samp->top_k = top_k; P.samp->temperature = temperature; P.samp->seed = seed;
 }
 // External truncate + flush + reseed (PAPER.md:131 with c := new_len).
 __global__ void k_rollback(DevPtrs P, int new_len, int tok) {
@@ -342,6 +349,7 @@ extern "C" int spd_step_many(spd_ctx *ctx, int32_t n_steps, spd_step_result *res
   int rc = sync_state(ctx);
   if (rc) return rc;
   static_assert(sizeof(StepResult) == sizeof(spd_step_result), "result layout");
+  static_assert(sizeof(SampleRecord) == sizeof(spd_sample_record) && kMaxTopK == SPD_MAX_TOPK, "sample record layout");
   memcpy(results, ctx->h_results, sizeof(StepResult) * n_steps);
   return SPD_OK;
 }
@@ -370,15 +378,41 @@ extern "C" int spd_set_forced(spd_ctx *ctx, const int32_t *truth, int32_t n_trut
   if (!ctx) return SPD_EINVAL;
   if (ctx->dead) return SPD_ECUDA;
   CU(cudaSetDevice(ctx->cfg.device));
+  if (p >= 0.f && ctx->sampling_on) return fail(ctx, SPD_ESTATE, "spd_set_forced: sampling verification is on%s");
   if (p < 0.f) {
     k_set_forced<<<1, 1, 0, ctx->sm>>>(ctx->P, 0, 0, 0ull, 0ull);
+    ctx->forced_on = 0;
   } else {
     if (p > 1.f || n_truth < 0 || n_truth > ctx->cfg.max_seq || (n_truth > 0 && !truth))
       return fail(ctx, SPD_EINVAL, "spd_set_forced: bad arguments%s");
+    ctx->forced_on = 1;
     if (n_truth) CU(cudaMemcpyAsync(ctx->P.truth, truth, sizeof(int32_t) * n_truth, cudaMemcpyHostToDevice, ctx->sm));
     unsigned long long thresh = (unsigned long long)floor((double)p * 9007199254740992.0);
     k_set_forced<<<1, 1, 0, ctx->sm>>>(ctx->P, 1, n_truth, thresh, (unsigned long long)seed);
   }
+  ++ctx->launches;
+  CU(cudaStreamSynchronize(ctx->sm));
+  return SPD_OK;
+}
+
+static void drop_graphs(spd_ctx *ctx) {   // a kernel parameter changed: captured graphs must be rebuilt
+  cudaStreamSynchronize(ctx->sm);
+  for (int e = 0; e < 2; ++e) {
+    if (ctx->graph[e]) cudaGraphExecDestroy(ctx->graph[e]);
+    ctx->graph[e] = nullptr; ctx->graph_tried[e] = 0;
+  }
+}
+
+extern "C" int spd_set_sampling(spd_ctx *ctx, float temperature, int32_t top_k, uint64_t seed) {
+  if (!ctx) return SPD_EINVAL;
+  if (ctx->dead) return SPD_ECUDA;
+  const int on = top_k >= 1;
+  if (on && (top_k > kMaxTopK || !(temperature > 0.f))) return fail(ctx, SPD_EINVAL, "spd_set_sampling: bad arguments%s");
+  if (on && ctx->forced_on) return fail(ctx, SPD_ESTATE, "spd_set_sampling: forced acceptance is on%s");
+  CU(cudaSetDevice(ctx->cfg.device));
+  if (ctx->P.sampling != on) { ctx->P.sampling = on; drop_graphs(ctx); }
+  ctx->sampling_on = on;
+  k_set_sampling<<<1, 1, 0, ctx->sm>>>(ctx->P, on, on ? top_k : 0, on ? temperature : 1.f, (unsigned long long)seed);
   ++ctx->launches;
   CU(cudaStreamSynchronize(ctx->sm));
   return SPD_OK;
@@ -394,12 +428,8 @@ extern "C" int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value) {
     int v = value ? 1 : 0;
     int32_t *field = option == SPD_OPT_DEBUG_LOGITS ? &ctx->P.debug_logits : &ctx->P.prof_on;
     if (v != *field) {
-      *field = v;                // kernel parameter: captured graphs must be rebuilt
-      cudaStreamSynchronize(ctx->sm);
-      for (int e = 0; e < 2; ++e) {
-        if (ctx->graph[e]) cudaGraphExecDestroy(ctx->graph[e]);
-        ctx->graph[e] = nullptr; ctx->graph_tried[e] = 0;
-      }
+      *field = v;
+      drop_graphs(ctx);
     }
     return SPD_OK;
   }
@@ -431,7 +461,7 @@ extern "C" int spd_debug_read(spd_ctx *ctx, int32_t what, int32_t index, void *h
       src = P.h + (size_t)st->hbuf[index] * D.d; want = sizeof(float) * D.d; break;
     case SPD_DBG_EXIT_LOGITS:
     case SPD_DBG_PDM_LOGITS:
-      if (!P.debug_logits && ctx->engine == 1) return fail(ctx, SPD_ESTATE, "debug_read: enable SPD_OPT_DEBUG_LOGITS first%s");
+      if (!P.debug_logits && !P.sampling && ctx->engine == 1) return fail(ctx, SPD_ESTATE, "debug_read: enable SPD_OPT_DEBUG_LOGITS first%s");
       src = what == SPD_DBG_EXIT_LOGITS ? P.logits_v : P.logits_p; want = sizeof(float) * D.V; break;
     case SPD_DBG_PDM_PRENORM: src = P.pdm_u; want = sizeof(float) * D.d; break;
     case SPD_DBG_PDM_FEAT: src = P.feat; want = sizeof(float) * D.d * D.n; break;
@@ -439,6 +469,9 @@ extern "C" int spd_debug_read(spd_ctx *ctx, int32_t what, int32_t index, void *h
     case SPD_DBG_HFIN:
       if (index < 0 || index >= D.max_seq) return fail(ctx, SPD_EINVAL, "debug_read: position out of range%s");
       src = P.hfin + (size_t)index * D.d; want = sizeof(float) * D.d; break;
+    case SPD_DBG_SAMPLE:
+      if (!P.sampling) return fail(ctx, SPD_ESTATE, "debug_read: sampling verification is off%s");
+      src = &P.samp->rec; want = sizeof(SampleRecord); break;
     case SPD_DBG_PHASE_PROFILE:
       src = P.prof; want = sizeof(unsigned long long) * kProfCtas * kProfPhases * kProfStamps; break;
     case SPD_DBG_RING: {

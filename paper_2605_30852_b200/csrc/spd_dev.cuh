@@ -18,6 +18,36 @@ constexpr int kBarWords = kBarGroup0 + 32 * (kMaxStages + 2);
 // Optional per-phase clock stamps of the fused kernel (SPD_OPT_PHASE_PROFILE): [cta][phase][stamp]
 constexpr int kProfCtas = 160, kProfPhases = 168, kProfStamps = 6;
 
+// Sampling verification ("under sampling we apply standard rejection
+// sampling", :141 "T=1 ... top-k=50 and top-p=1.0"; readings S-1..S-9 of DESIGN.md).
+constexpr int kMaxTopK = 64;        // largest top_k
+constexpr int kSampCap = 2048;      // survivors of the threshold scan (above that: exact k-round selection)
+
+// A filtered distribution: support in ascending token id, fp32 probabilities (S-2).
+struct SampleDist {
+  int32_t k;
+  int32_t id[kMaxTopK];
+  float p[kMaxTopK];
+};
+// What the sampler of the last cycle saw and decided (SPD_DBG_SAMPLE).
+struct SampleRecord {
+  SampleDist draft;                  // Q_t of this cycle's PDM
+  SampleDist target;                 // P of this cycle's exit (or of the prefill's final head)
+  float u_draft, u_accept, u_resid;  // S-6 uniforms (-1: not drawn)
+  int32_t succ_token;                // the judged token, its stored draft probability and its target probability
+  float succ_q, succ_p;
+  int32_t exact_rounds;              // how many of the two selections took the exact k-round path
+  int32_t pad_;
+};
+struct SampleState {
+  int32_t on, top_k;
+  float temperature;
+  int32_t pad_;
+  unsigned long long seed;
+  SampleDist q[kMaxStages];          // indexed by hidden-buffer id: the distribution the token living there was drawn from
+  SampleRecord rec;
+};
+
 enum Mode : int32_t { MODE_IDLE = 0, MODE_SPD = 1, MODE_PREFILL = 2, MODE_PREFILL_FINAL = 3 };
 
 struct StepResult {
@@ -85,6 +115,10 @@ struct DevPtrs {
   const uint16_t *const *attn_norm, *const *wq, *const *wk, *const *wv, *const *wo, *const *mlp_norm,
       *const *w_gate, *const *w_up, *const *w_down;   // device arrays of [L] device pointers
   int32_t debug_logits;
+  int32_t sampling;                  // kernel parameter: 1 = sampling verification (the head keeps full logit vectors)
+  SampleState *samp;
+  float *samp_val;                   // [kSampCap] survivors of the top-k threshold scan
+  int32_t *samp_idx;                 // [kSampCap]
   int32_t nsplit_max;
   unsigned long long *prof;          // [kProfCtas][kProfPhases][kProfStamps] clock stamps (fused engine)
   int32_t prof_on;

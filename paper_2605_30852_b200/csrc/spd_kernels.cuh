@@ -182,14 +182,180 @@ __device__ __forceinline__ void rope_table_fill(const DevPtrs &P, int tid, int n
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Sampling verification (NEXT-2).  All of it runs in the controller CTA at the end of a cycle.
+
+// S-6: u(seed, K, j) = (splitmix64(seed + 3 K + j) >> 40) * 2^-24.
+__device__ __forceinline__ float samp_uniform(unsigned long long seed, long long K, int j) {
+  return (float)(splitmix64(seed + 3ull * (unsigned long long)K + (unsigned long long)j) >> 40) * (1.0f / 16777216.0f);
+}
+
+// S-2: the top_k entries of logits[0..V) in the order (value descending, index ascending), listed in ascending
+// token id with p = softmax(l / T) over them.  Whole CTA (>= 64 threads); `out` is global or shared memory.
+//   1. tau = the k-th best argmax candidate: the candidates are distinct entries, so at least k logits are
+//      >= tau and every top-k entry is;  2. one scan keeps the entries >= tau (about k .. 2k of them for
+//      near-i.i.d. logits);  3. each survivor's rank among the survivors decides membership.
+//   If fewer than k candidates exist or more than kSampCap entries survive (heavy ties, adversarial logits):
+//   k exact rounds of "best entry after the previous one".
+struct TopkSmem {   // shared-memory scratch of topk_dist (the caller says where it lives)
+  double e[kMaxTopK];
+  float sel_v[kMaxTopK], red_v[32], tau;
+  int sel_i[kMaxTopK], red_i[32], cnt, nvalid;
+};
+__device__ __forceinline__ void topk_dist(const float *logits, int V, const float *cand_val, const int32_t *cand_idx,
+                                          int ncand, int top_k, float temperature, float *surv_val,
+                                          int32_t *surv_idx, SampleDist *out, int32_t *exact_rounds, TopkSmem *ts) {
+  float &s_tau = ts->tau;
+  float *s_sel_v = ts->sel_v, *s_red_v = ts->red_v;
+  double *s_e = ts->e;
+  int &s_cnt = ts->cnt, &s_nvalid = ts->nvalid;
+  int *s_sel_i = ts->sel_i, *s_red_i = ts->red_i;
+  const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nt >> 5;
+  const int k = min(min(top_k, V), kMaxTopK);
+  if (tid == 0) { s_tau = -INFINITY; s_cnt = 0; s_nvalid = 0; }
+  __syncthreads();
+  for (int i = tid; i < ncand; i += nt) {
+    const int ix = cand_idx[i];
+    if (ix < 0) continue;
+    const float v = cand_val[i];
+    int better = 0;
+    for (int j = 0; j < ncand; ++j) {
+      const int jx = cand_idx[j];
+      if (jx >= 0 && cand_better(cand_val[j], jx, v, ix)) ++better;
+    }
+    atomicAdd(&s_nvalid, 1);
+    if (better == k - 1) s_tau = v;
+  }
+  __syncthreads();
+  bool exact = s_nvalid < k && V > kSampCap;
+  if (!exact) {
+    const float tau = s_nvalid < k ? -INFINITY : s_tau;
+    for (int i = tid; i < V; i += nt) {
+      const float v = __ldcg(logits + i);
+      if (v >= tau) {
+        const int pos = atomicAdd(&s_cnt, 1);
+        if (pos < kSampCap) { surv_val[pos] = v; surv_idx[pos] = i; }
+      }
+    }
+    __syncthreads();
+    const int m = s_cnt;
+    if (m > kSampCap) exact = true;
+    else
+      for (int i = tid; i < m; i += nt) {
+        const float v = surv_val[i];
+        const int ix = surv_idx[i];
+        int better = 0;
+        for (int j = 0; j < m; ++j) better += cand_better(surv_val[j], surv_idx[j], v, ix) ? 1 : 0;
+        if (better < k) { s_sel_v[better] = v; s_sel_i[better] = ix; }
+      }
+  }
+  if (exact) {   // uniform over the CTA: s_nvalid, s_cnt are shared
+    if (tid == 0 && exact_rounds) *exact_rounds += 1;
+    float pv = INFINITY;
+    int pi = -1;
+    for (int r = 0; r < k; ++r) {
+      float bv = -INFINITY;
+      int bi = 0x7fffffff;
+      for (int i = tid; i < V; i += nt) {
+        const float v = __ldcg(logits + i);
+        if (cand_better(pv, pi, v, i) && cand_better(v, i, bv, bi)) { bv = v; bi = i; }   // after the previous pick
+      }
+      for (int o = 16; o > 0; o >>= 1) {
+        const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (cand_better(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+      }
+      if (lane == 0) { s_red_v[warp] = bv; s_red_i[warp] = bi; }
+      __syncthreads();
+      if (tid == 0) {
+        for (int w = 1; w < nwarp; ++w)
+          if (cand_better(s_red_v[w], s_red_i[w], bv, bi)) { bv = s_red_v[w]; bi = s_red_i[w]; }
+        s_sel_v[r] = bv; s_sel_i[r] = bi;
+      }
+      __syncthreads();
+      pv = s_sel_v[r]; pi = s_sel_i[r];
+    }
+  }
+  __syncthreads();
+  // ascending token id, then softmax((l - max) / T): exponentials and their sum in fp64, p rounded to fp32
+  float lv = 0.f;
+  int rank = 0, ix = 0;
+  if (tid < k) {
+    ix = s_sel_i[tid]; lv = s_sel_v[tid];
+    for (int j = 0; j < k; ++j) rank += s_sel_i[j] < ix ? 1 : 0;
+  }
+  const float mx = s_sel_v[0];
+  __syncthreads();
+  if (tid < k) {
+    out->id[rank] = ix;
+    s_e[rank] = exp(((double)lv - (double)mx) / (double)temperature);
+  }
+  __syncthreads();
+  if (tid < k) {
+    double Z = 0.0;
+    for (int j = 0; j < k; ++j) Z += s_e[j];
+    out->p[tid] = (float)(s_e[tid] / Z);
+  }
+  if (tid == 0) out->k = k;
+  __syncthreads();
+}
+
+__device__ __forceinline__ double dist_prob(const SampleDist *D, int token) {
+  for (int i = 0; i < D->k; ++i)
+    if (D->id[i] == token) return (double)D->p[i];
+  return 0.0;
+}
+// S-3: inverse CDF over weights in list order, fp64: the smallest i with u * W < w_0 + .. + w_i.
+__device__ __forceinline__ int pick_index(const double *w, int k, double u) {
+  double W = 0.0;
+  for (int i = 0; i < k; ++i) W += w[i];
+  double c = 0.0;
+  int last = -1;
+  for (int i = 0; i < k; ++i) {
+    c += w[i];
+    if (w[i] > 0.0) last = i;
+    if (u * W < c) return i;
+  }
+  return last;
+}
+__device__ __forceinline__ int sample_cdf(const SampleDist *D, double u) {
+  double w[kMaxTopK];
+  for (int i = 0; i < D->k; ++i) w[i] = (double)D->p[i];
+  return D->id[pick_index(w, D->k, u)];
+}
+// The replacement of a rejected token: drawn from norm(max(0, P - Q)).
+__device__ __forceinline__ int sample_residual(const SampleDist *Pt, const SampleDist *Q, double u) {
+  double w[kMaxTopK], W = 0.0;
+  for (int i = 0; i < Pt->k; ++i) {
+    const double r = (double)Pt->p[i] - dist_prob(Q, Pt->id[i]);
+    w[i] = r > 0.0 ? r : 0.0;
+    W += w[i];
+  }
+  if (!(W > 0.0))
+    for (int i = 0; i < Pt->k; ++i) w[i] = (double)Pt->p[i];
+  return Pt->id[pick_index(w, Pt->k, u)];
+}
+
 // Controller, last part of a cycle (one CTA, >= 32 threads): reduce the argmax candidates, verify,
 // accept / reject + rollback, shift the pipeline, enter the next token, record.
 // Needs >= 64 threads.  `ncand` candidates per head (verify = row 0, PDM = row 1 of cand_val/cand_idx).
-__device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand) {
-  __shared__ int s_y, s_draft, s_exit_buf, s_exit_pos, s_enter_tok, s_enter_buf, s_do_exit, s_do_enter;
+// `ts`: shared-memory scratch for the sampler (may be nullptr when P.sampling == 0).
+__device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, TopkSmem *ts) {
+  __shared__ int s_y, s_draft, s_exit_buf, s_exit_pos, s_enter_tok, s_enter_buf, s_do_exit, s_do_enter, s_keep_q;
   StepState *st = P.st;
   const Dims &D = P.dim;
   int n = D.n;
+  SampleState *ss = P.samp;
+  const bool sampling = P.sampling != 0;
+  if (sampling) {   // filtered distributions of this cycle's PDM and exit logits (the heads kept the full vectors)
+    if (threadIdx.x == 0) ss->rec.exact_rounds = 0;
+    if (st->run_pdm)
+      topk_dist(P.logits_p, D.V, P.cand_val + kMaxCand, P.cand_idx + kMaxCand, ncand, ss->top_k, ss->temperature,
+                P.samp_val, P.samp_idx, &ss->rec.draft, &ss->rec.exact_rounds, ts);
+    if (st->run_verify)
+      topk_dist(P.logits_v, D.V, P.cand_val, P.cand_idx, ncand, ss->top_k, ss->temperature, P.samp_val, P.samp_idx,
+                &ss->rec.target, &ss->rec.exact_rounds, ts);
+  }
   if (threadIdx.x < 64) {
     // warp 0 = verify, warp 1 = PDM; lowest index among equal maxima ((value, index) is a total order,
     // so the result does not depend on the reduction shape)
@@ -216,7 +382,20 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand) {
     StepResult r;
     r.step_index = (int)st->K; r.fill = st->fill; r.exited = 0; r.accepted = 0; r.emitted_token = -1;
     r.draft_token = -1; r.draft_forced = 0; r.discarded = 0;
-    s_do_exit = 0; s_do_enter = 0;
+    s_do_exit = 0; s_do_enter = 0; s_keep_q = 0;
+    if (sampling) {
+      ss->rec.u_draft = ss->rec.u_accept = ss->rec.u_resid = -1.f;
+      ss->rec.succ_token = -1; ss->rec.succ_q = ss->rec.succ_p = 0.f;
+      if (!st->run_pdm) ss->rec.draft.k = 0;
+      if (!st->run_verify) ss->rec.target.k = 0;
+      if (mode == MODE_SPD) {                 // x^ ~ Q_t (S-3, j = 0)
+        ss->rec.u_draft = samp_uniform(ss->seed, st->K, 0);
+        draft = sample_cdf(&ss->rec.draft, (double)ss->rec.u_draft);
+      } else if (mode == MODE_PREFILL_FINAL) {   // the first token is drawn from P as well (j = 2, K = 0)
+        ss->rec.u_resid = samp_uniform(ss->seed, 0, 2);
+        y = sample_cdf(&ss->rec.target, (double)ss->rec.u_resid);
+      }
+    }
     s_exit_buf = st->hbuf[n - 1]; s_exit_pos = st->pos[n - 1];
     int enter_tok = -1, enter_pos = -1;
     bool flush = false;
@@ -227,11 +406,26 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand) {
         s_do_exit = 1;
         st->c = st->pos[n - 1] + 1;
         st->N += 1;
-        r.exited = 1; r.emitted_token = y;
+        r.exited = 1;
         int succ = n > 1 ? st->tok[n - 2] : draft;   // the token one stage behind (C-2.12 for n = 1)
-        if (succ == y) {
+        bool ok = succ == y;                         // greedy: exact argmax match
+        if (sampling) {                              // sampling: standard rejection sampling
+          const SampleDist *Qs = n > 1 ? &ss->q[st->hbuf[n - 2]] : &ss->rec.draft;
+          const double qx = dist_prob(Qs, succ), px = dist_prob(&ss->rec.target, succ);
+          ss->rec.succ_token = succ; ss->rec.succ_q = (float)qx; ss->rec.succ_p = (float)px;
+          ss->rec.u_accept = samp_uniform(ss->seed, st->K, 1);
+          ok = (double)ss->rec.u_accept * qx < px;
+          if (ok) y = succ;
+          else {                                     // the replacement ~ norm(max(0, P - Q)) (j = 2)
+            ss->rec.u_resid = samp_uniform(ss->seed, st->K, 2);
+            y = sample_residual(&ss->rec.target, Qs, (double)ss->rec.u_resid);
+          }
+        }
+        r.emitted_token = y;
+        if (ok) {
           r.accepted = 1;
           enter_tok = draft; enter_pos = st->p_new + 1;
+          s_keep_q = sampling;
         } else {
           r.discarded = st->fill - 1;
           for (int l = 0; l < D.L; ++l) if (P.len[l] > st->c) P.len[l] = st->c;   // truncate
@@ -240,6 +434,7 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand) {
         }
       } else {
         enter_tok = draft; enter_pos = st->p_new + 1;
+        s_keep_q = sampling;
       }
     } else if (mode == MODE_PREFILL) {
       if (exited) { s_do_exit = 1; st->c = st->pos[n - 1] + 1; }
@@ -265,6 +460,11 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand) {
     else if (mode == MODE_PREFILL_FINAL) P.results[0] = r;
   }
   __syncthreads();
+  if (s_keep_q) {      // the entering draft keeps the distribution it was drawn from, filed under its hidden buffer
+    const int32_t *src = reinterpret_cast<const int32_t *>(&ss->rec.draft);
+    int32_t *dst = reinterpret_cast<int32_t *>(&ss->q[s_enter_buf]);
+    for (int i = threadIdx.x; i < (int)(sizeof(SampleDist) / 4); i += blockDim.x) dst[i] = src[i];
+  }
   int d = D.d;   // d % 8 == 0
   if (s_do_exit) {     // Hfin[e.pos] = e.h  (C-2.4) — read before the buffer is reused below
     const float4 *src = reinterpret_cast<const float4 *>(P.h + (size_t)s_exit_buf * d);

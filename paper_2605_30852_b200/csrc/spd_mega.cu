@@ -830,7 +830,7 @@ __device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v,
       const int row = u * kTileRows + r16;
       if ((vec ? do_p : do_v) && row < D.V) {
         if (cand_better(y, row, bv, bi)) { bv = y; bi = row; }
-        if (P.debug_logits) (vec ? P.logits_p : P.logits_v)[row] = y;
+        if (P.debug_logits | P.sampling) (vec ? P.logits_p : P.logits_v)[row] = y;
       }
     }
     ++ucount;
@@ -1225,7 +1225,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
       __threadfence();
     }
     __syncthreads();
-    controller_end(P, ncta);
+    controller_end(P, ncta, reinterpret_cast<TopkSmem *>(ring));   // the tile ring is idle: every tile of the cycle was consumed
     for (int i = tid; i < np * kMaxStages; i += kThreads) P.claim[i] = 0u;   // every producer is done claiming
     if (tid < kMaxStages + 2) gbar[32 * tid] = 0u;                           // ... and every CTA with its group counters
     __syncthreads();

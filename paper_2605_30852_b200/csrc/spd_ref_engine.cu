@@ -3,6 +3,7 @@
 // (and the kernels behind the spd_op_* entry points); the fused persistent engine (spd_mega.cu) is the
 // fast one.  The two engines use different reduction orders, so each is compared with the CPU oracle,
 // not bitwise with the other.
+#include "../../include/spd.h"
 #include "spd_engine.h"
 #include "spd_kernels.cuh"
 
@@ -28,7 +29,10 @@ __global__ void k_pdm_gather(DevPtrs P) {
     P.feat[(size_t)j * d + i] = src ? src[i] : 0.f;
 }
 
-__global__ void k_end(DevPtrs P, int ncand) { controller_end(P, ncand); }
+__global__ void k_end(DevPtrs P, int ncand) {
+  __shared__ TopkSmem ts;
+  controller_end(P, ncand, &ts);
+}
 
 // ------------------------------------------------------------------ per-op kernels -------------
 // which: 0 attn_norm, 1 mlp_norm (per stage); 2 verify head input; 3 PDM head input
@@ -308,6 +312,36 @@ __global__ void k_op_argmax(const float *x, int n, int *out) {
   }
 }
 
+// Chunk maxima of x (grid = ncand CTAs): the argmax candidates that seed topk_dist's threshold.
+__global__ void k_op_cand(const float *x, int n, float *cand_val, int32_t *cand_idx) {
+  __shared__ float sv[32];
+  __shared__ int si[32];
+  int chunk = (n + gridDim.x - 1) / gridDim.x;
+  int lo = blockIdx.x * chunk, hi = min(n, lo + chunk);
+  float bv = -INFINITY;
+  int bi = 0x7fffffff;
+  for (int i = lo + threadIdx.x; i < hi; i += blockDim.x)
+    if (cand_better(x[i], i, bv, bi)) { bv = x[i]; bi = i; }
+  for (int o = 16; o > 0; o >>= 1) {
+    float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+    int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+    if (cand_better(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+  }
+  if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = bv; si[threadIdx.x >> 5] = bi; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w)
+      if (cand_better(sv[w], si[w], bv, bi)) { bv = sv[w]; bi = si[w]; }
+    cand_val[blockIdx.x] = bv;
+    cand_idx[blockIdx.x] = lo < hi ? bi : -1;
+  }
+}
+__global__ void __launch_bounds__(256) k_op_topk(const float *x, int n, int top_k, float temperature, int ncand,
+                                                 const float *cand_val, const int32_t *cand_idx, float *surv_val,
+                                                 int32_t *surv_idx, SampleDist *out) {
+  __shared__ TopkSmem ts;
+  topk_dist(x, n, cand_val, cand_idx, ncand, top_k, temperature, surv_val, surv_idx, out, nullptr, &ts);
+}
 }  // namespace spd
 
 using namespace spd;
@@ -360,5 +394,22 @@ extern "C" int spd_op_silu_mul(const float *gate, const float *up, int32_t n, fl
 extern "C" int spd_op_argmax(const float *x, int32_t n, int32_t *out_index, void *stream) {
   if (!x || !out_index || n < 1) return 1;
   k_op_argmax<<<1, 1024, 0, (cudaStream_t)stream>>>(x, n, out_index);
+  return op_done();
+}
+
+static const int kOpCand = 128;
+extern "C" size_t spd_op_topk_scratch(void) { return (size_t)kOpCand * 8 + (size_t)kSampCap * 8; }
+extern "C" int spd_op_topk_softmax(const float *x, int32_t n, int32_t top_k, float temperature, int32_t use_candidates,
+                                   spd_sample_dist *out, void *scratch, void *stream) {
+  static_assert(sizeof(spd_sample_dist) == sizeof(SampleDist), "dist layout");
+  if (!x || !out || !scratch || n < 1 || top_k < 1 || top_k > kMaxTopK || !(temperature > 0.f)) return 1;
+  float *cand_val = (float *)scratch;
+  int32_t *cand_idx = (int32_t *)(cand_val + kOpCand);
+  float *surv_val = (float *)(cand_idx + kOpCand);
+  int32_t *surv_idx = (int32_t *)(surv_val + kSampCap);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (use_candidates) k_op_cand<<<kOpCand, 256, 0, s>>>(x, n, cand_val, cand_idx);
+  k_op_topk<<<1, 256, 0, s>>>(x, n, top_k, temperature, use_candidates ? kOpCand : 0, cand_val, cand_idx, surv_val,
+                              surv_idx, reinterpret_cast<SampleDist *>(out));
   return op_done();
 }

@@ -165,3 +165,140 @@ def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, en
         ora.close()
         if own:
             gpu.close()
+
+
+# ------------------------------------------------------------------ sampling verification (NEXT-2) ----
+
+@dataclasses.dataclass
+class SamplingReport:
+    status: str = "ok"
+    detail: str = ""
+    steps: int = 0
+    emitted: int = 0
+    accepts: int = 0
+    rejects: int = 0
+    max_logit_abs_err: float = 0.0
+    max_prob_err: float = 0.0
+    max_hidden_err: float = 0.0
+    ties: tuple = (0, 0, 0, 0)       # hints adopted: support, draft, accept, replacement
+    exact_rounds: int = 0
+    tokens: list = dataclasses.field(default_factory=list)
+
+    def summary(self) -> str:
+        return (f"{self.status} steps={self.steps} emitted={self.emitted} acc/rej={self.accepts}/{self.rejects} "
+                f"logit_abs={self.max_logit_abs_err:.2e} prob={self.max_prob_err:.2e} hidden={self.max_hidden_err:.2e} "
+                f"ties(support/draft/accept/repl)={self.ties} exact_rounds={self.exact_rounds} {self.detail}")
+
+
+def _dist_close(g, o, delta):
+    """Same support; probabilities within what a logit difference `delta` allows (|dp| <= (e^(2 delta) - 1) p)."""
+    gi, gp = g
+    if not np.array_equal(gi, o.ids):
+        return False, float("inf")
+    err = np.abs(gp.astype(np.float64) - o.p.astype(np.float64))
+    lim = np.expm1(2.0 * delta) * o.p.astype(np.float64) + 2e-7
+    return bool(np.all(err <= lim)), float(err.max()) if err.size else 0.0
+
+
+def run_sampling_parity(shape, weights_np, dev_weights, prompt, n_tokens, temperature, top_k, seed, engine=None,
+                        tensor_tol=CONTRACT, max_seq=None, max_steps=None) -> SamplingReport:
+    """GPU vs oracle in sampling mode, cycle by cycle.  Exact: step results (tokens, accept bits, fill,
+    committed length), uniforms, supports, KV lengths.  Within tolerance: logits (tensor_tol, C-2.18),
+    probabilities (bounded by the measured logit difference), hidden states.
+
+    Decisions taken on floating point (top-k membership at the k-th/k+1-th boundary, inverse-CDF draws, the
+    accept test) may legitimately differ where the uniform / the logit lies within the measured logit
+    difference of the decision boundary.  The oracle is told what the CUDA path decided
+    (ora_step_sample_follow) and adopts it ONLY in that case (band = 3 x the largest logit difference measured
+    so far; the adoptions are counted in `ties`); any other difference fails."""
+    from paper_2605_30852_b200 import SPD, OPT
+    rep = SamplingReport()
+    n = shape.n_stages
+    ms = max_seq or (len(prompt) + n_tokens * (n + 1) + 2 * n + 8)
+    ora = Oracle(shape, weights_np, max_seq=ms)
+    gpu = SPD(shape, dev_weights, max_seq=ms)
+
+    def fail(msg):
+        rep.status, rep.detail = "fail", msg
+        return rep
+
+    try:
+        if engine is not None:
+            gpu.set_option(OPT.ENGINE, engine)
+        ora.set_sampling(temperature, top_k, seed)
+        gpu.set_sampling(temperature, top_k, seed)
+        fo = ora.prefill(prompt, block=16)
+        fg = gpu.prefill(prompt)
+        lo, lg = ora.last("exit_logits"), gpu.last("exit_logits")
+        delta_run = float(np.max(np.abs(lo.astype(np.float64) - lg)))
+        maxabs = float(np.max(np.abs(lo)))
+        rep.max_logit_abs_err = delta_run
+        if delta_run > tensor_tol * maxabs:
+            return fail(f"prefill logits differ by {delta_run:.3e} (max|logit| {maxabs:.3f})")
+        orec, grec = ora.sample_record(), gpu.sample_record()
+        if grec["u_resid"] != orec["u_resid"]:
+            return fail("first-token uniform differs")
+        ok, perr = _dist_close(grec["target"], orec["target"], delta_run)
+        if fo != fg or not ok:
+            return fail(f"first token {fg} vs oracle {fo}, distributions close: {ok} (prob err {perr:.2e})")
+        rep.max_prob_err = perr
+        rep.tokens.append(fg)
+        limit = max_steps or 10 ** 9
+        while ora.emitted < n_tokens and rep.steps < limit:
+            rg = gpu.step()
+            grec = gpu.sample_record()
+            band = 3.0 * delta_run + 1e-6 * maxabs
+            ro = ora.step_sample_follow(draft_ids=grec["draft"][0], verify_ids=grec["target"][0] if rg.exited else None,
+                                        draft_token=rg.draft_token, accepted=rg.accepted if rg.exited else -1,
+                                        emitted_token=rg.emitted_token if rg.exited and not rg.accepted else -1,
+                                        logit_band=band, prob_eps=4.0 * band)
+            orec = ora.sample_record()
+            rep.steps += 1
+            rep.ties = orec["ties"]
+            rep.exact_rounds += grec["exact_rounds"]
+            # logits first: they bound everything else
+            d = float(np.max(np.abs(ora.last("pdm_logits").astype(np.float64) - gpu.last("pdm_logits"))))
+            if ro.exited:
+                d = max(d, float(np.max(np.abs(ora.last("exit_logits").astype(np.float64) - gpu.last("exit_logits")))))
+                maxabs = max(maxabs, float(np.max(np.abs(ora.last("exit_logits")))))
+            rep.max_logit_abs_err = max(rep.max_logit_abs_err, d)
+            if d > tensor_tol * maxabs:
+                return fail(f"step {rep.steps}: logits differ by {d:.3e} (max|logit| {maxabs:.3f})")
+            if tuple(ro) != tuple(rg):
+                return fail(f"step {rep.steps}: gpu {tuple(rg)} != oracle {tuple(ro)} (band {band:.2e}, "
+                            f"u = {orec['u_draft']:.7f}/{orec['u_accept']:.7f}/{orec['u_resid']:.7f})")
+            for key in ("u_draft", "u_accept", "u_resid"):
+                if float(grec[key]) != float(orec[key]):
+                    return fail(f"step {rep.steps}: {key} gpu {grec[key]} != oracle {orec[key]}")
+            ok, perr = _dist_close(grec["draft"], orec["draft"], max(d, delta_run))
+            if not ok:
+                return fail(f"step {rep.steps}: draft distribution differs (prob err {perr:.2e})")
+            rep.max_prob_err = max(rep.max_prob_err, perr)
+            if ro.exited:
+                ok, perr = _dist_close(grec["target"], orec["target"], max(d, delta_run))
+                if not ok or grec["succ_token"] != orec["succ_token"]:
+                    return fail(f"step {rep.steps}: target distribution / judged token differs (prob err {perr:.2e})")
+                rep.max_prob_err = max(rep.max_prob_err, perr)
+                if abs(grec["succ_q"] - orec["succ_q"]) > np.expm1(2 * max(d, delta_run)) * orec["succ_q"] + 2e-7:
+                    return fail(f"step {rep.steps}: stored draft probability of the judged token differs")
+                rep.emitted += 1
+                rep.tokens.append(ro.emitted_token)
+                rep.accepts += ro.accepted
+                rep.rejects += 1 - ro.accepted
+            delta_run = max(delta_run, d)
+            fill, c, slots = gpu.ring()
+            if fill != ora.fill or c != ora.committed_len:
+                return fail(f"step {rep.steps}: ring fill/committed differ")
+            for i in range(ora.fill):
+                pos, tok, k, h = ora.ring(i)
+                if slots[k] != (1, pos, tok):
+                    return fail(f"step {rep.steps}: depth {k} holds {slots[k]}, oracle ({pos},{tok})")
+                rep.max_hidden_err = max(rep.max_hidden_err, rel_err(gpu.hidden(k), h))
+            if rep.max_hidden_err > tensor_tol:
+                return fail(f"step {rep.steps}: hidden rel err {rep.max_hidden_err:.3e}")
+            if not np.array_equal(gpu.kv_len(), ora.kv_len()):
+                return fail(f"step {rep.steps}: KV lengths differ")
+        return rep
+    finally:
+        ora.close()
+        gpu.close()

@@ -1,0 +1,151 @@
+"""GPU-vs-oracle parity of sampling verification (-m gpu), through the C ABI, for both
+engines: the top-k + temperature filter as a single operation, the whole cycle in sampling mode against the
+oracle (tests/_parity.py::run_sampling_parity), the special case top_k = 1 == the greedy path, and the
+full-size shapes (vocabulary 151 936, top-k 50, T = 1: the paper's setting)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as ora
+import spd_inputs as si
+from tests._parity import run_sampling_parity
+from tests._util import TINY, shape_of
+
+pytestmark = pytest.mark.gpu
+ENGINES = [0, 1]
+
+
+def _inputs(shape, prompt_len, seed=1234, std=0.02, random_gains=False):
+    import paper_2605_30852_b200 as spd
+    w = si.make_weights(shape, seed=seed, std=std, random_gains=random_gains)
+    return dict(shape=shape, weights_np=w, dev_weights=spd.upload_weights(w), prompt=si.make_prompt(shape, seed, prompt_len))
+
+
+# ------------------------------------------------------------------ the filter as one operation ---
+
+@pytest.mark.parametrize("use_candidates", [True, False])
+@pytest.mark.parametrize("V,k,T", [(151936, 50, 1.0), (151936, 64, 0.7), (1024, 50, 1.0), (64, 50, 1.0), (10, 50, 2.0),
+                                   (4097, 1, 1.0), (2049, 7, 1.3)])
+def test_topk_softmax_op(V, k, T, use_candidates):
+    """Both selection paths (threshold scan seeded by chunk maxima; exact k rounds when there are no
+    candidates and V > 2048) against the oracle's k-pass selection: supports exact, probabilities 1e-6."""
+    import paper_2605_30852_b200 as spd
+    rng = np.random.default_rng(V * 131 + k)
+    x = (rng.standard_normal(V) * 1.3).astype(np.float32)
+    ids, p = spd.op_topk_softmax(torch.from_numpy(x).cuda(), k, T, use_candidates)
+    want = ora.op_topk_softmax(x, k, T)
+    assert np.array_equal(ids, want.ids)
+    np.testing.assert_allclose(p, want.p, rtol=0, atol=1e-6)
+
+
+@pytest.mark.parametrize("use_candidates", [True, False])
+def test_topk_softmax_op_ties_and_flat_vectors(use_candidates):
+    """Equal values: lower index first (C-2.8 order); an all-equal vector (every entry survives the threshold:
+    the exact path) and a vector with heavy duplication at the k-th value."""
+    import paper_2605_30852_b200 as spd
+    for x in (np.zeros(5000, np.float32),
+              np.repeat(np.array([3.0, 2.0, 1.0], np.float32), 3000),
+              np.concatenate([np.full(40, 5.0, np.float32), np.full(4000, 1.0, np.float32), np.full(10, 5.0, np.float32)])):
+        ids, p = spd.op_topk_softmax(torch.from_numpy(x).cuda(), 50, 1.0, use_candidates)
+        want = ora.op_topk_softmax(x, 50, 1.0)
+        assert np.array_equal(ids, want.ids)
+        np.testing.assert_allclose(p, want.p, rtol=0, atol=1e-6)
+
+
+# ------------------------------------------------------------------ the cycle in sampling mode ----
+
+@pytest.mark.parametrize("engine", ENGINES)
+@pytest.mark.parametrize("n", [1, 2, 4, 8])
+def test_tiny_v64_paper_setting(engine, n):
+    """top-k 50, T = 1 on a 64-token vocabulary so that the PDM's and the target's supports
+    overlap: accepts and rejects both occur, every pipeline width."""
+    shape = shape_of("tiny", n, vocab=64)
+    rep = run_sampling_parity(**_inputs(shape, 32, std=0.08, random_gains=True), n_tokens=48, temperature=1.0,
+                              top_k=50, seed=77, engine=engine, tensor_tol=5e-3)
+    print(f"sampling tiny V=64 n={n} engine={engine}:", rep.summary())
+    assert rep.status == "ok", rep.detail
+    if n > 1:
+        assert rep.accepts > 0 and rep.rejects > 0
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+@pytest.mark.parametrize("T,k,seed", [(1.0, 50, 5), (2.0, 64, 6), (0.7, 8, 7)])
+def test_tiny_baseline_vocab(engine, T, k, seed):
+    """BASELINE.json's tiny shape (vocabulary 1024): the supports rarely overlap, so almost every exit is a
+    reject followed by a replacement draw, truncation and reseed (rollback stress)."""
+    shape = shape_of("tiny", 2)
+    rep = run_sampling_parity(**_inputs(shape, 32, std=0.08, random_gains=True), n_tokens=40, temperature=T,
+                              top_k=k, seed=seed, engine=engine, tensor_tol=5e-3)
+    print(f"sampling tiny T={T} k={k} engine={engine}:", rep.summary())
+    assert rep.status == "ok", rep.detail
+    assert rep.rejects > 0
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+def test_top_k_one_is_the_greedy_path(engine):
+    """top_k = 1: every step result equals the greedy run of the same library ("exact argmax
+    match"), and the KV lengths agree."""
+    import paper_2605_30852_b200 as spd
+    shape = shape_of("tiny", 4)
+    inp = _inputs(shape, 32, std=0.08, random_gains=True)
+    a = spd.SPD(shape, inp["dev_weights"], max_seq=512)
+    b = spd.SPD(shape, inp["dev_weights"], max_seq=512)
+    try:
+        for g in (a, b):
+            g.set_option(spd.OPT.ENGINE, engine)
+        b.set_sampling(1.0, 1, 99)
+        assert a.prefill(inp["prompt"]) == b.prefill(inp["prompt"])
+        for _ in range(80):
+            assert tuple(a.step()) == tuple(b.step())
+        assert np.array_equal(a.kv_len(), b.kv_len())
+    finally:
+        a.close(); b.close()
+
+
+def test_sampling_errors_and_switching():
+    import paper_2605_30852_b200 as spd
+    shape = shape_of("tiny", 2)
+    inp = _inputs(shape, 16)
+    g = spd.SPD(shape, inp["dev_weights"], max_seq=256)
+    try:
+        for bad in ((1.0, 65), (0.0, 50), (-1.0, 50)):
+            with pytest.raises(spd.SpdError) as e:
+                g.set_sampling(bad[0], bad[1], 1)
+            assert e.value.status == 1                       # SPD_EINVAL
+        g.set_forced(np.zeros(8, np.int32), 0.5, 1)
+        with pytest.raises(spd.SpdError) as e:
+            g.set_sampling(1.0, 50, 1)
+        assert e.value.status == 2                           # SPD_ESTATE
+        g.set_forced(None, -1.0, 0)
+        g.set_sampling(1.0, 50, 1)
+        with pytest.raises(spd.SpdError) as e:
+            g.set_forced(np.zeros(8, np.int32), 0.5, 1)
+        assert e.value.status == 2
+        # sampling -> greedy -> sampling on a live sequence; the greedy stretch matches a never-sampled run
+        ref = spd.SPD(shape, inp["dev_weights"], max_seq=256)
+        g.set_sampling(1.0, 0, 0)
+        assert g.prefill(inp["prompt"]) == ref.prefill(inp["prompt"])
+        for _ in range(10):
+            assert tuple(g.step()) == tuple(ref.step())
+        ref.close()
+        g.set_sampling(1.0, 50, 3)
+        for _ in range(10):
+            r = g.step()
+            rec = g.sample_record()
+            assert len(rec["draft"][0]) == 50 and abs(float(rec["draft"][1].sum()) - 1.0) < 1e-5
+            assert r.draft_token in rec["draft"][0]
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+@pytest.mark.parametrize("name,prompt_len,gen", [("4b_n4", 24, 8), ("9b_n4", 20, 6)])
+def test_full_model_dims_paper_setting(engine, name, prompt_len, gen):
+    """The 4B/9B-class shapes (vocabulary 151 936) with top-k 50, T = 1: the threshold scan over the real
+    vocabulary inside the cycle, 148 per-CTA candidates (fused engine) / 128 chunk candidates (reference)."""
+    shape = si.CONFIGS[name]
+    rep = run_sampling_parity(**_inputs(shape, prompt_len), n_tokens=gen, temperature=1.0, top_k=50, seed=11,
+                              engine=engine, tensor_tol=1e-2, max_steps=4 * gen)
+    print(f"sampling {name} engine={engine}:", rep.summary())
+    assert rep.status == "ok", rep.detail
+    assert rep.exact_rounds == 0          # the threshold path was the one that ran
