@@ -290,6 +290,30 @@ def run_gpu(args, shape):
                          "mean_step_us": ms * 1e3 / len(log), "lossless_vs_greedy": bool(ok),
                          "fill_hist": {str(a): sum(1 for r in log if r.fill == a) for a in range(1, n + 1)}}
 
+    # ---- sampling verification (NEXT-2; PAPER.md:141 T=1, top-k 50): cycle latency next to the greedy path on the
+    # same fill pattern.  Random-init PDM and target supports are disjoint, so both runs reject at every exit
+    # (fill 1..n round robin); the difference is the cost of keeping the logit vectors + the top-k selection.
+    def timed_cycles(k):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        eng.step_many(n)
+        e0.record(stream)
+        log = eng.step_many(k)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e3 / k, log
+
+    ks = min(256, need - 2 * n)
+    rewind(-1.0)                                                # greedy, the PDM's own drafts
+    g_us, g_log = timed_cycles(ks)
+    eng.rollback(P, first)
+    eng.set_sampling(1.0, 50, args.seed)
+    s_us, s_log = timed_cycles(ks)
+    eng.set_sampling(1.0, 0, 0)
+    hist = lambda log: {str(a): sum(1 for r in log if r.fill == a) for a in range(1, n + 1)}
+    sampling = {"temperature": 1.0, "top_k": 50, "cycles": ks, "mean_step_us": s_us, "greedy_same_drafts_mean_step_us": g_us,
+                "overhead_us": s_us - g_us, "accept_rate": sum(r.accepted for r in s_log) / max(1, sum(r.exited for r in s_log)),
+                "fill_hist": hist(s_log), "greedy_fill_hist": hist(g_log)}
+
     local = {"step_us": step_us, "e2e_us": e2e_us, "kernel_us": step_us, "tokens_per_s": 1e6 / step_us,
              "hbm_gbs": by["full"] / step_us / 1e3, "gpu_launches": launches}
     tot = aggregate(local, world)
@@ -317,7 +341,8 @@ def run_gpu(args, shape):
         "e2e": {"value": tot["e2e_us"], "unit": "us", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": d2h,
                 "note": "spd_step(): launch + result/state D2H + stream sync per cycle; the cycle has no per-step host input "
                         "(ring, KV and lengths live on the device)"},
-        "gpu_launches": int(tot["gpu_launches"]), "clocks": clk, "p_sweep": sweep, "setup_s": t_setup,
+        "gpu_launches": int(tot["gpu_launches"]), "clocks": clk, "p_sweep": sweep, "sampling": sampling,
+        "setup_s": t_setup,
     }
     if world == 1 and not args.no_cpu_baseline:
         med, timed, threads = oracle_saturated_cycle_us(shape, w_np, ctx_mid, 3, budget_s=60.0)

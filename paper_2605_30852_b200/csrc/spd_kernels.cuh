@@ -230,13 +230,30 @@ __device__ __forceinline__ void topk_dist(const float *logits, int V, const floa
   bool exact = s_nvalid < k && V > kSampCap;
   if (!exact) {
     const float tau = s_nvalid < k ? -INFINITY : s_tau;
-    for (int i = tid; i < V; i += nt) {
-      const float v = __ldcg(logits + i);
+    auto keep = [&](float v, int i) {
       if (v >= tau) {
         const int pos = atomicAdd(&s_cnt, 1);
         if (pos < kSampCap) { surv_val[pos] = v; surv_idx[pos] = i; }
       }
+    };
+    // the vector sits in L2: 8 independent 16-byte loads per thread and round keep the one scanning SM busy
+    constexpr int U = 8;
+    const int n4 = (reinterpret_cast<uintptr_t>(logits) & 15) == 0 ? V >> 2 : 0;
+    const float4 *l4 = reinterpret_cast<const float4 *>(logits);
+    for (int base = 0; base < n4; base += nt * U) {
+      float4 v[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int i = base + u * nt + tid;
+        if (i < n4) v[u] = __ldcg(l4 + i);
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int i = base + u * nt + tid;
+        if (i < n4) { keep(v[u].x, 4 * i); keep(v[u].y, 4 * i + 1); keep(v[u].z, 4 * i + 2); keep(v[u].w, 4 * i + 3); }
+      }
     }
+    for (int i = 4 * n4 + tid; i < V; i += nt) keep(__ldcg(logits + i), i);
     __syncthreads();
     const int m = s_cnt;
     if (m > kSampCap) exact = true;
@@ -300,6 +317,12 @@ __device__ __forceinline__ void topk_dist(const float *logits, int V, const floa
   __syncthreads();
 }
 
+// Shared-memory working set of the sampler in the controller CTA.
+struct SampSmem {
+  TopkSmem tk;
+  SampleDist qd, pt, qs;            // this cycle's draft / target distributions, the judged token's stored one
+  double w[kMaxTopK];               // residual weights max(0, P - Q) over P's support
+};
 __device__ __forceinline__ double dist_prob(const SampleDist *D, int token) {
   for (int i = 0; i < D->k; ++i)
     if (D->id[i] == token) return (double)D->p[i];
@@ -319,28 +342,31 @@ __device__ __forceinline__ int pick_index(const double *w, int k, double u) {
   return last;
 }
 __device__ __forceinline__ int sample_cdf(const SampleDist *D, double u) {
-  double w[kMaxTopK];
-  for (int i = 0; i < D->k; ++i) w[i] = (double)D->p[i];
-  return D->id[pick_index(w, D->k, u)];
-}
-// The replacement of a rejected token: drawn from norm(max(0, P - Q)).
-__device__ __forceinline__ int sample_residual(const SampleDist *Pt, const SampleDist *Q, double u) {
-  double w[kMaxTopK], W = 0.0;
-  for (int i = 0; i < Pt->k; ++i) {
-    const double r = (double)Pt->p[i] - dist_prob(Q, Pt->id[i]);
-    w[i] = r > 0.0 ? r : 0.0;
-    W += w[i];
+  double W = 0.0;
+  for (int i = 0; i < D->k; ++i) W += (double)D->p[i];
+  double c = 0.0;
+  int last = -1;
+  for (int i = 0; i < D->k; ++i) {
+    c += (double)D->p[i];
+    if (D->p[i] > 0.f) last = i;
+    if (u * W < c) return D->id[i];
   }
-  if (!(W > 0.0))
-    for (int i = 0; i < Pt->k; ++i) w[i] = (double)Pt->p[i];
-  return Pt->id[pick_index(w, Pt->k, u)];
+  return D->id[last];
+}
+// The replacement of a rejected token: drawn from norm(max(0, P - Q)); w = those
+// weights over P's support (computed by the CTA in parallel), all zero -> P itself.
+__device__ __forceinline__ int sample_residual(const SampleDist *Pt, const double *w, double u) {
+  double W = 0.0;
+  for (int i = 0; i < Pt->k; ++i) W += w[i];
+  if (W > 0.0) return Pt->id[pick_index(w, Pt->k, u)];
+  return sample_cdf(Pt, u);
 }
 
 // Controller, last part of a cycle (one CTA, >= 32 threads): reduce the argmax candidates, verify,
 // accept / reject + rollback, shift the pipeline, enter the next token, record.
 // Needs >= 64 threads.  `ncand` candidates per head (verify = row 0, PDM = row 1 of cand_val/cand_idx).
-// `ts`: shared-memory scratch for the sampler (may be nullptr when P.sampling == 0).
-__device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, TopkSmem *ts) {
+// `sm`: shared-memory scratch for the sampler (may be nullptr when P.sampling == 0).
+__device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, SampSmem *sm) {
   __shared__ int s_y, s_draft, s_exit_buf, s_exit_pos, s_enter_tok, s_enter_buf, s_do_exit, s_do_enter, s_keep_q;
   StepState *st = P.st;
   const Dims &D = P.dim;
@@ -348,13 +374,33 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, Topk
   SampleState *ss = P.samp;
   const bool sampling = P.sampling != 0;
   if (sampling) {   // filtered distributions of this cycle's PDM and exit logits (the heads kept the full vectors)
-    if (threadIdx.x == 0) ss->rec.exact_rounds = 0;
+    if (threadIdx.x == 0) { ss->rec.exact_rounds = 0; sm->qd.k = 0; sm->pt.k = 0; sm->qs.k = 0; }
+    __syncthreads();
     if (st->run_pdm)
       topk_dist(P.logits_p, D.V, P.cand_val + kMaxCand, P.cand_idx + kMaxCand, ncand, ss->top_k, ss->temperature,
-                P.samp_val, P.samp_idx, &ss->rec.draft, &ss->rec.exact_rounds, ts);
+                P.samp_val, P.samp_idx, &sm->qd, &ss->rec.exact_rounds, &sm->tk);
     if (st->run_verify)
       topk_dist(P.logits_v, D.V, P.cand_val, P.cand_idx, ncand, ss->top_k, ss->temperature, P.samp_val, P.samp_idx,
-                &ss->rec.target, &ss->rec.exact_rounds, ts);
+                &sm->pt, &ss->rec.exact_rounds, &sm->tk);
+    // the judged token's stored distribution (n = 1: the draft of this very cycle, C-2.12) and the residual
+    // weights, which depend on P and Q only — ready before thread 0 takes the decisions
+    const bool judging = st->mode == MODE_SPD && st->occ[n - 1];
+    constexpr int DW = (int)(sizeof(SampleDist) / 4);
+    if (judging) {
+      const int32_t *src = n > 1 ? reinterpret_cast<const int32_t *>(&ss->q[st->hbuf[n - 2]])
+                                 : reinterpret_cast<const int32_t *>(&sm->qd);
+      for (int i = threadIdx.x; i < DW; i += blockDim.x) reinterpret_cast<int32_t *>(&sm->qs)[i] = src[i];
+    }
+    for (int i = threadIdx.x; i < DW; i += blockDim.x) {   // the record of this cycle (SPD_DBG_SAMPLE)
+      reinterpret_cast<int32_t *>(&ss->rec.draft)[i] = reinterpret_cast<const int32_t *>(&sm->qd)[i];
+      reinterpret_cast<int32_t *>(&ss->rec.target)[i] = reinterpret_cast<const int32_t *>(&sm->pt)[i];
+    }
+    __syncthreads();
+    if (judging && (int)threadIdx.x < sm->pt.k) {
+      const double r = (double)sm->pt.p[threadIdx.x] - dist_prob(&sm->qs, sm->pt.id[threadIdx.x]);
+      sm->w[threadIdx.x] = r > 0.0 ? r : 0.0;
+    }
+    __syncthreads();
   }
   if (threadIdx.x < 64) {
     // warp 0 = verify, warp 1 = PDM; lowest index among equal maxima ((value, index) is a total order,
@@ -386,14 +432,12 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, Topk
     if (sampling) {
       ss->rec.u_draft = ss->rec.u_accept = ss->rec.u_resid = -1.f;
       ss->rec.succ_token = -1; ss->rec.succ_q = ss->rec.succ_p = 0.f;
-      if (!st->run_pdm) ss->rec.draft.k = 0;
-      if (!st->run_verify) ss->rec.target.k = 0;
       if (mode == MODE_SPD) {                 // x^ ~ Q_t (S-3, j = 0)
         ss->rec.u_draft = samp_uniform(ss->seed, st->K, 0);
-        draft = sample_cdf(&ss->rec.draft, (double)ss->rec.u_draft);
+        draft = sample_cdf(&sm->qd, (double)ss->rec.u_draft);
       } else if (mode == MODE_PREFILL_FINAL) {   // the first token is drawn from P as well (j = 2, K = 0)
         ss->rec.u_resid = samp_uniform(ss->seed, 0, 2);
-        y = sample_cdf(&ss->rec.target, (double)ss->rec.u_resid);
+        y = sample_cdf(&sm->pt, (double)ss->rec.u_resid);
       }
     }
     s_exit_buf = st->hbuf[n - 1]; s_exit_pos = st->pos[n - 1];
@@ -410,15 +454,14 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, Topk
         int succ = n > 1 ? st->tok[n - 2] : draft;   // the token one stage behind (C-2.12 for n = 1)
         bool ok = succ == y;                         // greedy: exact argmax match
         if (sampling) {                              // sampling: standard rejection sampling
-          const SampleDist *Qs = n > 1 ? &ss->q[st->hbuf[n - 2]] : &ss->rec.draft;
-          const double qx = dist_prob(Qs, succ), px = dist_prob(&ss->rec.target, succ);
+          const double qx = dist_prob(&sm->qs, succ), px = dist_prob(&sm->pt, succ);
           ss->rec.succ_token = succ; ss->rec.succ_q = (float)qx; ss->rec.succ_p = (float)px;
           ss->rec.u_accept = samp_uniform(ss->seed, st->K, 1);
           ok = (double)ss->rec.u_accept * qx < px;
           if (ok) y = succ;
           else {                                     // the replacement ~ norm(max(0, P - Q)) (j = 2)
             ss->rec.u_resid = samp_uniform(ss->seed, st->K, 2);
-            y = sample_residual(&ss->rec.target, Qs, (double)ss->rec.u_resid);
+            y = sample_residual(&sm->pt, sm->w, (double)ss->rec.u_resid);
           }
         }
         r.emitted_token = y;
@@ -461,7 +504,7 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, Topk
   }
   __syncthreads();
   if (s_keep_q) {      // the entering draft keeps the distribution it was drawn from, filed under its hidden buffer
-    const int32_t *src = reinterpret_cast<const int32_t *>(&ss->rec.draft);
+    const int32_t *src = reinterpret_cast<const int32_t *>(&sm->qd);
     int32_t *dst = reinterpret_cast<int32_t *>(&ss->q[s_enter_buf]);
     for (int i = threadIdx.x; i < (int)(sizeof(SampleDist) / 4); i += blockDim.x) dst[i] = src[i];
   }

@@ -1225,7 +1225,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
       __threadfence();
     }
     __syncthreads();
-    controller_end(P, ncta, reinterpret_cast<TopkSmem *>(ring));   // the tile ring is idle: every tile of the cycle was consumed
+    controller_end(P, ncta, reinterpret_cast<SampSmem *>(ring));   // the tile ring is idle: every tile of the cycle was consumed
     for (int i = tid; i < np * kMaxStages; i += kThreads) P.claim[i] = 0u;   // every producer is done claiming
     if (tid < kMaxStages + 2) gbar[32 * tid] = 0u;                           // ... and every CTA with its group counters
     __syncthreads();

@@ -30,8 +30,8 @@ __global__ void k_pdm_gather(DevPtrs P) {
 }
 
 __global__ void k_end(DevPtrs P, int ncand) {
-  __shared__ TopkSmem ts;
-  controller_end(P, ncand, &ts);
+  __shared__ SampSmem sm;
+  controller_end(P, ncand, &sm);
 }
 
 // ------------------------------------------------------------------ per-op kernels -------------
