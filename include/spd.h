@@ -195,7 +195,7 @@ typedef struct {
   int32_t succ_token;      /* the judged token (-1: none), its stored draft probability, its target probability */
   float succ_q, succ_p;
   int32_t exact_rounds;    /* selections of this cycle that took the exact k-round path (0..2)          */
-  int32_t pad_;
+  int32_t prefiltered;     /* selections served by the head pass's threshold list, no scan (0..2)       */
 } spd_sample_record;
 int spd_set_sampling(spd_ctx *ctx, float temperature, int32_t top_k, uint64_t seed);
 

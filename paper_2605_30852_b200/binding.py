@@ -47,7 +47,7 @@ class _Dist(C.Structure):
 class _SampleRec(C.Structure):
     _fields_ = [("draft", _Dist), ("target", _Dist), ("u_draft", C.c_float), ("u_accept", C.c_float),
                 ("u_resid", C.c_float), ("succ_token", C.c_int32), ("succ_q", C.c_float), ("succ_p", C.c_float),
-                ("exact_rounds", C.c_int32), ("pad_", C.c_int32)]
+                ("exact_rounds", C.c_int32), ("prefiltered", C.c_int32)]
 
 
 def _dist_out(d: _Dist):
@@ -262,7 +262,7 @@ class SPD:
         self._check(lib().spd_debug_read(self._h, DBG.SAMPLE, 0, C.addressof(r), C.sizeof(r)))
         return dict(draft=_dist_out(r.draft), target=_dist_out(r.target), u_draft=r.u_draft, u_accept=r.u_accept,
                     u_resid=r.u_resid, succ_token=r.succ_token, succ_q=r.succ_q, succ_p=r.succ_p,
-                    exact_rounds=r.exact_rounds)
+                    exact_rounds=r.exact_rounds, prefiltered=r.prefiltered)
 
     def set_option(self, option: int, value: int):
         self._check(lib().spd_set_option(self._h, option, value))

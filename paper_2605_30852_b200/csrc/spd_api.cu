@@ -124,6 +124,8 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
   Q.samp = cv.take<SampleState>(1);
   Q.samp_val = cv.take<float>(kSampCap);
   Q.samp_idx = cv.take<int32_t>(kSampCap);
+  Q.pre_val = cv.take<float>(2 * kSampCap);
+  Q.pre_idx = cv.take<int32_t>(2 * kSampCap);
   const uint16_t **tabs[9];
   for (int i = 0; i < 9; ++i) tabs[i] = cv.take<const uint16_t *>(D.L);
   Q.attn_norm = tabs[0]; Q.wq = tabs[1]; Q.wk = tabs[2]; Q.wv = tabs[3]; Q.wo = tabs[4];
@@ -168,6 +170,8 @@ __global__ void k_set_forced(DevPtrs P, int on, int n_truth, unsigned long long 
 }
 __global__ void k_set_sampling(DevPtrs P, int on, int top_k, float temperature, unsigned long long seed) {
   P.samp->on = on; P.samp->top_k = top_k; P.samp->temperature = temperature; P.samp->seed = seed;
+  P.samp->pre_cnt[0] = P.samp->pre_cnt[1] = 0;
+  P.samp->tau_guess[0] = P.samp->tau_guess[1] = INFINITY;
 }
 // External truncate + flush + reseed (PAPER.md:131 with c := new_len).
 __global__ void k_rollback(DevPtrs P, int new_len, int tok) {

@@ -37,13 +37,15 @@ struct SampleRecord {
   int32_t succ_token;                // the judged token, its stored draft probability and its target probability
   float succ_q, succ_p;
   int32_t exact_rounds;              // how many of the two selections took the exact k-round path
-  int32_t pad_;
+  int32_t prefiltered;               // ... and how many used the head pass's threshold list (no scan)
 };
 struct SampleState {
   int32_t on, top_k;
   float temperature;
   int32_t pad_;
   unsigned long long seed;
+  int32_t pre_cnt[2];                // entries the head pass listed this cycle (0 verify, 1 PDM); may exceed kSampCap
+  float tau_guess[2];                // the list threshold of the next head pass (+inf: none yet)
   SampleDist q[kMaxStages];          // indexed by hidden-buffer id: the distribution the token living there was drawn from
   SampleRecord rec;
 };
@@ -119,6 +121,8 @@ struct DevPtrs {
   SampleState *samp;
   float *samp_val;                   // [kSampCap] survivors of the top-k threshold scan
   int32_t *samp_idx;                 // [kSampCap]
+  float *pre_val;                    // [2][kSampCap] logits >= tau_guess listed by the fused head pass
+  int32_t *pre_idx;                  // [2][kSampCap]
   int32_t nsplit_max;
   unsigned long long *prof;          // [kProfCtas][kProfPhases][kProfStamps] clock stamps (fused engine)
   int32_t prof_on;

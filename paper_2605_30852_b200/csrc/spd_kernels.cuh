@@ -201,10 +201,23 @@ struct TopkSmem {   // shared-memory scratch of topk_dist (the caller says where
   double e[kMaxTopK];
   float sel_v[kMaxTopK], red_v[32], tau;
   int sel_i[kMaxTopK], red_i[32], cnt, nvalid;
+  float sv[kSampCap];               // the survivors, staged for the all-pairs ranking
+  int si[kSampCap];
+};
+//   0. (fused engine) the head pass itself listed every logit >= a guessed threshold (the previous cycle's k-th
+//      value minus a margin) while the value was in a register: if that list holds between k and kSampCap
+//      entries it contains the whole top-k and replaces steps 1-2 (no second pass over the logits); otherwise
+//      the scan runs.  pre_cnt < 0: no such list.  *next_guess receives the threshold for the next cycle.
+struct TopkPre {
+  const float *val;
+  const int32_t *idx;
+  int cnt;
 };
 __device__ __forceinline__ void topk_dist(const float *logits, int V, const float *cand_val, const int32_t *cand_idx,
                                           int ncand, int top_k, float temperature, float *surv_val,
-                                          int32_t *surv_idx, SampleDist *out, int32_t *exact_rounds, TopkSmem *ts) {
+                                          int32_t *surv_idx, SampleDist *out, int32_t *exact_rounds, TopkSmem *ts,
+                                          TopkPre pre = TopkPre{nullptr, nullptr, -1}, int32_t *prefiltered = nullptr,
+                                          float *next_guess = nullptr) {
   float &s_tau = ts->tau;
   float *s_sel_v = ts->sel_v, *s_red_v = ts->red_v;
   double *s_e = ts->e;
@@ -214,7 +227,13 @@ __device__ __forceinline__ void topk_dist(const float *logits, int V, const floa
   const int k = min(min(top_k, V), kMaxTopK);
   if (tid == 0) { s_tau = -INFINITY; s_cnt = 0; s_nvalid = 0; }
   __syncthreads();
-  for (int i = tid; i < ncand; i += nt) {
+  const bool use_pre = pre.cnt >= k && pre.cnt <= kSampCap;
+  if (use_pre) {
+    if (tid == 0 && prefiltered) *prefiltered += 1;
+    surv_val = const_cast<float *>(pre.val);
+    surv_idx = const_cast<int32_t *>(pre.idx);
+  }
+  for (int i = tid; i < (use_pre ? 0 : ncand); i += nt) {
     const int ix = cand_idx[i];
     if (ix < 0) continue;
     const float v = cand_val[i];
@@ -227,7 +246,7 @@ __device__ __forceinline__ void topk_dist(const float *logits, int V, const floa
     if (better == k - 1) s_tau = v;
   }
   __syncthreads();
-  bool exact = s_nvalid < k && V > kSampCap;
+  bool exact = !use_pre && s_nvalid < k && V > kSampCap;
   if (!exact) {
     const float tau = s_nvalid < k ? -INFINITY : s_tau;
     auto keep = [&](float v, int i) {
@@ -238,7 +257,7 @@ __device__ __forceinline__ void topk_dist(const float *logits, int V, const floa
     };
     // the vector sits in L2: 8 independent 16-byte loads per thread and round keep the one scanning SM busy
     constexpr int U = 8;
-    const int n4 = (reinterpret_cast<uintptr_t>(logits) & 15) == 0 ? V >> 2 : 0;
+    const int n4 = use_pre ? 0 : ((reinterpret_cast<uintptr_t>(logits) & 15) == 0 ? V >> 2 : 0);
     const float4 *l4 = reinterpret_cast<const float4 *>(logits);
     for (int base = 0; base < n4; base += nt * U) {
       float4 v[U];
@@ -253,18 +272,21 @@ __device__ __forceinline__ void topk_dist(const float *logits, int V, const floa
         if (i < n4) { keep(v[u].x, 4 * i); keep(v[u].y, 4 * i + 1); keep(v[u].z, 4 * i + 2); keep(v[u].w, 4 * i + 3); }
       }
     }
-    for (int i = 4 * n4 + tid; i < V; i += nt) keep(__ldcg(logits + i), i);
+    for (int i = 4 * n4 + tid; i < (use_pre ? 0 : V); i += nt) keep(__ldcg(logits + i), i);
     __syncthreads();
-    const int m = s_cnt;
+    const int m = use_pre ? pre.cnt : s_cnt;
     if (m > kSampCap) exact = true;
-    else
+    else {
+      for (int i = tid; i < m; i += nt) { ts->sv[i] = __ldcg(surv_val + i); ts->si[i] = __ldcg(surv_idx + i); }
+      __syncthreads();
       for (int i = tid; i < m; i += nt) {
-        const float v = surv_val[i];
-        const int ix = surv_idx[i];
+        const float v = ts->sv[i];
+        const int ix = ts->si[i];
         int better = 0;
-        for (int j = 0; j < m; ++j) better += cand_better(surv_val[j], surv_idx[j], v, ix) ? 1 : 0;
+        for (int j = 0; j < m; ++j) better += cand_better(ts->sv[j], ts->si[j], v, ix) ? 1 : 0;
         if (better < k) { s_sel_v[better] = v; s_sel_i[better] = ix; }
       }
+    }
   }
   if (exact) {   // uniform over the CTA: s_nvalid, s_cnt are shared
     if (tid == 0 && exact_rounds) *exact_rounds += 1;
@@ -302,6 +324,10 @@ __device__ __forceinline__ void topk_dist(const float *logits, int V, const floa
     for (int j = 0; j < k; ++j) rank += s_sel_i[j] < ix ? 1 : 0;
   }
   const float mx = s_sel_v[0];
+  if (tid == 0 && next_guess) {   // next cycle's list threshold: this cycle's k-th value minus a margin
+    const float kth = s_sel_v[k - 1];
+    *next_guess = kth - fmaxf(0.5f * (mx - kth), 0.1f + 0.05f * fabsf(kth));
+  }
   __syncthreads();
   if (tid < k) {
     out->id[rank] = ix;
@@ -366,7 +392,8 @@ __device__ __forceinline__ int sample_residual(const SampleDist *Pt, const doubl
 // accept / reject + rollback, shift the pipeline, enter the next token, record.
 // Needs >= 64 threads.  `ncand` candidates per head (verify = row 0, PDM = row 1 of cand_val/cand_idx).
 // `sm`: shared-memory scratch for the sampler (may be nullptr when P.sampling == 0).
-__device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, SampSmem *sm) {
+// `with_lists`: the head pass filled the threshold lists (fused engine).
+__device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, SampSmem *sm, bool with_lists = false) {
   __shared__ int s_y, s_draft, s_exit_buf, s_exit_pos, s_enter_tok, s_enter_buf, s_do_exit, s_do_enter, s_keep_q;
   StepState *st = P.st;
   const Dims &D = P.dim;
@@ -374,14 +401,19 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, Samp
   SampleState *ss = P.samp;
   const bool sampling = P.sampling != 0;
   if (sampling) {   // filtered distributions of this cycle's PDM and exit logits (the heads kept the full vectors)
-    if (threadIdx.x == 0) { ss->rec.exact_rounds = 0; sm->qd.k = 0; sm->pt.k = 0; sm->qs.k = 0; }
+    if (threadIdx.x == 0) { ss->rec.exact_rounds = 0; ss->rec.prefiltered = 0; sm->qd.k = 0; sm->pt.k = 0; sm->qs.k = 0; }
     __syncthreads();
+    // head-pass lists (fused engine; row 0 = verify, row 1 = PDM); the reference engine has none
+    const int cnt_v = with_lists ? __ldcg(&ss->pre_cnt[0]) : -1, cnt_p = with_lists ? __ldcg(&ss->pre_cnt[1]) : -1;
     if (st->run_pdm)
       topk_dist(P.logits_p, D.V, P.cand_val + kMaxCand, P.cand_idx + kMaxCand, ncand, ss->top_k, ss->temperature,
-                P.samp_val, P.samp_idx, &sm->qd, &ss->rec.exact_rounds, &sm->tk);
+                P.samp_val, P.samp_idx, &sm->qd, &ss->rec.exact_rounds, &sm->tk,
+                TopkPre{P.pre_val + kSampCap, P.pre_idx + kSampCap, cnt_p}, &ss->rec.prefiltered, &ss->tau_guess[1]);
     if (st->run_verify)
       topk_dist(P.logits_v, D.V, P.cand_val, P.cand_idx, ncand, ss->top_k, ss->temperature, P.samp_val, P.samp_idx,
-                &sm->pt, &ss->rec.exact_rounds, &sm->tk);
+                &sm->pt, &ss->rec.exact_rounds, &sm->tk, TopkPre{P.pre_val, P.pre_idx, cnt_v}, &ss->rec.prefiltered,
+                &ss->tau_guess[0]);
+    if (threadIdx.x < 2) ss->pre_cnt[threadIdx.x] = 0;
     // the judged token's stored distribution (n = 1: the draft of this very cycle, C-2.12) and the residual
     // weights, which depend on P and Q only — ready before thread 0 takes the decisions
     const bool judging = st->mode == MODE_SPD && st->occ[n - 1];

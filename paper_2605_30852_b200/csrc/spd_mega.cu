@@ -780,6 +780,8 @@ __device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v,
   float bv = -INFINITY;
   int bi = 0x7fffffff;
   int ucount = 0;
+  // sampling: every logit >= the guessed k-th value is listed while it is in a register (topk_dist, step 0)
+  const float tguess = P.sampling ? __ldcg(&P.samp->tau_guess[lane >> 4]) : INFINITY;
   while (true) {
     const uint32_t s0 = seq;
     mbar_wait(&full[s0 % kStages], (s0 / kStages) & 1);
@@ -831,6 +833,10 @@ __device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v,
       if ((vec ? do_p : do_v) && row < D.V) {
         if (cand_better(y, row, bv, bi)) { bv = y; bi = row; }
         if (P.debug_logits | P.sampling) (vec ? P.logits_p : P.logits_v)[row] = y;
+        if (y >= tguess) {
+          const int pos = atomicAdd(&P.samp->pre_cnt[vec], 1);
+          if (pos < kSampCap) { P.pre_val[vec * kSampCap + pos] = y; P.pre_idx[vec * kSampCap + pos] = row; }
+        }
       }
     }
     ++ucount;
@@ -1225,7 +1231,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
       __threadfence();
     }
     __syncthreads();
-    controller_end(P, ncta, reinterpret_cast<SampSmem *>(ring));   // the tile ring is idle: every tile of the cycle was consumed
+    controller_end(P, ncta, reinterpret_cast<SampSmem *>(ring), true);   // the tile ring is idle: every tile of the cycle was consumed
     for (int i = tid; i < np * kMaxStages; i += kThreads) P.claim[i] = 0u;   // every producer is done claiming
     if (tid < kMaxStages + 2) gbar[32 * tid] = 0u;                           // ... and every CTA with its group counters
     __syncthreads();

@@ -182,12 +182,13 @@ class SamplingReport:
     max_hidden_err: float = 0.0
     ties: tuple = (0, 0, 0, 0)       # hints adopted: support, draft, accept, replacement
     exact_rounds: int = 0
+    prefiltered: int = 0             # selections served by the fused head pass's threshold list (no scan)
     tokens: list = dataclasses.field(default_factory=list)
 
     def summary(self) -> str:
         return (f"{self.status} steps={self.steps} emitted={self.emitted} acc/rej={self.accepts}/{self.rejects} "
                 f"logit_abs={self.max_logit_abs_err:.2e} prob={self.max_prob_err:.2e} hidden={self.max_hidden_err:.2e} "
-                f"ties(support/draft/accept/repl)={self.ties} exact_rounds={self.exact_rounds} {self.detail}")
+                f"ties(support/draft/accept/repl)={self.ties} exact_rounds={self.exact_rounds} prefiltered={self.prefiltered} {self.detail}")
 
 
 def _dist_close(g, o, delta):
@@ -256,6 +257,7 @@ def run_sampling_parity(shape, weights_np, dev_weights, prompt, n_tokens, temper
             rep.steps += 1
             rep.ties = orec["ties"]
             rep.exact_rounds += grec["exact_rounds"]
+            rep.prefiltered += grec["prefiltered"]
             # logits first: they bound everything else
             d = float(np.max(np.abs(ora.last("pdm_logits").astype(np.float64) - gpu.last("pdm_logits"))))
             if ro.exited:

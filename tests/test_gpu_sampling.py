@@ -148,4 +148,8 @@ def test_full_model_dims_paper_setting(engine, name, prompt_len, gen):
                               engine=engine, tensor_tol=1e-2, max_steps=4 * gen)
     print(f"sampling {name} engine={engine}:", rep.summary())
     assert rep.status == "ok", rep.detail
-    assert rep.exact_rounds == 0          # the threshold path was the one that ran
+    assert rep.exact_rounds == 0          # the threshold paths were the ones that ran
+    if engine == 1:                       # most selections came from the head pass's own list, without a scan
+        assert rep.prefiltered >= rep.steps // 2, rep.summary()
+    else:
+        assert rep.prefiltered == 0
