@@ -29,9 +29,22 @@ def declared_symbols():
 def test_library_exports_every_declared_symbol(lib):
     syms = declared_symbols()
     assert {"spd_create", "spd_prefill", "spd_step", "spd_rollback", "spd_query_sizes", "spd_destroy",
-            "spd_step_many", "spd_set_forced", "spd_debug_read", "spd_last_error"} <= set(syms)
+            "spd_step_many", "spd_set_forced", "spd_debug_read", "spd_last_error", "spd_set_sampling",
+            "spd_op_topk_softmax"} <= set(syms)
     for s in syms:
         assert hasattr(lib, s), s
+
+
+def test_sample_record_layout_matches_the_header(lib):
+    """The binding's ctypes mirror of spd_sample_record / spd_sample_dist has the header's field order and size."""
+    from paper_2605_30852_b200.binding import _Dist, _SampleRec, MAX_TOPK
+    text = open(os.path.join(ROOT, "include", "spd.h")).read()
+    assert int(re.search(r"#define SPD_MAX_TOPK (\d+)", text).group(1)) == MAX_TOPK == 64
+    assert C.sizeof(_Dist) == 4 + 8 * MAX_TOPK and C.sizeof(_SampleRec) == 2 * C.sizeof(_Dist) + 32
+    body = re.search(r"typedef struct \{([^}]*)\} spd_sample_record;", text, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = re.findall(r"\b([a-z_]+)\s*[,;]", body)
+    assert names == [k for k, _ in _SampleRec._fields_]
 
 
 def test_query_sizes_and_validation(lib):
@@ -62,6 +75,9 @@ def test_no_gpu_means_no_compute_not_a_fallback(lib):
     assert lib.spd_create(C.byref(cfg), C.byref(w), C.byref(bufs), C.byref(h)) == 4  # SPD_ECUDA
     assert not h.value
     assert lib.spd_step(None, None) == 1 and lib.spd_destroy(None) == 1
+    assert lib.spd_set_sampling(None, 1.0, 50, 1) == 1                       # SPD_EINVAL: null ctx
+    assert lib.spd_op_topk_softmax(None, 8, 4, 1.0, 1, None, None, None) == 1
+    assert lib.spd_op_topk_scratch() >= 2 * 2048 * 4
     assert b"null" in lib.spd_last_error(None)
 
 

@@ -153,3 +153,82 @@ def test_full_model_dims_paper_setting(engine, name, prompt_len, gen):
         assert rep.prefiltered >= rep.steps // 2, rep.summary()
     else:
         assert rep.prefiltered == 0
+
+
+@pytest.mark.timeout(900)
+def test_full_size_sampling_decisions_recomputed_by_the_oracle():
+    """BASELINE.json configs[3] (9b_n4) at its full 2048-token prompt, in bench.py's launch configuration, in
+    sampling mode (T = 1, top-k 50).  The oracle cannot run this prefill, but every cycle's outputs can be
+    recomputed one by one from what the cycle itself exposes: the filtered distributions from the library's own
+    logit vectors (oracle top-k softmax: supports exact, probabilities 1e-6), the uniforms from (seed, K, j), and
+    every decision (draft token, accept bit, replacement) by the oracle's decision functions applied to the
+    recorded fp32 distributions — fp64 on identical inputs on both sides, hence exact.  Plus the any-size
+    invariants: the judged token carries the distribution it was drawn from, KV lengths equal the committed
+    length after a reject, fill pattern.  Then top_k = 1 on the same prompt: identical to the greedy run."""
+    import paper_2605_30852_b200 as spd
+    shape = si.CONFIGS["9b_n4"]
+    n, P, V = shape.n_stages, shape.prompt_len, shape.vocab
+    w = si.make_weights(shape, seed=1234)
+    prompt = si.make_prompt(shape, 1234)
+    wd = spd.upload_weights(w)
+    eng = spd.SPD(shape, wd, max_seq=P + 256)
+    seed, T, K50 = 4242, 1.0, 50
+    try:
+        eng.set_sampling(T, K50, seed)
+        first = eng.prefill(prompt)
+        rec = eng.sample_record()
+        want = ora.op_topk_softmax(eng.last("exit_logits"), K50, T)
+        assert np.array_equal(rec["target"][0], want.ids)
+        np.testing.assert_allclose(rec["target"][1], want.p, rtol=0, atol=1e-6)
+        assert rec["u_resid"] == ora.op_uniform(seed, 0, 2)
+        assert first == ora.op_sample_cdf(ora.Dist(*rec["target"]), rec["u_resid"])
+        in_flight, prev_fill, rejects, prefiltered = {}, 1, 0, 0
+        for step in range(1, 41):
+            p_new = [s for s in eng.ring()[2] if s[0]][0][1]
+            r = eng.step()
+            rec = eng.sample_record()
+            prefiltered += rec["prefiltered"]
+            assert r.step_index == step and r.fill == prev_fill and rec["exact_rounds"] == 0
+            Q = ora.Dist(*rec["draft"])
+            want = ora.op_topk_softmax(eng.last("pdm_logits"), K50, T)
+            assert np.array_equal(Q.ids, want.ids)
+            np.testing.assert_allclose(Q.p, want.p, rtol=0, atol=1e-6)
+            assert rec["u_draft"] == ora.op_uniform(seed, step, 0)
+            assert r.draft_token == ora.op_sample_cdf(Q, rec["u_draft"])
+            if r.exited:
+                c = r.committed_len
+                x, Qx = in_flight[c]
+                Pt = ora.Dist(*rec["target"])
+                want = ora.op_topk_softmax(eng.last("exit_logits"), K50, T)
+                assert np.array_equal(Pt.ids, want.ids)
+                np.testing.assert_allclose(Pt.p, want.p, rtol=0, atol=1e-6)
+                assert rec["succ_token"] == x and rec["u_accept"] == ora.op_uniform(seed, step, 1)
+                qx = float(Qx.p[list(Qx.ids).index(x)])
+                assert rec["succ_q"] == np.float32(qx)
+                assert r.accepted == ora.op_accept(Pt, Qx, x, rec["u_accept"])
+                if r.accepted:
+                    assert r.emitted_token == x
+                    in_flight[p_new + 1] = (r.draft_token, Q)
+                    prev_fill = r.fill
+                else:
+                    rejects += 1
+                    assert rec["u_resid"] == ora.op_uniform(seed, step, 2)
+                    assert r.emitted_token == ora.op_sample_residual(Pt, Qx, rec["u_resid"])
+                    assert np.all(eng.kv_len() == c) and r.discarded == r.fill - 1
+                    fill, cc, slots = eng.ring()
+                    assert fill == 1 and cc == c and slots[0] == (1, c, r.emitted_token)
+                    in_flight, prev_fill = {}, 1
+            else:
+                in_flight[p_new + 1] = (r.draft_token, Q)
+                prev_fill = r.fill + 1
+        assert rejects >= 5 and prefiltered >= 30
+        # top_k = 1 from the same prefill state == the greedy run (PAPER.md:129 "exact argmax match")
+        eng.set_sampling(1.0, 1, 1)
+        f1 = eng.prefill(prompt)
+        s_tokens, _ = eng.generate(12, chunk=8)
+        eng.set_sampling(1.0, 0, 0)
+        f0 = eng.prefill(prompt)
+        g_tokens, _ = eng.generate(12, chunk=8)
+        assert f0 == f1 and s_tokens == g_tokens
+    finally:
+        eng.close()
