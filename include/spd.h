@@ -179,6 +179,8 @@ int spd_set_forced(spd_ctx *ctx, const int32_t *truth, int32_t n_truth, float p,
  *     token, K = step_index of the cycle (0 in spd_prefill).
  * The emitted tokens are distributed exactly as autoregressive sampling from the filtered target (not
  * token-identical to any other run).  top_k < 1 switches back to greedy.  top_k = 1 is the greedy path.
+ * Switched on in the middle of a sequence, the tokens already in flight count as deterministic drafts
+ * (Q = one-hot: accepted with probability P(x)).
  * SPD_EINVAL: top_k > SPD_MAX_TOPK or temperature <= 0.  SPD_ESTATE: forced acceptance is on (and
  * spd_set_forced while sampling is on).  Logits must be finite.  May be called before or after spd_prefill. */
 #define SPD_MAX_TOPK 64

@@ -306,6 +306,12 @@ int ora_set_sampling(ora_ctx *o, float temperature, int32_t top_k, uint64_t seed
   if (top_k < 1) { o->sampling_on = 0; return 0; }
   if (top_k > ORA_MAX_TOPK || !(temperature > 0.f) || o->forced_on) return -1;
   o->sampling_on = 1; o->top_k = top_k; o->temperature = temperature; o->samp_seed = seed;
+  /* tokens already in flight were not drawn from a filtered distribution: whoever put them there acted as a
+   * deterministic drafter, Q = one-hot on the token (accepted with probability P(x)) */
+  for (int i = 0; i < o->a; ++i) {
+    memset(&o->r_q[i], 0, sizeof(ora_dist));
+    o->r_q[i].k = 1; o->r_q[i].id[0] = o->r_tok[i]; o->r_q[i].p[0] = 1.f;
+  }
   return 0;
 }
 

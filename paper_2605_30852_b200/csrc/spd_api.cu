@@ -170,6 +170,7 @@ __global__ void k_set_forced(DevPtrs P, int on, int n_truth, unsigned long long 
 }
 __global__ void k_set_sampling(DevPtrs P, int on, int top_k, float temperature, unsigned long long seed) {
   P.samp->on = on; P.samp->top_k = top_k; P.samp->temperature = temperature; P.samp->seed = seed;
+  for (int b = 0; b < kMaxStages; ++b) P.samp->q[b].k = 0;   // nothing in flight carries a draft distribution yet
   P.samp->pre_cnt[0] = P.samp->pre_cnt[1] = 0;
   P.samp->tau_guess[0] = P.samp->tau_guess[1] = INFINITY;
 }

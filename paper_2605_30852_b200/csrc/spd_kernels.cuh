@@ -428,6 +428,11 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, Samp
       reinterpret_cast<int32_t *>(&ss->rec.target)[i] = reinterpret_cast<const int32_t *>(&sm->pt)[i];
     }
     __syncthreads();
+    if (judging && sm->qs.k == 0) {   // in flight since before sampling was switched on: a deterministic draft, Q one-hot
+      __syncthreads();
+      if (threadIdx.x == 0) { sm->qs.k = 1; sm->qs.id[0] = st->tok[n - 2]; sm->qs.p[0] = 1.f; }
+      __syncthreads();
+    }
     if (judging && (int)threadIdx.x < sm->pt.k) {
       const double r = (double)sm->pt.p[threadIdx.x] - dist_prob(&sm->qs, sm->pt.id[threadIdx.x]);
       sm->w[threadIdx.x] = r > 0.0 ? r : 0.0;

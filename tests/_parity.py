@@ -202,7 +202,7 @@ def _dist_close(g, o, delta):
 
 
 def run_sampling_parity(shape, weights_np, dev_weights, prompt, n_tokens, temperature, top_k, seed, engine=None,
-                        tensor_tol=CONTRACT, max_seq=None, max_steps=None) -> SamplingReport:
+                        tensor_tol=CONTRACT, max_seq=None, max_steps=None, greedy_steps=0) -> SamplingReport:
     """GPU vs oracle in sampling mode, cycle by cycle.  Exact: step results (tokens, accept bits, fill,
     committed length), uniforms, supports, KV lengths.  Within tolerance: logits (tensor_tol, C-2.18),
     probabilities (bounded by the measured logit difference), hidden states.
@@ -226,8 +226,11 @@ def run_sampling_parity(shape, weights_np, dev_weights, prompt, n_tokens, temper
     try:
         if engine is not None:
             gpu.set_option(OPT.ENGINE, engine)
-        ora.set_sampling(temperature, top_k, seed)
-        gpu.set_sampling(temperature, top_k, seed)
+        if greedy_steps:      # greedy prefill + cycles first; sampling is switched on with tokens in flight
+            gpu.set_option(OPT.DEBUG_LOGITS, 1)
+        else:
+            ora.set_sampling(temperature, top_k, seed)
+            gpu.set_sampling(temperature, top_k, seed)
         fo = ora.prefill(prompt, block=16)
         fg = gpu.prefill(prompt)
         lo, lg = ora.last("exit_logits"), gpu.last("exit_logits")
@@ -236,13 +239,23 @@ def run_sampling_parity(shape, weights_np, dev_weights, prompt, n_tokens, temper
         rep.max_logit_abs_err = delta_run
         if delta_run > tensor_tol * maxabs:
             return fail(f"prefill logits differ by {delta_run:.3e} (max|logit| {maxabs:.3f})")
-        orec, grec = ora.sample_record(), gpu.sample_record()
-        if grec["u_resid"] != orec["u_resid"]:
-            return fail("first-token uniform differs")
-        ok, perr = _dist_close(grec["target"], orec["target"], delta_run)
-        if fo != fg or not ok:
-            return fail(f"first token {fg} vs oracle {fo}, distributions close: {ok} (prob err {perr:.2e})")
-        rep.max_prob_err = perr
+        if greedy_steps:
+            if fo != fg:
+                return fail(f"greedy first token {fg} vs oracle {fo}")
+            for i in range(greedy_steps):
+                rg, ro = gpu.step(), ora.step()
+                if tuple(rg) != tuple(ro):
+                    return fail(f"greedy step {i + 1}: gpu {tuple(rg)} != oracle {tuple(ro)}")
+            ora.set_sampling(temperature, top_k, seed)
+            gpu.set_sampling(temperature, top_k, seed)
+        else:
+            orec, grec = ora.sample_record(), gpu.sample_record()
+            if grec["u_resid"] != orec["u_resid"]:
+                return fail("first-token uniform differs")
+            ok, perr = _dist_close(grec["target"], orec["target"], delta_run)
+            if fo != fg or not ok:
+                return fail(f"first token {fg} vs oracle {fo}, distributions close: {ok} (prob err {perr:.2e})")
+            rep.max_prob_err = perr
         rep.tokens.append(fg)
         limit = max_steps or 10 ** 9
         while ora.emitted < n_tokens and rep.steps < limit:

@@ -82,6 +82,19 @@ def test_tiny_baseline_vocab(engine, T, k, seed):
 
 
 @pytest.mark.parametrize("engine", ENGINES)
+@pytest.mark.parametrize("n,greedy_steps", [(4, 5), (4, 2), (8, 11), (1, 3)])
+def test_sampling_switched_on_with_tokens_in_flight(engine, n, greedy_steps):
+    """Greedy prefill and cycles first, then spd_set_sampling on the live pipeline: the tokens already in flight
+    were drafted deterministically and are judged with Q = one-hot (accepted with probability P(x)); the step
+    counter K (hence the uniforms) continues."""
+    shape = shape_of("tiny", n, vocab=64)
+    rep = run_sampling_parity(**_inputs(shape, 32, std=0.08, random_gains=True), n_tokens=30, temperature=1.0,
+                              top_k=50, seed=31, engine=engine, tensor_tol=5e-3, greedy_steps=greedy_steps)
+    print(f"sampling switched on after {greedy_steps} greedy cycles, n={n} engine={engine}:", rep.summary())
+    assert rep.status == "ok", rep.detail
+
+
+@pytest.mark.parametrize("engine", ENGINES)
 def test_top_k_one_is_the_greedy_path(engine):
     """top_k = 1: every step result equals the greedy run of the same library ("exact argmax
     match"), and the KV lengths agree."""

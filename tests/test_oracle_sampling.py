@@ -209,6 +209,31 @@ def test_sampling_and_forcing_exclude_each_other():
     o.close()
 
 
+def test_switching_sampling_on_with_tokens_in_flight_judges_them_as_deterministic_drafts():
+    """Tokens drafted greedily before ora_set_sampling are judged with Q = one-hot: accept iff u < P(x)."""
+    n = 4
+    shape = shape_of("tiny", n, vocab=64)
+    o = Oracle(shape, si.make_weights(shape, seed=1234, std=0.08, random_gains=True), max_seq=512)
+    o.prefill(si.make_prompt(shape, 1))
+    for _ in range(6):
+        o.step()
+    o.set_sampling(1.0, 50, 5)
+    judged = 0
+    while judged < 3:
+        x = o.ring(1)[1] if o.fill > 1 else None
+        r = o.step_sample_follow()
+        rec = o.sample_record()
+        if r.exited:
+            judged += 1
+            assert rec["succ_token"] == x and rec["succ_q"] == 1.0
+            px = dense(rec["target"], shape.vocab)[x]
+            assert r.accepted == int(rec["u_accept"] < px)
+            if not r.accepted:
+                assert r.emitted_token != x
+                break
+    o.close()
+
+
 def test_cycle_bookkeeping_in_sampling_mode():
     """Every accepted token was in flight with the distribution it was drawn from; rollback identity and
     fill pattern as in the greedy cycle; the record exposes P, Q and the uniforms of S-6."""
