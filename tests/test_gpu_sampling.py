@@ -245,3 +245,40 @@ def test_full_size_sampling_decisions_recomputed_by_the_oracle():
         assert f0 == f1 and s_tokens == g_tokens
     finally:
         eng.close()
+
+
+@pytest.mark.parametrize("engine", ENGINES)
+@pytest.mark.parametrize("n", [1, 2, 4])
+def test_gpu_sampled_spd_is_distributed_as_autoregressive_sampling(engine, n):
+    """The defining property under sampling, checked on the CUDA path without any follow
+    protocol: 2500 seeds of sampled SPD on a micro decoder (V = 24, top-3, T = 1); the joint law of the first
+    three emitted tokens against the exact autoregressive sampling law that the ORACLE's whole-prefix logits
+    define (chi-square; seeds fixed, so the test is deterministic)."""
+    import paper_2605_30852_b200 as spd
+    from tests.test_oracle_sampling import chi_square, exact_ar_distribution, MK, MT
+    shape = TINY.replace(name="micro_gpu", d_model=128, n_layers=4, n_stages=n, n_q_heads=2, n_kv_heads=1, head_dim=64,
+                         d_ffn=96, vocab=24, prompt_len=6, gen_len=8)
+    w = si.make_weights(shape, seed=4321, std=0.25, random_gains=True)
+    prompt = si.make_prompt(shape, 3)
+    depth, runs = 3, 2500
+    want = exact_ar_distribution(n, prompt, depth, shape=shape, w=w)
+    g = spd.SPD(shape, spd.upload_weights(w), max_seq=128)
+    counts = {k: 0 for k in want}
+    accepted = exits = 0
+    try:
+        g.set_option(spd.OPT.ENGINE, engine)
+        for seed in range(runs):
+            g.set_sampling(MT, MK, 5000 + seed)
+            toks = [g.prefill(prompt)]
+            while len(toks) < depth:
+                for r in g.step_many(n + 1):
+                    if r.exited:
+                        toks.append(r.emitted_token)
+                        accepted += r.accepted
+                        exits += 1
+            counts[tuple(toks[:depth])] += 1     # KeyError: a token outside the target's support was emitted
+    finally:
+        g.close()
+    chi2, cells, pval = chi_square(want, counts, runs)
+    print(f"gpu sampled law n={n} engine={engine}: chi2 {chi2:.1f} over {cells} cells, p = {pval:.3f}, acceptance {accepted}/{exits}")
+    assert pval > 1e-3

@@ -296,12 +296,12 @@ def micro_weights(n):
     return si.make_weights(MICRO.replace(n_stages=n), seed=4321, std=0.25, random_gains=True)
 
 
-def exact_ar_distribution(n, prompt, depth):
+def exact_ar_distribution(n, prompt, depth, shape=None, w=None):
     """P(t_1..t_depth) of autoregressive sampling from the filtered target distribution, by whole-prefix
     recompute: each factor is library top-k softmax of the logits the oracle's prefill gives for
     prompt + prefix (the PDM and the pipeline play no part)."""
-    shape = MICRO.replace(n_stages=n)
-    o = Oracle(shape, micro_weights(n), max_seq=64)
+    shape = shape or MICRO.replace(n_stages=n)
+    o = Oracle(shape, w if w is not None else micro_weights(n), max_seq=64)
     dist = {(): 1.0}
     for _ in range(depth):
         nxt = {}
@@ -313,6 +313,20 @@ def exact_ar_distribution(n, prompt, depth):
         dist = nxt
     o.close()
     return dist
+
+
+def chi_square(want, counts, runs):
+    """Pearson chi-square of observed outcome counts against the exact law (rare outcomes pooled into one cell)."""
+    keys = sorted(want, key=lambda k: -want[k])
+    exp = np.array([want[k] * runs for k in keys])
+    obs = np.array([counts[k] for k in keys], dtype=np.float64)
+    big = exp >= 8.0
+    e = np.append(exp[big], exp[~big].sum())
+    c = np.append(obs[big], obs[~big].sum())
+    if e[-1] < 8.0:
+        e[-2] += e[-1]; c[-2] += c[-1]; e, c = e[:-1], c[:-1]
+    chi2 = float(((c - e) ** 2 / e).sum())
+    return chi2, len(e), float(scipy.stats.chi2.sf(chi2, len(e) - 1))
 
 
 @pytest.mark.parametrize("n,drafter", [(2, "pdm"), (4, "pdm"), (1, "pdm"), (2, "fixed"), (4, "random")])
@@ -339,16 +353,7 @@ def test_sampled_spd_is_distributed_as_autoregressive_sampling(n, drafter):
         accepted += sum(r.accepted for r in log)
         exits += sum(r.exited for r in log)
     o.close()
-    keys = sorted(want, key=lambda k: -want[k])
-    exp = np.array([want[k] * runs for k in keys])
-    obs = np.array([counts[k] for k in keys], dtype=np.float64)
-    big = exp >= 8.0                                        # pool the rare outcomes into one cell
-    e = np.append(exp[big], exp[~big].sum())
-    c = np.append(obs[big], obs[~big].sum())
-    if e[-1] < 8.0:
-        e[-2] += e[-1]; c[-2] += c[-1]; e, c = e[:-1], c[:-1]
-    chi2 = float(((c - e) ** 2 / e).sum())
-    pval = float(scipy.stats.chi2.sf(chi2, len(e) - 1))
-    assert pval > 1e-3, f"chi2 {chi2:.1f} over {len(e)} cells, p = {pval:.2e}, acceptance {accepted}/{exits}"
+    chi2, cells, pval = chi_square(want, counts, runs)
+    assert pval > 1e-3, f"chi2 {chi2:.1f} over {cells} cells, p = {pval:.2e}, acceptance {accepted}/{exits}"
     if drafter == "pdm" and n > 1:
         assert 0 < accepted < exits                          # both branches of the verifier were exercised
