@@ -326,7 +326,7 @@ __device__ __forceinline__ void topk_dist(const float *logits, int V, const floa
   const float mx = s_sel_v[0];
   if (tid == 0 && next_guess) {   // next cycle's list threshold: this cycle's k-th value minus a margin
     const float kth = s_sel_v[k - 1];
-    *next_guess = kth - fmaxf(0.5f * (mx - kth), 0.1f + 0.05f * fabsf(kth));
+    *next_guess = kth - fmaxf(0.25f * (mx - kth), 0.1f + 0.05f * fabsf(kth));
   }
   __syncthreads();
   if (tid < k) {
