@@ -11,7 +11,10 @@
  *          every greedy SPD run must reproduce (PAPER.md:125 "lossless", :129 "exact argmax match").
  *   O-SPD  the SPD cycle, step by step: n-stage token pipeline, pre-step Pipeline
  *          Draft Module on the depth staircase (PAPER.md:77-85 Eq.1-2, :102-107 Eq.5, :115),
- *          streaming greedy verification and rollback.
+ *          streaming greedy verification and rollback; with
+ *          ora_set_sampling, verification by standard rejection sampling —
+ *          pinned by tests/test_oracle_sampling.py (library softmax, the lossless identity measured in u,
+ *          top_k = 1 == greedy, the exact autoregressive sampling law on a micro decoder).
  *
  * Numeric contract (C-2.17): every tensor is fp32 except K/V cache rows, which are rounded to bf16
  * (round-to-nearest-even) when appended; weights are bf16 widened exactly.  Every reduction (dot
@@ -112,7 +115,7 @@ void ora_get_last(const ora_ctx *, int32_t what, float *out);
 /* top1-top2 gap and max|logit| of the last verify (which=0) / PDM (which=1) argmax (C-4). */
 void ora_get_margin(const ora_ctx *, int32_t which, float *gap, float *maxabs);
 
-/* ---- NEXT-2: sampling verification (readings S-1..S-9 of DESIGN.md §2) ----------
+/* ---- NEXT-2: sampling verification (readings S-1..S-10 of DESIGN.md §11) ----------
  * PAPER.md:129 "under sampling we apply standard rejection sampling"; PAPER.md:131 on a reject the
  * pipeline is reseeded "from x ~ P(x | x_1:t-n+1)"; "Sampling runs (T=1) use top-k=50 and
  * top-p=1.0".  Standard rejection sampling of speculative decoding: a token x drafted from Q is accepted
