@@ -75,8 +75,9 @@ void ora_op_rmsnorm(const float *x, const uint16_t *gain, int32_t d, float eps, 
 
 /* out = W x, W bf16 [rows, k] row-major. */
 void ora_op_gemv(const uint16_t *w, int32_t rows, int32_t k, const float *x, float *out) {
-  /* rows are independent, so threading never changes a value; tiny products stay on the calling thread */
-#pragma omp parallel for schedule(static) if ((size_t)rows * (size_t)k >= 32768)
+  /* rows are independent, so threading never changes a value; products below 2^20 multiply-adds (every product of
+   * the small test models) stay on the calling thread: no worker wake-ups or spinning between tiny regions */
+#pragma omp parallel for schedule(static) if ((size_t)rows * (size_t)k >= 1048576)
   for (int r = 0; r < rows; ++r) out[r] = (float)dot_row(w + (size_t)r * k, x, k);
 }
 
@@ -84,7 +85,7 @@ void ora_op_gemv(const uint16_t *w, int32_t rows, int32_t k, const float *x, flo
  * weight row is read once per block; each (t, r) value is the same dot_row call as in ora_op_gemv. */
 static void gemv_block(const uint16_t *w, int rows, int k, const float *x, int ldx, float *y, int ldy,
                        int nt) {
-#pragma omp parallel for schedule(static) if ((size_t)rows * (size_t)k * (size_t)nt >= 32768)
+#pragma omp parallel for schedule(static) if ((size_t)rows * (size_t)k * (size_t)nt >= 1048576)
   for (int r = 0; r < rows; ++r)
     for (int t = 0; t < nt; ++t) y[(size_t)t * ldy + r] = (float)dot_row(w + (size_t)r * k, x + (size_t)t * ldx, k);
 }
@@ -113,7 +114,7 @@ void ora_op_attention(const float *q, const uint16_t *kc, const uint16_t *vc, in
                       int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, float *out) {
   int group = n_q_heads / n_kv_heads;
   size_t row = (size_t)n_kv_heads * head_dim;
-#pragma omp parallel for schedule(static) if ((size_t)n_q_heads * (size_t)t_len * (size_t)head_dim >= 32768)
+#pragma omp parallel for schedule(static) if ((size_t)n_q_heads * (size_t)t_len * (size_t)head_dim >= 1048576)
   for (int hq = 0; hq < n_q_heads; ++hq) {
     int kvh = hq / group;
     const float *qh = q + (size_t)hq * head_dim;
