@@ -314,6 +314,35 @@ def run_gpu(args, shape):
                 "overhead_us": s_us - g_us, "accept_rate": sum(r.accepted for r in s_log) / max(1, sum(r.exited for r in s_log)),
                 "fill_hist": hist(s_log), "greedy_fill_hist": hist(g_log)}
 
+    # ---- ... and at SATURATION.  Random-init drafts are never accepted under sampling, so the saturated sampling cycle
+    # (fill n, exit, target top-k, accept test) is timed on an "echo" re-initialisation of the SAME device tensors:
+    # W_o = W_down = 0 (every layer leaves the residual stream untouched; all bytes are still streamed) and
+    # W_p = [I 0 .. 0], so the PDM's logits for a token equal the target's bit for bit, Q = P, and every draft is
+    # accepted (u * Q(x) < P(x) for every u < 1).  The greedy cycle is timed on the same tensors beside it.
+    eng.close()
+    for l in range(shape.n_layers):
+        w_dev["wo"][l].zero_()
+        w_dev["w_down"][l].zero_()
+    w_dev["pdm_proj"].zero_()
+    w_dev["pdm_proj"][:, :shape.d_model].fill_diagonal_(0x3F80)          # bf16 1.0
+    w_dev["pdm_norm"].copy_(w_dev["final_norm"])
+    eng = spd.SPD(shape, w_dev, max_seq=P + 2 * ks + 8 * n + 64, device=local_rank)
+    if args.engine is not None:
+        eng.set_option(spd.OPT.ENGINE, args.engine)
+    stream = eng.stream_main
+    eng.set_sampling(1.0, 50, args.seed)
+    first_e = eng.prefill(prompt)
+    ss_us, ss_log = timed_cycles(ks)
+    eng.set_sampling(1.0, 0, 0)
+    eng.rollback(P, first_e)
+    sg_us, sg_log = timed_cycles(ks)
+    acc = lambda log: sum(r.accepted for r in log) / max(1, sum(r.exited for r in log))
+    sampling["saturated"] = {"init": "echo (W_o = W_down = 0, W_p = [I 0 .. 0]): Q = P, every draft is accepted",
+                             "cycles": ks, "mean_step_us": ss_us, "greedy_mean_step_us": sg_us, "overhead_us": ss_us - sg_us,
+                             "accept_rate": acc(ss_log), "greedy_accept_rate": acc(sg_log),
+                             "tokens_per_s": sum(r.exited for r in ss_log) / (ss_us * ks) * 1e6,
+                             "all_fill_n": all(r.fill == n for r in ss_log) and all(r.fill == n for r in sg_log)}
+
     local = {"step_us": step_us, "e2e_us": e2e_us, "kernel_us": step_us, "tokens_per_s": 1e6 / step_us,
              "hbm_gbs": by["full"] / step_us / 1e3, "gpu_launches": launches}
     tot = aggregate(local, world)

@@ -324,9 +324,11 @@ __device__ __forceinline__ void topk_dist(const float *logits, int V, const floa
     for (int j = 0; j < k; ++j) rank += s_sel_i[j] < ix ? 1 : 0;
   }
   const float mx = s_sel_v[0];
-  if (tid == 0 && next_guess) {   // next cycle's list threshold: this cycle's k-th value minus a margin
+  if (tid == 0 && next_guess) {   // next cycle's list threshold: this cycle's k-th value minus a margin that follows the
+    // LOCAL spacing of the order statistics (rank k/2 to rank k), not the maximum: a peaked distribution (one
+    // dominant logit) must not drag the threshold below the bulk, or every logit would be listed
     const float kth = s_sel_v[k - 1];
-    *next_guess = kth - fmaxf(0.25f * (mx - kth), 0.1f + 0.05f * fabsf(kth));
+    *next_guess = kth - fmaxf(1.25f * (s_sel_v[(k - 1) / 2] - kth), 0.1f + 0.05f * fabsf(kth));
   }
   __syncthreads();
   if (tid < k) {
