@@ -143,6 +143,22 @@ def make_weights(shape: ModelShape, seed: int = 1234, std: float = 0.02, random_
     return w
 
 
+def make_echo(shape: ModelShape, weights: dict) -> dict:
+    """The "echo" re-initialisation used to reach saturation under sampling verification: a copy of
+    `weights` with W_o = W_down = 0 (every layer leaves the residual stream untouched), W_p = [I 0 .. 0] (the PDM
+    reads the newest token's embedding) and the PDM's norm gain = the final norm's.  The PDM's logits for a token
+    then equal the target's logits for it, so the draft distribution equals the target distribution."""
+    d, n = shape.d_model, shape.n_stages
+    w = dict(weights)
+    w["wo"] = [np.zeros_like(x) for x in weights["wo"]]
+    w["w_down"] = [np.zeros_like(x) for x in weights["w_down"]]
+    proj = np.zeros((d, n * d), dtype=np.uint16)
+    proj[np.arange(d), np.arange(d)] = 0x3F80          # bf16 1.0
+    w["pdm_proj"] = proj
+    w["pdm_norm"] = weights["final_norm"].copy()
+    return w
+
+
 def make_prompt(shape: ModelShape, seed: int = 1, length: int | None = None) -> np.ndarray:
     """Prompt token ids, uniform on [0, vocab), int32."""
     n = shape.prompt_len if length is None else length

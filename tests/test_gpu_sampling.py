@@ -82,6 +82,26 @@ def test_tiny_baseline_vocab(engine, T, k, seed):
 
 
 @pytest.mark.parametrize("engine", ENGINES)
+@pytest.mark.parametrize("n,T,k", [(2, 1.0, 50), (4, 30.0, 50), (8, 30.0, 64), (4, 30.0, 5)])
+def test_echo_initialisation_accepts_every_draft(engine, n, T, k):
+    """bench.py's saturation vehicle (spd_inputs.make_echo): Q = P, so standard rejection sampling accepts every
+    draft (u Q(x) < P(x) for all u < 1) and the pipeline stays saturated; T = 30 flattens the echo's dominant
+    logit so that the draws are not degenerate.  Long runs of accepts exercise the stored-Q path (the judged
+    token's distribution filed under its hidden buffer n - 1 cycles earlier) on both engines, against the oracle."""
+    shape = shape_of("tiny", n)
+    inp = _inputs(shape, 32, std=0.08, random_gains=True)
+    inp["weights_np"] = si.make_echo(shape, inp["weights_np"])
+    import paper_2605_30852_b200 as spd
+    inp["dev_weights"] = spd.upload_weights(inp["weights_np"])
+    rep = run_sampling_parity(**inp, n_tokens=60, temperature=T, top_k=k, seed=13, engine=engine, tensor_tol=5e-3)
+    print(f"sampling echo n={n} T={T} k={k} engine={engine}:", rep.summary())
+    assert rep.status == "ok", rep.detail
+    assert rep.rejects == 0 and rep.accepts == 59 and rep.steps == 59 + n - 1
+    if T > 1:
+        assert len(set(rep.tokens)) > 10          # the draws are spread over the support, not one echoed token
+
+
+@pytest.mark.parametrize("engine", ENGINES)
 @pytest.mark.parametrize("n,greedy_steps", [(4, 5), (4, 2), (8, 11), (1, 3)])
 def test_sampling_switched_on_with_tokens_in_flight(engine, n, greedy_steps):
     """Greedy prefill and cycles first, then spd_set_sampling on the live pipeline: the tokens already in flight

@@ -234,6 +234,28 @@ def test_switching_sampling_on_with_tokens_in_flight_judges_them_as_deterministi
     o.close()
 
 
+@pytest.mark.parametrize("n", [1, 4])
+def test_echo_initialisation_makes_the_draft_distribution_equal_the_target(n):
+    """spd_inputs.make_echo: identity layers and W_p = [I 0 .. 0] => the distribution a token is drafted from equals,
+    bit for bit, the target distribution that judges it n - 1 cycles later; every draft is accepted."""
+    shape = shape_of("tiny", n)
+    w = si.make_echo(shape, si.make_weights(shape, seed=1234, std=0.08, random_gains=True))
+    o = Oracle(shape, w, max_seq=256)
+    o.set_sampling(30.0, 50, 3)
+    o.prefill(PROMPT)
+    drafted = {}
+    for _ in range(40):
+        p_new = o.ring(o.fill - 1)[0]
+        r = o.step_sample_follow()
+        rec = o.sample_record()
+        drafted[p_new + 1] = rec["draft"]
+        if r.exited:
+            Q = drafted[r.committed_len]
+            assert r.accepted == 1
+            assert np.array_equal(Q.ids, rec["target"].ids) and np.array_equal(Q.p, rec["target"].p)
+    o.close()
+
+
 def test_cycle_bookkeeping_in_sampling_mode():
     """Every accepted token was in flight with the distribution it was drawn from; rollback identity and
     fill pattern as in the greedy cycle; the record exposes P, Q and the uniforms of S-6."""
