@@ -781,7 +781,7 @@ __device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v,
   int bi = 0x7fffffff;
   int ucount = 0;
   // sampling: every logit >= the guessed k-th value is listed while it is in a register (topk_dist, step 0)
-  float tguess = P.sampling ? __ldcg(&P.samp->tau_guess[lane >> 4]) : INFINITY;
+  const float tguess = P.sampling ? __ldcg(&P.samp->tau_guess[lane >> 4]) : INFINITY;
   while (true) {
     const uint32_t s0 = seq;
     mbar_wait(&full[s0 % kStages], (s0 / kStages) & 1);
@@ -836,7 +836,6 @@ __device__ __forceinline__ void head_stream(const DevPtrs &P, int nc, bool do_v,
         if (y >= tguess) {
           const int pos = atomicAdd(&P.samp->pre_cnt[vec], 1);
           if (pos < kSampCap) { P.pre_val[vec * kSampCap + pos] = y; P.pre_idx[vec * kSampCap + pos] = row; }
-          else tguess = INFINITY;   // the list overflowed (the controller will scan instead): stop hitting the counter
         }
       }
     }
