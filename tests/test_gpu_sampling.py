@@ -172,13 +172,13 @@ def test_sampling_errors_and_switching():
 
 
 @pytest.mark.parametrize("engine", ENGINES)
-@pytest.mark.parametrize("name,prompt_len,gen", [("4b_n4", 24, 8), ("9b_n4", 20, 6)])
+@pytest.mark.parametrize("name,prompt_len,gen", [("4b_n4", 24, 8), ("9b_n4", 20, 6), ("4b_n8", 18, 5), ("9b_n16", 20, 3)])
 def test_full_model_dims_paper_setting(engine, name, prompt_len, gen):
     """The 4B/9B-class shapes (vocabulary 151 936) with top-k 50, T = 1: the threshold scan over the real
     vocabulary inside the cycle, 148 per-CTA candidates (fused engine) / 128 chunk candidates (reference)."""
     shape = si.CONFIGS[name]
     rep = run_sampling_parity(**_inputs(shape, prompt_len), n_tokens=gen, temperature=1.0, top_k=50, seed=11,
-                              engine=engine, tensor_tol=1e-2, max_steps=4 * gen)
+                              engine=engine, tensor_tol=1e-2, max_steps=shape.n_stages * gen)
     print(f"sampling {name} engine={engine}:", rep.summary())
     assert rep.status == "ok", rep.detail
     assert rep.exact_rounds == 0          # the threshold paths were the ones that ran
