@@ -568,12 +568,14 @@ int ora_step(ora_ctx *o, int32_t draft_override, ora_step_result *out) {
 }
 
 /* A tie hint (test hook): `hint` is the token the CUDA path chose.  If it
- * is not the oracle's argmax but its oracle logit lies within band * max|logit| of the oracle's maximum,
- * both are valid choices at the stated logit tolerance: the oracle continues with the hint and counts a
- * tie.  Otherwise the oracle keeps its own argmax (and the caller reports the mismatch). */
-static int apply_hint(const float *logits, int own, int hint, int vocab, float band, float maxabs, int32_t *ties) {
-  if (hint < 0 || hint >= vocab || hint == own) return own;
-  if (logits[own] - logits[hint] <= band * maxabs) { *ties += 1; return hint; }
+ * is not the oracle's argmax but its oracle logit lies within `band` (ABSOLUTE, in logit units: the test
+ * passes a small multiple of the logit difference it measured between the two implementations) of the
+ * oracle's maximum, both are valid choices at that measured difference: the oracle continues with the hint
+ * and counts a tie.  band <= 0, an out-of-range hint, or a hint further below the maximum: the oracle
+ * keeps its own argmax (and the caller reports the mismatch). */
+static int apply_hint(const float *logits, int own, int hint, int vocab, float band, int32_t *ties) {
+  if (hint < 0 || hint >= vocab || hint == own || !(band > 0.f)) return own;
+  if (logits[own] - logits[hint] <= band) { *ties += 1; return hint; }
   return own;
 }
 
@@ -620,7 +622,7 @@ static int step_impl(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int
   }
   ora_op_gemv(o->w.pdm_proj, d, n * d, o->pdm_feat, o->pdm_u);
   int draft = head_argmax(o, o->pdm_u, o->w.pdm_norm, o->pdm_logits, 1);
-  draft = apply_hint(o->pdm_logits, draft, draft_hint, c->vocab, band, o->maxabs[1], &o->ties[1]);
+  draft = apply_hint(o->pdm_logits, draft, draft_hint, c->vocab, band, &o->ties[1]);
   ora_dist Qd; /* the distribution the entering draft is drawn from (sampling mode) */
   memset(&Qd, 0, sizeof Qd);
   if (o->sampling_on) { /* x^ ~ Q_t = filtered PDM distribution (S-2, S-3; j = 0) */
@@ -663,7 +665,7 @@ static int step_impl(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int
     memcpy(o->hfin + (size_t)e_pos * d, o->r_h, sizeof(float) * d);
     o->c = e_pos + 1;
     int y = head_argmax(o, o->r_h, o->w.final_norm, o->exit_logits, 0);
-    y = apply_hint(o->exit_logits, y, verify_hint, c->vocab, band, o->maxabs[0], &o->ties[0]);
+    y = apply_hint(o->exit_logits, y, verify_hint, c->vocab, band, &o->ties[0]);
     o->emitted += 1;
     r.exited = 1;
     /* pop the oldest */

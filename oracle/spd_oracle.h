@@ -76,8 +76,10 @@ int ora_prefill(ora_ctx *, const int32_t *tokens, int32_t n_tokens, int32_t bloc
 int ora_step(ora_ctx *, int32_t draft_override, ora_step_result *out);
 /* The same cycle with tie hints (test hook): draft_hint / verify_hint are
  * the tokens the CUDA path chose (-1: none).  A hint that is not the oracle's argmax but whose oracle
- * logit is within band * max|logit| of the oracle's maximum is adopted (both are valid at the stated
- * logit tolerance) and counted by ora_get_ties; any other hint is ignored. */
+ * logit is within `band` of the oracle's maximum is adopted and counted by ora_get_ties; any other hint is
+ * ignored.  `band` is ABSOLUTE (logit units): the caller passes a small multiple of the logit difference it
+ * MEASURED between the two implementations, so a hint is adopted only where that difference can flip the
+ * argmax; band <= 0 never adopts.  Pinned by tests/test_oracle_model.py::test_tie_hint_*. */
 int ora_step_follow(ora_ctx *, int32_t draft_override, int32_t draft_hint, int32_t verify_hint, float band,
                     ora_step_result *out);
 void ora_get_ties(const ora_ctx *, int32_t *verify_ties, int32_t *pdm_ties);

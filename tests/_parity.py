@@ -6,12 +6,15 @@ pre-norm vector, logits, KV lengths (exact) and KV rows.
 
 Token exactness and ties.  The CUDA path accumulates in fp32, the oracle
 in fp64; through 32 random-init layers that difference grows to ~1e-3 of the logit scale, while the
-top-1/top-2 gap of 151 936 near-i.i.d. logits is below that for a few percent of the argmaxes.  Where
-the two argmaxes differ, the CUDA token is accepted only if its ORACLE logit lies within
-2 * logit_tol * max|logit| of the oracle's maximum — i.e. only if the disagreement is implied by the
-logit tolerance that is asserted anyway (several results are then correct; the rest must be valid).
-The oracle then follows that token (ora_step_follow) so every later cycle is still compared exactly.
-Any other token difference is a failure.
+top-1/top-2 gap of 151 936 near-i.i.d. logits is below that for a small share of the argmaxes.  Protocol:
+(1) every CUDA token must be the argmax (lowest index) of the CUDA path's OWN logit vector — exact;
+(2) that vector must match the oracle's within the tensor tolerance;
+(3) where the two argmaxes still differ, the CUDA token is adopted only if its ORACLE logit lies within
+    band = 3 x the largest |gpu - oracle| logit difference MEASURED so far in the run (not the asserted
+    tolerance) of the oracle's maximum; the oracle then follows that token (ora_step_follow) so every later
+    cycle is still compared exactly.  Adoptions are counted (verify_ties / pdm_ties) and bounded by
+    assert_ties(): zero whenever the smallest top-1/top-2 margin of the run exceeds twice the measured logit
+    error, else a small share of the argmaxes.  Any other token difference is a failure.
 """
 from __future__ import annotations
 
@@ -47,13 +50,27 @@ class Report:
     rejects: int = 0
     verify_ties: int = 0
     pdm_ties: int = 0
+    argmaxes: int = 0             # greedy decisions compared (first token + one per PDM pass + one per exit)
+    max_logit_abs_err: float = 0.0
     tokens: list = dataclasses.field(default_factory=list)
 
     def summary(self) -> str:
         return (f"{self.status} steps={self.steps} emitted={self.emitted} acc/rej={self.accepts}/{self.rejects} "
                 f"hidden={self.max_hidden_err:.2e} pdm={self.max_pdm_err:.2e} logits={self.max_logit_err:.2e} "
                 f"kvflip={self.kv_flip_frac:.2e} min_margin={self.min_margin:.2e} "
-                f"ties(verify/pdm)={self.verify_ties}/{self.pdm_ties} {self.detail}")
+                f"ties(verify/pdm)={self.verify_ties}/{self.pdm_ties} of {self.argmaxes} argmaxes "
+                f"logit_abs={self.max_logit_abs_err:.2e} {self.detail}")
+
+
+def assert_ties(rep: "Report", share: float = 0.05):
+    """north_star: "emitted token ids exact".  Zero adoptions wherever the run's smallest top-1/top-2 margin exceeds
+    twice the measured logit error (then no argmax can legitimately flip); otherwise at most `share` of the argmaxes
+    (>= 1).  Both quantities are relative to max|logit| (C-2.18 metric)."""
+    ties = rep.verify_ties + rep.pdm_ties
+    if rep.min_margin > 2.0 * rep.max_logit_err:
+        assert ties == 0, f"{ties} tie adoptions although min margin {rep.min_margin:.2e} > 2 x logit error {rep.max_logit_err:.2e}"
+    else:
+        assert ties <= max(1, int(share * rep.argmaxes)), f"{ties} tie adoptions in {rep.argmaxes} argmaxes"
 
 
 def kv_compare(gpu, ora, layers, rows, rep: Report, tol: float):
@@ -74,11 +91,10 @@ def kv_compare(gpu, ora, layers, rows, rep: Report, tol: float):
 def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, engine=None, tensor_every=1,
                tensor_tol=CONTRACT, check_logits=True, prefill_block=16, max_seq=None, gpu=None) -> Report:
     """forced = (truth tokens, p, seed) or None (the PDM's own drafts).  tensor_tol bounds hidden states,
-    the PDM vector and logits (C-2.18 metric); the tie band is 2 * tensor_tol."""
+    the PDM vector and logits (C-2.18 metric); the tie band is 3 x the measured logit difference (module doc)."""
     from paper_2605_30852_b200 import SPD, OPT
     rep = Report()
     n = shape.n_stages
-    band = 2.0 * tensor_tol
     ms = max_seq or (len(prompt) + n_tokens * (n + 1) + 2 * n + 8)
     ora = Oracle(shape, weights_np, max_seq=ms)
     own = gpu is None
@@ -92,11 +108,22 @@ def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, en
     try:
         if engine is not None:
             gpu.set_option(OPT.ENGINE, engine)
-        gpu.set_option(OPT.DEBUG_LOGITS, 1 if check_logits else 0)
+        gpu.set_option(OPT.DEBUG_LOGITS, 1)      # the measured logit difference sets the tie band
         fo = ora.prefill(prompt, block=prefill_block)
         fg = gpu.prefill(prompt)
         gap, mx = ora.margin(0)
         rep.min_margin = gap / mx
+        lg_g, lg_o = gpu.last("exit_logits"), ora.last("exit_logits")
+        delta_run = float(np.max(np.abs(lg_g.astype(np.float64) - lg_o)))
+        maxabs = float(mx)
+        rep.max_logit_abs_err = delta_run
+        rep.max_logit_err = delta_run / maxabs
+        rep.argmaxes = 1
+        if int(np.argmax(lg_g)) != fg:
+            return fail(f"first token {fg} is not the argmax of the CUDA path's own logits ({int(np.argmax(lg_g))})")
+        if rep.max_logit_err > tensor_tol:
+            return fail(f"prefill logits rel err {rep.max_logit_err:.3e}")
+        band = 3.0 * delta_run + 1e-6 * maxabs
         P = len(prompt)
         e = rel_err(gpu.hfin(P - 1), ora.hfin(P - 1))
         rep.max_hidden_err = max(rep.max_hidden_err, e)
@@ -104,7 +131,7 @@ def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, en
             return fail(f"prefill final hidden state rel err {e:.3e}")
         if fo != fg:
             lg = ora.last("exit_logits")
-            if lg[fo] - lg[fg] <= band * mx:
+            if lg[fo] - lg[fg] <= band:
                 rep.verify_ties += 1
                 ora.rollback(P, fg)          # both are valid first tokens at the logit tolerance: follow the GPU
             else:
@@ -121,15 +148,37 @@ def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, en
         v0 = rep.verify_ties
         while ora.emitted < n_tokens:
             rg = gpu.step()
+            band = 3.0 * delta_run + 1e-6 * maxabs
             ro = ora.step_follow(-1 if rg.draft_forced else rg.draft_token, rg.emitted_token if rg.exited else -1, band)
             rep.steps += 1
+            rep.argmaxes += 1 + (1 if rg.exited else 0)
+            # (1) the CUDA tokens are the argmax (lowest index) of the CUDA path's own logit vectors; (2) the measured
+            # logit difference of this cycle widens the band of the following cycles
+            lp_g, lp_o = gpu.last("pdm_logits"), ora.last("pdm_logits")
+            if not rg.draft_forced and int(np.argmax(lp_g)) != rg.draft_token:
+                return fail(f"step {rep.steps}: draft {rg.draft_token} is not the argmax of the CUDA PDM logits")
+            d = float(np.max(np.abs(lp_g.astype(np.float64) - lp_o)))
+            maxabs = max(maxabs, float(np.max(np.abs(lp_o))))
+            rep.max_logit_err = max(rep.max_logit_err, rel_err(lp_g, lp_o))
+            if rg.exited:
+                le_g, le_o = gpu.last("exit_logits"), ora.last("exit_logits")
+                if int(np.argmax(le_g)) != rg.emitted_token:
+                    return fail(f"step {rep.steps}: emitted {rg.emitted_token} is not the argmax of the CUDA exit logits")
+                d = max(d, float(np.max(np.abs(le_g.astype(np.float64) - le_o))))
+                maxabs = max(maxabs, float(np.max(np.abs(le_o))))
+                rep.max_logit_err = max(rep.max_logit_err, rel_err(le_g, le_o))
+            delta_run = max(delta_run, d)
+            rep.max_logit_abs_err = delta_run
+            if rep.max_logit_err > tensor_tol:
+                return fail(f"step {rep.steps}: logits rel err {rep.max_logit_err:.3e} > {tensor_tol}")
             vt, pt = ora.ties()
             rep.verify_ties, rep.pdm_ties = v0 + vt, pt
             if tuple(ro) != tuple(rg):
                 gv, mv = ora.margin(0)
                 gp, mp = ora.margin(1)
                 return fail(f"step {rep.steps}: gpu {tuple(rg)} != oracle {tuple(ro)} "
-                            f"(verify margin {gv / mv:.2e}, PDM margin {gp / mp:.2e}, band {band:.1e})")
+                            f"(verify margin {gv / mv:.2e}, PDM margin {gp / mp:.2e}, band {band:.1e} abs = "
+                            f"{band / maxabs:.1e} of max|logit|)")
             if ro.exited:
                 rep.emitted += 1
                 rep.tokens.append(ro.emitted_token)
@@ -149,11 +198,6 @@ def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, en
                         return fail(f"step {rep.steps}: depth {k} holds {slots[k]}, oracle ({pos},{tok})")
                     rep.max_hidden_err = max(rep.max_hidden_err, rel_err(gpu.hidden(k), h))
                 rep.max_pdm_err = max(rep.max_pdm_err, rel_err(gpu.last("pdm_prenorm"), ora.last("pdm_prenorm")))
-                if check_logits:
-                    e = rel_err(gpu.last("pdm_logits"), ora.last("pdm_logits"))
-                    if ro.exited:
-                        e = max(e, rel_err(gpu.last("exit_logits"), ora.last("exit_logits")))
-                    rep.max_logit_err = max(rep.max_logit_err, e)
                 if not np.array_equal(gpu.kv_len(), ora.kv_len()):
                     return fail(f"step {rep.steps}: KV lengths differ")
                 worst = max(rep.max_hidden_err, rep.max_pdm_err, rep.max_logit_err)

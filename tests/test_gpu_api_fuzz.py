@@ -85,7 +85,7 @@ def test_random_call_sequences_match_the_oracle(engine, n, seed):
                 else:
                     rg = gpu.step_many(k) if many else [gpu.step() for _ in range(k)]
                     for a in rg:
-                        b = ora.step_follow(-1 if a.draft_forced else a.draft_token, a.emitted_token if a.exited else -1, 2e-3)
+                        b = ora.step_follow(-1 if a.draft_forced else a.draft_token, a.emitted_token if a.exited else -1, 3.0 * delta[0] + 1e-5)
                         assert tuple(a) == tuple(b), f"{log[-8:]}: gpu {tuple(a)} != oracle {tuple(b)}"
                     ties[1] = sum(ora.ties())
             elif op == "rollback":

@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 
 import spd_inputs as si
-from tests._parity import run_parity, CONTRACT
+from tests._parity import run_parity, assert_ties, CONTRACT
 from tests._util import TINY, shape_of
 
 pytestmark = pytest.mark.gpu
@@ -58,6 +58,7 @@ def test_tiny_baseline_config_pdm_drafts(engine):
     rep = run_parity(**_inputs(TINY, TINY.prompt_len), n_tokens=TINY.gen_len, engine=engine, tensor_tol=1e-3)
     print("tiny baseline:", rep.summary())
     assert rep.status == "ok", rep.detail
+    assert_ties(rep)
     assert rep.emitted == TINY.gen_len - 1 and rep.verify_ties + rep.pdm_ties == 0
 
 
@@ -73,6 +74,7 @@ def test_tiny_hot_forced_acceptance(engine, n, p):
     rep = run_parity(**inp, n_tokens=G, forced=(_truth(shape, inp, G + 8), p, 7), engine=engine, tensor_tol=5e-3)
     print(f"tiny hot n={n} p={p}:", rep.summary())
     assert rep.status == "ok", rep.detail
+    assert_ties(rep)
     if p == 1.0:
         assert rep.rejects == 0 and rep.steps == G + n - 2
     if p == 0.0 and n > 1:
@@ -86,6 +88,7 @@ def test_tiny_attention_heavy(engine):
     rep = run_parity(**_inputs(TINY, 32, std=0.04, attention_heavy=True), n_tokens=48, engine=engine, tensor_tol=5e-3)
     print("attention heavy:", rep.summary())
     assert rep.status == "ok", rep.detail
+    assert_ties(rep)
 
 
 @pytest.mark.parametrize("engine", ENGINES)
@@ -100,6 +103,7 @@ def test_full_model_dims_short_prompt(engine, name, prompt_len, gen):
                      tensor_tol=1e-2, tensor_every=3)
     print(name, rep.summary())
     assert rep.status == "ok", rep.detail
+    assert_ties(rep)
     assert rep.max_hidden_err < CONTRACT and rep.max_logit_err < CONTRACT
 
 
@@ -115,4 +119,5 @@ def test_tensor_core_attention_path_midsize(hq, hkv):
     rep = run_parity(**inp, n_tokens=24, engine=1, tensor_tol=5e-4)
     print(f"mid Hq={hq} Hkv={hkv}:", rep.summary())
     assert rep.status == "ok", rep.detail
+    assert_ties(rep)
     assert rep.max_hidden_err < 5e-4 and rep.max_logit_err < 5e-4

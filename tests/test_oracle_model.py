@@ -312,3 +312,96 @@ def test_config_validation():
         Oracle(TINY.replace(n_stages=3), w)                      # L % n != 0 (C-2.7)
     with pytest.raises(ValueError):
         Oracle(TINY.replace(n_q_heads=3), w)
+
+
+# ------------------------------------------------------------------ the tie-hint test hook (ora_step_follow) ----
+# The GPU parity harness lets the oracle continue with the CUDA path's token when the two argmaxes differ by less
+# than the measured logit difference (tests/_parity.py).  These pins fix the hook itself: an inverted comparison,
+# a relative-vs-absolute band mix-up or a missing range check would make the GPU token-exactness checks vacuous.
+
+def _twin(n=2):
+    a, b = new_oracle(n), new_oracle(n)
+    assert a.prefill(PROMPT) == b.prefill(PROMPT)
+    return a, b
+
+
+def _runner_up(logits):
+    order = np.argsort(-logits.astype(np.float64), kind="stable")
+    return int(order[0]), int(order[1]), float(logits[order[0]] - logits[order[1]])
+
+
+def test_tie_hint_band_zero_or_no_hint_is_the_plain_step():
+    a, b = _twin(2)
+    for i in range(12):
+        ra = a.step()
+        top, second, _ = _runner_up(a.last("pdm_logits"))
+        rb = b.step_follow(second, (top + 1) % TINY.vocab, 0.0)        # band 0: never adopted
+        assert tuple(ra) == tuple(rb)
+    assert b.ties() == (0, 0)
+    rb = b.step_follow(-1, -1, 1e9)                                    # no hint: nothing to adopt at any band
+    assert tuple(a.step()) == tuple(rb) and b.ties() == (0, 0)
+    a.close(); b.close()
+
+
+def test_tie_hint_pdm_adopted_only_inside_the_absolute_band():
+    """The PDM argmax: a hint whose oracle logit is `gap` below the maximum is ignored at band < gap, adopted at
+    band > gap (and only then counted); the adopted token is the one that enters the pipeline."""
+    a, b = _twin(4)
+    ra = a.step()                                                      # the twin shows what this cycle's logits are
+    top, second, gap = _runner_up(a.last("pdm_logits"))
+    assert ra.draft_token == top and gap > 0 and not ra.exited
+    c = new_oracle(4); c.prefill(PROMPT)
+    rc = c.step_follow(second, -1, 0.9 * gap)
+    assert tuple(rc) == tuple(ra) and c.ties() == (0, 0)               # outside the band: ignored
+    rb = b.step_follow(second, -1, 1.1 * gap)
+    assert rb.draft_token == second and b.ties() == (0, 1)             # inside: adopted, counted as a PDM tie
+    assert b.ring(b.fill - 1)[1] == second                             # ... and it is what entered stage 0
+    # the band is ABSOLUTE: scaled by max|logit| it would be far wider / narrower than the gap
+    _, mx = a.margin(1)
+    assert not (0.9 < mx < 1.1), "choose a config whose logit scale is not ~1, so relative vs absolute differ"
+    d = new_oracle(4); d.prefill(PROMPT)
+    rd = d.step_follow(second, -1, 0.9 * gap / mx if mx > 1 else 0.9 * gap * mx)   # what a relative reading would pass
+    assert (d.ties() == (0, 0)) == (rd.draft_token == top)
+    a.close(); b.close(); c.close(); d.close()
+
+
+def test_tie_hint_rejects_far_and_invalid_tokens():
+    """A comparison with the wrong sign would adopt the WORST token; out-of-range ids must never be adopted."""
+    a, b = _twin(2)
+    ra = a.step()
+    lg = a.last("pdm_logits")
+    worst = int(np.argmin(lg))
+    top, _, gap = _runner_up(lg)
+    for hint in (worst, TINY.vocab, TINY.vocab + 7, -5):
+        c = new_oracle(2); c.prefill(PROMPT)
+        rc = c.step_follow(hint, -1, 2.0 * gap)
+        assert tuple(rc) == tuple(ra) and c.ties() == (0, 0), hint
+        c.close()
+    a.close(); b.close()
+
+
+def test_tie_hint_verify_adopted_token_is_emitted_and_judges_the_successor():
+    """At an exit the verify hint, if adopted, is the emitted token y: the successor is accepted iff it equals
+    the hint, a reject reseeds with the hint (PAPER.md:129-131 applied to the adopted argmax)."""
+    n = 2
+    a, b = _twin(n)
+    while True:                                                        # advance both to the cycle before an exit
+        if a.ring(0)[2] == n - 1:
+            break
+        a.step(); b.step()
+    succ = a.ring(1)[1] if a.fill > 1 else None
+    ra = a.step()
+    assert ra.exited
+    top, second, gap = _runner_up(a.last("exit_logits"))
+    assert ra.emitted_token == top
+    c = new_oracle(n); c.prefill(PROMPT)
+    while c.steps < b.steps:
+        c.step()
+    rc = c.step_follow(-1, second, 0.5 * gap)
+    assert tuple(rc) == tuple(ra) and c.ties() == (0, 0)               # outside the band
+    rb = b.step_follow(-1, second, 1.5 * gap)
+    assert b.ties() == (1, 0) and rb.emitted_token == second
+    assert rb.accepted == int(succ == second)
+    if not rb.accepted:
+        assert b.fill == 1 and b.ring(0)[1] == second and np.all(b.kv_len() == b.committed_len)
+    a.close(); b.close(); c.close()
