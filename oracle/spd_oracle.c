@@ -128,12 +128,15 @@ void ora_op_attention(const float *q, const uint16_t *kc, const uint16_t *vc, in
     double *w = (double *)malloc(sizeof(double) * (size_t)t_len);
     double denom = 0.0;
     for (int t = 0; t < t_len; ++t) { w[t] = exp((double)s[t] - (double)m); denom += w[t]; }
-    for (int e = 0; e < head_dim; ++e) {
-      double acc = 0.0;
-      for (int t = 0; t < t_len; ++t)
-        acc += w[t] * (double)bf16_to_f32(vc[(size_t)t * row + (size_t)kvh * head_dim + e]);
-      out[(size_t)hq * head_dim + e] = (float)(acc / denom);
+    /* o_e = sum_t w_t V[t][e] / denom: every element's sum runs over t in ascending order; the t loop is the outer
+     * one only so that a V row is read contiguously (same operations per element, same order, same result) */
+    double *acc = (double *)calloc((size_t)head_dim, sizeof(double));
+    for (int t = 0; t < t_len; ++t) {
+      const uint16_t *vr = vc + (size_t)t * row + (size_t)kvh * head_dim;
+      for (int e = 0; e < head_dim; ++e) acc[e] += w[t] * (double)bf16_to_f32(vr[e]);
     }
+    for (int e = 0; e < head_dim; ++e) out[(size_t)hq * head_dim + e] = (float)(acc[e] / denom);
+    free(acc);
     free(w);
     free(s);
   }
