@@ -122,6 +122,9 @@ enum {
   SPD_DBG_RING = 8,        /* int32[2 + 3n]: fill a, committed c, then per depth k: occupied, pos, tok */
   SPD_DBG_HFIN = 9,        /* [position] fp32[d]: final hidden state of a committed position        */
   SPD_DBG_SAMPLE = 11,     /* spd_sample_record of the last cycle (needs spd_set_sampling)                */
+  SPD_DBG_Q = 12,          /* [stage k] fp32[n_q_heads*hd]: q (after RoPE) of the token that ran stage k in the
+                              last cycle, at that stage's LAST layer (k+1)*L/n - 1 (per-kernel attention parity)  */
+  SPD_DBG_ATT = 13,        /* [stage k] fp32[n_q_heads*hd]: that layer's attention output (input of the O GEMV)   */
   SPD_DBG_PHASE_PROFILE = 10 /* uint64[160][168][6]: per (CTA, phase) clock stamps of the last fused cycle:
                               0 inputs ready, 1 activations staged, 2 tiles consumed, 3/4 producer issued the
                               phase's first/last tile (SM clock); 5 = %globaltimer at stamp 0; phase 167 holds

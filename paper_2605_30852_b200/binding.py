@@ -34,7 +34,7 @@ class OPT:
 
 class DBG:
     SLOT_HIDDEN, EXIT_LOGITS, PDM_LOGITS, PDM_PRENORM, PDM_FEAT, KV_K, KV_V, KV_LEN, RING, HFIN, PHASE_PROFILE, \
-        SAMPLE = range(12)
+        SAMPLE, Q, ATT = range(14)
 
 
 MAX_TOPK = 64
@@ -300,6 +300,14 @@ class SPD:
 
     def hidden(self, depth: int) -> np.ndarray:
         return self.debug_read(DBG.SLOT_HIDDEN, depth, np.float32, self.shape.d_model)
+
+    def stage_q(self, stage: int) -> np.ndarray:
+        """q (after RoPE) of the token that ran `stage` in the last cycle, at the stage's last layer (SPD_DBG_Q)."""
+        return self.debug_read(DBG.Q, stage, np.float32, self.shape.n_q_heads * self.shape.head_dim)
+
+    def stage_att(self, stage: int) -> np.ndarray:
+        """The attention output of that layer (SPD_DBG_ATT)."""
+        return self.debug_read(DBG.ATT, stage, np.float32, self.shape.n_q_heads * self.shape.head_dim)
 
     def hfin(self, pos: int) -> np.ndarray:
         return self.debug_read(DBG.HFIN, pos, np.float32, self.shape.d_model)

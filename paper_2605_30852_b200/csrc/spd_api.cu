@@ -474,6 +474,10 @@ extern "C" int spd_debug_read(spd_ctx *ctx, int32_t what, int32_t index, void *h
     case SPD_DBG_HFIN:
       if (index < 0 || index >= D.max_seq) return fail(ctx, SPD_EINVAL, "debug_read: position out of range%s");
       src = P.hfin + (size_t)index * D.d; want = sizeof(float) * D.d; break;
+    case SPD_DBG_Q:
+    case SPD_DBG_ATT:
+      if (index < 0 || index >= D.n) return fail(ctx, SPD_EINVAL, "debug_read: stage out of range%s");
+      src = (what == SPD_DBG_Q ? P.q : P.att) + (size_t)index * D.Hq * D.hd; want = sizeof(float) * D.Hq * D.hd; break;
     case SPD_DBG_SAMPLE:
       if (!P.sampling) return fail(ctx, SPD_ESTATE, "debug_read: sampling verification is off%s");
       src = &P.samp->rec; want = sizeof(SampleRecord); break;

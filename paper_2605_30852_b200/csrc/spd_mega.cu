@@ -1311,8 +1311,9 @@ static void make_layout(const Dims &D, MegaLayout *ML, size_t *total) {
 static bool mega_supported(const Dims &D) {
   int qd = D.Hq * D.hd;
   int G = D.Hq / D.Hkv;
+  // 2 + 5 * (L / n) phases must fit the claim-counter / profile tables (P.claim is [kProfPhases][kMaxStages])
   return D.d <= kXFloats / 2 && qd <= kXFloats && D.F <= kXFloats && (G == 1 || G == 2 || G == 4 || G == 8) &&
-         (qd + 2 * D.Hkv * D.hd) % 2 == 0 && D.hd % 2 == 0;
+         (qd + 2 * D.Hkv * D.hd) % 2 == 0 && D.hd % 2 == 0 && 2 + 5 * D.per <= kProfPhases;
 }
 
 size_t mega_repack_bytes(const Dims &D) {
@@ -1337,7 +1338,7 @@ int mega_create(const DevPtrs &P, const uint16_t *const *const *src, void *repac
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   int smem = kStages * kTileBytes + kXFloats * 4 + 2 * kStages * 8 + 64 * 8 + 16 * 4 + 32 * 4 + 16 * 4 + 128 * 4 + (int)sizeof(Sched);
-  if (!coop || sms < D.n) return -1;
+  if (!coop || sms < D.n || sms > kMaxCand) return -1;   // one argmax candidate slot per CTA
   if (cudaFuncSetAttribute(k_spd_cycle, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
     cudaGetLastError();
     return -1;
