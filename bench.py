@@ -262,6 +262,7 @@ def run_gpu(args, shape):
     _, _, l1 = eng.counters()
     launches = l1 - l0
     assert all(r.fill == n and r.exited and r.accepted for r in res), "timed steps must be saturated accept steps"
+    timed_lat = [us for _, us in cycle_latencies_us(eng, res, 512)]      # device stamps of the timed cycles themselves
     ctx_mid = (res[0].committed_len + res[-1].committed_len) // 2 + n // 2
     by = step_bytes(shape, ctx_mid)
 
@@ -276,13 +277,25 @@ def run_gpu(args, shape):
 
     # ---- acceptance sweep (tokens/s at the config's p values; not part of the timed K steps) --------
     sweep = {}
+    fill_samples = []
+    SW_CHUNK = 32
     for p in shape.p_sweep:
         rewind(p)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        toks_p, log = eng.generate(G, chunk=32)
+        toks_p, log, unread = [], [], 0
+        while len(toks_p) < G - 1:
+            chunk_log = eng.step_many(SW_CHUNK)
+            log += chunk_log
+            toks_p += [r.emitted_token for r in chunk_log if r.exited]
+            unread += SW_CHUNK
+            if unread + SW_CHUNK > 1024:                      # the device keeps the stamps of the last 1024 cycles
+                fill_samples += cycle_latencies_us(eng, log[-unread:], SW_CHUNK)
+                unread = 0
         e1.record(stream)
         torch.cuda.synchronize()
+        if unread:
+            fill_samples += cycle_latencies_us(eng, log[-unread:], SW_CHUNK)
         ms = e0.elapsed_time(e1)
         emitted = sum(r.exited for r in log)
         ok = ([first] + toks_p)[:G] == list(truth[:G])
@@ -357,7 +370,7 @@ def run_gpu(args, shape):
         "dtype": "bf16 weights, f32 activations/accumulation", "data": "synthetic",
         "config": {"workload": f"{shape.name}: d={shape.d_model} L={shape.n_layers} n={n} F={shape.d_ffn} V={shape.vocab}, "
                                f"prompt {P}, saturated cycles at forced p=1.0 (context ~{ctx_mid})",
-                   "engine": "fused persistent cycle kernel" if launches == args.steps * world else "reference (kernel per op)",
+                   "engine": "fused persistent cycle kernel" if launches == args.steps else "reference (kernel per op)",
                    "l2": "working set %.1f GB per step >> 126 MB L2: no flush needed" % (by["full"] / 1e9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "tokens_per_s": tot["tokens_per_s"], "hbm_gbs": tot["hbm_gbs"],
@@ -370,6 +383,9 @@ def run_gpu(args, shape):
         "e2e": {"value": tot["e2e_us"], "unit": "us", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": d2h,
                 "note": "spd_step(): launch + result/state D2H + stream sync per cycle; the cycle has no per-step host input "
                         "(ring, KV and lengths live on the device)"},
+        "step_us_stats": {**percentiles(timed_lat), "unit": "us",
+                          "source": "finish-stamp differences (%globaltimer, SPD_DBG_CYCLE_TIMES) of the timed back-to-back cycles"},
+        "by_fill": by_fill_table(shape, fill_samples, peak),
         "gpu_launches": int(tot["gpu_launches"]), "clocks": clk, "p_sweep": sweep, "sampling": sampling,
         "setup_s": t_setup,
     }
@@ -380,6 +396,51 @@ def run_gpu(args, shape):
                                           f"of length {ctx_mid}"}
     print(json.dumps(line), flush=True)
     eng.close()
+
+
+def percentiles(x) -> dict:
+    a = np.asarray(x, dtype=np.float64)
+    if a.size == 0:
+        return {"n": 0}
+    return {"n": int(a.size), "median": float(np.median(a)), "p10": float(np.percentile(a, 10)),
+            "p90": float(np.percentile(a, 90)), "mean": float(a.mean())}
+
+
+def cycle_latencies_us(eng, log, chunk: int):
+    """Per-cycle step latency from the device's own stamps (SPD_DBG_CYCLE_TIMES): the difference of the finish stamps
+    (%globaltimer) of consecutive back-to-back cycles.  `log` = the StepResults of cycles enqueued in chunks of
+    `chunk` (a host sync separates chunks, so the first cycle of a chunk has no back-to-back predecessor and is
+    left out).  Only the last 1024 cycles are on the device.  Returns [(StepResult, latency_us)]."""
+    tail = log[-1024:]
+    off = len(log) - len(tail)
+    ts = eng.cycle_times([r.step_index for r in tail])
+    out = []
+    for j in range(1, len(tail)):
+        if (off + j) % chunk == 0 or tail[j].step_index != tail[j - 1].step_index + 1:
+            continue
+        out.append((tail[j], (ts[j, 1] - ts[j - 1, 1]) / 1e3))
+    return out
+
+
+def by_fill_table(shape, samples, peak_gbs: float) -> dict:
+    """latency and GB/s per fill level a.  B(a) = (a/n) layer weights + KV rows of a tokens + E + W_p
+    (reporting.step_bytes; a cycle without an exit still runs the PDM's pass over the tied E)."""
+    n = shape.n_stages
+    out = {}
+    for a in range(1, n + 1):
+        for exited in (0, 1):
+            sel = [(r, us) for r, us in samples if r.fill == a and r.exited == exited]
+            if not sel:
+                continue
+            st = percentiles([us for _, us in sel])
+            ctx = int(np.median([r.committed_len for r, _ in sel])) + a // 2
+            by = step_bytes(shape, ctx, fill=a, exited=bool(exited))
+            gbs = by["full"] / st["median"] / 1e3
+            out[f"{a}{'' if exited == (a == n) else ('+exit' if exited else '-noexit')}"] = {
+                **st, "unit": "us", "exited": bool(exited), "algorithmic_bytes": by["full"], "algorithmic_bytes_strict": by["strict"],
+                "gbs": gbs, "frac_of_8tbs": gbs / NOMINAL_HBM_GBS, "frac_of_8tbs_strict": by["strict"] / st["median"] / 1e3 / NOMINAL_HBM_GBS,
+                "frac_of_measured_peak": gbs / peak_gbs}
+    return out
 
 
 def eng_state_bytes() -> int:

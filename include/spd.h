@@ -125,6 +125,9 @@ enum {
   SPD_DBG_Q = 12,          /* [stage k] fp32[n_q_heads*hd]: q (after RoPE) of the token that ran stage k in the
                               last cycle, at that stage's LAST layer (k+1)*L/n - 1 (per-kernel attention parity)  */
   SPD_DBG_ATT = 13,        /* [stage k] fp32[n_q_heads*hd]: that layer's attention output (input of the O GEMV)   */
+  SPD_DBG_CYCLE_TIMES = 14,/* uint64[1024][2]: %globaltimer (ns) at which the controller of the cycle with step_index K
+                              began [(K-1) % 1024][0] (kernel entry of the fused engine) and finished [..][1]; the
+                              difference of consecutive finish stamps of back-to-back cycles is the step latency   */
   SPD_DBG_PHASE_PROFILE = 10 /* uint64[160][168][6]: per (CTA, phase) clock stamps of the last fused cycle:
                               0 inputs ready, 1 activations staged, 2 tiles consumed, 3/4 producer issued the
                               phase's first/last tile (SM clock); 5 = %globaltimer at stamp 0; phase 167 holds

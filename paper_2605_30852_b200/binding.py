@@ -34,7 +34,7 @@ class OPT:
 
 class DBG:
     SLOT_HIDDEN, EXIT_LOGITS, PDM_LOGITS, PDM_PRENORM, PDM_FEAT, KV_K, KV_V, KV_LEN, RING, HFIN, PHASE_PROFILE, \
-        SAMPLE, Q, ATT = range(14)
+        SAMPLE, Q, ATT, CYCLE_TIMES = range(15)
 
 
 MAX_TOPK = 64
@@ -320,6 +320,12 @@ class SPD:
         if rows == 0:
             return np.zeros((0, w), dtype=np.uint16)
         return self.debug_read(DBG.KV_V if which else DBG.KV_K, layer, np.uint16, rows * w).reshape(rows, w)
+
+    def cycle_times(self, step_indices) -> np.ndarray:
+        """int64[len, 2]: (begin, end) %globaltimer stamps in ns of the cycles with the given step_index values (the
+        device keeps the last 1024 cycles; SPD_DBG_CYCLE_TIMES)."""
+        ring = self.debug_read(DBG.CYCLE_TIMES, 0, np.uint64, 2 * 1024).reshape(1024, 2).astype(np.int64)
+        return ring[(np.asarray(step_indices, dtype=np.int64) - 1) % 1024]
 
     def phase_profile(self) -> np.ndarray:
         """uint64[160, 168, 6] clock stamps of the last fused cycle (see SPD_DBG_PHASE_PROFILE in spd.h)."""

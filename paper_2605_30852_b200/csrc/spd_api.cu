@@ -118,6 +118,7 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
   Q.truth = cv.take<int32_t>(D.max_seq);
   Q.pf_tokens = cv.take<int32_t>(D.max_seq);
   Q.results = cv.take<StepResult>(kResultRing);
+  Q.cycle_ts = cv.take<unsigned long long>(2 * (size_t)kResultRing);
   Q.bar = cv.take<unsigned int>(kBarWords);
   Q.claim = cv.take<unsigned int>((size_t)kProfPhases * kMaxStages);
   Q.prof = cv.take<unsigned long long>((size_t)kProfCtas * kProfPhases * kProfStamps);
@@ -481,6 +482,8 @@ extern "C" int spd_debug_read(spd_ctx *ctx, int32_t what, int32_t index, void *h
     case SPD_DBG_SAMPLE:
       if (!P.sampling) return fail(ctx, SPD_ESTATE, "debug_read: sampling verification is off%s");
       src = &P.samp->rec; want = sizeof(SampleRecord); break;
+    case SPD_DBG_CYCLE_TIMES:
+      src = P.cycle_ts; want = sizeof(unsigned long long) * 2 * kResultRing; break;
     case SPD_DBG_PHASE_PROFILE:
       src = P.prof; want = sizeof(unsigned long long) * kProfCtas * kProfPhases * kProfStamps; break;
     case SPD_DBG_RING: {

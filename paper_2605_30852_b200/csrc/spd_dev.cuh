@@ -110,6 +110,7 @@ struct DevPtrs {
   int32_t *truth;                    // [max_seq]
   int32_t *pf_tokens;                // [max_seq]
   StepResult *results;               // [kResultRing]
+  unsigned long long *cycle_ts;      // [kResultRing][2] %globaltimer (ns) when the cycle's controller began / ended, filed like results
   unsigned int *bar;                 // grid-barrier words (fused engine)
   unsigned int *claim;               // [kProfPhases][kMaxStages] work-claim counters of one cycle (fused engine)
   uint16_t *kv;                      // K/V cache
@@ -142,6 +143,12 @@ __device__ __forceinline__ uint16_t f32_to_bf16(float f) {
   uint32_t u = __float_as_uint(f);
   u += 0x7fffu + ((u >> 16) & 1u);
   return (uint16_t)(u >> 16);
+}
+
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
 }
 
 __device__ __forceinline__ float warp_sum(float v) {

@@ -161,6 +161,7 @@ __device__ __forceinline__ void controller_begin(const DevPtrs &P) {
   st->forced_now = 0;
   if (st->mode == MODE_SPD) {
     st->K += 1;
+    P.cycle_ts[2 * ((st->K - 1) % kResultRing)] = globaltimer_ns();   // entry stamp of cycle K (SPD_DBG_CYCLE_TIMES)
     if (st->forced_on) {
       unsigned long long draw = splitmix64(st->forced_seed + (unsigned long long)st->K) >> 11;
       int ti = st->p_new + 1 - st->prompt_len;
@@ -396,7 +397,7 @@ __device__ __forceinline__ int sample_residual(const SampleDist *Pt, const doubl
 // `sm`: shared-memory scratch for the sampler (may be nullptr when P.sampling == 0).
 // `with_lists`: the head pass filled the threshold lists (fused engine).
 __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, SampSmem *sm, bool with_lists = false) {
-  __shared__ int s_y, s_draft, s_exit_buf, s_exit_pos, s_enter_tok, s_enter_buf, s_do_exit, s_do_enter, s_keep_q;
+  __shared__ int s_y, s_draft, s_exit_buf, s_exit_pos, s_enter_tok, s_enter_buf, s_do_exit, s_do_enter, s_keep_q, s_stamp;
   StepState *st = P.st;
   const Dims &D = P.dim;
   int n = D.n;
@@ -468,6 +469,7 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, Samp
     r.step_index = (int)st->K; r.fill = st->fill; r.exited = 0; r.accepted = 0; r.emitted_token = -1;
     r.draft_token = -1; r.draft_forced = 0; r.discarded = 0;
     s_do_exit = 0; s_do_enter = 0; s_keep_q = 0;
+    s_stamp = mode == MODE_SPD ? (r.step_index - 1) % kResultRing : -1;
     if (sampling) {
       ss->rec.u_draft = ss->rec.u_accept = ss->rec.u_resid = -1.f;
       ss->rec.succ_token = -1; ss->rec.succ_q = ss->rec.succ_p = 0.f;
@@ -562,6 +564,8 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, Samp
       dst[i] = make_float4(bf16_lo(w.x), bf16_hi(w.x), bf16_lo(w.y), bf16_hi(w.y));
     }
   }
+  __syncthreads();
+  if (threadIdx.x == 0 && s_stamp >= 0) P.cycle_ts[2 * s_stamp + 1] = globaltimer_ns();   // the cycle's state is final
 }
 
 }  // namespace spd

@@ -150,11 +150,6 @@ __device__ __forceinline__ void split_bf16x2(float x0, float x1, uint32_t &hi, u
 // Orders generic-proxy accesses (st.global of the KV append) against async-proxy accesses (TMA reads).
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
-__device__ __forceinline__ unsigned long long globaltimer_ns() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-  return t;
-}
 __device__ __forceinline__ void prof_stamp(const DevPtrs &P, int cta, int phase, int stamp) {
   if (P.prof_on && cta < kProfCtas && phase < kProfPhases)
     P.prof[((size_t)cta * kProfPhases + phase) * kProfStamps + stamp] = (unsigned long long)clock64();

@@ -1,6 +1,10 @@
 """Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (-m gpu).
 
-The oracle cannot run a 2048-token 9B-class prefill in test time, so at full size the CUDA path is checked
+The oracle's 2048-token 9B-class prefill takes ~10 minutes on 16 host cores (the 4096-token one ~20) and the driver
+gives the whole GPU suite 20 minutes, so at full size the CUDA path is checked
+(0) against the ORACLE's values at the full prompt length, stored by tests/golden/fullsize_golden.py (SPD_FULL_TIER=live
+    recomputes them in-process): prefill result, first 32 emitted tokens, hidden states, logits, slot states
+    (tests/_fullsize.py);
 (a) on sampled outputs the oracle CAN compute one by one — K/V rows of layer 0 at any position (a function
     of that position's token only) and the whole depth of the first prompt positions (causal: they do not
     depend on the 2040 tokens after them);
@@ -18,6 +22,7 @@ import pytest
 
 import oracle as ora
 import spd_inputs as si
+from tests._fullsize import LIVE, golden_for, oracle_tier
 from tests._parity import run_parity, assert_ties, rel_err, CONTRACT
 
 pytestmark = pytest.mark.gpu
@@ -65,8 +70,18 @@ def test_full_prompt_sampled_oracle_outputs_and_invariants(name, G):
     wd = spd.upload_weights(w)
     max_seq = P + G * (n + 1) + 4 * n + 16
     eng = spd.SPD(shape, wd, max_seq=max_seq)
+    eng.set_option(spd.OPT.DEBUG_LOGITS, 1)
     first = eng.prefill(prompt)
     assert np.all(eng.kv_len() == P)
+
+    # ---- (0) the oracle tier of SURVEY C-4 at the full prompt: prefill result (first token, final hidden states,
+    #      K/V rows of layers {0, L/2-1, L-1}), the first 32 (n = 16: 8) emitted tokens with their final hidden states
+    #      and exit logits, spot-checked in-flight slot states, the PDM on the kernel's own slots --------------------
+    tier = oracle_tier(eng, shape, w, golden_for(name), first)
+    print(f"{name} full-prompt oracle tier ({'live oracle' if LIVE else 'stored oracle values'}):", tier.summary())
+    assert tier.accepts > 0 and tier.rejects > 0 and tier.slots_checked > 0 and tier.pdm_checked > 0
+    assert tier.ties <= 1 and (tier.ties == 0 or tier.min_margin <= 2.0 * tier.max_logit_err)
+    eng.rollback(P, first)
 
     # ---- (a) sampled outputs the oracle computes one by one -------------------------------------
     k_gpu, v_gpu = eng.kv(0, 0, P), eng.kv(0, 1, P)

@@ -405,3 +405,28 @@ def test_tie_hint_verify_adopted_token_is_emitted_and_judges_the_successor():
     if not rb.accepted:
         assert b.fill == 1 and b.ring(0)[1] == second and np.all(b.kv_len() == b.committed_len)
     a.close(); b.close(); c.close()
+
+
+def test_longer_prefill_restricted_to_a_prefix_is_the_shorter_prefill():
+    """Causality, as used by tests/golden/fullsize_golden.py (one 4096-token prefill serves the 2048-token config):
+    cache rows and final hidden states below P of a 2P-token prefill equal the P-token prefill's bitwise, and an
+    oracle loaded with those rows (ora_load_kv + ora_assume_prefilled) decodes the same greedy tokens."""
+    shape = shape_of("tiny")
+    w = weights("tiny")
+    long_prompt = si.make_prompt(shape, 1, 2 * P)
+    assert np.array_equal(long_prompt[:P], PROMPT)
+    a = Oracle(shape, w, max_seq=2 * P + 32)
+    a.prefill(long_prompt, block=16)
+    b = Oracle(shape, w, max_seq=P + 32)
+    first = b.prefill(PROMPT, block=16)
+    for l in range(shape.n_layers):
+        for which in (0, 1):
+            assert np.array_equal(a.kv(l, which, P), b.kv(l, which, P))
+    for pos in (0, P // 2, P - 1):
+        assert np.array_equal(a.hfin(pos), b.hfin(pos))
+    c = Oracle(shape, w, max_seq=P + 32)
+    for l in range(shape.n_layers):
+        c.load_kv(l, a.kv(l, 0, P), a.kv(l, 1, P))
+    c.assume_prefilled(P, first)
+    assert [b.ar_step() for _ in range(12)] == [c.ar_step() for _ in range(12)]
+    a.close(); b.close(); c.close()
