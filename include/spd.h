@@ -106,7 +106,10 @@ enum {
   SPD_OPT_ENGINE = 0,      /* 0 = one kernel per operation (reference engine), 1 = persistent fused
                               step kernel (default when available)                               */
   SPD_OPT_DEBUG_LOGITS = 1,/* 1 = also write full verify/PDM logit vectors (for parity tests)    */
-  SPD_OPT_PHASE_PROFILE = 2/* 1 = the fused kernel records per-phase clock stamps (SPD_DBG_PHASE_PROFILE) */
+  SPD_OPT_PHASE_PROFILE = 2,/* 1 = the fused kernel records per-phase clock stamps (SPD_DBG_PHASE_PROFILE) */
+  SPD_OPT_PREFILL = 3      /* 1 = batched tensor-core prefill (tcgen05 GEMMs over chunks of the prompt; default when the
+                              configuration supports it: d_model, n_q_heads*head_dim, d_ffn multiples of 64),
+                              0 = the prompt runs through the decode kernel, one token entering per cycle          */
 };
 
 /* spd_debug_read selectors.  `index` meaning in brackets. */
@@ -144,10 +147,14 @@ int spd_create(const spd_config *cfg, const spd_weights *w, const spd_buffers *b
 int spd_destroy(spd_ctx *ctx);
 
 /* Prefill (outside the paper's timed region): runs the prompt (HOST int32 ids,
- * 1 <= n_tokens < max_seq - 1) through all layers with the same kernels as the step, n tokens
- * pipelined over the n stages.  Afterwards: committed length = n_tokens, every layer holds n_tokens
- * KV rows, *first_token = argmax of the last position's logits is the single in-flight token, K = 0.
- * May be called again to start a new sequence. */
+ * 1 <= n_tokens < max_seq - 1) through all layers.  Default (SPD_OPT_PREFILL = 1): layer by layer over chunks of
+ * 1024 prompt tokens — GEMMs with M = tokens on the tcgen05 tensor cores (fp32 activations as three bf16 parts, exact,
+ * against the exact bf16 weights, fp32 accumulation in TMEM), causal GQA attention over the cache, the same RMSNorm /
+ * RoPE / bf16 KV append / SwiGLU arithmetic as the step.  SPD_OPT_PREFILL = 0: the prompt runs through the step's
+ * own kernel, n tokens pipelined over the n stages (one full weight sweep per token).  Either way, afterwards:
+ * committed length = n_tokens, every layer holds n_tokens KV rows, the final hidden state of every prompt position is
+ * kept (Eq. 5 warm-up features), *first_token = argmax of the last position's logits is the single in-flight
+ * token, K = 0.  May be called again to start a new sequence. */
 int spd_prefill(spd_ctx *ctx, const int32_t *tokens, int32_t n_tokens, int32_t *first_token);
 
 /* One SPD cycle including verification and, on reject, the internal rollback.  Returns after the
@@ -234,6 +241,10 @@ int spd_op_attention(const float *q, const uint16_t *kc, const uint16_t *vc, int
                      int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, float *out, float *scratch,
                      void *stream);
 size_t spd_op_attention_scratch(int32_t t_len, int32_t n_q_heads, int32_t head_dim);
+/* The prefill GEMM as one operation: y[M, N] = x[M, K] . W[N, K]^T, x fp32 (split exactly into three bf16 parts), W bf16 row-major,
+ * y fp32, on the tcgen05 tensor cores.  K % 64 == 0, N % 4 == 0.  scratch: DEVICE, >= spd_op_gemm_scratch(M, K) bytes. */
+int spd_op_gemm(const float *x, const uint16_t *w, int32_t m, int32_t n, int32_t k, float *y, void *scratch, void *stream);
+size_t spd_op_gemm_scratch(int32_t m, int32_t k);
 /* out[i] = silu(gate[i]) * up[i] */
 int spd_op_silu_mul(const float *gate, const float *up, int32_t n, float *out, void *stream);
 /* argmax with lowest-index ties of x[0..n); result int32 on the device */

@@ -30,6 +30,7 @@ class OPT:
     ENGINE = 0
     DEBUG_LOGITS = 1
     PHASE_PROFILE = 2
+    PREFILL = 3
 
 
 class DBG:
@@ -127,6 +128,9 @@ def lib():
         L.spd_last_error.restype = C.c_char_p
         L.spd_op_rmsnorm.argtypes = [vp, vp, i32, f32, vp, vp]
         L.spd_op_gemv.argtypes = [vp, i32, i32, vp, vp, vp]
+        L.spd_op_gemm.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp]
+        L.spd_op_gemm_scratch.argtypes = [i32, i32]
+        L.spd_op_gemm_scratch.restype = C.c_size_t
         L.spd_op_rope.argtypes = [vp, i32, i32, i32, f32, vp]
         L.spd_op_attention.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp]
         L.spd_op_attention_scratch.argtypes = [i32, i32, i32]
@@ -359,6 +363,16 @@ def op_gemv(w: torch.Tensor, x: torch.Tensor, stream=None) -> torch.Tensor:
     rows, k = w.shape
     out = torch.empty(rows, dtype=torch.float32, device=x.device)
     _chk(lib().spd_op_gemv(w.data_ptr(), rows, k, x.data_ptr(), out.data_ptr(), _s(stream)), "spd_op_gemv")
+    return out
+
+
+def op_gemm(x: torch.Tensor, w: torch.Tensor, stream=None) -> torch.Tensor:
+    """y[M, N] = x[M, K] . w[N, K]^T with the prefill's tcgen05 GEMM (x fp32, w bf16 bits as int16/uint16)."""
+    m, k = x.shape
+    n = w.shape[0]
+    out = torch.empty((m, n), dtype=torch.float32, device=x.device)
+    scratch = torch.empty(lib().spd_op_gemm_scratch(m, k), dtype=torch.uint8, device=x.device)
+    _chk(lib().spd_op_gemm(x.data_ptr(), w.data_ptr(), m, n, k, out.data_ptr(), scratch.data_ptr(), _s(stream)), "spd_op_gemm")
     return out
 
 

@@ -24,6 +24,8 @@ struct spd_ctx {
   int engine;
   int has_mega;
   MegaPlan mega;
+  int prefill_mode;        // 1: batched tensor-core prefill (spd_prefill.cu), 0: the decode kernel's prefill mode
+  PrefillPlan *pf;
   StepResult *h_results;   // pinned
   StepState *h_state;      // pinned mirror
   int prefilled, dead;
@@ -127,6 +129,19 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
   Q.samp_idx = cv.take<int32_t>(kSampCap);
   Q.pre_val = cv.take<float>(2 * kSampCap);
   Q.pre_idx = cv.take<int32_t>(2 * kSampCap);
+  if (prefill_supported(D)) {
+    size_t mc = (size_t)prefill_chunk_tokens(D);
+    size_t ymax = qd + 2 * kd > 2 * (size_t)D.F ? qd + 2 * kd : 2 * (size_t)D.F;
+    if ((size_t)D.d > ymax) ymax = D.d;
+    size_t xmax = (size_t)D.d > qd ? D.d : qd;
+    if ((size_t)D.F > xmax) xmax = D.F;
+    Q.pf_chunk = (int32_t)mc;
+    Q.pf_H = cv.take<float>(mc * D.d);
+    Q.pf_Q = cv.take<float>(mc * qd);
+    Q.pf_Y = cv.take<float>(mc * ymax);
+    Q.pf_plane = mc * xmax;
+    Q.pf_x3 = cv.take<uint16_t>(3 * mc * xmax);
+  }
   const uint16_t **tabs[9];
   for (int i = 0; i < 9; ++i) tabs[i] = cv.take<const uint16_t *>(D.L);
   Q.attn_norm = tabs[0]; Q.wq = tabs[1]; Q.wk = tabs[2]; Q.wv = tabs[3]; Q.wo = tabs[4];
@@ -166,6 +181,11 @@ __global__ void k_state_init(DevPtrs P, int mode, int pf_n) {
   for (int l = threadIdx.x; l < P.dim.L; l += blockDim.x) P.len[l] = 0;
 }
 __global__ void k_set_mode(DevPtrs P, int mode) { P.st->mode = mode; }
+// After the batched prefill: every layer holds n rows, the committed length is n, nothing is in flight.
+__global__ void k_prefill_done(DevPtrs P, int n) {
+  if (threadIdx.x == 0) { P.st->c = n; P.st->pf_next = n; }
+  for (int l = threadIdx.x; l < P.dim.L; l += blockDim.x) P.len[l] = n;
+}
 __global__ void k_set_forced(DevPtrs P, int on, int n_truth, unsigned long long thresh, unsigned long long seed) {
   P.st->forced_on = on; P.st->n_truth = n_truth; P.st->forced_thresh = thresh; P.st->forced_seed = seed;
 }
@@ -240,6 +260,8 @@ extern "C" int spd_create(const spd_config *cfg, const spd_weights *w, const spd
   ctx->engine = 0;
   int mrc = mega_create(P, src, bufs->repack, need.repack_bytes, ctx->sm, &ctx->mega);
   if (mrc == 0) { ctx->has_mega = 1; ctx->engine = 1; }
+  ctx->pf = (PrefillPlan *)calloc(1, sizeof(PrefillPlan));
+  ctx->prefill_mode = (ctx->pf && prefill_create(P, src, ctx->pf) == 0) ? 1 : 0;
   CUC(cudaStreamSynchronize(ctx->sm));
   CUC(cudaGetLastError());
 #undef CUC
@@ -257,6 +279,7 @@ extern "C" int spd_destroy(spd_ctx *ctx) {
   cudaEventDestroy(ctx->ev_join);
   cudaFreeHost(ctx->h_results);
   cudaFreeHost(ctx->h_state);
+  free(ctx->pf);
   free(ctx);
   return SPD_OK;
 }
@@ -313,16 +336,29 @@ extern "C" int spd_prefill(spd_ctx *ctx, const int32_t *tokens, int32_t n_tokens
   CU(cudaSetDevice(ctx->cfg.device));
   ctx->prefilled = 0;
   CU(cudaMemcpyAsync(ctx->P.pf_tokens, tokens, sizeof(int32_t) * n_tokens, cudaMemcpyHostToDevice, ctx->sm));
-  k_state_init<<<1, 256, 0, ctx->sm>>>(ctx->P, MODE_PREFILL, n_tokens);
-  ++ctx->launches;
-  // cycle 0 only enters token 0; cycles 1..P-1 forward and enter; n more drain the pipeline
-  int total = n_tokens + ctx->cfg.n_stages;
-  for (int i = 0; i < total; ++i) {
-    int rc = enqueue_cycle(ctx);
-    if (rc) return rc;
+  if (ctx->prefill_mode == 1) {
+    // batched prefill: per-layer tcgen05 GEMMs + causal attention over chunks of the prompt (spd_prefill.cu); the
+    // state is then what the pipelined prefill leaves before its final cycle: c = len[l] = P, nothing in flight
+    k_state_init<<<1, 256, 0, ctx->sm>>>(ctx->P, MODE_PREFILL_FINAL, n_tokens);
+    ++ctx->launches;
+    if (prefill_run(ctx->P, *ctx->pf, n_tokens, ctx->sm, &ctx->launches)) {
+      ctx->dead = 1;
+      return fail(ctx, SPD_ECUDA, "batched prefill launch failed%s");
+    }
+    k_prefill_done<<<1, 256, 0, ctx->sm>>>(ctx->P, n_tokens);
+    ++ctx->launches;
+  } else {
+    k_state_init<<<1, 256, 0, ctx->sm>>>(ctx->P, MODE_PREFILL, n_tokens);
+    ++ctx->launches;
+    // cycle 0 only enters token 0; cycles 1..P-1 forward and enter; n more drain the pipeline
+    int total = n_tokens + ctx->cfg.n_stages;
+    for (int i = 0; i < total; ++i) {
+      int rc = enqueue_cycle(ctx);
+      if (rc) return rc;
+    }
+    k_set_mode<<<1, 1, 0, ctx->sm>>>(ctx->P, MODE_PREFILL_FINAL);
+    ++ctx->launches;
   }
-  k_set_mode<<<1, 1, 0, ctx->sm>>>(ctx->P, MODE_PREFILL_FINAL);
-  ++ctx->launches;
   int rc = enqueue_cycle(ctx);
   if (rc) return rc;
   CU(cudaMemcpyAsync(ctx->h_results, ctx->P.results, sizeof(StepResult), cudaMemcpyDeviceToHost, ctx->sm));
@@ -430,6 +466,10 @@ extern "C" int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value) {
     if (value == 0 || (value == 1 && ctx->has_mega)) { ctx->engine = value; return SPD_OK; }
     return fail(ctx, SPD_EINVAL, "engine not available%s");
   }
+  if (option == SPD_OPT_PREFILL) {
+    if (value == 0 || (value == 1 && ctx->pf && ctx->pf->available)) { ctx->prefill_mode = value; return SPD_OK; }
+    return fail(ctx, SPD_EINVAL, "batched prefill not available for this configuration%s");
+  }
   if (option == SPD_OPT_DEBUG_LOGITS || option == SPD_OPT_PHASE_PROFILE) {
     int v = value ? 1 : 0;
     int32_t *field = option == SPD_OPT_DEBUG_LOGITS ? &ctx->P.debug_logits : &ctx->P.prof_on;
@@ -514,4 +554,14 @@ extern "C" int spd_debug_read(spd_ctx *ctx, int32_t what, int32_t index, void *h
   if (bytes != want) return fail(ctx, SPD_EINVAL, "debug_read: size mismatch%s");
   CU(cudaMemcpy(host_out, src, want, cudaMemcpyDeviceToHost));
   return SPD_OK;
+}
+
+// ------------------------------------------------------------------ the prefill GEMM as one operation ----------
+extern "C" size_t spd_op_gemm_scratch(int32_t m, int32_t k) { return (size_t)3 * (m > 0 ? m : 0) * (k > 0 ? k : 0) * sizeof(uint16_t); }
+extern "C" int spd_op_gemm(const float *x, const uint16_t *w, int32_t m, int32_t n, int32_t k, float *y, void *scratch,
+                           void *stream) {
+  if (!x || !w || !y || !scratch || m < 1 || n < 1 || k < 64 || k % 64 || n % 4) return SPD_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return SPD_ECUDA;
+  return prefill_op_gemm(x, w, m, n, k, y, scratch, (cudaStream_t)stream) == 0 ? SPD_OK : SPD_ECUDA;
 }

@@ -124,6 +124,13 @@ struct DevPtrs {
   int32_t *samp_idx;                 // [kSampCap]
   float *pre_val;                    // [2][kSampCap] logits >= tau_guess listed by the fused head pass
   int32_t *pre_idx;                  // [2][kSampCap]
+  // batched prefill scratch (spd_prefill.cu), sized for pf_chunk tokens
+  float *pf_H;                       // [pf_chunk][d] residual streams of the chunk
+  float *pf_Q;                       // [pf_chunk][Hq*hd] q after RoPE
+  float *pf_Y;                       // [pf_chunk][max(Hq*hd + 2 Hkv*hd, 2 F, d)] GEMM output
+  uint16_t *pf_x3;                   // [3][pf_chunk * max(d, Hq*hd, F)] bf16 hi / mid / lo parts of the GEMM input
+  size_t pf_plane;                   // elements per part
+  int32_t pf_chunk;
   int32_t nsplit_max;
   unsigned long long *prof;          // [kProfCtas][kProfPhases][kProfStamps] clock stamps (fused engine)
   int32_t prof_on;

@@ -24,4 +24,19 @@ int mega_create(const DevPtrs &P, const uint16_t *const *const *src, void *repac
                 cudaStream_t stream, MegaPlan *plan);
 int mega_enqueue_step(const DevPtrs &P, const MegaPlan &plan, cudaStream_t sm, long long *launches);
 
+
+// Batched tensor-core prefill (spd_prefill.cu).
+constexpr int kPrefillChunk = 1024;      // prompt tokens per pass over the layers (scratch is sized for it)
+constexpr int kPrefillMaxLayers = 128;
+struct PrefillPlan {
+  int available;
+  const uint16_t *w[9][kPrefillMaxLayers];   // host copy of the per-layer device pointers, spd_weights order
+};
+bool prefill_supported(const Dims &D);
+int prefill_chunk_tokens(const Dims &D);
+int prefill_create(const DevPtrs &P, const uint16_t *const *const *src, PrefillPlan *plan);
+// Positions [0, n_tokens) of P.pf_tokens through all layers: K/V rows appended, Hfin written.  Returns 0 on success.
+int prefill_run(const DevPtrs &P, const PrefillPlan &plan, int n_tokens, cudaStream_t st, long long *launches);
+int prefill_op_gemm(const float *x, const uint16_t *w, int M, int N, int K, float *y, void *scratch, cudaStream_t st);
+
 }  // namespace spd

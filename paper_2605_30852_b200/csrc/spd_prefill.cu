@@ -1,0 +1,618 @@
+// spd_prefill.cu — batched prefill: the step BEFORE the path.
+//
+// PAPER.md:158 excludes prefill from the timed region; the decode kernel can run a prompt (one token enters per
+// cycle), but that streams every layer's weights once per prompt token.  Prefill is the one genuine contraction of the
+// scope — M = prompt tokens — so here it runs layer by layer over a chunk of the prompt as GEMMs on the 5th-generation
+// tensor cores: tcgen05.mma (one elected thread issues), operands staged in shared memory by TMA
+// (cp.async.bulk.tensor, 128-byte swizzle), accumulators in TMEM, read back with tcgen05.ld for the epilogue.
+//
+// Numeric contract (C-2.17): weights bf16, activations fp32.  An fp32 activation x is represented EXACTLY as three bf16
+// parts, x = hi + mid + lo (hi = RNE(x), mid = RNE(x - hi), lo = x - hi - mid: 3 x 8 = 24 mantissa bits); all three
+// multiply the exact bf16 weights into the SAME fp32 accumulator (three MMAs per k step), so every product is exact and
+// the only difference from the decode path's GEMV is the order / rounding of the fp32 accumulation.  (Two parts — 16
+// mantissa bits, 2^-17 per term — were measured first: K/V rounding flips and hidden-state error 10-15x those of the
+// GEMV path on the small test models; with three parts they are the same.)  K/V rows are rounded to bf16 (RNE) when
+// appended.
+//
+// Per layer and chunk of <= kChunk tokens (positions p0 .. p0 + M - 1):
+//   k_pf_norm_split   X = RMSNorm(H; g) -> (hi, mid, lo)                       [M, d]
+//   k_pf_gemm         Y = X . [Wq; Wk; Wv]^T                               [M, qd + 2 kd]      tcgen05
+//   k_pf_rope_append  q -> RoPE -> Q fp32; k -> RoPE -> bf16 cache row; v -> bf16 cache row
+//   k_pf_attention    causal GQA attention of the chunk over cache rows 0 .. pos -> (hi, mid, lo) [M, qd]
+//   k_pf_gemm         Y = att . Wo^T;  k_pf_residual  H += Y
+//   k_pf_norm_split   X = RMSNorm(H; g2);  k_pf_gemm  Y = X . [Wg; Wu]^T;  k_pf_silu_split  act = silu(g) * u -> (hi, mid, lo)
+//   k_pf_gemm         Y = act . Wd^T;  k_pf_residual  H += Y
+// then Hfin[p0 + t] = H[t]; the first token comes from the decode kernel's MODE_PREFILL_FINAL cycle (one pass over E).
+#include <cuda.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "spd_engine.h"
+#include "spd_kernels.cuh"
+
+namespace spd {
+
+constexpr int kGemmBM = 128;              // tokens per tile (TMEM lanes)
+constexpr int kGemmBN = 256;              // output features per tile (TMEM fp32 columns)
+constexpr int kGemmBK = 64;               // bf16 elements per k block = one 128-byte swizzle row
+constexpr int kGemmStages = 2;
+constexpr int kGemmThreads = 192;         // warp 0: TMA producer, warp 1: MMA issuer + TMEM owner, warps 2..5: epilogue
+constexpr int kGemmStageBytes = (3 * kGemmBM + kGemmBN) * kGemmBK * 2;   // A hi + A mid + A lo + B = 80 KB
+constexpr int kGemmSmem = kGemmStages * kGemmStageBytes + 1024 /*alignment*/ + 256 /*barriers*/;
+
+// ------------------------------------------------------------------ PTX wrappers ------------------------------
+__device__ __forceinline__ uint32_t pf_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void pf_mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(pf_smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void pf_mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(pf_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void pf_mbar_wait(uint64_t *bar, uint32_t parity) {
+  uint32_t ok = 0;
+  while (!ok) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(pf_smem_u32(bar)), "r"(parity) : "memory");
+  }
+}
+__device__ __forceinline__ void pf_tma_load_2d(void *dst, const CUtensorMap *tmap, int c0, int c1, uint64_t *bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+      ::"r"(pf_smem_u32(dst)), "l"(tmap), "r"(c0), "r"(c1), "r"(pf_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// D[tmem] (+)= A[smem desc] . B[smem desc]^T, bf16 x bf16 -> fp32, issued by ONE thread for the CTA
+__device__ __forceinline__ void tc_mma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// mbarrier arrive when every tcgen05 operation issued so far by this thread has completed
+__device__ __forceinline__ void tc_commit(uint64_t *bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(pf_smem_u32(bar)) : "memory");
+}
+// 32 lanes x 32 consecutive fp32 columns of TMEM -> 32 registers per thread (thread = lane)
+__device__ __forceinline__ void tc_ld_32x32(uint32_t taddr, float (&v)[32]) {
+  uint32_t r[32];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// Shared-memory matrix descriptor of a K-major tile whose rows are 128 bytes (64 bf16), 128-byte swizzled as TMA
+// wrote them: start address (>> 4), stride between 8-row groups = 1024 bytes (>> 4), descriptor version 1 (sm_100),
+// layout type 2 = SWIZZLE_128B.  The leading-dimension offset is unused for swizzled K-major operands.
+__device__ __forceinline__ uint64_t tc_smem_desc(uint32_t smem_addr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr & 0x3ffffu) >> 4);            // bits [0, 14)
+  d |= (uint64_t)1 << 16;                                  // leading byte offset (ignored), bits [16, 30)
+  d |= (uint64_t)(1024 >> 4) << 32;                        // stride byte offset, bits [32, 46)
+  d |= (uint64_t)1 << 46;                                  // version, bits [46, 48)
+  d |= (uint64_t)2 << 61;                                  // layout type, bits [61, 64)
+  return d;
+}
+// Instruction descriptor of kind::f16: D fp32, A and B bf16, both K-major, M x N tile.
+__host__ __device__ constexpr uint32_t tc_idesc_bf16(int M, int N) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+// ------------------------------------------------------------------ the GEMM ----------------------------------
+// Y[m, col0 + n] = sum_k (Xhi[m, k] + Xlo[m, k]) * W_seg[n, k] for up to three weight matrices (segments) that share X:
+// blockIdx.x runs over the 256-row tiles of the segments back to back, blockIdx.y over 128-token tiles.
+struct GemmArgs {
+  CUtensorMap a_hi, a_mid, a_lo;   // [rows >= M, K] bf16, box {64, 128}
+  CUtensorMap b[3];                // [N_seg, K] bf16, box {64, 256}
+  int seg_tiles[3];                // 256-row tiles of each segment (0: unused)
+  int seg_n[3];                    // rows of each segment
+  int seg_col0[3];                 // first output column of each segment
+  int M, K, ldy;
+  float *y;                        // [M, ldy] fp32
+};
+
+__global__ void __launch_bounds__(kGemmThreads, 1) k_pf_gemm(const __grid_constant__ GemmArgs A) {
+  extern __shared__ uint8_t pf_smem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>(((uintptr_t)pf_smem_raw + 1023) & ~(uintptr_t)1023);   // swizzle atoms: 1024-byte aligned
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + kGemmStages * kGemmStageBytes);
+  uint64_t *empty = full + kGemmStages;
+  uint64_t *tmem_full = empty + kGemmStages;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_full + 1);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int seg = 0, tile = blockIdx.x;
+  while (seg < 2 && tile >= A.seg_tiles[seg]) { tile -= A.seg_tiles[seg]; ++seg; }
+  const int n0 = tile * kGemmBN, m0 = blockIdx.y * kGemmBM;
+  const int nkb = A.K / kGemmBK;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kGemmStages; ++s) { pf_mbar_init(&full[s], 1); pf_mbar_init(&empty[s], 1); }
+    pf_mbar_init(tmem_full, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {   // TMEM: 256 fp32 columns x 128 lanes for the accumulator tile
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(pf_smem_u32(tmem_slot)), "r"((uint32_t)kGemmBN) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_d = *tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {   // ===== TMA producer =====
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % kGemmStages, it = kb / kGemmStages;
+        pf_mbar_wait(&empty[s], (it & 1) ^ 1);
+        uint8_t *st = smem + (size_t)s * kGemmStageBytes;
+        pf_mbar_expect_tx(&full[s], kGemmStageBytes);
+        pf_tma_load_2d(st, &A.a_hi, kb * kGemmBK, m0, &full[s]);
+        pf_tma_load_2d(st + kGemmBM * 128, &A.a_mid, kb * kGemmBK, m0, &full[s]);
+        pf_tma_load_2d(st + 2 * kGemmBM * 128, &A.a_lo, kb * kGemmBK, m0, &full[s]);
+        pf_tma_load_2d(st + 3 * kGemmBM * 128, &A.b[seg], kb * kGemmBK, n0, &full[s]);
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {   // ===== MMA issuer =====
+      constexpr uint32_t idesc = tc_idesc_bf16(kGemmBM, kGemmBN);
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % kGemmStages, it = kb / kGemmStages;
+        pf_mbar_wait(&full[s], it & 1);
+        tc_fence_after();
+        const uint32_t a_hi = pf_smem_u32(smem + (size_t)s * kGemmStageBytes);
+        const uint32_t a_mid = a_hi + kGemmBM * 128, a_lo = a_hi + 2 * kGemmBM * 128, b = a_hi + 3 * kGemmBM * 128;
+#pragma unroll
+        for (int k = 0; k < kGemmBK / 16; ++k) {      // UMMA_K = 16 bf16 = 32 bytes inside the 128-byte swizzle row
+          const uint64_t bd = tc_smem_desc(b + k * 32);
+          tc_mma_bf16(tmem_d, tc_smem_desc(a_hi + k * 32), bd, idesc, (kb | k) ? 1u : 0u);
+          tc_mma_bf16(tmem_d, tc_smem_desc(a_mid + k * 32), bd, idesc, 1u);
+          tc_mma_bf16(tmem_d, tc_smem_desc(a_lo + k * 32), bd, idesc, 1u);
+        }
+        tc_commit(&empty[s]);                         // the slot is free once these MMAs have read it
+      }
+      tc_commit(tmem_full);                           // the accumulator tile is complete
+    }
+  } else {             // ===== epilogue: TMEM -> registers -> Y (a warp owns the 32 TMEM lanes 32 * (warp % 4) ..) =====
+    pf_mbar_wait(tmem_full, 0);
+    tc_fence_after();
+    const int lg = warp & 3;
+    const int m = m0 + lg * 32 + lane;
+    const int nseg = A.seg_n[seg];
+    float *yrow = A.y + (size_t)m * A.ldy + A.seg_col0[seg] + n0;
+    for (int c = 0; c < kGemmBN; c += 32) {
+      if (n0 + c >= nseg) break;                      // uniform over the warp
+      float v[32];
+      tc_ld_32x32(tmem_d + ((uint32_t)(lg * 32) << 16) + (uint32_t)c, v);
+      if (m < A.M) {
+        if (n0 + c + 32 <= nseg) {
+#pragma unroll
+          for (int i = 0; i < 32; i += 4) *reinterpret_cast<float4 *>(yrow + c + i) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+        } else {
+          for (int i = 0; i < 32; ++i) if (n0 + c + i < nseg) yrow[c + i] = v[i];
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)kGemmBN) : "memory");
+  }
+}
+
+// ------------------------------------------------------------------ elementwise kernels ------------------------
+// x = hi + mid + lo exactly (finite x; each residual is exact in fp32 and the last one fits 8 mantissa bits)
+struct Split3 { uint16_t hi, mid, lo; };
+__device__ __forceinline__ Split3 pf_split(float x) {
+  Split3 s;
+  s.hi = f32_to_bf16(x);
+  const float r1 = x - bf16_to_f32(s.hi);
+  s.mid = f32_to_bf16(r1);
+  s.lo = f32_to_bf16(r1 - bf16_to_f32(s.mid));
+  return s;
+}
+
+// H[t] = E[tok[p0 + t]] (token entry, a0)
+__global__ void k_pf_embed(const uint16_t *embed, const int32_t *tokens, int p0, int d, float *H) {
+  const int t = blockIdx.x;
+  const uint16_t *e = embed + (size_t)tokens[p0 + t] * d;
+  for (int i = threadIdx.x; i < d; i += blockDim.x) H[(size_t)t * d + i] = bf16_to_f32(e[i]);
+}
+
+// X = RMSNorm(H[t]; gain) -> bf16 hi / mid / lo rows (a1.1 / a1.6).  One CTA per token; the sum of squares uses the
+// decode path's block_rms_scale tree.
+__global__ void k_pf_norm_split(const float *H, const uint16_t *gain, int d, float eps, uint16_t *x3, size_t plane) {
+  __shared__ float red[33];
+  const int t = blockIdx.x;
+  const float *h = H + (size_t)t * d;
+  const float r = block_rms_scale(h, d, eps, red);
+  for (int i = threadIdx.x; i < d; i += blockDim.x) {
+    const Split3 sp = pf_split(h[i] * r * bf16_to_f32(gain[i]));
+    const size_t o = (size_t)t * d + i;
+    x3[o] = sp.hi; x3[plane + o] = sp.mid; x3[2 * plane + o] = sp.lo;
+  }
+}
+
+// Y row = [q (qd) | k (kd) | v (kd)]: RoPE (C-2.14, angles in double) on q and k; q -> Q fp32; k, v -> bf16 cache rows
+// at position p0 + t (a1.3).  One CTA per token.
+__global__ void k_pf_rope_append(const float *Y, int ldy, DevPtrs P, int layer, int p0, float *Q) {
+  const Dims &D = P.dim;
+  __shared__ float2 cs[64];
+  const int t = blockIdx.x, pos = p0 + t, half = D.hd / 2, qd = D.Hq * D.hd, kd = D.Hkv * D.hd;
+  if (threadIdx.x < half) {
+    double s_, c_;
+    sincos((double)pos * P.inv_freq[threadIdx.x], &s_, &c_);
+    cs[threadIdx.x] = make_float2((float)c_, (float)s_);
+  }
+  __syncthreads();
+  const float *y = Y + (size_t)t * ldy;
+  for (int j = threadIdx.x; j < (D.Hq + D.Hkv) * half; j += blockDim.x) {
+    const int hh = j / half, i = j - hh * half;
+    const float2 c = cs[i];
+    if (hh < D.Hq) {
+      const float a = y[hh * D.hd + i], b = y[hh * D.hd + i + half];
+      float *q = Q + (size_t)t * qd + hh * D.hd;
+      q[i] = a * c.x - b * c.y;
+      q[i + half] = b * c.x + a * c.y;
+    } else {
+      const int kh = hh - D.Hq;
+      const float a = y[qd + kh * D.hd + i], b = y[qd + kh * D.hd + i + half];
+      uint16_t *dst = P.kv + kv_offset(D, layer, 0, kh) + (size_t)pos * D.hd;
+      dst[i] = f32_to_bf16(a * c.x - b * c.y);
+      dst[i + half] = f32_to_bf16(b * c.x + a * c.y);
+    }
+  }
+  for (int j = threadIdx.x; j < kd; j += blockDim.x) {
+    const int kh = j / D.hd, i = j - kh * D.hd;
+    P.kv[kv_offset(D, layer, 1, kh) + (size_t)pos * D.hd + i] = f32_to_bf16(y[qd + kd + j]);
+  }
+}
+
+// H += Y (residual, a1.5 / a1.8)
+__global__ void k_pf_residual(float *H, const float *Y, int ldy, int d, int M) {
+  const size_t n = (size_t)M * d;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t t = i / d, c = i - t * d;
+    H[i] += Y[t * ldy + c];
+  }
+}
+
+// act = silu(gate) * up -> bf16 hi / mid / lo (a1.7); Y row = [gate (F) | up (F)]
+__global__ void k_pf_silu_split(const float *Y, int ldy, int F, int M, uint16_t *x3, size_t plane) {
+  const size_t n = (size_t)M * F;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t t = i / F, c = i - t * F;
+    const Split3 sp = pf_split(silu_mul(Y[t * ldy + c], Y[t * ldy + F + c]));
+    x3[i] = sp.hi; x3[plane + i] = sp.mid; x3[2 * plane + i] = sp.lo;
+  }
+}
+
+// Hfin[p0 + t] = H[t]
+__global__ void k_pf_store_hfin(const float *H, float *hfin, int p0, int d, int M) {
+  const size_t n = (size_t)M * d;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    hfin[(size_t)p0 * d + i] = H[i];
+}
+
+// fp32 matrix -> bf16 hi / mid / lo (spd_op_gemm's input split)
+__global__ void k_pf_split(const float *x, size_t n, uint16_t *x3, size_t plane) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const Split3 sp = pf_split(x[i]);
+    x3[i] = sp.hi; x3[plane + i] = sp.mid; x3[2 * plane + i] = sp.lo;
+  }
+}
+
+// ------------------------------------------------------------------ causal prefill attention (a1.4) ------------
+// One CTA = one kv head x a block of TQ = 64 / G chunk tokens: R = 64 query rows (token-major, row = tq * G + g), all
+// of them reading the same K/V rows.  Cache rows 0 .. pos (causal incl. self) are visited in tiles of 64 rows, widened
+// to fp32 in shared memory; scores, online softmax (running max / sum per row) and P.V in fp32 on the CUDA cores —
+// 4 flop per K/V byte at M = 1 is the decode path's problem; at prefill the GEMMs dominate.
+// Thread (ty, tx) = (tid / 16, tid % 16) owns score rows 4 ty .. 4 ty + 3 x columns tx, tx + 16, tx + 32, tx + 48 and
+// output rows 4 ty .. 4 ty + 3 x head-dim elements tx * HD/16 ..; every sum runs in a fixed order.
+template <int HD>
+__global__ void __launch_bounds__(256, 1) k_pf_attention(DevPtrs P, int layer, int p0, int M, const float *Q,
+                                                         uint16_t *x3, size_t plane) {
+  constexpr int R = 64, TK = 64, LDK = HD + 4, EPT = HD / 16;
+  const Dims &D = P.dim;
+  const int G = D.Hq / D.Hkv, TQ = R / G, qd = D.Hq * HD;
+  extern __shared__ float pf_att_smem[];
+  float *Qs = pf_att_smem;               // [R][LDK]
+  float *Ks = Qs + R * LDK;              // [TK][LDK]
+  float *Vs = Ks + TK * LDK;             // [TK][LDK]
+  float *Ss = Vs + TK * LDK;             // [R][TK + 1]
+  float *m_s = Ss + R * (TK + 1);        // [R] running max
+  float *l_s = m_s + R;                  // [R] running sum
+  float *c_s = l_s + R;                  // [R] correction of this tile
+  const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+  const int kvh = blockIdx.y, t0 = blockIdx.x * TQ;
+  const float scale = 1.0f / sqrtf((float)HD);
+  for (int i = tid; i < R * (HD / 4); i += 256) {          // Q rows of this block (zero for tokens beyond M)
+    const int r = i / (HD / 4), c4 = i - r * (HD / 4);
+    const int t = t0 + r / G, g = r % G;
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (t < M) v = *reinterpret_cast<const float4 *>(Q + (size_t)t * qd + (size_t)(kvh * G + g) * HD + 4 * c4);
+    *reinterpret_cast<float4 *>(Qs + r * LDK + 4 * c4) = v;
+  }
+  if (tid < R) { m_s[tid] = -INFINITY; l_s[tid] = 0.f; }
+  float acc[4][EPT];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) acc[i][e] = 0.f;
+  const int last_pos = p0 + min(t0 + TQ, M) - 1;            // the newest row any token of the block attends to
+  const uint16_t *kc = P.kv + kv_offset(D, layer, 0, kvh), *vc = P.kv + kv_offset(D, layer, 1, kvh);
+  for (int r0 = 0; r0 <= last_pos; r0 += TK) {
+    __syncthreads();                                         // the previous tile is consumed (and Qs / m / l are written)
+    for (int i = tid; i < TK * (HD / 8); i += 256) {         // 16-byte chunks of K and V rows -> fp32
+      const int r = i / (HD / 8), c8 = i - r * (HD / 8);
+      uint4 kw = make_uint4(0u, 0u, 0u, 0u), vw = kw;
+      if (r0 + r <= last_pos) {
+        kw = *reinterpret_cast<const uint4 *>(kc + (size_t)(r0 + r) * HD + 8 * c8);
+        vw = *reinterpret_cast<const uint4 *>(vc + (size_t)(r0 + r) * HD + 8 * c8);
+      }
+      float *kd = Ks + r * LDK + 8 * c8, *vd = Vs + r * LDK + 8 * c8;
+      *reinterpret_cast<float4 *>(kd) = make_float4(bf16_lo(kw.x), bf16_hi(kw.x), bf16_lo(kw.y), bf16_hi(kw.y));
+      *reinterpret_cast<float4 *>(kd + 4) = make_float4(bf16_lo(kw.z), bf16_hi(kw.z), bf16_lo(kw.w), bf16_hi(kw.w));
+      *reinterpret_cast<float4 *>(vd) = make_float4(bf16_lo(vw.x), bf16_hi(vw.x), bf16_lo(vw.y), bf16_hi(vw.y));
+      *reinterpret_cast<float4 *>(vd + 4) = make_float4(bf16_lo(vw.z), bf16_hi(vw.z), bf16_lo(vw.w), bf16_hi(vw.w));
+    }
+    __syncthreads();
+    // ---- scores of the tile: s[i][j] = q[4 ty + i] . k[tx + 16 j], scaled, causally masked -> Ss ----
+    {
+      float s[4][4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) s[i][j] = 0.f;
+#pragma unroll 4
+      for (int k = 0; k < HD; k += 4) {
+        float4 qv[4], kv4[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) qv[i] = *reinterpret_cast<const float4 *>(Qs + (4 * ty + i) * LDK + k);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) kv4[j] = *reinterpret_cast<const float4 *>(Ks + (tx + 16 * j) * LDK + k);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            s[i][j] = fmaf(qv[i].x, kv4[j].x, s[i][j]); s[i][j] = fmaf(qv[i].y, kv4[j].y, s[i][j]);
+            s[i][j] = fmaf(qv[i].z, kv4[j].z, s[i][j]); s[i][j] = fmaf(qv[i].w, kv4[j].w, s[i][j]);
+          }
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const int r = 4 * ty + i, pos = p0 + t0 + r / G;     // this query row's position
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int c = tx + 16 * j;
+          Ss[r * (TK + 1) + c] = (r0 + c <= pos) ? s[i][j] * scale : -INFINITY;
+        }
+      }
+    }
+    __syncthreads();
+    // ---- online softmax: 4 threads per row, 16 columns each ----
+    {
+      const int r = tid >> 2, part = tid & 3;
+      float *srow = Ss + r * (TK + 1) + 16 * part;
+      float mx = -INFINITY;
+#pragma unroll
+      for (int c = 0; c < 16; ++c) mx = fmaxf(mx, srow[c]);
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
+      const float m_old = m_s[r], m_new = fmaxf(m_old, mx);
+      float sum = 0.f;
+#pragma unroll
+      for (int c = 0; c < 16; ++c) {
+        const float pr = (m_new == -INFINITY) ? 0.f : expf(srow[c] - m_new);   // a fully masked row (token beyond M) stays 0
+        srow[c] = pr;
+        sum += pr;
+      }
+      sum += __shfl_xor_sync(0xffffffffu, sum, 1);
+      sum += __shfl_xor_sync(0xffffffffu, sum, 2);
+      __syncwarp();
+      if (part == 0) {
+        const float corr = (m_old == -INFINITY) ? 0.f : expf(m_old - m_new);
+        c_s[r] = corr;
+        l_s[r] = fmaf(l_s[r], corr, sum);
+        m_s[r] = m_new;
+      }
+    }
+    __syncthreads();
+    // ---- O = O * corr + P . V ----
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float corr = c_s[4 * ty + i];
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) acc[i][e] *= corr;
+    }
+#pragma unroll 4
+    for (int c = 0; c < TK; ++c) {
+      float vv[EPT];
+#pragma unroll
+      for (int e = 0; e < EPT; e += 4) {
+        const float4 t4 = *reinterpret_cast<const float4 *>(Vs + c * LDK + tx * EPT + e);
+        vv[e] = t4.x; vv[e + 1] = t4.y; vv[e + 2] = t4.z; vv[e + 3] = t4.w;
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float pr = Ss[(4 * ty + i) * (TK + 1) + c];
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) acc[i][e] = fmaf(pr, vv[e], acc[i][e]);
+      }
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int r = 4 * ty + i, t = t0 + r / G, g = r % G;
+    if (t >= M) continue;
+    const float l = l_s[r];
+    const size_t o = (size_t)t * qd + (size_t)(kvh * G + g) * HD + tx * EPT;
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+      const Split3 sp = pf_split(acc[i][e] / l);
+      x3[o + e] = sp.hi; x3[plane + o + e] = sp.mid; x3[2 * plane + o + e] = sp.lo;
+    }
+  }
+}
+
+// ------------------------------------------------------------------ host side ----------------------------------
+typedef CUresult (*PfEncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                               const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static PfEncodeFn pf_encoder() {
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  return (PfEncodeFn)fn;
+}
+
+// bf16 matrix [rows, K] row-major -> tensor map with boxes of 64 columns (128 bytes, swizzled) x box_rows rows
+static int pf_make_map(PfEncodeFn enc, CUtensorMap *tm, const void *base, int rows, int K, int box_rows) {
+  cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+  cuuint64_t gstr[1] = {(cuuint64_t)K * 2};
+  cuuint32_t box[2] = {(cuuint32_t)kGemmBK, (cuuint32_t)box_rows}, estr[2] = {1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), gdim, gstr, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? 0 : -1;
+}
+
+static int pf_launch_gemm(PfEncodeFn enc, const uint16_t *x3, size_t plane, int x_rows, int M, int K,
+                          const uint16_t *const *w, const int *w_rows, int nseg, float *y, int ldy, cudaStream_t st,
+                          long long *launches) {
+  GemmArgs A;
+  memset(&A, 0, sizeof A);
+  if (pf_make_map(enc, &A.a_hi, x3, x_rows, K, kGemmBM) || pf_make_map(enc, &A.a_mid, x3 + plane, x_rows, K, kGemmBM) ||
+      pf_make_map(enc, &A.a_lo, x3 + 2 * plane, x_rows, K, kGemmBM))
+    return -1;
+  int tiles = 0, col = 0;
+  for (int s = 0; s < nseg; ++s) {
+    if (pf_make_map(enc, &A.b[s], w[s], w_rows[s], K, kGemmBN)) return -1;
+    A.seg_tiles[s] = (w_rows[s] + kGemmBN - 1) / kGemmBN;
+    A.seg_n[s] = w_rows[s];
+    A.seg_col0[s] = col;
+    col += w_rows[s];
+    tiles += A.seg_tiles[s];
+  }
+  A.M = M; A.K = K; A.ldy = ldy; A.y = y;
+  dim3 grid(tiles, (M + kGemmBM - 1) / kGemmBM);
+  k_pf_gemm<<<grid, kGemmThreads, kGemmSmem, st>>>(A);
+  if (launches) *launches += 1;
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+bool prefill_supported(const Dims &D) {
+  const int qd = D.Hq * D.hd;
+  const int G = D.Hq / D.Hkv;
+  return D.d % kGemmBK == 0 && qd % kGemmBK == 0 && D.F % kGemmBK == 0 && (D.hd == 64 || D.hd == 128) &&
+         (G == 1 || G == 2 || G == 4 || G == 8) && D.d % 8 == 0;
+}
+
+int prefill_chunk_tokens(const Dims &D) {
+  int c = ((D.max_seq + kGemmBM - 1) / kGemmBM) * kGemmBM;
+  return c < kPrefillChunk ? c : kPrefillChunk;
+}
+
+int prefill_create(const DevPtrs &P, const uint16_t *const *const *src, PrefillPlan *plan) {
+  memset(plan, 0, sizeof *plan);
+  const Dims &D = P.dim;
+  if (!prefill_supported(D) || !P.pf_H || D.L > kPrefillMaxLayers) return -1;
+  PfEncodeFn enc = pf_encoder();
+  if (!enc) return -1;
+  static bool attr_done = false;
+  if (!attr_done) {
+    if (cudaFuncSetAttribute(k_pf_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem) != cudaSuccess ||
+        cudaFuncSetAttribute(k_pf_attention<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(k_pf_attention<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024) != cudaSuccess) {
+      cudaGetLastError();
+      return -1;
+    }
+    attr_done = true;
+  }
+  for (int i = 0; i < 9; ++i)
+    for (int l = 0; l < D.L; ++l) plan->w[i][l] = src[i][l];
+  plan->available = 1;
+  return 0;
+}
+
+// Runs positions [0, n_tokens) through all layers (KV rows appended, Hfin written).  Tokens are in P.pf_tokens.
+int prefill_run(const DevPtrs &P, const PrefillPlan &plan, int n_tokens, cudaStream_t st, long long *launches) {
+  if (!plan.available) return -1;
+  PfEncodeFn enc = pf_encoder();
+  if (!enc) return -1;
+  const Dims &D = P.dim;
+  const int qd = D.Hq * D.hd, kd = D.Hkv * D.hd, Mc = P.pf_chunk;
+  const int G = D.Hq / D.Hkv, TQ = 64 / G;
+  const size_t att_smem = (size_t)(3 * 64 * (D.hd + 4) + 64 * 65 + 3 * 64) * sizeof(float);
+  long long cnt = 0;
+  for (int p0 = 0; p0 < n_tokens; p0 += Mc) {
+    const int M = n_tokens - p0 < Mc ? n_tokens - p0 : Mc;
+    const int eb = (int)(((size_t)M * D.F + 255) / 256 < 4096 ? ((size_t)M * D.F + 255) / 256 : 4096);
+    k_pf_embed<<<M, 256, 0, st>>>(P.embed, P.pf_tokens, p0, D.d, P.pf_H);
+    ++cnt;
+    for (int l = 0; l < D.L; ++l) {
+      // spd_weights order: 0 attn_norm 1 wq 2 wk 3 wv 4 wo 5 mlp_norm 6 w_gate 7 w_up 8 w_down
+      k_pf_norm_split<<<M, 256, 0, st>>>(P.pf_H, plan.w[0][l], D.d, D.eps, P.pf_x3, P.pf_plane);
+      const uint16_t *wqkv[3] = {plan.w[1][l], plan.w[2][l], plan.w[3][l]};
+      const int nqkv[3] = {qd, kd, kd};
+      if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, D.d, wqkv, nqkv, 3, P.pf_Y, qd + 2 * kd, st, &cnt)) return -1;
+      k_pf_rope_append<<<M, 256, 0, st>>>(P.pf_Y, qd + 2 * kd, P, l, p0, P.pf_Q);
+      dim3 ag((M + TQ - 1) / TQ, D.Hkv);
+      if (D.hd == 128) k_pf_attention<128><<<ag, 256, att_smem, st>>>(P, l, p0, M, P.pf_Q, P.pf_x3, P.pf_plane);
+      else k_pf_attention<64><<<ag, 256, att_smem, st>>>(P, l, p0, M, P.pf_Q, P.pf_x3, P.pf_plane);
+      const uint16_t *wo[1] = {plan.w[4][l]};
+      const int no[1] = {D.d};
+      if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, qd, wo, no, 1, P.pf_Y, D.d, st, &cnt)) return -1;
+      k_pf_residual<<<eb, 256, 0, st>>>(P.pf_H, P.pf_Y, D.d, D.d, M);
+      k_pf_norm_split<<<M, 256, 0, st>>>(P.pf_H, plan.w[5][l], D.d, D.eps, P.pf_x3, P.pf_plane);
+      const uint16_t *wgu[2] = {plan.w[6][l], plan.w[7][l]};
+      const int ngu[2] = {D.F, D.F};
+      if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, D.d, wgu, ngu, 2, P.pf_Y, 2 * D.F, st, &cnt)) return -1;
+      k_pf_silu_split<<<eb, 256, 0, st>>>(P.pf_Y, 2 * D.F, D.F, M, P.pf_x3, P.pf_plane);
+      const uint16_t *wd[1] = {plan.w[8][l]};
+      if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, D.F, wd, no, 1, P.pf_Y, D.d, st, &cnt)) return -1;
+      k_pf_residual<<<eb, 256, 0, st>>>(P.pf_H, P.pf_Y, D.d, D.d, M);
+      cnt += 7;
+    }
+    k_pf_store_hfin<<<eb, 256, 0, st>>>(P.pf_H, P.hfin, p0, D.d, M);
+    ++cnt;
+  }
+  if (launches) *launches += cnt;
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+// spd_op_gemm: Y[M, N] = X[M, K] . W[N, K]^T with the prefill GEMM (X fp32 -> bf16 hi + mid + lo, exact).  scratch: 3 * M * K bf16.
+int prefill_op_gemm(const float *x, const uint16_t *w, int M, int N, int K, float *y, void *scratch, cudaStream_t st) {
+  if (K % kGemmBK || M < 1 || N < 1 || N % 4) return -1;
+  PfEncodeFn enc = pf_encoder();
+  if (!enc) return -1;
+  if (cudaFuncSetAttribute(k_pf_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem) != cudaSuccess) return -1;
+  uint16_t *x3 = (uint16_t *)scratch;
+  const size_t plane = (size_t)M * K;
+  k_pf_split<<<1024, 256, 0, st>>>(x, plane, x3, plane);
+  const uint16_t *ws[1] = {w};
+  const int ns[1] = {N};
+  return pf_launch_gemm(enc, x3, plane, M, M, K, ws, ns, 1, y, N, st, nullptr);
+}
+
+}  // namespace spd

@@ -89,7 +89,7 @@ def kv_compare(gpu, ora, layers, rows, rep: Report, tol: float):
 
 
 def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, engine=None, tensor_every=1,
-               tensor_tol=CONTRACT, check_logits=True, prefill_block=16, max_seq=None, gpu=None) -> Report:
+               tensor_tol=CONTRACT, check_logits=True, prefill_block=16, max_seq=None, gpu=None, prefill_mode=None) -> Report:
     """forced = (truth tokens, p, seed) or None (the PDM's own drafts).  tensor_tol bounds hidden states,
     the PDM vector and logits (C-2.18 metric); the tie band is 3 x the measured logit difference (module doc)."""
     from paper_2605_30852_b200 import SPD, OPT
@@ -108,6 +108,8 @@ def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, en
     try:
         if engine is not None:
             gpu.set_option(OPT.ENGINE, engine)
+        if prefill_mode is not None:             # 1: batched tensor-core prefill (the default), 0: through the decode kernel
+            gpu.set_option(OPT.PREFILL, prefill_mode)
         gpu.set_option(OPT.DEBUG_LOGITS, 1)      # the measured logit difference sets the tie band
         fo = ora.prefill(prompt, block=prefill_block)
         fg = gpu.prefill(prompt)

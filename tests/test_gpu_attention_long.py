@@ -54,7 +54,8 @@ def test_fused_attention_at_graded_context_lengths(P, hq, hkv):
     shape = si.ModelShape("mid", 512, 4, 2, hq, hkv, 128, 1024, 2048, P, 16, ())
     w, wd, prompt = _inputs(shape, P)
     G = 16
-    rep = run_parity(shape=shape, weights_np=w, dev_weights=wd, prompt=prompt, n_tokens=G, engine=1, tensor_tol=5e-4)
+    rep = run_parity(shape=shape, weights_np=w, dev_weights=wd, prompt=prompt, n_tokens=G, engine=1, tensor_tol=5e-4,
+                     prefill_mode=0)       # the prompt runs through the decode kernel: its attention is what is under test
     print(f"mid P={P} Hq={hq} Hkv={hkv}:", rep.summary())
     assert rep.status == "ok", rep.detail
     assert_ties(rep)
@@ -62,6 +63,7 @@ def test_fused_attention_at_graded_context_lengths(P, hq, hkv):
     # (a) per kernel, on the kernel's own inputs
     gpu = spd.SPD(shape, wd, max_seq=P + 64)
     gpu.set_option(spd.OPT.ENGINE, 1)
+    gpu.set_option(spd.OPT.PREFILL, 0)
     gpu.prefill(prompt)
     worst = 0.0
     for _ in range(10):
@@ -88,13 +90,14 @@ def test_attention_mid_phase_flush_with_small_cta_groups():
     # peaked; measured 1.2e-3 on hfin[0] with BOTH engines, 6e-5 beyond position 1000), hence 2e-3 here; the per-kernel
     # check below stays at 1e-4
     rep = run_parity(shape=shape, weights_np=w, dev_weights=wd, prompt=prompt, n_tokens=G, forced=(truth, 1.0, 1),
-                     engine=1, tensor_tol=2e-3, tensor_every=4)
+                     engine=1, tensor_tol=2e-3, tensor_every=4, prefill_mode=0)
     print("flush n=32:", rep.summary())
     assert rep.status == "ok", rep.detail
     assert_ties(rep)
     assert rep.rejects == 0 and rep.steps == G + shape.n_stages - 2
     gpu = spd.SPD(shape, wd, max_seq=P + 128)
     gpu.set_option(spd.OPT.ENGINE, 1)
+    gpu.set_option(spd.OPT.PREFILL, 0)
     first = gpu.prefill(prompt)
     assert first == int(truth[0])
     gpu.set_forced(truth, 1.0, 1)

@@ -116,7 +116,7 @@ def test_tensor_core_attention_path_midsize(hq, hkv):
     _need_engine(1)
     shape = si.ModelShape("mid", 512, 4, 2, hq, hkv, 128, 1024, 2048, 300, 24, ())
     inp = _inputs(shape, 300, std=0.04, attention_heavy=True)
-    rep = run_parity(**inp, n_tokens=24, engine=1, tensor_tol=5e-4)
+    rep = run_parity(**inp, n_tokens=24, engine=1, tensor_tol=5e-4, prefill_mode=0)   # the decode kernel's attention, prompt included
     print(f"mid Hq={hq} Hkv={hkv}:", rep.summary())
     assert rep.status == "ok", rep.detail
     assert_ties(rep)
