@@ -41,20 +41,18 @@ def _rope(x: np.ndarray, positions: np.ndarray, base: float) -> np.ndarray:
     return np.concatenate([z.real, z.imag], axis=-1)
 
 
-def forward_nocache(shape, weights, tokens, keep_hidden: bool = False) -> dict:
-    """Full-sequence forward.  Returns {"logits": [T, V] f64, "final": [T, d] pre-norm final hidden,
-    "k": [L][T, Hkv*hd] bf16-rounded f64, "v": same, "hidden": [L+1, T, d] if keep_hidden}."""
-    tokens = np.asarray(tokens, dtype=np.int64)
-    T = len(tokens)
-    d, Hq, Hkv, hd = shape.d_model, shape.n_q_heads, shape.n_kv_heads, shape.head_dim
+def decoder_nocache(shape, weights, h: np.ndarray, n_layers: int, keep_hidden: bool = False) -> dict:
+    """`n_layers` decoder layers over the input rows h [T, d] (row t = position t), whole sequence at once.
+    Returns {"final": [T, d], "k", "v": per layer [T, Hkv*hd] bf16-rounded f64, "hidden": [n_layers+1, T, d]}."""
+    T = h.shape[0]
+    Hq, Hkv, hd = shape.n_q_heads, shape.n_kv_heads, shape.head_dim
     eps, base = float(np.float32(shape.rms_eps)), float(np.float32(shape.rope_base))
-    E = _w(weights["embed"])
-    h = E[tokens]                                           # [T, d]
+    h = np.array(h, dtype=np.float64)
     pos = np.arange(T)
     causal = np.tril(np.ones((T, T), dtype=bool))           # row = query position, col = key position
     hidden = [h.copy()] if keep_hidden else None
     ks, vs = [], []
-    for l in range(shape.n_layers):
+    for l in range(n_layers):
         x = _rmsnorm(h, _w(weights["attn_norm"][l]), eps)
         q = (x @ _w(weights["wq"][l]).T).astype(np.float32).astype(np.float64).reshape(T, Hq, hd)
         k = (x @ _w(weights["wk"][l]).T).astype(np.float32).astype(np.float64).reshape(T, Hkv, hd)
@@ -79,11 +77,46 @@ def forward_nocache(shape, weights, tokens, keep_hidden: bool = False) -> dict:
         h = h + ((g / (1.0 + np.exp(-g))) * u) @ _w(weights["w_down"][l]).T
         if keep_hidden:
             hidden.append(h.copy())
-    logits = _rmsnorm(h, _w(weights["final_norm"]), eps) @ E.T
-    out = {"logits": logits, "final": h, "k": ks, "v": vs}
+    out = {"final": h, "k": ks, "v": vs}
     if keep_hidden:
         out["hidden"] = np.stack(hidden)
     return out
+
+
+def forward_nocache(shape, weights, tokens, keep_hidden: bool = False) -> dict:
+    """Full-sequence forward.  Returns {"logits": [T, V] f64, "final": [T, d] pre-norm final hidden,
+    "k": [L][T, Hkv*hd] bf16-rounded f64, "v": same, "hidden": [L+1, T, d] if keep_hidden}."""
+    tokens = np.asarray(tokens, dtype=np.int64)
+    E = _w(weights["embed"])
+    out = decoder_nocache(shape, weights, E[tokens], shape.n_layers, keep_hidden)
+    out["logits"] = _rmsnorm(out["final"], _w(weights["final_norm"]), float(np.float32(shape.rms_eps))) @ E.T
+    return out
+
+
+def pdm_paper_ref(shape, weights, pdm_weights, tokens, depths) -> dict:
+    """The paper's Pipeline Draft Module, whole prefix at once, float64 (pins oracle/spd_oracle.c's cached version).
+    tokens: the sequence x_1..x_t (verified prefix + in-flight tokens); depths[t] = stages that token has completed
+    when drafting begins (n for the verified prefix; Eq. 2 / Eq. 5).
+      H^l   = the target's hidden state after layer l, l = 0 the embedding (PAPER.md:91), from the whole-prefix target;
+      B     = [0, L/4, L/2, 3L/4, L-1] (L = 32: [0, 8, 16, 24, 31], PAPER.md:91);
+      f(k)  = max{i | b_i <= min(L, k L/n)} (Eq. 3);  g_t^k = FC_f(k) Concat(H_t^b0 .. H_t^bf) (Eq. 4);
+      h     = the L_s-layer decoder over (g_1 .. g_t), last position (Eq. 1); logits = W_lm RMSNorm(h)."""
+    L, n, d = shape.n_layers, shape.n_stages, shape.d_model
+    tokens = np.asarray(tokens, dtype=np.int64)
+    T = len(tokens)
+    B = sorted({0, L // 4, L // 2, (3 * L) // 4, L - 1})
+    hid = forward_nocache(shape, weights, tokens, keep_hidden=True)["hidden"].astype(np.float32).astype(np.float64)
+    g = np.zeros((T, d))
+    for t in range(T):
+        lmax = min(L, int(depths[t]) * L // n)
+        f = max(i for i, b in enumerate(B) if b <= lmax)
+        cat = np.concatenate([hid[B[i], t] for i in range(f + 1)])
+        g[t] = (_w(pdm_weights["fc"][f]) @ cat).astype(np.float32).astype(np.float64)
+    dec = decoder_nocache(shape, pdm_weights, g, pdm_weights["n_layers"])
+    h = dec["final"][-1]
+    logits = _w(pdm_weights["head"]) @ _rmsnorm(h, _w(pdm_weights["final_norm"]), float(np.float32(shape.rms_eps)))
+    return {"logits": logits, "hidden": h, "features": g, "anchors": B, "k": dec["k"], "v": dec["v"],
+            "token": int(pdm_weights["vocab_map"][int(np.argmax(logits))])}
 
 
 def pdm_ref(shape, weights, feats: np.ndarray) -> dict:

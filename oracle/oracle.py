@@ -25,6 +25,11 @@ class _Weights(C.Structure):
                [("final_norm", C.c_void_p), ("pdm_proj", C.c_void_p), ("pdm_norm", C.c_void_p)]
 
 
+class _PdmWeights(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("vocab", C.c_int32), ("fc", _PP)] + [(k, _PP) for k in _LAYER_NAMES] + \
+               [("final_norm", C.c_void_p), ("head", C.c_void_p), ("vocab_map", C.c_void_p)]
+
+
 class _Res(C.Structure):
     _fields_ = [(k, C.c_int32) for k in ("step_index", "fill", "exited", "accepted", "emitted_token",
                                           "draft_token", "draft_forced", "discarded", "committed_len")]
@@ -138,6 +143,13 @@ def lib():
         L.ora_set_sampling.argtypes = [C.c_void_p, C.c_float, C.c_int32, C.c_uint64]
         L.ora_step_sample_follow.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_Hints), C.POINTER(_Res)]
         L.ora_get_sample_record.argtypes = [C.c_void_p, C.POINTER(_SampleRec)]
+        L.ora_pdm_attach.argtypes = [C.c_void_p, C.POINTER(_PdmWeights)]
+        L.ora_pdm_anchors.argtypes = [C.c_void_p, C.c_void_p]
+        L.ora_pdm_f.argtypes = [C.c_void_p, C.c_int32]
+        L.ora_pdm_get_anchor.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
+        L.ora_pdm_get_last.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+        L.ora_pdm_last_rows.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_void_p]
+        L.ora_pdm_get_kv.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.POINTER(C.c_int32)]
         _lib = L
     return _lib
 
@@ -260,6 +272,63 @@ class Oracle:
         return dict(draft=_dist_out(r.draft), target=_dist_out(r.target), u_draft=r.u_draft, u_accept=r.u_accept,
                     u_resid=r.u_resid, succ_token=r.succ_token, succ_q=r.succ_q, succ_p=r.succ_p,
                     ties=(r.ties_support, r.ties_draft, r.ties_accept, r.ties_resid))
+
+    # -- NEXT-1: the paper's PDM -------------------------------------------------------------
+    def attach_pdm(self, pw: dict):
+        """pw = spd_inputs.make_pdm_weights(...).  Before prefill."""
+        w = _PdmWeights()
+        w.n_layers, w.vocab = pw["n_layers"], pw["vocab"]
+        self.pdm_vocab = pw["vocab"]
+        for name in ["fc"] + _LAYER_NAMES:
+            arrs = [_u16(x) for x in pw[name]]
+            self._keep.extend(arrs)
+            tab = (C.c_void_p * len(arrs))(*[x.ctypes.data for x in arrs])
+            self._keep.append(tab)
+            setattr(w, name, C.cast(tab, _PP))
+        for name in ("final_norm", "head"):
+            arr = _u16(pw[name])
+            self._keep.append(arr)
+            setattr(w, name, arr.ctypes.data)
+        vm = np.ascontiguousarray(pw["vocab_map"], dtype=np.int32)
+        self._keep.append(vm)
+        w.vocab_map = vm.ctypes.data
+        if lib().ora_pdm_attach(self._h, C.byref(w)):
+            raise ValueError("ora_pdm_attach")
+
+    def pdm_anchors(self) -> list:
+        b = np.zeros(8, dtype=np.int32)
+        m = lib().ora_pdm_anchors(self._h, _p(b))
+        return [int(x) for x in b[:m]]
+
+    def pdm_f(self, k: int) -> int:
+        return lib().ora_pdm_f(self._h, k)
+
+    def pdm_anchor(self, pos: int, i: int) -> np.ndarray:
+        out = np.zeros(self.shape.d_model, dtype=np.float32)
+        lib().ora_pdm_get_anchor(self._h, pos, i, _p(out))
+        return out
+
+    def pdm_rows(self):
+        """(first position, per-row depths k) of the last PDM run."""
+        first, rows = C.c_int32(), C.c_int32()
+        lib().ora_pdm_last_rows(self._h, C.byref(first), C.byref(rows), None)
+        depths = np.zeros(rows.value, dtype=np.int32)
+        lib().ora_pdm_last_rows(self._h, C.byref(first), C.byref(rows), _p(depths))
+        return first.value, depths
+
+    def pdm_last(self, what: str) -> np.ndarray:
+        first, depths = self.pdm_rows()
+        idx = {"logits": 0, "hidden": 1, "features": 2}[what]
+        n = {0: self.pdm_vocab, 1: self.shape.d_model, 2: len(depths) * self.shape.d_model}[idx]
+        out = np.zeros(n, dtype=np.float32)
+        lib().ora_pdm_get_last(self._h, idx, _p(out))
+        return out.reshape(len(depths), -1) if idx == 2 else out
+
+    def pdm_kv(self, layer: int, which: int, rows: int):
+        out = np.zeros((rows, self.shape.n_kv_heads * self.shape.head_dim), dtype=np.uint16)
+        fin = C.c_int32()
+        lib().ora_pdm_get_kv(self._h, layer, which, rows, _p(out), C.byref(fin))
+        return out, fin.value
 
     def ar_step(self) -> int:
         nxt = C.c_int32(-1)

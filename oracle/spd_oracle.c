@@ -200,6 +200,17 @@ struct ora_ctx {
   uint64_t samp_seed;
   ora_dist *r_q;     /* [n] the draft distribution each in-flight token was drawn from */
   ora_sample_record rec;
+  /* NEXT-1 the paper's PDM */
+  int32_t pdm_on, pdm_m, pdm_anchor[ORA_PDM_MAX_ANCHORS];
+  ora_pdm_weights pw;
+  float *anch;       /* [max_seq][m][d]  H_pos^{b_i}: the residual stream entering layer b_i */
+  uint16_t *pkc, *pvc; /* [L_s][max_seq][Hkv*hd] bf16: the PDM's own KV cache */
+  int32_t pdm_final; /* F: positions whose PDM cache rows are final (depth n) */
+  float *pdm_x;      /* [rows][d] features / residual streams of the rows of the last PDM run */
+  float *pdm_g;      /* [rows][d] the features g as built (kept for the pins) */
+  float *pdm_lg;     /* [V_s] */
+  float *pdm_h;      /* [d] */
+  int32_t pdm_rows, pdm_first, pdm_cap, *pdm_depth;
   /* scratch */
   float *x, *q, *kk, *vv, *att, *o, *g, *u, *act, *dn, *z;
 };
@@ -308,7 +319,7 @@ int32_t ora_op_sample_residual(const ora_dist *P, const ora_dist *Q, double u) {
 
 int ora_set_sampling(ora_ctx *o, float temperature, int32_t top_k, uint64_t seed) {
   if (top_k < 1) { o->sampling_on = 0; return 0; }
-  if (top_k > ORA_MAX_TOPK || !(temperature > 0.f) || o->forced_on) return -1;
+  if (top_k > ORA_MAX_TOPK || !(temperature > 0.f) || o->forced_on || o->pdm_on) return -1;   /* P-9: the paper's PDM is greedy only */
   o->sampling_on = 1; o->top_k = top_k; o->temperature = temperature; o->samp_seed = seed;
   /* tokens already in flight were not drawn from a filtered distribution: whoever put them there acted as a
    * deterministic drafter, Q = one-hot on the token (accepted with probability P(x)) */
@@ -413,6 +424,7 @@ void ora_destroy(ora_ctx *o) {
   free(o->r_h); free(o->exit_logits); free(o->pdm_logits); free(o->pdm_u); free(o->pdm_feat);
   free(o->x); free(o->q); free(o->kk); free(o->vv); free(o->att); free(o->o); free(o->g); free(o->u);
   free(o->act); free(o->dn); free(o->z); free(o->r_q);
+  free(o->anch); free(o->pkc); free(o->pvc); free(o->pdm_x); free(o->pdm_g); free(o->pdm_lg); free(o->pdm_h); free(o->pdm_depth);
   free(o);
 }
 
@@ -421,42 +433,79 @@ static void embed_row(const ora_ctx *o, int tok, float *h) {
   for (int i = 0; i < o->cfg.d_model; ++i) h[i] = bf16_to_f32(e[i]);
 }
 
+/* A stack of decoder layers with its KV cache: the target's L layers, or the PDM's L_s layers (same structure, C-2.13 /
+ * reading P-3).  len == NULL: rows may be rewritten (the PDM refreshes its trailing rows every cycle). */
+typedef struct {
+  const uint16_t *const *attn_norm, *const *wq, *const *wk, *const *wv, *const *wo, *const *mlp_norm, *const *w_gate,
+      *const *w_up, *const *w_down;
+  uint16_t *kc, *vc;
+  int32_t *len;
+  int32_t capture;   /* 1: the target stack — capture the anchors H^b of the paper's PDM on the way (Eq. 4) */
+} layer_set;
+
+static layer_set target_set(ora_ctx *o) {
+  layer_set S = {o->w.attn_norm, o->w.wq, o->w.wk, o->w.wv, o->w.wo, o->w.mlp_norm, o->w.w_gate, o->w.w_up, o->w.w_down,
+                 o->kc, o->vc, o->len, 1};
+  return S;
+}
+
+static layer_set pdm_set(ora_ctx *o) {
+  layer_set S = {o->pw.attn_norm, o->pw.wq, o->pw.wk, o->pw.wv, o->pw.wo, o->pw.mlp_norm, o->pw.w_gate, o->pw.w_up,
+                 o->pw.w_down, o->pkc, o->pvc, NULL, 0};
+  return S;
+}
+
+/* PAPER.md:91 "H_t^l denote the hidden state of token x_t after layer l (l = 0 is the embedding)": the residual stream
+ * ENTERING layer l.  Stored for the anchors l in B when the paper's PDM is attached. */
+static void capture_anchor(ora_ctx *o, int l, const float *h, int pos) {
+  if (!o->pdm_on) return;
+  for (int i = 0; i < o->pdm_m; ++i)
+    if (o->pdm_anchor[i] == l)
+      memcpy(o->anch + ((size_t)pos * o->pdm_m + i) * o->cfg.d_model, h, sizeof(float) * (size_t)o->cfg.d_model);
+}
+
 /* The per-token attention sub-step of Layer: RoPE(q,k,pos); require len[l]==pos; append bf16(k),
  * bf16(v) as row pos; attend over rows 0..pos (causal incl. self).  Returns -1 if the causality
  * precondition of north_star ("every earlier-position token already deeper") is violated. */
-static int attend_token(ora_ctx *o, int l, int pos, float *q, float *kk, const float *vv, float *att) {
+static int attend_token(ora_ctx *o, const layer_set *S, int l, int pos, float *q, float *kk, const float *vv, float *att) {
   const ora_config *c = &o->cfg;
   size_t row = kv_row(c);
   ora_op_rope(q, c->n_q_heads, c->head_dim, pos, c->rope_base);
   ora_op_rope(kk, c->n_kv_heads, c->head_dim, pos, c->rope_base);
-  if (o->len[l] != pos || pos >= c->max_seq) return -1;
-  uint16_t *kd = o->kc + ((size_t)l * c->max_seq + pos) * row;
-  uint16_t *vd = o->vc + ((size_t)l * c->max_seq + pos) * row;
+  if (pos >= c->max_seq || (S->len && S->len[l] != pos)) return -1;
+  uint16_t *kd = S->kc + ((size_t)l * c->max_seq + pos) * row;
+  uint16_t *vd = S->vc + ((size_t)l * c->max_seq + pos) * row;
   for (size_t i = 0; i < row; ++i) { kd[i] = ora_op_f32_to_bf16(kk[i]); vd[i] = ora_op_f32_to_bf16(vv[i]); }
-  o->len[l] = pos + 1;
-  ora_op_attention(q, o->kc + (size_t)l * c->max_seq * row, o->vc + (size_t)l * c->max_seq * row, pos + 1,
+  if (S->len) S->len[l] = pos + 1;
+  ora_op_attention(q, S->kc + (size_t)l * c->max_seq * row, S->vc + (size_t)l * c->max_seq * row, pos + 1,
                    c->n_q_heads, c->n_kv_heads, c->head_dim, att);
   return 0;
 }
 
 /* Layer(l, h, pos) of C-1: pre-norm attention block then pre-norm SwiGLU block, residual stream h. */
-static int layer_forward(ora_ctx *o, int l, float *h, int pos) {
+static int layer_forward_set(ora_ctx *o, const layer_set *S, int l, float *h, int pos) {
   const ora_config *c = &o->cfg;
   int d = c->d_model, qd = c->n_q_heads * c->head_dim, kd = c->n_kv_heads * c->head_dim, F = c->d_ffn;
-  ora_op_rmsnorm(h, o->w.attn_norm[l], d, c->rms_eps, o->x);
-  ora_op_gemv(o->w.wq[l], qd, d, o->x, o->q);
-  ora_op_gemv(o->w.wk[l], kd, d, o->x, o->kk);
-  ora_op_gemv(o->w.wv[l], kd, d, o->x, o->vv);
-  if (attend_token(o, l, pos, o->q, o->kk, o->vv, o->att)) return -1;
-  ora_op_gemv(o->w.wo[l], d, qd, o->att, o->o);
+  if (S->capture) capture_anchor(o, l, h, pos);
+  ora_op_rmsnorm(h, S->attn_norm[l], d, c->rms_eps, o->x);
+  ora_op_gemv(S->wq[l], qd, d, o->x, o->q);
+  ora_op_gemv(S->wk[l], kd, d, o->x, o->kk);
+  ora_op_gemv(S->wv[l], kd, d, o->x, o->vv);
+  if (attend_token(o, S, l, pos, o->q, o->kk, o->vv, o->att)) return -1;
+  ora_op_gemv(S->wo[l], d, qd, o->att, o->o);
   for (int i = 0; i < d; ++i) h[i] += o->o[i];
-  ora_op_rmsnorm(h, o->w.mlp_norm[l], d, c->rms_eps, o->x);
-  ora_op_gemv(o->w.w_gate[l], F, d, o->x, o->g);
-  ora_op_gemv(o->w.w_up[l], F, d, o->x, o->u);
+  ora_op_rmsnorm(h, S->mlp_norm[l], d, c->rms_eps, o->x);
+  ora_op_gemv(S->w_gate[l], F, d, o->x, o->g);
+  ora_op_gemv(S->w_up[l], F, d, o->x, o->u);
   ora_op_silu_mul(o->g, o->u, F, o->act);
-  ora_op_gemv(o->w.w_down[l], d, F, o->act, o->dn);
+  ora_op_gemv(S->w_down[l], d, F, o->act, o->dn);
   for (int i = 0; i < d; ++i) h[i] += o->dn[i];
   return 0;
+}
+
+static int layer_forward(ora_ctx *o, int l, float *h, int pos) {
+  layer_set S = target_set(o);
+  return layer_forward_set(o, &S, l, h, pos);
 }
 
 /* logits = E . RMSNorm(h, gain); returns argmax and records the margin. */
@@ -488,12 +537,14 @@ static int layer_forward_block(ora_ctx *o, int l, float *H, int t0, int t1) {
   float *G = (float *)malloc(sizeof(float) * (size_t)nt * F);
   float *U = (float *)malloc(sizeof(float) * (size_t)nt * F);
   int rc = 0;
+  layer_set S = target_set(o);
+  for (int t = 0; t < nt; ++t) capture_anchor(o, l, H + (size_t)(t0 + t) * d, t0 + t);
   for (int t = 0; t < nt; ++t) ora_op_rmsnorm(H + (size_t)(t0 + t) * d, o->w.attn_norm[l], d, c->rms_eps, X + (size_t)t * d);
   gemv_block(o->w.wq[l], qd, d, X, d, Q, qd, nt);
   gemv_block(o->w.wk[l], kd, d, X, d, Kb, kd, nt);
   gemv_block(o->w.wv[l], kd, d, X, d, Vb, kd, nt);
   for (int t = 0; t < nt && !rc; ++t)
-    rc = attend_token(o, l, t0 + t, Q + (size_t)t * qd, Kb + (size_t)t * kd, Vb + (size_t)t * kd, A + (size_t)t * qd);
+    rc = attend_token(o, &S, l, t0 + t, Q + (size_t)t * qd, Kb + (size_t)t * kd, Vb + (size_t)t * kd, A + (size_t)t * qd);
   if (!rc) {
     gemv_block(o->w.wo[l], d, qd, A, qd, O, d, nt);
     for (int t = 0; t < nt; ++t)
@@ -521,6 +572,7 @@ int ora_prefill(ora_ctx *o, const int32_t *tokens, int32_t P, int32_t block, int
   for (int i = 0; i < P; ++i)
     if (tokens[i] < 0 || tokens[i] >= c->vocab) return -1;
   for (int l = 0; l < L; ++l) o->len[l] = 0;
+  o->pdm_final = 0;   /* the first cycle's PDM run builds the prompt's full-depth rows */
   if (block <= 1) {
     for (int pos = 0; pos < P; ++pos) {
       float *h = o->hfin + (size_t)pos * d;
@@ -559,6 +611,136 @@ int ora_set_forced(ora_ctx *o, const int32_t *truth, int32_t n_truth, float p, u
   o->truth = truth; o->n_truth = n_truth; o->forced_on = 1; o->forced_seed = seed;
   o->forced_thresh = (uint64_t)floor((double)p * 9007199254740992.0); /* floor(p * 2^53) */
   return 0;
+}
+
+/* ------------------------------------------------------------------ NEXT-1: the paper's PDM ---- */
+
+static int apply_hint(const float *logits, int own, int hint, int vocab, float band, int32_t *ties);
+
+/* Reading P-1: B = [0, L/4, L/2, 3L/4, L-1] (integer division), duplicates removed — for L = 32 the paper's
+ * [0, 8, 16, 24, 31] (the last anchor is taken literally as L-1, C-2.6). */
+static int anchor_set(int L, int32_t *b) {
+  int cand[5] = {0, L / 4, L / 2, (3 * L) / 4, L - 1}, m = 0;
+  for (int i = 0; i < 5; ++i)
+    if (m == 0 || cand[i] > b[m - 1]) b[m++] = cand[i];
+  return m;
+}
+
+int32_t ora_pdm_anchors(const ora_ctx *o, int32_t *anchors) {
+  int32_t b[ORA_PDM_MAX_ANCHORS];
+  int m = anchor_set(o->cfg.n_layers, b);
+  if (anchors) memcpy(anchors, b, sizeof(int32_t) * (size_t)m);
+  return m;
+}
+
+/* Eq. 3: l_max(k) = min(L, k L/n); f(k) = max{ i | b_i <= l_max(k) }. */
+int32_t ora_pdm_f(const ora_ctx *o, int32_t k) {
+  int32_t b[ORA_PDM_MAX_ANCHORS];
+  int m = anchor_set(o->cfg.n_layers, b), L = o->cfg.n_layers, n = o->cfg.n_stages;
+  int lmax = k * (L / n) < L ? k * (L / n) : L, f = 0;
+  for (int i = 0; i < m; ++i)
+    if (b[i] <= lmax) f = i;
+  return f;
+}
+
+int ora_pdm_attach(ora_ctx *o, const ora_pdm_weights *pw) {
+  const ora_config *c = &o->cfg;
+  if (!pw || pw->n_layers < 1 || pw->vocab < 1 || pw->vocab > c->vocab || o->sampling_on || o->prefilled) return -1;
+  if (!pw->fc || !pw->attn_norm || !pw->wq || !pw->wk || !pw->wv || !pw->wo || !pw->mlp_norm || !pw->w_gate || !pw->w_up ||
+      !pw->w_down || !pw->final_norm || !pw->head || !pw->vocab_map)
+    return -1;
+  for (int i = 0; i < pw->vocab; ++i)
+    if (pw->vocab_map[i] < 0 || pw->vocab_map[i] >= c->vocab || (i > 0 && pw->vocab_map[i] <= pw->vocab_map[i - 1])) return -1;
+  o->pw = *pw;
+  o->pdm_m = anchor_set(c->n_layers, o->pdm_anchor);
+  size_t row = kv_row(c);
+  o->anch = (float *)calloc((size_t)c->max_seq * o->pdm_m * c->d_model, 4);
+  o->pkc = (uint16_t *)calloc((size_t)pw->n_layers * c->max_seq * row, 2);
+  o->pvc = (uint16_t *)calloc((size_t)pw->n_layers * c->max_seq * row, 2);
+  o->pdm_lg = (float *)calloc((size_t)pw->vocab, 4);
+  o->pdm_h = (float *)calloc((size_t)c->d_model, 4);
+  o->pdm_cap = 0;
+  o->pdm_final = 0;
+  o->pdm_on = 1;
+  return 0;
+}
+
+/* The draft of one cycle (see spd_oracle.h).  Returns the drafted TARGET token id. */
+static int pdm_paper_draft(ora_ctx *o, int32_t draft_hint, float band) {
+  const ora_config *c = &o->cfg;
+  int d = c->d_model, n = c->n_stages, m = o->pdm_m;
+  int a = o->a, p_new = o->r_pos[a - 1];
+  int first = o->pdm_final, rows = p_new - first + 1;
+  if (rows > o->pdm_cap) {
+    free(o->pdm_x); free(o->pdm_g); free(o->pdm_depth);
+    o->pdm_cap = rows + 64;
+    o->pdm_x = (float *)calloc((size_t)o->pdm_cap * d, 4);
+    o->pdm_g = (float *)calloc((size_t)o->pdm_cap * d, 4);
+    o->pdm_depth = (int32_t *)calloc((size_t)o->pdm_cap, 4);
+  }
+  o->pdm_rows = rows; o->pdm_first = first;
+  float *cat = (float *)malloc(sizeof(float) * (size_t)m * d);
+  /* features (Eq. 4): committed positions q < c take the full-depth rule k = n (Eq. 2 / Eq. 5); an in-flight token
+   * takes its depth BEFORE this cycle's forward (pre-step); the newest contributes only g^0 */
+  for (int r = 0; r < rows; ++r) {
+    int q = first + r, k;
+    if (q < o->c) k = n;
+    else k = o->r_k[q - o->c];
+    o->pdm_depth[r] = k;
+    int f = ora_pdm_f(o, k);
+    for (int i = 0; i <= f; ++i) {
+      float *dst = cat + (size_t)i * d;
+      /* an in-flight token's deepest eligible state H^{k L/n} is the residual stream it currently holds (the input of
+       * its next stage; k = 0: the embedding row) — the capture below layer_forward stores it only when that stage runs */
+      if (q >= o->c && o->pdm_anchor[i] == k * (c->n_layers / n)) memcpy(dst, o->r_h + (size_t)(q - o->c) * d, sizeof(float) * d);
+      else memcpy(dst, o->anch + ((size_t)q * m + i) * d, sizeof(float) * d);
+    }
+    ora_op_gemv(o->pw.fc[f], d, (f + 1) * d, cat, o->pdm_x + (size_t)r * d);
+  }
+  free(cat);
+  memcpy(o->pdm_g, o->pdm_x, sizeof(float) * (size_t)rows * d);
+  /* the PDM decoder over those rows, layer by layer, rows in position order (causal); every row rewrites its K/V row
+   * of the PDM cache (the trailing features are refreshed on every advance) */
+  layer_set S = pdm_set(o);
+  for (int l = 0; l < o->pw.n_layers; ++l)
+    for (int r = 0; r < rows; ++r)
+      if (layer_forward_set(o, &S, l, o->pdm_x + (size_t)r * d, first + r)) return -1;
+  o->pdm_final = o->c;   /* rows below c were built at depth n: final */
+  /* independent head on the last position (Eq. 1), reduced vocabulary */
+  memcpy(o->pdm_h, o->pdm_x + (size_t)(rows - 1) * d, sizeof(float) * d);
+  ora_op_rmsnorm(o->pdm_h, o->pw.final_norm, d, c->rms_eps, o->z);
+  ora_op_gemv(o->pw.head, o->pw.vocab, d, o->z, o->pdm_lg);
+  top2_margin(o->pdm_lg, o->pw.vocab, &o->gap[1], &o->maxabs[1]);
+  int idx = ora_op_argmax(o->pdm_lg, o->pw.vocab);
+  int hint_idx = -1;
+  if (draft_hint >= 0)
+    for (int i = 0; i < o->pw.vocab; ++i)
+      if (o->pw.vocab_map[i] == draft_hint) hint_idx = i;
+  idx = apply_hint(o->pdm_lg, idx, hint_idx, o->pw.vocab, band, &o->ties[1]);
+  return o->pw.vocab_map[idx];
+}
+
+void ora_pdm_get_anchor(const ora_ctx *o, int32_t pos, int32_t i, float *out) {
+  memcpy(out, o->anch + ((size_t)pos * o->pdm_m + i) * o->cfg.d_model, 4 * (size_t)o->cfg.d_model);
+}
+
+void ora_pdm_get_last(const ora_ctx *o, int32_t what, float *out) {
+  if (what == 0) memcpy(out, o->pdm_lg, 4 * (size_t)o->pw.vocab);
+  else if (what == 1) memcpy(out, o->pdm_h, 4 * (size_t)o->cfg.d_model);
+  else if (what == 2) memcpy(out, o->pdm_g, 4 * (size_t)o->pdm_rows * o->cfg.d_model);
+}
+
+void ora_pdm_last_rows(const ora_ctx *o, int32_t *first_pos, int32_t *rows, int32_t *depths) {
+  if (first_pos) *first_pos = o->pdm_first;
+  if (rows) *rows = o->pdm_rows;
+  if (depths) memcpy(depths, o->pdm_depth, 4 * (size_t)o->pdm_rows);
+}
+
+void ora_pdm_get_kv(const ora_ctx *o, int32_t layer, int32_t which, int32_t rows, uint16_t *out, int32_t *final_len) {
+  size_t row = kv_row(&o->cfg);
+  const uint16_t *src = (which ? o->pvc : o->pkc) + (size_t)layer * o->cfg.max_seq * row;
+  memcpy(out, src, 2 * row * (size_t)rows);
+  if (final_len) *final_len = o->pdm_final;
 }
 
 /* One SPD cycle — "Step" of C-1, in the paper's order: (1) read the ring, (2) PDM on PRE-step
@@ -623,9 +805,15 @@ static int step_impl(ora_ctx *o, int32_t draft_override, int32_t draft_hint, int
     else if (q >= 0) memcpy(f, o->hfin + (size_t)q * d, sizeof(float) * d);
     else memset(f, 0, sizeof(float) * d);
   }
-  ora_op_gemv(o->w.pdm_proj, d, n * d, o->pdm_feat, o->pdm_u);
-  int draft = head_argmax(o, o->pdm_u, o->w.pdm_norm, o->pdm_logits, 1);
-  draft = apply_hint(o->pdm_logits, draft, draft_hint, c->vocab, band, &o->ties[1]);
+  int draft;
+  if (o->pdm_on) {   /* NEXT-1: the paper's PDM replaces the simplified one (same pre-step schedule) */
+    draft = pdm_paper_draft(o, draft_hint, band);
+    if (draft < 0) return -2;
+  } else {
+    ora_op_gemv(o->w.pdm_proj, d, n * d, o->pdm_feat, o->pdm_u);
+    draft = head_argmax(o, o->pdm_u, o->w.pdm_norm, o->pdm_logits, 1);
+    draft = apply_hint(o->pdm_logits, draft, draft_hint, c->vocab, band, &o->ties[1]);
+  }
   ora_dist Qd; /* the distribution the entering draft is drawn from (sampling mode) */
   memset(&Qd, 0, sizeof Qd);
   if (o->sampling_on) { /* x^ ~ Q_t = filtered PDM distribution (S-2, S-3; j = 0) */
@@ -735,6 +923,7 @@ int ora_rollback(ora_ctx *o, int32_t new_len, int32_t reseed_token) {
   if (!o->prefilled) return -1;
   if (new_len < 0 || new_len > o->c || reseed_token < 0 || reseed_token >= o->cfg.vocab) return -1;
   o->c = new_len;
+  if (o->pdm_final > new_len) o->pdm_final = new_len;
   o->emitted = new_len - o->prompt_len + 1; /* tokens emitted up to and including the reseed token */
   for (int l = 0; l < o->cfg.n_layers; ++l)
     if (o->len[l] > new_len) o->len[l] = new_len;

@@ -24,6 +24,9 @@
  * Parity pins: see tests/test_oracle_*.py.  The simplified PDM (linear n*d->d + RMSNorm + tied
  * head, BASELINE.json) has no counterpart in the paper: draft-token parity vs the paper is
  * UNPINNED ("parity unpinned"); it is pinned only as a pure function of its n slot vectors.
+ * The paper's own PDM (ora_pdm_attach, NEXT-1) is pinned by tests/test_oracle_pdm.py: a float64 whole-prefix
+ * numpy model of the PDM decoder over the feature sequence (no cache), the anchors against O-AR's per-layer
+ * trace, f(k) against Eq. 3 by brute force, the staircase layouts of Eq. 2 / Eq. 5, lossless-ness unchanged.
  */
 #ifndef SPD_ORACLE_H
 #define SPD_ORACLE_H
@@ -116,6 +119,47 @@ void ora_get_hfin(const ora_ctx *, int32_t pos, float *out /* [d] */);
 void ora_get_last(const ora_ctx *, int32_t what, float *out);
 /* top1-top2 gap and max|logit| of the last verify (which=0) / PDM (which=1) argmax (C-4). */
 void ora_get_margin(const ora_ctx *, int32_t which, float *gap, float *maxabs);
+
+/* ---- NEXT-1: the paper's Pipeline Draft Module (readings P-1..P-9 of DESIGN.md section 14) ----
+ * PAPER.md:71 "an L_s-layer Transformer decoder f_theta with an independent LM head W_lm"; :77-85 Eq. 1-2 the
+ * depth-conditioned feature sequence G_t and the depth staircase; :91-100 Eq. 3-4 multi-depth feature aggregation
+ * (anchors B with b_0 = 0, l_max(k) = min(L, k L/n), f(k) = max{i | b_i <= l_max(k)},
+ * g_t^k = FC_f(k)(Concat(H_t^b0 .. H_t^bf(k)))); :102-107 Eq. 5 warm-up layout; :115 pre-step features; :139 reduced
+ * vocabulary head; :299 App. A.1 PDM KV cache ("caching appends only the trailing (n+1) refreshed features each step").
+ *
+ * One cycle's draft (replaces the simplified PDM when attached):
+ *   rows q = F .. p_new, F = positions whose cached PDM rows are already final (depth n), p_new = newest position;
+ *   depth k(q) = n for committed q < c, else the in-flight token's completed stages BEFORE this cycle's forward;
+ *   g_q = FC_f(k(q)) . Concat(H_q^b0 .. H_q^bf) (H^b = the target's residual stream entering layer b; H^0 = E[tok]);
+ *   the L_s PDM layers (the target's layer structure, C-2.13, own weights) run over those rows in position order, each
+ *   row rewriting its K/V row of the PDM cache and attending rows 0 .. q; then F := c;
+ *   x^ = vocab_map[argmax(W_lm . RMSNorm(h_last; g_pdm))].
+ * Tensors fp32, reductions fp64, K/V rows bf16 — the same numeric contract as the target (C-2.17). */
+#define ORA_PDM_MAX_ANCHORS 8
+typedef struct {
+  int32_t n_layers;                    /* L_s >= 1 */
+  int32_t vocab;                       /* V_s <= V: rows of the independent head */
+  const uint16_t *const *fc;           /* [m] -> [d, (i+1) d]: FC_i multiplies Concat(H^b0 .. H^bi) */
+  const uint16_t *const *attn_norm, *const *wq, *const *wk, *const *wv, *const *wo, *const *mlp_norm, *const *w_gate,
+      *const *w_up, *const *w_down;    /* [L_s] each, shapes as the target's */
+  const uint16_t *final_norm;          /* [d] */
+  const uint16_t *head;                /* [V_s, d] */
+  const int32_t *vocab_map;            /* [V_s] draft index -> target token id, strictly ascending */
+} ora_pdm_weights;
+/* Attaches the paper's PDM (before ora_prefill).  -1: bad arguments or sampling is on (greedy only, reading P-9). */
+int ora_pdm_attach(ora_ctx *, const ora_pdm_weights *);
+/* The anchor set B of the ctx's L (reading P-1: [0, L/4, L/2, 3L/4, L-1], duplicates removed); returns m. */
+int32_t ora_pdm_anchors(const ora_ctx *, int32_t *anchors /* [ORA_PDM_MAX_ANCHORS] */);
+/* f(k) of Eq. 3 for the ctx's (L, n). */
+int32_t ora_pdm_f(const ora_ctx *, int32_t k);
+/* H_pos^{b_i} as captured by the target's forward (fp32 [d]). */
+void ora_pdm_get_anchor(const ora_ctx *, int32_t pos, int32_t i, float *out);
+/* Last PDM run: what 0 = logits [V_s], 1 = final hidden h_last [d] (pre-norm), 2 = features g of its rows [rows, d]. */
+void ora_pdm_get_last(const ora_ctx *, int32_t what, float *out);
+/* Rows of the last PDM run: first position, row count, per-row depth k (may be NULL). */
+void ora_pdm_last_rows(const ora_ctx *, int32_t *first_pos, int32_t *rows, int32_t *depths);
+/* K or V rows of one PDM layer as bf16 bits, [rows, Hkv*hd]; *final_len = F. */
+void ora_pdm_get_kv(const ora_ctx *, int32_t layer, int32_t which, int32_t rows, uint16_t *out, int32_t *final_len);
 
 /* ---- NEXT-2: sampling verification (readings S-1..S-10 of DESIGN.md §11) ----------
  * PAPER.md:129 "under sampling we apply standard rejection sampling"; PAPER.md:131 on a reject the

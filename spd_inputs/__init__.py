@@ -12,7 +12,9 @@ norm gains are 1.0 (or, for the test-only variant, U[0.5, 1.5] rounded to bf16);
 ids are uniform on [0, vocab).
 """
 from .gen import (CONFIGS, ModelShape, make_weights, make_prompt, f32_to_bf16_bits,
-                  bf16_bits_to_f32, layer_tensor_names, make_kv_filler, make_tensor, shapes_of, make_echo)
+                  bf16_bits_to_f32, layer_tensor_names, make_kv_filler, make_tensor, shapes_of, make_echo,
+                  make_pdm_weights, pdm_anchor_count)
 
 __all__ = ["CONFIGS", "ModelShape", "make_weights", "make_prompt", "f32_to_bf16_bits",
-           "bf16_bits_to_f32", "layer_tensor_names", "make_kv_filler", "make_tensor", "shapes_of", "make_echo"]
+           "bf16_bits_to_f32", "layer_tensor_names", "make_kv_filler", "make_tensor", "shapes_of", "make_echo",
+           "make_pdm_weights", "pdm_anchor_count"]

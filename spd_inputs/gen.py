@@ -143,6 +143,32 @@ def make_weights(shape: ModelShape, seed: int = 1234, std: float = 0.02, random_
     return w
 
 
+def pdm_anchor_count(n_layers: int) -> int:
+    """How many FC matrices the paper's PDM needs: the anchor list [0, L/4, L/2, 3L/4, L-1] without duplicates (sizes
+    only; which layers they are is the method's business and lives on both sides separately)."""
+    return len(sorted({0, n_layers // 4, n_layers // 2, (3 * n_layers) // 4, n_layers - 1}))
+
+
+def make_pdm_weights(shape: ModelShape, pdm_layers: int, pdm_vocab: int, seed: int = 1234, std: float = 0.02,
+                     random_gains: bool = False) -> dict:
+    """Weights of the paper's Pipeline Draft Module (NEXT-1) as uint16 bf16-bit arrays: "fc" = [m] matrices
+    [d, (i+1) d] (std / sqrt(i+1), so every aggregated feature has the scale of one projected state), the nine
+    per-layer tensors of `pdm_layers` decoder layers (the target's shapes, own values), "final_norm" [d], "head"
+    [pdm_vocab, d], and "vocab_map": int32 [pdm_vocab], a seeded strictly ascending subset of the token ids."""
+    d = shape.d_model
+    m = pdm_anchor_count(shape.n_layers)
+    sp = seed + 7777                                    # the PDM's tensors never alias the target's
+    w = {"n_layers": int(pdm_layers), "vocab": int(pdm_vocab)}
+    w["fc"] = [_normal_bf16(sp, 20, i, d * (i + 1) * d, std / float(np.sqrt(i + 1))).reshape(d, (i + 1) * d) for i in range(m)]
+    for name in layer_tensor_names():
+        w[name] = [make_tensor(shape, name, l, sp, std, random_gains, 1.0) for l in range(pdm_layers)]
+    w["final_norm"] = _gain_bf16(sp, 22, -1, d, random_gains)
+    w["head"] = _normal_bf16(sp, 21, -1, pdm_vocab * d, std).reshape(pdm_vocab, d)
+    rng = np.random.Generator(np.random.PCG64([seed, 4711]))
+    w["vocab_map"] = np.sort(rng.choice(shape.vocab, size=pdm_vocab, replace=False)).astype(np.int32)
+    return w
+
+
 def make_echo(shape: ModelShape, weights: dict) -> dict:
     """The "echo" re-initialisation used to reach saturation under sampling verification: a copy of
     `weights` with W_o = W_down = 0 (every layer leaves the residual stream untouched), W_p = [I 0 .. 0] (the PDM
