@@ -131,6 +131,13 @@ enum {
   SPD_DBG_CYCLE_TIMES = 14,/* uint64[1024][2]: %globaltimer (ns) at which the controller of the cycle with step_index K
                               began [(K-1) % 1024][0] (kernel entry of the fused engine) and finished [..][1]; the
                               difference of consecutive finish stamps of back-to-back cycles is the step latency   */
+  SPD_DBG_PDM2_LOGITS = 15,/* fp32[V_s]: logits of the paper PDM's last draft (reduced vocabulary)                   */
+  SPD_DBG_PDM2_HIDDEN = 16,/* fp32[d]: its last row's hidden state before the final norm                            */
+  SPD_DBG_PDM2_RUN = 17,   /* int32[3]: first position, row count of the last draft, F (final rows)                 */
+  SPD_DBG_PDM2_FEAT = 18,  /* [rows] fp32[rows, d]: the features g of those rows (Eq. 4)                             */
+  SPD_DBG_PDM2_K = 19,     /* [PDM layer] bf16 [rows, n_kv_heads*hd] of the PDM's cache, rows = bytes / row size    */
+  SPD_DBG_PDM2_V = 20,
+  SPD_DBG_ANCHOR = 21,     /* [position * 8 + i] fp32[d]: H^{b_i} of that position                                  */
   SPD_DBG_PHASE_PROFILE = 10 /* uint64[160][168][6]: per (CTA, phase) clock stamps of the last fused cycle:
                               0 inputs ready, 1 activations staged, 2 tiles consumed, 3/4 producer issued the
                               phase's first/last tile (SM clock); 5 = %globaltimer at stamp 0; phase 167 holds
@@ -213,6 +220,37 @@ typedef struct {
   int32_t prefiltered;     /* selections served by the head pass's threshold list, no scan (0..2)       */
 } spd_sample_record;
 int spd_set_sampling(spd_ctx *ctx, float temperature, int32_t top_k, uint64_t seed);
+
+/* ---- The paper's Pipeline Draft Module ----------------------------------------------------
+ * PAPER.md:71 "an L_s-layer Transformer decoder f_theta with an independent LM head"; :91-100 Eq. 3-4 (anchors
+ * B = [0, L/4, L/2, 3L/4, L-1] — [0, 8, 16, 24, 31] for L = 32 —, l_max(k) = min(L, k L/n), f(k) = max{i | b_i <= l_max(k)},
+ * g_t^k = FC_f(k)(Concat(H_t^b0 .. H_t^bf(k))), H^b = the target's residual stream entering layer b); :102-107 Eq. 5;
+ * :115 pre-step features; :139 reduced-vocabulary head; :299 the PDM's KV cache, whose trailing n + 1 rows are rewritten
+ * every cycle.  Once attached it REPLACES the simplified PDM of spd_weights (pdm_proj / pdm_norm are then unused): every
+ * cycle, before the stage forward, the rows F .. p_new (F = positions whose rows are final, p_new = newest position)
+ * run through FC_f(k) and the L_s PDM layers (the target's layer structure C-2.13 with its own weights and its own
+ * cache), the last row goes through RMSNorm(final_norm) and the head, and draft = vocab_map[argmax].  spd_prefill
+ * also builds the prompt's full-depth rows; spd_rollback rewinds F.  Greedy verification only (spd_set_sampling then
+ * returns SPD_ESTATE, reading P-9).  Weights: DEVICE pointers to bf16 bit patterns, row-major [out, in]; the per-layer
+ * members and `fc` are HOST arrays of DEVICE pointers (read during spd_pdm_attach only); vocab_map is a DEVICE int32
+ * array, strictly ascending target token ids.  Buffers: DEVICE, sizes from spd_pdm_query_sizes, 256-byte aligned,
+ * caller-owned until spd_destroy.  Attach before spd_prefill (SPD_ESTATE afterwards); SPD_EINVAL on bad arguments. */
+typedef struct spd_pdm_weights {
+  int32_t n_layers;                 /* L_s >= 1 */
+  int32_t vocab;                    /* V_s <= vocab */
+  const uint16_t *const *fc;        /* [m] -> [d, (i+1) d], m = anchors (5 unless L < 8) */
+  const uint16_t *const *attn_norm, *const *wq, *const *wk, *const *wv, *const *wo, *const *mlp_norm, *const *w_gate,
+      *const *w_up, *const *w_down; /* [L_s] each, shapes as spd_weights */
+  const uint16_t *final_norm;       /* [d] */
+  const uint16_t *head;             /* [V_s, d] */
+  const int32_t *vocab_map;         /* DEVICE int32[V_s] */
+} spd_pdm_weights;
+typedef struct {
+  size_t kv_bytes;   /* the PDM's cache: bf16 [L_s][K|V][kv_head][max_seq][head_dim] */
+  size_t work_bytes; /* row scratch, anchors H^b of every position [max_seq][m][d] fp32 */
+} spd_pdm_sizes;
+int spd_pdm_query_sizes(const spd_config *cfg, int32_t pdm_layers, int32_t pdm_vocab, spd_pdm_sizes *out);
+int spd_pdm_attach(spd_ctx *ctx, const spd_pdm_weights *w, void *pdm_kv, void *pdm_work);
 
 int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value);
 

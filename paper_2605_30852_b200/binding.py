@@ -35,7 +35,7 @@ class OPT:
 
 class DBG:
     SLOT_HIDDEN, EXIT_LOGITS, PDM_LOGITS, PDM_PRENORM, PDM_FEAT, KV_K, KV_V, KV_LEN, RING, HFIN, PHASE_PROFILE, \
-        SAMPLE, Q, ATT, CYCLE_TIMES = range(15)
+        SAMPLE, Q, ATT, CYCLE_TIMES, PDM2_LOGITS, PDM2_HIDDEN, PDM2_RUN, PDM2_FEAT, PDM2_K, PDM2_V, ANCHOR = range(22)
 
 
 MAX_TOPK = 64
@@ -77,6 +77,15 @@ class _Sizes(C.Structure):
 class _Buffers(C.Structure):
     _fields_ = [("repack", C.c_void_p), ("kv", C.c_void_p), ("work", C.c_void_p),
                 ("stream_main", C.c_void_p), ("stream_pdm", C.c_void_p)]
+
+
+class _PdmWeights(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("vocab", C.c_int32), ("fc", _PP)] + [(k, _PP) for k in _LAYER_NAMES] + \
+               [("final_norm", C.c_void_p), ("head", C.c_void_p), ("vocab_map", C.c_void_p)]
+
+
+class _PdmSizes(C.Structure):
+    _fields_ = [("kv_bytes", C.c_size_t), ("work_bytes", C.c_size_t)]
 
 
 class _Res(C.Structure):
@@ -131,6 +140,8 @@ def lib():
         L.spd_op_gemm.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp]
         L.spd_op_gemm_scratch.argtypes = [i32, i32]
         L.spd_op_gemm_scratch.restype = C.c_size_t
+        L.spd_pdm_query_sizes.argtypes = [vp, i32, i32, vp]
+        L.spd_pdm_attach.argtypes = [vp, vp, vp, vp]
         L.spd_op_rope.argtypes = [vp, i32, i32, i32, f32, vp]
         L.spd_op_attention.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp]
         L.spd_op_attention_scratch.argtypes = [i32, i32, i32]
@@ -150,6 +161,22 @@ def upload_weights(weights: dict, device: int = 0) -> dict:
 
     out = {}
     for k, v in weights.items():
+        out[k] = [up(x) for x in v] if isinstance(v, (list, tuple)) else up(v)
+    return out
+
+
+def upload_pdm_weights(pw: dict, device: int = 0) -> dict:
+    """spd_inputs.make_pdm_weights(...) -> CUDA tensors (bf16 bits as int16; vocab_map int32)."""
+    dev = torch.device("cuda", device)
+
+    def up(a):
+        return torch.from_numpy(np.ascontiguousarray(a).view(np.int16)).to(dev)
+
+    out = {"n_layers": int(pw["n_layers"]), "vocab": int(pw["vocab"]),
+           "vocab_map": torch.from_numpy(np.ascontiguousarray(pw["vocab_map"], dtype=np.int32)).to(dev)}
+    for k, v in pw.items():
+        if k in out:
+            continue
         out[k] = [up(x) for x in v] if isinstance(v, (list, tuple)) else up(v)
     return out
 
@@ -227,6 +254,51 @@ class SPD:
             self.close()
         except Exception:
             pass
+
+    # ------------------------------------------------------------------ NEXT-1: the paper's PDM
+    def attach_pdm(self, dev_pdm: dict):
+        """dev_pdm = upload_pdm_weights(spd_inputs.make_pdm_weights(...)).  Before prefill."""
+        cfg = _cfg_of(self.shape, self.max_seq, self.device)
+        sz = _PdmSizes()
+        self._check(lib().spd_pdm_query_sizes(C.byref(cfg), dev_pdm["n_layers"], dev_pdm["vocab"], C.byref(sz)))
+        dev = torch.device("cuda", self.device)
+        self._pdm_kv = torch.zeros(sz.kv_bytes, dtype=torch.uint8, device=dev)
+        self._pdm_work = torch.empty(sz.work_bytes, dtype=torch.uint8, device=dev)
+        self._pdm_w = dev_pdm
+        self.pdm_vocab = dev_pdm["vocab"]
+        w = _PdmWeights()
+        w.n_layers, w.vocab = dev_pdm["n_layers"], dev_pdm["vocab"]
+        for name in ["fc"] + _LAYER_NAMES:
+            ts = dev_pdm[name]
+            assert all(t.is_cuda and t.is_contiguous() and t.element_size() == 2 for t in ts)
+            tab = (C.c_void_p * len(ts))(*[t.data_ptr() for t in ts])
+            self._tabs.append(tab)
+            setattr(w, name, C.cast(tab, _PP))
+        w.final_norm, w.head = dev_pdm["final_norm"].data_ptr(), dev_pdm["head"].data_ptr()
+        assert dev_pdm["vocab_map"].dtype == torch.int32
+        w.vocab_map = dev_pdm["vocab_map"].data_ptr()
+        torch.cuda.synchronize(dev)
+        self._check(lib().spd_pdm_attach(self._h, C.byref(w), self._pdm_kv.data_ptr(), self._pdm_work.data_ptr()))
+
+    def pdm_run(self):
+        """(first position, rows, F) of the paper PDM's last draft."""
+        r = self.debug_read(DBG.PDM2_RUN, 0, np.int32, 3)
+        return int(r[0]), int(r[1]), int(r[2])
+
+    def pdm_last(self, what: str) -> np.ndarray:
+        if what == "logits":
+            return self.debug_read(DBG.PDM2_LOGITS, 0, np.float32, self.pdm_vocab)
+        if what == "hidden":
+            return self.debug_read(DBG.PDM2_HIDDEN, 0, np.float32, self.shape.d_model)
+        rows = self.pdm_run()[1]
+        return self.debug_read(DBG.PDM2_FEAT, rows, np.float32, rows * self.shape.d_model).reshape(rows, -1)
+
+    def pdm_kv(self, layer: int, which: int, rows: int) -> np.ndarray:
+        w = self.shape.n_kv_heads * self.shape.head_dim
+        return self.debug_read(DBG.PDM2_V if which else DBG.PDM2_K, layer, np.uint16, rows * w).reshape(rows, w)
+
+    def anchor(self, pos: int, i: int) -> np.ndarray:
+        return self.debug_read(DBG.ANCHOR, pos * 8 + i, np.float32, self.shape.d_model)
 
     # ------------------------------------------------------------------ the path
     def prefill(self, tokens) -> int:

@@ -24,6 +24,7 @@ struct spd_ctx {
   int engine;
   int has_mega;
   MegaPlan mega;
+  PdmPlan *pdm;            // the paper's PDM, if attached (spd_pdm_attach)
   int prefill_mode;        // 1: batched tensor-core prefill (spd_prefill.cu), 0: the decode kernel's prefill mode
   PrefillPlan *pf;
   StepResult *h_results;   // pinned
@@ -280,6 +281,7 @@ extern "C" int spd_destroy(spd_ctx *ctx) {
   cudaFreeHost(ctx->h_results);
   cudaFreeHost(ctx->h_state);
   free(ctx->pf);
+  pdm_destroy(ctx->pdm);
   free(ctx);
   return SPD_OK;
 }
@@ -288,6 +290,8 @@ extern "C" const char *spd_last_error(const spd_ctx *ctx) { return ctx ? ctx->er
 
 // ------------------------------------------------------------------ running cycles -------------
 static int enqueue_raw(spd_ctx *ctx, long long *cnt) {
+  // NEXT-1: the paper's PDM drafts from the pre-step state, in front of the cycle's kernels
+  if (ctx->pdm && pdm_enqueue_draft(ctx->P, ctx->pdm, ctx->sm, cnt)) return -1;
   if (ctx->engine == 1) return mega_enqueue_step(ctx->P, ctx->mega, ctx->sm, cnt);
   return ref_enqueue_step(ctx->P, ctx->sm, ctx->sp, ctx->ev_fork, ctx->ev_join, cnt);
 }
@@ -359,6 +363,10 @@ extern "C" int spd_prefill(spd_ctx *ctx, const int32_t *tokens, int32_t n_tokens
     k_set_mode<<<1, 1, 0, ctx->sm>>>(ctx->P, MODE_PREFILL_FINAL);
     ++ctx->launches;
   }
+  if (ctx->pdm && pdm_prefill(ctx->P, ctx->pdm, n_tokens, ctx->sm, &ctx->launches)) {
+    ctx->dead = 1;
+    return fail(ctx, SPD_ECUDA, "PDM prefill launch failed%s");
+  }
   int rc = enqueue_cycle(ctx);
   if (rc) return rc;
   CU(cudaMemcpyAsync(ctx->h_results, ctx->P.results, sizeof(StepResult), cudaMemcpyDeviceToHost, ctx->sm));
@@ -413,6 +421,7 @@ extern "C" int spd_rollback(spd_ctx *ctx, int32_t new_len, int32_t reseed_token)
   CU(cudaSetDevice(ctx->cfg.device));
   k_rollback<<<1, 256, 0, ctx->sm>>>(ctx->P, new_len, reseed_token);
   ++ctx->launches;
+  if (ctx->pdm) { pdm_rollback(ctx->pdm, new_len, ctx->sm); ++ctx->launches; }
   return sync_state(ctx);
 }
 
@@ -451,6 +460,7 @@ extern "C" int spd_set_sampling(spd_ctx *ctx, float temperature, int32_t top_k, 
   const int on = top_k >= 1;
   if (on && (top_k > kMaxTopK || !(temperature > 0.f))) return fail(ctx, SPD_EINVAL, "spd_set_sampling: bad arguments%s");
   if (on && ctx->forced_on) return fail(ctx, SPD_ESTATE, "spd_set_sampling: forced acceptance is on%s");
+  if (on && ctx->pdm) return fail(ctx, SPD_ESTATE, "spd_set_sampling: the paper's PDM is attached (greedy verification only)%s");
   CU(cudaSetDevice(ctx->cfg.device));
   if (ctx->P.sampling != on) { ctx->P.sampling = on; drop_graphs(ctx); }
   ctx->sampling_on = on;
@@ -522,6 +532,15 @@ extern "C" int spd_debug_read(spd_ctx *ctx, int32_t what, int32_t index, void *h
     case SPD_DBG_SAMPLE:
       if (!P.sampling) return fail(ctx, SPD_ESTATE, "debug_read: sampling verification is off%s");
       src = &P.samp->rec; want = sizeof(SampleRecord); break;
+    case SPD_DBG_PDM2_LOGITS: case SPD_DBG_PDM2_HIDDEN: case SPD_DBG_PDM2_RUN: case SPD_DBG_PDM2_FEAT:
+    case SPD_DBG_PDM2_K: case SPD_DBG_PDM2_V:
+      if (!ctx->pdm) return fail(ctx, SPD_ESTATE, "debug_read: the paper's PDM is not attached%s");
+      if (pdm_debug_read(P, ctx->pdm, what - SPD_DBG_PDM2_LOGITS, index, host_out, bytes))
+        return fail(ctx, SPD_EINVAL, "debug_read: bad PDM selector arguments%s");
+      return SPD_OK;
+    case SPD_DBG_ANCHOR:
+      if (!ctx->pdm || index < 0 || index / 8 >= D.max_seq || index % 8 >= P.pdm_m) return fail(ctx, SPD_EINVAL, "debug_read: bad anchor index%s");
+      src = P.anch + ((size_t)(index / 8) * P.pdm_m + index % 8) * D.d; want = sizeof(float) * D.d; break;
     case SPD_DBG_CYCLE_TIMES:
       src = P.cycle_ts; want = sizeof(unsigned long long) * 2 * kResultRing; break;
     case SPD_DBG_PHASE_PROFILE:
@@ -564,4 +583,29 @@ extern "C" int spd_op_gemm(const float *x, const uint16_t *w, int32_t m, int32_t
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return SPD_ECUDA;
   return prefill_op_gemm(x, w, m, n, k, y, scratch, (cudaStream_t)stream) == 0 ? SPD_OK : SPD_ECUDA;
+}
+
+// ------------------------------------------------------------------ the paper's PDM (NEXT-1) -------------------
+extern "C" int spd_pdm_query_sizes(const spd_config *cfg, int32_t pdm_layers, int32_t pdm_vocab, spd_pdm_sizes *out) {
+  if (!validate(cfg) || !out || pdm_layers < 1 || pdm_layers > kPrefillMaxLayers || pdm_vocab < 1 || pdm_vocab > cfg->vocab)
+    return SPD_EINVAL;
+  Dims D = make_dims(cfg);
+  out->kv_bytes = pdm_kv_bytes(D, pdm_layers);
+  out->work_bytes = pdm_work_bytes(D, pdm_layers, pdm_vocab);
+  return SPD_OK;
+}
+
+extern "C" int spd_pdm_attach(spd_ctx *ctx, const spd_pdm_weights *w, void *pdm_kv, void *pdm_work) {
+  if (!ctx) return SPD_EINVAL;
+  if (ctx->dead) return SPD_ECUDA;
+  if (ctx->prefilled || ctx->pdm) return fail(ctx, SPD_ESTATE, "spd_pdm_attach: attach once, before spd_prefill%s");
+  if (ctx->sampling_on) return fail(ctx, SPD_ESTATE, "spd_pdm_attach: sampling verification is on%s");
+  if (!w || !pdm_kv || !pdm_work || !w->fc || !w->attn_norm || !w->wq || !w->wk || !w->wv || !w->wo || !w->mlp_norm ||
+      !w->w_gate || !w->w_up || !w->w_down || !w->final_norm || !w->head || !w->vocab_map)
+    return fail(ctx, SPD_EINVAL, "spd_pdm_attach: missing argument%s");
+  CU(cudaSetDevice(ctx->cfg.device));
+  ctx->pdm = pdm_create(&ctx->P, w, pdm_kv, pdm_work, ctx->sm);
+  if (!ctx->pdm) return fail(ctx, SPD_EINVAL, "spd_pdm_attach: bad PDM configuration%s");
+  drop_graphs(ctx);   // the kernels' parameters changed
+  return SPD_OK;
 }

@@ -124,6 +124,12 @@ struct DevPtrs {
   int32_t *samp_idx;                 // [kSampCap]
   float *pre_val;                    // [2][kSampCap] logits >= tau_guess listed by the fused head pass
   int32_t *pre_idx;                  // [2][kSampCap]
+  // the paper's Pipeline Draft Module (spd_pdm.cu, NEXT-1); paper_pdm == 0: the simplified PDM of BASELINE.json
+  int32_t paper_pdm;
+  int32_t pdm_m;                     // anchors
+  int32_t pdm_anchor[8];             // B = [0, L/4, L/2, 3L/4, L-1]
+  float *anch;                       // [max_seq][m][d] H_pos^{b_i}: the residual stream entering layer b_i
+  int32_t *pdm_draft;                // the token the paper's PDM drafted for this cycle
   // batched prefill scratch (spd_prefill.cu), sized for pf_chunk tokens
   float *pf_H;                       // [pf_chunk][d] residual streams of the chunk
   float *pf_Q;                       // [pf_chunk][Hq*hd] q after RoPE
@@ -156,6 +162,14 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
   return t;
+}
+
+// Anchor index of `layer` in the paper PDM's anchor set, or -1.
+__device__ __forceinline__ int anchor_index(const DevPtrs &P, int layer) {
+  if (!P.paper_pdm) return -1;
+  for (int i = 0; i < P.pdm_m; ++i)
+    if (P.pdm_anchor[i] == layer) return i;
+  return -1;
 }
 
 __device__ __forceinline__ float warp_sum(float v) {

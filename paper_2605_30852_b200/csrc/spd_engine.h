@@ -39,4 +39,21 @@ int prefill_create(const DevPtrs &P, const uint16_t *const *const *src, PrefillP
 int prefill_run(const DevPtrs &P, const PrefillPlan &plan, int n_tokens, cudaStream_t st, long long *launches);
 int prefill_op_gemm(const float *x, const uint16_t *w, int M, int N, int K, float *y, void *scratch, cudaStream_t st);
 
+
+// The paper's Pipeline Draft Module (spd_pdm.cu).
+constexpr int kPdmMaxRows = 40;          // >= kMaxStages + 1 rows per draft (n + 1)
+struct PdmPlan;
+}  // namespace spd
+struct spd_pdm_weights;
+namespace spd {
+int pdm_anchor_set(int L, int32_t *b);
+size_t pdm_kv_bytes(const Dims &D, int Ls);
+size_t pdm_work_bytes(const Dims &D, int Ls, int Vs);
+PdmPlan *pdm_create(DevPtrs *P, const ::spd_pdm_weights *w, void *kv, void *work, cudaStream_t st);
+void pdm_destroy(PdmPlan *plan);
+int pdm_enqueue_draft(const DevPtrs &P, const PdmPlan *pl, cudaStream_t st, long long *launches);
+int pdm_prefill(const DevPtrs &P, const PdmPlan *pl, int n_tokens, cudaStream_t st, long long *launches);
+int pdm_rollback(const PdmPlan *pl, int new_len, cudaStream_t st);
+int pdm_debug_read(const DevPtrs &P, const PdmPlan *pl, int what, int index, void *out, size_t bytes);
+
 }  // namespace spd

@@ -156,7 +156,7 @@ __device__ __forceinline__ void controller_begin(const DevPtrs &P) {
   for (int k = 0; k < n; ++k) fill += st->occ[k];
   st->fill = fill;
   st->p_new = st->occ[0] ? st->pos[0] : -1;
-  st->run_pdm = st->mode == MODE_SPD;
+  st->run_pdm = st->mode == MODE_SPD && !P.paper_pdm;   // the paper's PDM runs in its own kernels before the cycle
   st->run_verify = (st->mode == MODE_SPD && st->occ[n - 1]) || st->mode == MODE_PREFILL_FINAL;
   st->forced_now = 0;
   if (st->mode == MODE_SPD) {
@@ -485,6 +485,7 @@ __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, Samp
     int enter_tok = -1, enter_pos = -1;
     bool flush = false;
     if (mode == MODE_SPD) {
+      if (P.paper_pdm) draft = *P.pdm_draft;        // NEXT-1: drafted by spd_pdm.cu's kernels on the pre-step state
       if (st->forced_now) { draft = P.truth[st->p_new + 1 - st->prompt_len]; r.draft_forced = 1; }
       r.draft_token = draft;
       if (exited) {

@@ -889,7 +889,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
     }
     S.n_act = a;
     S.p_new = st->occ[0] ? st->pos[0] : -1;
-    S.run_pdm = st->mode == MODE_SPD;
+    S.run_pdm = st->mode == MODE_SPD && !P.paper_pdm;
     S.run_verify = (st->mode == MODE_SPD && st->occ[D.n - 1]) || st->mode == MODE_PREFILL_FINAL;
     // CTA c serves active stage c mod a (every group gets the same mix of SMs); PDM slot c mod n
     S.my_stage = a > 0 ? S.act[cta % a] : -1;
@@ -1118,6 +1118,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_spd_cycle(DevPtrs P, MegaLayout
             const float *h = P.h + (size_t)S.hbuf[k] * D.d;
             const uint16_t *g = t == PH_QKV ? P.attn_norm[layer] : P.mlp_norm[layer];
             float ss = consumer_sum(stage_copy(h, xs, D.d), red);
+            if (t == PH_QKV && S.my_idx == 0) {   // NEXT-1: H^layer of the paper PDM's anchor set (the raw residual stream)
+              const int ai = anchor_index(P, layer);
+              if (ai >= 0 && S.pos[k] < D.max_seq) {
+                float4 *dst = reinterpret_cast<float4 *>(P.anch + ((size_t)S.pos[k] * P.pdm_m + ai) * D.d);
+                const float4 *src = reinterpret_cast<const float4 *>(xs);
+                for (int i = tid; i < (D.d >> 2); i += kConsumerThreads) dst[i] = src[i];   // this thread's own float4s
+              }
+            }
             stage_scale(xs, g, D.d, 1.0f / sqrtf(ss / (float)D.d + D.eps));
             K = D.d;
           } else if (t == PH_O) {

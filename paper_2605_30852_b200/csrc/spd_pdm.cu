@@ -1,0 +1,496 @@
+// spd_pdm.cu — the paper's Pipeline Draft Module on the device.
+//
+// PAPER.md:71 "an L_s-layer Transformer decoder with an independent LM head"; :91-100 Eq. 3-4: anchors B (b_0 = 0;
+// [0, 8, 16, 24, 31] for L = 32), l_max(k) = min(L, k L/n), f(k) = max{i | b_i <= l_max(k)},
+// g_t^k = FC_f(k)(Concat(H_t^b0 .. H_t^bf(k))); :102-107 Eq. 5 warm-up layout; :115 pre-step features; :139 reduced
+// vocabulary head; :299 "caching appends only the trailing (n+1) refreshed features each step".
+//
+// One draft = a short kernel sequence on the cycle's stream BEFORE the cycle kernel (pre-step state, no dependency on
+// the cycle's forward):  k_pdm_begin (which rows: positions F .. p_new, their depths; F := c) -> k_pdm_features (Eq. 4,
+// one GEMV per row against FC_f(k)) -> per PDM layer: RMSNorm, QKV, RoPE + bf16 append into the PDM's own cache (rows are
+// REwritten: in-flight features deepen every cycle), split-KV attention, O + residual, RMSNorm, gate/up + SiLU.mul,
+// down + residual -> RMSNorm + head GEMV over the reduced vocabulary -> argmax -> vocab_map -> the token the controller
+// of the cycle kernel enters into stage 0.  M = rows <= n + 1 vectors share every weight row that is streamed (the
+// M = 2 head pass of the cycle kernel generalised); a row's result never depends on which other rows share the pass.
+// The paper hides this work on a dedicated GPU; on one GPU its bytes come out of the same HBM, so it is
+// reported as what it costs.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/spd.h"
+#include "spd_engine.h"
+#include "spd_kernels.cuh"
+
+namespace spd {
+
+struct PdmRun {                       // written by k_pdm_begin, read by every other kernel of the draft
+  int32_t first, rows, final_len;     // rows = positions first .. first + rows - 1; final_len = F
+  int32_t depth[kPdmMaxRows];         // completed stages k of each row's token (n: committed)
+  int32_t f[kPdmMaxRows];             // Eq. 3
+  int32_t hbuf[kPdmMaxRows];          // in-flight rows: hidden buffer of the token (its current residual stream); else -1
+};
+
+struct PdmPtrs {
+  int32_t Ls, Vs;
+  PdmRun *run;
+  float *G, *X, *XN, *Y, *Q, *ATT, *ACT;      // [kPdmMaxRows][d | d | d | max(qd + 2 kd, 2 F) | qd | qd | F]
+  float *part_o;                      // [kPdmMaxRows][Hq][nsplit][hd]
+  float2 *part_ml;
+  float *logits, *z;                  // [Vs], [d]
+  float *cand_val;                    // [kPdmCand]
+  int32_t *cand_idx;
+  uint16_t *kv;                       // the PDM's own cache: [L_s][K|V][kv head][max_seq][hd] bf16
+  const uint16_t *const *fc;          // device table of the m FC matrices (selected per row by f(k))
+  const uint16_t *final_norm, *head;
+  const int32_t *vocab_map;
+};
+constexpr int kPdmCand = 128;
+
+// ------------------------------------------------------------------ which rows ---------------------------------
+// fixed_rows > 0: PDM prefill chunk (committed positions, depth n); else the cycle's rows from the device state.
+__global__ void k_pdm_begin(DevPtrs P, PdmPtrs PD, int fixed_first, int fixed_rows) {
+  if (threadIdx.x != 0) return;
+  const Dims &D = P.dim;
+  PdmRun *R = PD.run;
+  const StepState *st = P.st;
+  int first, rows;
+  if (fixed_rows > 0) { first = fixed_first; rows = fixed_rows; }
+  else if (st->mode != MODE_SPD || !st->occ[0]) { R->rows = 0; return; }
+  else { first = R->final_len; rows = st->pos[0] - first + 1; }
+  if (rows < 1 || rows > kPdmMaxRows) { P.st->err = 2; R->rows = 0; return; }
+  for (int r = 0; r < rows; ++r) {
+    const int q = first + r;
+    int k = D.n, hb = -1;
+    if (fixed_rows <= 0 && q >= st->c) {          // in flight: depth = stages completed BEFORE this cycle's forward
+      k = st->pos[0] - q;
+      if (k < 0 || k >= D.n || !st->occ[k] || st->pos[k] != q) { P.st->err = 2; R->rows = 0; return; }
+      hb = st->hbuf[k];
+    }
+    const int lmax = min(D.L, k * D.per);
+    int f = 0;
+    for (int i = 0; i < P.pdm_m; ++i)
+      if (P.pdm_anchor[i] <= lmax) f = i;
+    R->depth[r] = k; R->f[r] = f; R->hbuf[r] = hb;
+  }
+  R->first = first; R->rows = rows;
+  if (fixed_rows <= 0) R->final_len = st->c;       // rows below c were built at depth n: final
+}
+
+__global__ void k_pdm_set_final(PdmPtrs PD, int final_len, int only_lower) {
+  if (!only_lower || PD.run->final_len > final_len) PD.run->final_len = final_len;
+}
+
+// ------------------------------------------------------------------ Eq. 4: g = FC_f . Concat(anchors) ------------
+// grid (ceil(d / 8), kPdmMaxRows); a warp per output element.  An in-flight token's deepest eligible anchor
+// H^{k L/n} is the residual stream it currently holds (k = 0: the embedding row).
+__global__ void k_pdm_features(DevPtrs P, PdmPtrs PD) {
+  const Dims &D = P.dim;
+  const PdmRun *R = PD.run;
+  const int r = blockIdx.y;
+  if (r >= R->rows) return;
+  const int o = blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (o >= D.d) return;
+  const int f = R->f[r], q = R->first + r, k = R->depth[r], hb = R->hbuf[r];
+  const uint16_t *wrow = PD.fc[f] + (size_t)o * (f + 1) * D.d;
+  float acc = 0.f;
+  for (int i = 0; i <= f; ++i) {
+    const float *src = (hb >= 0 && P.pdm_anchor[i] == k * D.per) ? P.h + (size_t)hb * D.d
+                                                                 : P.anch + ((size_t)q * P.pdm_m + i) * D.d;
+    acc += warp_dot_row(wrow + (size_t)i * D.d, src, D.d);
+  }
+  if ((threadIdx.x & 31) == 0) { PD.X[(size_t)r * D.d + o] = acc; PD.G[(size_t)r * D.d + o] = acc; }
+}
+
+// XN[r] = RMSNorm(X[r]; gain); grid kPdmMaxRows.  last_only: only the last row (head input, final norm), into PD.z.
+__global__ void k_pdm_norm(DevPtrs P, PdmPtrs PD, const uint16_t *gain, int last_only) {
+  __shared__ float red[33];
+  const PdmRun *R = PD.run;
+  const Dims &D = P.dim;
+  int r = blockIdx.x;
+  if (last_only) { if (r != 0 || R->rows < 1) return; r = R->rows - 1; }
+  else if (r >= R->rows) return;
+  const uint16_t *g = last_only ? PD.final_norm : gain;
+  block_rmsnorm(PD.X + (size_t)r * D.d, g, D.d, D.eps, last_only ? PD.z : PD.XN + (size_t)r * D.d, red);
+}
+
+// ------------------------------------------------------------------ M-row GEMV ----------------------------------
+// Y[r][col0_s + n] (+)= W_s[n] . X[r] for every row r of the run and up to three weight matrices (segments) that share X.
+// A warp owns 4 consecutive weight rows and streams them once; 8 x-rows per pass share every 16-byte weight chunk.
+// Lane l takes the 8-element chunks l, l + 32, ...; one fp32 FMA chain per (weight row, x row), then the xor tree:
+// a value depends only on (weight row, x row), never on the batch.
+struct RowsGemv {
+  const uint16_t *w[3];
+  int n[3], col0[3];
+  int nseg, K, ldx, ldy, residual, last_only;
+  const float *x;
+  float *y;
+};
+
+__global__ void __launch_bounds__(256) k_pdm_rows_gemv(PdmPtrs PD, RowsGemv A) {
+  const PdmRun *R = PD.run;
+  int rows = R->rows, r_first = 0;
+  if (rows < 1) return;
+  if (A.last_only) { r_first = 0; rows = 1; }        // x and y are single vectors (the head: x = PD.z)
+  const int lane = threadIdx.x & 31;
+  int n4 = (blockIdx.x * 8 + (threadIdx.x >> 5)) * 4, seg = 0;     // first of this warp's 4 weight rows
+  while (seg < A.nseg && n4 >= ((A.n[seg] + 3) & ~3)) { n4 -= (A.n[seg] + 3) & ~3; ++seg; }
+  if (seg >= A.nseg) return;
+  const int nrow = A.n[seg], nchunk = A.K >> 3;
+  const uint4 *wp[4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) wp[j] = reinterpret_cast<const uint4 *>(A.w[seg] + (size_t)min(n4 + j, nrow - 1) * A.K);
+  for (int rb = 0; rb < rows; rb += 8) {
+    const int nr = min(8, rows - rb);
+    float acc[4][8];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+      for (int r = 0; r < 8; ++r) acc[j][r] = 0.f;
+    for (int c = lane; c < nchunk; c += 32) {
+      uint4 wv[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) wv[j] = __ldg(wp[j] + c);
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        if (r < nr) {
+          const float4 *xp = reinterpret_cast<const float4 *>(A.x + (size_t)(r_first + rb + r) * A.ldx) + 2 * c;
+          const float4 xa = xp[0], xb = xp[1];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            float a = acc[j][r];
+            a = fmaf(bf16_lo(wv[j].x), xa.x, a); a = fmaf(bf16_hi(wv[j].x), xa.y, a);
+            a = fmaf(bf16_lo(wv[j].y), xa.z, a); a = fmaf(bf16_hi(wv[j].y), xa.w, a);
+            a = fmaf(bf16_lo(wv[j].z), xb.x, a); a = fmaf(bf16_hi(wv[j].z), xb.y, a);
+            a = fmaf(bf16_lo(wv[j].w), xb.z, a); a = fmaf(bf16_hi(wv[j].w), xb.w, a);
+            acc[j][r] = a;
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const float v = warp_sum(acc[j][r]);
+        if (lane == 0 && r < nr && n4 + j < nrow) {
+          float *dst = A.y + (size_t)(A.last_only ? 0 : rb + r) * A.ldy + A.col0[seg] + n4 + j;
+          *dst = A.residual ? *dst + v : v;
+        }
+      }
+  }
+}
+
+// Y row = [q | k | v]: RoPE (C-2.14) on q and k; q -> Q; k, v -> bf16 rows of the PDM cache at the row's position
+// (REwritten every cycle for in-flight positions).  grid kPdmMaxRows.
+__global__ void k_pdm_rope_append(DevPtrs P, PdmPtrs PD, int layer) {
+  const Dims &D = P.dim;
+  const PdmRun *R = PD.run;
+  __shared__ float2 cs[64];
+  const int r = blockIdx.x;
+  if (r >= R->rows) return;
+  const int pos = R->first + r, half = D.hd / 2, qd = D.Hq * D.hd, kd = D.Hkv * D.hd, ldy = qd + 2 * kd;
+  if (threadIdx.x < half) {
+    double s_, c_;
+    sincos((double)pos * P.inv_freq[threadIdx.x], &s_, &c_);
+    cs[threadIdx.x] = make_float2((float)c_, (float)s_);
+  }
+  __syncthreads();
+  const float *y = PD.Y + (size_t)r * ldy;
+  for (int j = threadIdx.x; j < (D.Hq + D.Hkv) * half; j += blockDim.x) {
+    const int hh = j / half, i = j - hh * half;
+    const float2 c = cs[i];
+    if (hh < D.Hq) {
+      const float a = y[hh * D.hd + i], b = y[hh * D.hd + i + half];
+      float *q = PD.Q + (size_t)r * qd + hh * D.hd;
+      q[i] = a * c.x - b * c.y;
+      q[i + half] = b * c.x + a * c.y;
+    } else {
+      const int kh = hh - D.Hq;
+      const float a = y[qd + kh * D.hd + i], b = y[qd + kh * D.hd + i + half];
+      uint16_t *dst = PD.kv + kv_offset(D, layer, 0, kh) + (size_t)pos * D.hd;
+      dst[i] = f32_to_bf16(a * c.x - b * c.y);
+      dst[i + half] = f32_to_bf16(b * c.x + a * c.y);
+    }
+  }
+  for (int j = threadIdx.x; j < kd; j += blockDim.x) {
+    const int kh = j / D.hd, i = j - kh * D.hd;
+    PD.kv[kv_offset(D, layer, 1, kh) + (size_t)pos * D.hd + i] = f32_to_bf16(y[qd + kd + j]);
+  }
+}
+
+// Split-KV attention of every row over the PDM cache rows 0 .. pos (fixed 128-row splits merged in split order, as the
+// target's): grid (split, kv head, kPdmMaxRows), one warp per q head of the group.
+template <int HD>
+__global__ void k_pdm_attn_partial(DevPtrs P, PdmPtrs PD, int layer) {
+  const Dims &D = P.dim;
+  const PdmRun *R = PD.run;
+  const int r = blockIdx.z;
+  if (r >= R->rows) return;
+  const int T = R->first + r + 1, split = blockIdx.x, t0 = split * kAttnSplit;
+  if (t0 >= T) return;
+  const int t1 = min(T, t0 + kAttnSplit), kvh = blockIdx.y, group = D.Hq / D.Hkv;
+  const int hq = kvh * group + (threadIdx.x >> 5);
+  const uint16_t *kc = PD.kv + kv_offset(D, layer, 0, kvh), *vc = PD.kv + kv_offset(D, layer, 1, kvh);
+  const size_t slot = ((size_t)r * D.Hq + hq) * P.nsplit_max + split;
+  attn_partial_warp<HD>(PD.Q + ((size_t)r * D.Hq + hq) * HD, kc, vc, t0, t1, PD.part_o + slot * HD, PD.part_ml + slot);
+}
+
+// grid (q head, kPdmMaxRows); block = hd threads
+__global__ void k_pdm_attn_merge(DevPtrs P, PdmPtrs PD) {
+  const Dims &D = P.dim;
+  const PdmRun *R = PD.run;
+  const int r = blockIdx.y, hq = blockIdx.x;
+  if (r >= R->rows) return;
+  const int nsplit = (R->first + r + kAttnSplit) / kAttnSplit;
+  const size_t slot = ((size_t)r * D.Hq + hq) * P.nsplit_max;
+  PD.ATT[((size_t)r * D.Hq + hq) * D.hd + threadIdx.x] =
+      attn_merge_elem(PD.part_o + slot * D.hd, PD.part_ml + slot, nsplit, D.hd, threadIdx.x);
+}
+
+// ACT[r] = silu(gate) * up; Y row = [gate (F) | up (F)]
+__global__ void k_pdm_silu(DevPtrs P, PdmPtrs PD) {
+  const Dims &D = P.dim;
+  const int r = blockIdx.y;
+  if (r >= PD.run->rows) return;
+  const float *y = PD.Y + (size_t)r * 2 * D.F;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < D.F; i += gridDim.x * blockDim.x)
+    PD.ACT[(size_t)r * D.F + i] = silu_mul(y[i], y[D.F + i]);
+}
+
+// argmax (max value, lowest index) of the reduced-vocabulary logits -> the drafted TARGET token id.
+__global__ void k_pdm_argmax_cand(PdmPtrs PD) {
+  __shared__ float sv[32];
+  __shared__ int si[32];
+  if (PD.run->rows < 1) return;
+  const int V = PD.Vs, chunk = (V + gridDim.x - 1) / gridDim.x;
+  const int lo = blockIdx.x * chunk, hi = min(V, lo + chunk);
+  float bv = -INFINITY;
+  int bi = 0x7fffffff;
+  for (int i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+    const float v = PD.logits[i];
+    if (cand_better(v, i, bv, bi)) { bv = v; bi = i; }
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+    if (cand_better(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+  }
+  if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = bv; si[threadIdx.x >> 5] = bi; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w)
+      if (cand_better(sv[w], si[w], bv, bi)) { bv = sv[w]; bi = si[w]; }
+    PD.cand_val[blockIdx.x] = bv;
+    PD.cand_idx[blockIdx.x] = lo < hi ? bi : -1;
+  }
+}
+__global__ void k_pdm_argmax_final(DevPtrs P, PdmPtrs PD) {
+  if (threadIdx.x != 0 || PD.run->rows < 1) return;
+  float bv = -INFINITY;
+  int bi = 0x7fffffff;
+  for (int i = 0; i < kPdmCand; ++i)
+    if (PD.cand_idx[i] >= 0 && cand_better(PD.cand_val[i], PD.cand_idx[i], bv, bi)) { bv = PD.cand_val[i]; bi = PD.cand_idx[i]; }
+  *P.pdm_draft = PD.vocab_map[bi];
+}
+
+// ------------------------------------------------------------------ host side ----------------------------------
+struct PdmPlan {
+  PdmPtrs PD;
+  int Ls, Vs;
+  const uint16_t *w[9][kPrefillMaxLayers];   // host copy of the per-layer device pointers
+};
+
+static size_t pdm_carve(const Dims &D, int Ls, int Vs, int m, int nsplit, void *base, PdmPtrs *PD, float **anch,
+                        int32_t **draft) {
+  char *b = (char *)base;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { off = (off + 255) & ~(size_t)255; void *p = b ? b + off : nullptr; off += bytes; return p; };
+  const size_t R = kPdmMaxRows, qd = (size_t)D.Hq * D.hd, kd = (size_t)D.Hkv * D.hd;
+  const size_t ymax = qd + 2 * kd > 2 * (size_t)D.F ? qd + 2 * kd : 2 * (size_t)D.F;
+  PdmPtrs Q;
+  memset(&Q, 0, sizeof Q);
+  Q.Ls = Ls; Q.Vs = Vs;
+  Q.run = (PdmRun *)take(sizeof(PdmRun));
+  Q.G = (float *)take(R * D.d * 4); Q.X = (float *)take(R * D.d * 4); Q.XN = (float *)take(R * D.d * 4);
+  Q.Y = (float *)take(R * ymax * 4); Q.Q = (float *)take(R * qd * 4); Q.ATT = (float *)take(R * qd * 4);
+  Q.ACT = (float *)take(R * D.F * 4);
+  Q.part_o = (float *)take(R * D.Hq * nsplit * D.hd * 4);
+  Q.part_ml = (float2 *)take(R * D.Hq * nsplit * 8);
+  Q.logits = (float *)take((size_t)Vs * 4); Q.z = (float *)take((size_t)D.d * 4);
+  Q.cand_val = (float *)take(kPdmCand * 4); Q.cand_idx = (int32_t *)take(kPdmCand * 4);
+  Q.fc = (const uint16_t *const *)take(8 * sizeof(void *));
+  int32_t *dr = (int32_t *)take(64);
+  float *an = (float *)take((size_t)D.max_seq * m * D.d * 4);
+  if (PD) *PD = Q;
+  if (anch) *anch = an;
+  if (draft) *draft = dr;
+  return (off + 255) & ~(size_t)255;
+}
+
+int pdm_anchor_set(int L, int32_t *b) {
+  int cand[5] = {0, L / 4, L / 2, (3 * L) / 4, L - 1}, m = 0;
+  for (int i = 0; i < 5; ++i)
+    if (m == 0 || cand[i] > b[m - 1]) b[m++] = cand[i];
+  return m;
+}
+
+size_t pdm_kv_bytes(const Dims &D, int Ls) { return (size_t)Ls * 2 * D.Hkv * D.max_seq * D.hd * sizeof(uint16_t); }
+size_t pdm_work_bytes(const Dims &D, int Ls, int Vs) {
+  int32_t b[8];
+  const int m = pdm_anchor_set(D.L, b);
+  return pdm_carve(D, Ls, Vs, m, (D.max_seq + kAttnSplit - 1) / kAttnSplit, nullptr, nullptr, nullptr, nullptr);
+}
+
+PdmPlan *pdm_create(DevPtrs *P, const spd_pdm_weights *w, void *kv, void *work, cudaStream_t st) {
+  const Dims &D = P->dim;
+  if (w->n_layers < 1 || w->n_layers > kPrefillMaxLayers || w->vocab < 1 || w->vocab > D.V) return nullptr;
+  PdmPlan *plan = (PdmPlan *)calloc(1, sizeof(PdmPlan));
+  if (!plan) return nullptr;
+  int32_t b[8];
+  const int m = pdm_anchor_set(D.L, b);
+  float *anch;
+  int32_t *draft;
+  const size_t bytes = pdm_carve(D, w->n_layers, w->vocab, m, P->nsplit_max, work, &plan->PD, &anch, &draft);
+  plan->Ls = w->n_layers; plan->Vs = w->vocab;
+  plan->PD.kv = (uint16_t *)kv;
+  plan->PD.final_norm = w->final_norm; plan->PD.head = w->head; plan->PD.vocab_map = w->vocab_map;
+  const uint16_t *const *src[9] = {w->attn_norm, w->wq, w->wk, w->wv, w->wo, w->mlp_norm, w->w_gate, w->w_up, w->w_down};
+  for (int i = 0; i < 9; ++i)
+    for (int l = 0; l < w->n_layers; ++l) {
+      if (!src[i][l]) { free(plan); return nullptr; }
+      plan->w[i][l] = src[i][l];
+    }
+  for (int i = 0; i < m; ++i)
+    if (!w->fc[i]) { free(plan); return nullptr; }
+  if (cudaMemsetAsync(work, 0, bytes - (size_t)D.max_seq * m * D.d * 4, st) != cudaSuccess ||
+      cudaMemcpyAsync((void *)plan->PD.fc, w->fc, sizeof(void *) * m, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+      cudaStreamSynchronize(st) != cudaSuccess) {
+    free(plan);
+    return nullptr;
+  }
+  P->paper_pdm = 1; P->pdm_m = m;
+  for (int i = 0; i < m; ++i) P->pdm_anchor[i] = b[i];
+  P->anch = anch; P->pdm_draft = draft;
+  return plan;
+}
+
+void pdm_destroy(PdmPlan *plan) { free(plan); }
+
+static int pdm_launch_gemv(const PdmPlan *pl, const uint16_t *const *w, const int *n, int nseg, int K, const float *x, int ldx,
+                           float *y, int ldy, int residual, int last_only, cudaStream_t st) {
+  RowsGemv A;
+  memset(&A, 0, sizeof A);
+  int total4 = 0, col = 0;
+  for (int s = 0; s < nseg; ++s) {
+    A.w[s] = w[s]; A.n[s] = n[s]; A.col0[s] = col;
+    col += n[s];
+    total4 += (n[s] + 3) / 4;
+  }
+  A.nseg = nseg; A.K = K; A.ldx = ldx; A.ldy = ldy; A.residual = residual; A.last_only = last_only; A.x = x; A.y = y;
+  k_pdm_rows_gemv<<<(total4 + 7) / 8, 256, 0, st>>>(pl->PD, A);
+  return 0;
+}
+
+// The kernels of one draft after k_pdm_begin (shared by the cycle and the PDM prefill).
+static void pdm_enqueue_body(const DevPtrs &P, const PdmPlan *pl, bool head, cudaStream_t st, long long *cnt) {
+  const Dims &D = P.dim;
+  const PdmPtrs &PD = pl->PD;
+  const int R = kPdmMaxRows, qd = D.Hq * D.hd, kd = D.Hkv * D.hd, group = D.Hq / D.Hkv;
+  k_pdm_features<<<dim3((D.d + 7) / 8, R), 256, 0, st>>>(P, PD); ++*cnt;
+  for (int l = 0; l < pl->Ls; ++l) {
+    k_pdm_norm<<<R, 256, 0, st>>>(P, PD, pl->w[0][l], 0); ++*cnt;
+    const uint16_t *wqkv[3] = {pl->w[1][l], pl->w[2][l], pl->w[3][l]};
+    const int nqkv[3] = {qd, kd, kd};
+    pdm_launch_gemv(pl, wqkv, nqkv, 3, D.d, PD.XN, D.d, PD.Y, qd + 2 * kd, 0, 0, st); ++*cnt;
+    k_pdm_rope_append<<<R, 256, 0, st>>>(P, PD, l); ++*cnt;
+    dim3 ga(P.nsplit_max, D.Hkv, R);
+    if (D.hd == 128) k_pdm_attn_partial<128><<<ga, group * 32, 0, st>>>(P, PD, l);
+    else k_pdm_attn_partial<64><<<ga, group * 32, 0, st>>>(P, PD, l);
+    ++*cnt;
+    k_pdm_attn_merge<<<dim3(D.Hq, R), D.hd, 0, st>>>(P, PD); ++*cnt;
+    const uint16_t *wo[1] = {pl->w[4][l]};
+    const int nd[1] = {D.d};
+    pdm_launch_gemv(pl, wo, nd, 1, qd, PD.ATT, qd, PD.X, D.d, 1, 0, st); ++*cnt;
+    k_pdm_norm<<<R, 256, 0, st>>>(P, PD, pl->w[5][l], 0); ++*cnt;
+    const uint16_t *wgu[2] = {pl->w[6][l], pl->w[7][l]};
+    const int ngu[2] = {D.F, D.F};
+    pdm_launch_gemv(pl, wgu, ngu, 2, D.d, PD.XN, D.d, PD.Y, 2 * D.F, 0, 0, st); ++*cnt;
+    k_pdm_silu<<<dim3((D.F + 255) / 256, R), 256, 0, st>>>(P, PD); ++*cnt;
+    const uint16_t *wd[1] = {pl->w[8][l]};
+    pdm_launch_gemv(pl, wd, nd, 1, D.F, PD.ACT, D.F, PD.X, D.d, 1, 0, st); ++*cnt;
+  }
+  if (head) {
+    k_pdm_norm<<<1, 256, 0, st>>>(P, PD, nullptr, 1); ++*cnt;
+    const uint16_t *wh[1] = {PD.head};
+    const int nv[1] = {pl->Vs};
+    pdm_launch_gemv(pl, wh, nv, 1, D.d, PD.z, D.d, PD.logits, pl->Vs, 0, 1, st); ++*cnt;
+    k_pdm_argmax_cand<<<kPdmCand, 256, 0, st>>>(PD); ++*cnt;
+    k_pdm_argmax_final<<<1, 32, 0, st>>>(P, PD); ++*cnt;
+  }
+}
+
+// The draft of one cycle, enqueued in front of the cycle kernel.
+int pdm_enqueue_draft(const DevPtrs &P, const PdmPlan *pl, cudaStream_t st, long long *launches) {
+  long long cnt = 0;
+  k_pdm_begin<<<1, 32, 0, st>>>(P, pl->PD, 0, 0); ++cnt;
+  pdm_enqueue_body(P, pl, true, st, &cnt);
+  if (launches) *launches += cnt;
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+// After the target's prefill: the full-depth rows of positions 0 .. n_tokens - 1, then F = n_tokens.
+int pdm_prefill(const DevPtrs &P, const PdmPlan *pl, int n_tokens, cudaStream_t st, long long *launches) {
+  long long cnt = 0;
+  const int RB = 32;
+  for (int p0 = 0; p0 < n_tokens; p0 += RB) {
+    const int rows = n_tokens - p0 < RB ? n_tokens - p0 : RB;
+    k_pdm_begin<<<1, 32, 0, st>>>(P, pl->PD, p0, rows); ++cnt;
+    pdm_enqueue_body(P, pl, false, st, &cnt);
+  }
+  k_pdm_set_final<<<1, 1, 0, st>>>(pl->PD, n_tokens, 0); ++cnt;
+  if (launches) *launches += cnt;
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+int pdm_rollback(const PdmPlan *pl, int new_len, cudaStream_t st) {
+  k_pdm_set_final<<<1, 1, 0, st>>>(pl->PD, new_len, 1);
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+// what: 0 logits [Vs], 1 last row's hidden state [d], 2 run header int32[3] (first, rows, F), 3 features G [rows][d]
+// (index = rows), 4 / 5 K / V rows of PDM layer `index` ([rows][Hkv*hd], rows = bytes / row size)
+int pdm_debug_read(const DevPtrs &P, const PdmPlan *pl, int what, int index, void *out, size_t bytes) {
+  const Dims &D = P.dim;
+  const PdmPtrs &PD = pl->PD;
+  PdmRun run;
+  if (cudaMemcpy(&run, PD.run, sizeof run, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+  if (what == 0) return bytes == (size_t)pl->Vs * 4 && cudaMemcpy(out, PD.logits, bytes, cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : -1;
+  if (what == 1) {
+    if (bytes != (size_t)D.d * 4 || run.rows < 1) return -1;
+    return cudaMemcpy(out, PD.X + (size_t)(run.rows - 1) * D.d, bytes, cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : -1;
+  }
+  if (what == 2) {
+    if (bytes != 12) return -1;
+    int32_t h[3] = {run.first, run.rows, run.final_len};
+    memcpy(out, h, 12);
+    return 0;
+  }
+  if (what == 3) {
+    if (index != run.rows || bytes != (size_t)run.rows * D.d * 4) return -1;
+    return cudaMemcpy(out, PD.G, bytes, cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : -1;
+  }
+  if (what == 4 || what == 5) {
+    const size_t rowb = (size_t)D.Hkv * D.hd * 2;
+    if (index < 0 || index >= pl->Ls || bytes % rowb || bytes / rowb > (size_t)D.max_seq) return -1;
+    const size_t rows = bytes / rowb;
+    for (int hh = 0; hh < D.Hkv && rows; ++hh)
+      if (cudaMemcpy2D((char *)out + (size_t)hh * D.hd * 2, rowb, PD.kv + kv_offset(D, index, what == 5, hh), (size_t)D.hd * 2,
+                       (size_t)D.hd * 2, rows, cudaMemcpyDeviceToHost) != cudaSuccess)
+        return -1;
+    return 0;
+  }
+  return -1;
+}
+
+}  // namespace spd

@@ -301,6 +301,15 @@ __global__ void k_pf_silu_split(const float *Y, int ldy, int F, int M, uint16_t 
   }
 }
 
+// NEXT-1: H^layer of the paper PDM's anchor set for the chunk's positions: anch[p0 + t][ai] = H[t]
+__global__ void k_pf_store_anchor(const float *H, float *anch, int p0, int d, int M, int m, int ai) {
+  const size_t n = (size_t)M * d;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t t = i / d, c = i - t * d;
+    anch[((size_t)(p0 + t) * m + ai) * d + c] = H[i];
+  }
+}
+
 // Hfin[p0 + t] = H[t]
 __global__ void k_pf_store_hfin(const float *H, float *hfin, int p0, int d, int M) {
   const size_t n = (size_t)M * d;
@@ -572,6 +581,9 @@ int prefill_run(const DevPtrs &P, const PrefillPlan &plan, int n_tokens, cudaStr
     ++cnt;
     for (int l = 0; l < D.L; ++l) {
       // spd_weights order: 0 attn_norm 1 wq 2 wk 3 wv 4 wo 5 mlp_norm 6 w_gate 7 w_up 8 w_down
+      if (P.paper_pdm)
+        for (int ai = 0; ai < P.pdm_m; ++ai)
+          if (P.pdm_anchor[ai] == l) { k_pf_store_anchor<<<eb, 256, 0, st>>>(P.pf_H, P.anch, p0, D.d, M, P.pdm_m, ai); ++cnt; }
       k_pf_norm_split<<<M, 256, 0, st>>>(P.pf_H, plan.w[0][l], D.d, D.eps, P.pf_x3, P.pf_plane);
       const uint16_t *wqkv[3] = {plan.w[1][l], plan.w[2][l], plan.w[3][l]};
       const int nqkv[3] = {qd, kd, kd};

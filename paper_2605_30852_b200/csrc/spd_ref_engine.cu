@@ -45,6 +45,10 @@ __global__ void k_rmsnorm(DevPtrs P, int which, int pass) {
     if (!st->occ[k]) return;
     int layer = k * D.per + pass;
     const uint16_t *g = which == 0 ? P.attn_norm[layer] : P.mlp_norm[layer];
+    const int ai = which == 0 ? anchor_index(P, layer) : -1;
+    if (ai >= 0 && st->pos[k] < D.max_seq)   // NEXT-1: H^layer of the paper PDM's anchor set
+      for (int i = threadIdx.x; i < D.d; i += blockDim.x)
+        P.anch[((size_t)st->pos[k] * P.pdm_m + ai) * D.d + i] = P.h[(size_t)st->hbuf[k] * D.d + i];
     block_rmsnorm(P.h + (size_t)st->hbuf[k] * D.d, g, D.d, D.eps, P.x + (size_t)k * D.d, red);
   } else if (which == 2) {
     if (!st->run_verify) return;
