@@ -341,6 +341,50 @@ def run_gpu(args, shape):
     # W_p = [I 0 .. 0], so the PDM's logits for a token equal the target's bit for bit, Q = P, and every draft is
     # accepted (u * Q(x) < P(x) for every u < 1).  The greedy cycle is timed on the same tensors beside it.
     eng.close()
+
+    # ---- NEXT-1: the paper's Pipeline Draft Module (PAPER.md:71, :91-100, :121 "L_s ~ L/n - 1", :139, :299) in place of the
+    # simplified one: L_s = L/n - 1 layers (>= 1), a 32000-entry head; saturated cycles at forced p = 1 on the same target.
+    paper = None
+    if not args.no_paper_pdm:
+        Ls, Vs = max(1, shape.n_layers // n - 1), min(32000, shape.vocab)
+        pw = si.make_pdm_weights(shape, Ls, Vs, seed=args.seed + rank)
+        eng2 = spd.SPD(shape, w_dev, max_seq=P + 4 * args.steps + 8 * n + 64, device=local_rank)
+        eng2.attach_pdm(spd.upload_pdm_weights(pw, local_rank))
+        if args.engine is not None:
+            eng2.set_option(spd.OPT.ENGINE, args.engine)
+        s2 = eng2.stream_main
+        q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        eng2.prefill(prompt)
+        q0.record(s2)
+        f2 = eng2.prefill(prompt)
+        q1.record(s2)
+        torch.cuda.synchronize()
+        pdm_prefill_ms = q0.elapsed_time(q1)
+        eng2.set_forced(truth, 1.0, args.seed)
+        eng2.step_many(n + args.warmup)
+        kp = min(args.steps, 200)
+        q0.record(s2)
+        plog = eng2.step_many(kp)
+        q1.record(s2)
+        torch.cuda.synchronize()
+        pdm_cycle_us = q0.elapsed_time(q1) * 1e3 / kp
+        m_anch = si.pdm_anchor_count(shape.n_layers)
+        d = shape.d_model
+        Lt, anchors = shape.n_layers, sorted({0, shape.n_layers // 4, shape.n_layers // 2, 3 * shape.n_layers // 4, shape.n_layers - 1})
+        # a saturated draft has one row per depth k = 0 .. n; row k reads FC_f(k), (f(k) + 1) d x d (Eq. 3-4)
+        fc_bytes = sum(2 * d * d * sum(1 for b in anchors if b <= min(Lt, k * (Lt // n))) for k in range(n + 1))
+        pdm_bytes = fc_bytes + 2 * Ls * shape.layer_params() + 2 * Vs * d + (n + 1) * Ls * 4 * shape.n_kv_heads * shape.head_dim * ctx_mid
+        paper = {"pdm_layers": Ls, "pdm_vocab": Vs, "rows_per_draft": n + 1, "cycles": kp,
+                 "cycle_us_with_paper_pdm": pdm_cycle_us, "cycle_us_simplified_pdm": step_us, "pdm_cost_us": pdm_cycle_us - step_us,
+                 "pdm_algorithmic_bytes": pdm_bytes, "pdm_gbs": pdm_bytes / max(pdm_cycle_us - step_us, 1e-9) / 1e3,
+                 "masked_on_a_dedicated_gpu": bool(pdm_cycle_us - step_us < step_us),
+                 "note": "the draft's kernels run in front of the cycle kernel on the same GPU (the paper hides them on a dedicated rank, "
+                         "PAPER.md:119); 'masked' = the draft takes less than one cycle (PAPER.md:121)",
+                 "prefill_ms_incl_pdm_rows": pdm_prefill_ms, "all_saturated_accepts": all(r.fill == n and r.accepted for r in plog),
+                 "first_token_matches": bool(f2 == first)}
+        eng2.close()
+        del eng2, pw
+
     for l in range(shape.n_layers):
         w_dev["wo"][l].zero_()
         w_dev["w_down"][l].zero_()
@@ -394,7 +438,7 @@ def run_gpu(args, shape):
         "step_us_stats": {**percentiles(timed_lat), "unit": "us",
                           "source": "finish-stamp differences (%globaltimer, SPD_DBG_CYCLE_TIMES) of the timed back-to-back cycles"},
         "by_fill": by_fill_table(shape, fill_samples, peak),
-        "prefill": prefill_report(shape, P, prefill_ms),
+        "prefill": prefill_report(shape, P, prefill_ms), "paper_pdm": paper,
         "gpu_launches": int(tot["gpu_launches"]), "clocks": clk, "p_sweep": sweep, "sampling": sampling,
         "setup_s": t_setup,
     }
@@ -483,6 +527,7 @@ def main():
     ap.add_argument("--engine", type=int, default=None, help="0 reference engine, 1 fused engine (default: library default)")
     ap.add_argument("--seed", type=int, default=1234)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-paper-pdm", action="store_true", help="skip the NEXT-1 leg (the paper's PDM in place of the simplified one)")
     args = ap.parse_args()
     shape = si.CONFIGS[args.config]
     if args.impl == "reference":

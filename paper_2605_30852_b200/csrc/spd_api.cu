@@ -136,6 +136,7 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
     if ((size_t)D.d > ymax) ymax = D.d;
     size_t xmax = (size_t)D.d > qd ? D.d : qd;
     if ((size_t)D.F > xmax) xmax = D.F;
+    if (5 * (size_t)D.d > xmax) xmax = 5 * (size_t)D.d;   // the paper PDM's prefill: K = m d concatenated anchors (m <= 5)
     Q.pf_chunk = (int32_t)mc;
     Q.pf_H = cv.take<float>(mc * D.d);
     Q.pf_Q = cv.take<float>(mc * qd);
@@ -363,7 +364,7 @@ extern "C" int spd_prefill(spd_ctx *ctx, const int32_t *tokens, int32_t n_tokens
     k_set_mode<<<1, 1, 0, ctx->sm>>>(ctx->P, MODE_PREFILL_FINAL);
     ++ctx->launches;
   }
-  if (ctx->pdm && pdm_prefill(ctx->P, ctx->pdm, n_tokens, ctx->sm, &ctx->launches)) {
+  if (ctx->pdm && pdm_prefill(ctx->P, ctx->pdm, n_tokens, ctx->prefill_mode, ctx->sm, &ctx->launches)) {
     ctx->dead = 1;
     return fail(ctx, SPD_ECUDA, "PDM prefill launch failed%s");
   }

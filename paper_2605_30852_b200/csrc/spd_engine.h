@@ -37,6 +37,11 @@ int prefill_chunk_tokens(const Dims &D);
 int prefill_create(const DevPtrs &P, const uint16_t *const *const *src, PrefillPlan *plan);
 // Positions [0, n_tokens) of P.pf_tokens through all layers: K/V rows appended, Hfin written.  Returns 0 on success.
 int prefill_run(const DevPtrs &P, const PrefillPlan &plan, int n_tokens, cudaStream_t st, long long *launches);
+int prefill_pdm_rows(const DevPtrs &P, const uint16_t *const (*w)[kPrefillMaxLayers], int n_layers, uint16_t *pdm_kv,
+                     const uint16_t *fc_full, int n_tokens, cudaStream_t st, long long *launches);
+int skinny_gemm(const uint16_t *x3, size_t plane, int K, int NB, const uint16_t *const *w, const int *w_rows, int nseg,
+                float *part, size_t part_floats, const int *rows_ptr, int rows_fixed, float *dst, int ldd, int residual,
+                cudaStream_t st, long long *launches);
 int prefill_op_gemm(const float *x, const uint16_t *w, int M, int N, int K, float *y, void *scratch, cudaStream_t st);
 
 
@@ -52,7 +57,7 @@ size_t pdm_work_bytes(const Dims &D, int Ls, int Vs);
 PdmPlan *pdm_create(DevPtrs *P, const ::spd_pdm_weights *w, void *kv, void *work, cudaStream_t st);
 void pdm_destroy(PdmPlan *plan);
 int pdm_enqueue_draft(const DevPtrs &P, const PdmPlan *pl, cudaStream_t st, long long *launches);
-int pdm_prefill(const DevPtrs &P, const PdmPlan *pl, int n_tokens, cudaStream_t st, long long *launches);
+int pdm_prefill(const DevPtrs &P, const PdmPlan *pl, int n_tokens, int batched, cudaStream_t st, long long *launches);
 int pdm_rollback(const PdmPlan *pl, int new_len, cudaStream_t st);
 int pdm_debug_read(const DevPtrs &P, const PdmPlan *pl, int what, int index, void *out, size_t bytes);
 

@@ -37,6 +37,11 @@ struct PdmPtrs {
   float *G, *X, *XN, *Y, *Q, *ATT, *ACT;      // [kPdmMaxRows][d | d | d | max(qd + 2 kd, 2 F) | qd | qd | F]
   float *part_o;                      // [kPdmMaxRows][Hq][nsplit][hd]
   float2 *part_ml;
+  uint16_t *x3;                       // [3][48][max(d, qd, F)] the GEMM input rows as three exact bf16 parts (skinny GEMM)
+  size_t plane;                       // elements per part
+  float *part;                        // split-K partial sums of the skinny GEMM
+  size_t part_floats;
+  int32_t use_tc;                     // 1: tcgen05 skinny GEMM, 0: CUDA-core M-row GEMV
   float *logits, *z;                  // [Vs], [d]
   float *cand_val;                    // [kPdmCand]
   int32_t *cand_idx;
@@ -102,6 +107,16 @@ __global__ void k_pdm_features(DevPtrs P, PdmPtrs PD) {
   if ((threadIdx.x & 31) == 0) { PD.X[(size_t)r * D.d + o] = acc; PD.G[(size_t)r * D.d + o] = acc; }
 }
 
+// fp32 -> three bf16 parts, x = hi + mid + lo exactly; written to row r of the skinny GEMM's input planes (row stride K)
+__device__ __forceinline__ void pdm_put3(const PdmPtrs &PD, int r, int K, int i, float x) {
+  const uint16_t hi = f32_to_bf16(x);
+  const float r1 = x - bf16_to_f32(hi);
+  const uint16_t mid = f32_to_bf16(r1);
+  const uint16_t lo = f32_to_bf16(r1 - bf16_to_f32(mid));
+  const size_t o = (size_t)r * K + i;
+  PD.x3[o] = hi; PD.x3[PD.plane + o] = mid; PD.x3[2 * PD.plane + o] = lo;
+}
+
 // XN[r] = RMSNorm(X[r]; gain); grid kPdmMaxRows.  last_only: only the last row (head input, final norm), into PD.z.
 __global__ void k_pdm_norm(DevPtrs P, PdmPtrs PD, const uint16_t *gain, int last_only) {
   __shared__ float red[33];
@@ -111,73 +126,107 @@ __global__ void k_pdm_norm(DevPtrs P, PdmPtrs PD, const uint16_t *gain, int last
   if (last_only) { if (r != 0 || R->rows < 1) return; r = R->rows - 1; }
   else if (r >= R->rows) return;
   const uint16_t *g = last_only ? PD.final_norm : gain;
-  block_rmsnorm(PD.X + (size_t)r * D.d, g, D.d, D.eps, last_only ? PD.z : PD.XN + (size_t)r * D.d, red);
+  float *out = last_only ? PD.z : PD.XN + (size_t)r * D.d;
+  block_rmsnorm(PD.X + (size_t)r * D.d, g, D.d, D.eps, out, red);
+  if (PD.use_tc) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < D.d; i += blockDim.x) pdm_put3(PD, last_only ? 0 : r, D.d, i, out[i]);
+  }
 }
 
 // ------------------------------------------------------------------ M-row GEMV ----------------------------------
 // Y[r][col0_s + n] (+)= W_s[n] . X[r] for every row r of the run and up to three weight matrices (segments) that share X.
-// A warp owns 4 consecutive weight rows and streams them once; 8 x-rows per pass share every 16-byte weight chunk.
-// Lane l takes the 8-element chunks l, l + 32, ...; one fp32 FMA chain per (weight row, x row), then the xor tree:
-// a value depends only on (weight row, x row), never on the batch.
+// The x rows live in REGISTERS: thread t of a CTA owns the 8-element chunks t and t + 256 of a 4096-column K pass for up
+// to 8 x rows; the CTA then streams its `wr` weight rows once per pass — a weight row's 4096-column slice is one 8 KB
+// coalesced read by the 256 threads, multiplied into every x row while in registers (the M = 2 head pass of the cycle
+// kernel generalised) — so the x traffic from L2 is M / (2 wr) of the weight traffic and nothing in the main loop waits on
+// shared memory.  Per (weight row, x row): one fp32 FMA chain per thread over its chunks, the warp xor tree, the warp
+// partials of all passes added in (pass, warp) order by one thread: a value depends only on (weight row, x row), never
+// on which other rows share the pass.
+constexpr int kRgRows = 8;               // x rows per pass over the weights
+constexpr int kRgMaxWr = 32;             // weight rows per CTA
 struct RowsGemv {
   const uint16_t *w[3];
   int n[3], col0[3];
-  int nseg, K, ldx, ldy, residual, last_only;
+  int nseg, K, ldx, ldy, residual, last_only, wr;
   const float *x;
   float *y;
 };
 
-__global__ void __launch_bounds__(256) k_pdm_rows_gemv(PdmPtrs PD, RowsGemv A) {
+__global__ void __launch_bounds__(256, 1) k_pdm_rows_gemv(PdmPtrs PD, RowsGemv A) {
+  __shared__ float part[8][kRgMaxWr][kRgRows];        // [warp][weight row][x row]
   const PdmRun *R = PD.run;
-  int rows = R->rows, r_first = 0;
+  int rows = R->rows;
   if (rows < 1) return;
-  if (A.last_only) { r_first = 0; rows = 1; }        // x and y are single vectors (the head: x = PD.z)
-  const int lane = threadIdx.x & 31;
-  int n4 = (blockIdx.x * 8 + (threadIdx.x >> 5)) * 4, seg = 0;     // first of this warp's 4 weight rows
-  while (seg < A.nseg && n4 >= ((A.n[seg] + 3) & ~3)) { n4 -= (A.n[seg] + 3) & ~3; ++seg; }
+  if (A.last_only) rows = 1;                          // x and y are single vectors (the head: x = PD.z)
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, wr = A.wr;
+  int n0 = blockIdx.x * wr, seg = 0;                  // first of this CTA's weight rows
+  while (seg < A.nseg) {
+    const int padded = (A.n[seg] + wr - 1) / wr * wr;
+    if (n0 < padded) break;
+    n0 -= padded; ++seg;
+  }
   if (seg >= A.nseg) return;
-  const int nrow = A.n[seg], nchunk = A.K >> 3;
-  const uint4 *wp[4];
+  const int nrow = A.n[seg], nw = min(wr, nrow - n0), nchunk = A.K >> 3;
+  const uint4 *wbase = reinterpret_cast<const uint4 *>(A.w[seg] + (size_t)n0 * A.K);
+  for (int rb = 0; rb < rows; rb += kRgRows) {
+    const int nr = min(kRgRows, rows - rb);
+    for (int i = tid; i < 8 * kRgMaxWr * kRgRows; i += 256) (&part[0][0][0])[i] = 0.f;
+    __syncthreads();
+    for (int k0 = 0; k0 < nchunk; k0 += 512) {        // K passes of 512 chunks
+      float4 xr[kRgRows][4];                          // [x row][chunk 0: a, b; chunk 1: a, b]
+      const int c0 = k0 + tid, c1 = k0 + 256 + tid;
+      const bool v0 = c0 < nchunk, v1 = c1 < nchunk;
 #pragma unroll
-  for (int j = 0; j < 4; ++j) wp[j] = reinterpret_cast<const uint4 *>(A.w[seg] + (size_t)min(n4 + j, nrow - 1) * A.K);
-  for (int rb = 0; rb < rows; rb += 8) {
-    const int nr = min(8, rows - rb);
-    float acc[4][8];
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-#pragma unroll
-      for (int r = 0; r < 8; ++r) acc[j][r] = 0.f;
-    for (int c = lane; c < nchunk; c += 32) {
-      uint4 wv[4];
-#pragma unroll
-      for (int j = 0; j < 4; ++j) wv[j] = __ldg(wp[j] + c);
-#pragma unroll
-      for (int r = 0; r < 8; ++r) {
+      for (int r = 0; r < kRgRows; ++r) {
+        const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+        xr[r][0] = xr[r][1] = xr[r][2] = xr[r][3] = z;
         if (r < nr) {
-          const float4 *xp = reinterpret_cast<const float4 *>(A.x + (size_t)(r_first + rb + r) * A.ldx) + 2 * c;
-          const float4 xa = xp[0], xb = xp[1];
+          const float4 *xp = reinterpret_cast<const float4 *>(A.x + (size_t)(rb + r) * A.ldx);
+          if (v0) { xr[r][0] = xp[2 * c0]; xr[r][1] = xp[2 * c0 + 1]; }
+          if (v1) { xr[r][2] = xp[2 * c1]; xr[r][3] = xp[2 * c1 + 1]; }
+        }
+      }
+#pragma unroll 4
+      for (int j = 0; j < nw; ++j) {
+        const uint4 *wp = wbase + (size_t)j * nchunk;
+        const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
+        const uint4 w0 = v0 ? __ldg(wp + c0) : z4, w1 = v1 ? __ldg(wp + c1) : z4;
+        float acc[kRgRows];
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            float a = acc[j][r];
-            a = fmaf(bf16_lo(wv[j].x), xa.x, a); a = fmaf(bf16_hi(wv[j].x), xa.y, a);
-            a = fmaf(bf16_lo(wv[j].y), xa.z, a); a = fmaf(bf16_hi(wv[j].y), xa.w, a);
-            a = fmaf(bf16_lo(wv[j].z), xb.x, a); a = fmaf(bf16_hi(wv[j].z), xb.y, a);
-            a = fmaf(bf16_lo(wv[j].w), xb.z, a); a = fmaf(bf16_hi(wv[j].w), xb.w, a);
-            acc[j][r] = a;
+        for (int r = 0; r < kRgRows; ++r) {
+          float a = 0.f;
+          if (r < nr) {
+            a = fmaf(bf16_lo(w0.x), xr[r][0].x, a); a = fmaf(bf16_hi(w0.x), xr[r][0].y, a);
+            a = fmaf(bf16_lo(w0.y), xr[r][0].z, a); a = fmaf(bf16_hi(w0.y), xr[r][0].w, a);
+            a = fmaf(bf16_lo(w0.z), xr[r][1].x, a); a = fmaf(bf16_hi(w0.z), xr[r][1].y, a);
+            a = fmaf(bf16_lo(w0.w), xr[r][1].z, a); a = fmaf(bf16_hi(w0.w), xr[r][1].w, a);
+            a = fmaf(bf16_lo(w1.x), xr[r][2].x, a); a = fmaf(bf16_hi(w1.x), xr[r][2].y, a);
+            a = fmaf(bf16_lo(w1.y), xr[r][2].z, a); a = fmaf(bf16_hi(w1.y), xr[r][2].w, a);
+            a = fmaf(bf16_lo(w1.z), xr[r][3].x, a); a = fmaf(bf16_hi(w1.z), xr[r][3].y, a);
+            a = fmaf(bf16_lo(w1.w), xr[r][3].z, a); a = fmaf(bf16_hi(w1.w), xr[r][3].w, a);
+          }
+          acc[r] = a;
+        }
+#pragma unroll
+        for (int r = 0; r < kRgRows; ++r) {
+          if (r < nr) {
+            const float v = warp_sum(acc[r]);
+            if (lane == 0) part[warp][j][r] += v;     // this lane's own slot: passes accumulate in order
           }
         }
       }
     }
+    __syncthreads();
+    for (int i = tid; i < nw * nr; i += 256) {
+      const int j = i / nr, r = i - j * nr;
+      float v = 0.f;
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
-#pragma unroll
-      for (int r = 0; r < 8; ++r) {
-        const float v = warp_sum(acc[j][r]);
-        if (lane == 0 && r < nr && n4 + j < nrow) {
-          float *dst = A.y + (size_t)(A.last_only ? 0 : rb + r) * A.ldy + A.col0[seg] + n4 + j;
-          *dst = A.residual ? *dst + v : v;
-        }
-      }
+      for (int w = 0; w < 8; ++w) v += part[w][j][r];
+      float *dst = A.y + (size_t)(rb + r) * A.ldy + A.col0[seg] + n0 + j;
+      *dst = A.residual ? *dst + v : v;
+    }
+    __syncthreads();
   }
 }
 
@@ -244,8 +293,9 @@ __global__ void k_pdm_attn_merge(DevPtrs P, PdmPtrs PD) {
   if (r >= R->rows) return;
   const int nsplit = (R->first + r + kAttnSplit) / kAttnSplit;
   const size_t slot = ((size_t)r * D.Hq + hq) * P.nsplit_max;
-  PD.ATT[((size_t)r * D.Hq + hq) * D.hd + threadIdx.x] =
-      attn_merge_elem(PD.part_o + slot * D.hd, PD.part_ml + slot, nsplit, D.hd, threadIdx.x);
+  const float v = attn_merge_elem(PD.part_o + slot * D.hd, PD.part_ml + slot, nsplit, D.hd, threadIdx.x);
+  PD.ATT[((size_t)r * D.Hq + hq) * D.hd + threadIdx.x] = v;
+  if (PD.use_tc) pdm_put3(PD, r, D.Hq * D.hd, hq * D.hd + threadIdx.x, v);
 }
 
 // ACT[r] = silu(gate) * up; Y row = [gate (F) | up (F)]
@@ -254,8 +304,11 @@ __global__ void k_pdm_silu(DevPtrs P, PdmPtrs PD) {
   const int r = blockIdx.y;
   if (r >= PD.run->rows) return;
   const float *y = PD.Y + (size_t)r * 2 * D.F;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < D.F; i += gridDim.x * blockDim.x)
-    PD.ACT[(size_t)r * D.F + i] = silu_mul(y[i], y[D.F + i]);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < D.F; i += gridDim.x * blockDim.x) {
+    const float v = silu_mul(y[i], y[D.F + i]);
+    PD.ACT[(size_t)r * D.F + i] = v;
+    if (PD.use_tc) pdm_put3(PD, r, D.F, i, v);
+  }
 }
 
 // argmax (max value, lowest index) of the reduced-vocabulary logits -> the drafted TARGET token id.
@@ -298,6 +351,8 @@ __global__ void k_pdm_argmax_final(DevPtrs P, PdmPtrs PD) {
 struct PdmPlan {
   PdmPtrs PD;
   int Ls, Vs;
+  const uint16_t *fc_full;                   // FC_{m-1}: the full-depth rule (k = n)
+  int NB;                                    // activation rows per skinny-GEMM tile: n + 1 rounded up to 16
   const uint16_t *w[9][kPrefillMaxLayers];   // host copy of the per-layer device pointers
 };
 
@@ -317,6 +372,12 @@ static size_t pdm_carve(const Dims &D, int Ls, int Vs, int m, int nsplit, void *
   Q.ACT = (float *)take(R * D.F * 4);
   Q.part_o = (float *)take(R * D.Hq * nsplit * D.hd * 4);
   Q.part_ml = (float2 *)take(R * D.Hq * nsplit * 8);
+  const size_t xmax = (size_t)D.d > qd ? ((size_t)D.d > (size_t)D.F ? D.d : D.F) : (qd > (size_t)D.F ? qd : D.F);
+  const size_t nmax = ymax > (size_t)Vs ? ymax : (size_t)Vs;
+  Q.plane = 48 * xmax;
+  Q.x3 = (uint16_t *)take(3 * Q.plane * 2);
+  Q.part_floats = 16 * 48 * nmax;                     // ksplit <= 16, NB <= 48
+  Q.part = (float *)take(Q.part_floats * 4);
   Q.logits = (float *)take((size_t)Vs * 4); Q.z = (float *)take((size_t)D.d * 4);
   Q.cand_val = (float *)take(kPdmCand * 4); Q.cand_idx = (int32_t *)take(kPdmCand * 4);
   Q.fc = (const uint16_t *const *)take(8 * sizeof(void *));
@@ -353,6 +414,8 @@ PdmPlan *pdm_create(DevPtrs *P, const spd_pdm_weights *w, void *kv, void *work, 
   int32_t *draft;
   const size_t bytes = pdm_carve(D, w->n_layers, w->vocab, m, P->nsplit_max, work, &plan->PD, &anch, &draft);
   plan->Ls = w->n_layers; plan->Vs = w->vocab;
+  plan->NB = (D.n + 1 + 15) / 16 * 16;
+  plan->PD.use_tc = prefill_supported(D) && plan->NB <= 48 ? 1 : 0;
   plan->PD.kv = (uint16_t *)kv;
   plan->PD.final_norm = w->final_norm; plan->PD.head = w->head; plan->PD.vocab_map = w->vocab_map;
   const uint16_t *const *src[9] = {w->attn_norm, w->wq, w->wk, w->wv, w->wo, w->mlp_norm, w->w_gate, w->w_up, w->w_down};
@@ -363,6 +426,7 @@ PdmPlan *pdm_create(DevPtrs *P, const spd_pdm_weights *w, void *kv, void *work, 
     }
   for (int i = 0; i < m; ++i)
     if (!w->fc[i]) { free(plan); return nullptr; }
+  plan->fc_full = w->fc[m - 1];
   if (cudaMemsetAsync(work, 0, bytes - (size_t)D.max_seq * m * D.d * 4, st) != cudaSuccess ||
       cudaMemcpyAsync((void *)plan->PD.fc, w->fc, sizeof(void *) * m, cudaMemcpyHostToDevice, st) != cudaSuccess ||
       cudaStreamSynchronize(st) != cudaSuccess) {
@@ -379,16 +443,22 @@ void pdm_destroy(PdmPlan *plan) { free(plan); }
 
 static int pdm_launch_gemv(const PdmPlan *pl, const uint16_t *const *w, const int *n, int nseg, int K, const float *x, int ldx,
                            float *y, int ldy, int residual, int last_only, cudaStream_t st) {
+  if (pl->PD.use_tc)     // the producers of x also wrote its three bf16 parts into PD.x3 (row stride K)
+    return skinny_gemm(pl->PD.x3, pl->PD.plane, K, pl->NB, w, n, nseg, pl->PD.part, pl->PD.part_floats, &pl->PD.run->rows,
+                       last_only ? 1 : 0, y, ldy, residual, st, nullptr);
   RowsGemv A;
   memset(&A, 0, sizeof A);
-  int total4 = 0, col = 0;
+  int total = 0, col = 0, nmax = 0;
+  for (int s = 0; s < nseg; ++s) nmax = n[s] > nmax ? n[s] : nmax;
+  const int wr = nmax >= 8192 ? 32 : 16;              // weight rows per CTA: >= 256 CTAs for the narrow matrices
   for (int s = 0; s < nseg; ++s) {
     A.w[s] = w[s]; A.n[s] = n[s]; A.col0[s] = col;
     col += n[s];
-    total4 += (n[s] + 3) / 4;
+    total += (n[s] + wr - 1) / wr;
   }
+  A.wr = wr;
   A.nseg = nseg; A.K = K; A.ldx = ldx; A.ldy = ldy; A.residual = residual; A.last_only = last_only; A.x = x; A.y = y;
-  k_pdm_rows_gemv<<<(total4 + 7) / 8, 256, 0, st>>>(pl->PD, A);
+  k_pdm_rows_gemv<<<total, 256, 0, st>>>(pl->PD, A);
   return 0;
 }
 
@@ -402,7 +472,7 @@ static void pdm_enqueue_body(const DevPtrs &P, const PdmPlan *pl, bool head, cud
     k_pdm_norm<<<R, 256, 0, st>>>(P, PD, pl->w[0][l], 0); ++*cnt;
     const uint16_t *wqkv[3] = {pl->w[1][l], pl->w[2][l], pl->w[3][l]};
     const int nqkv[3] = {qd, kd, kd};
-    pdm_launch_gemv(pl, wqkv, nqkv, 3, D.d, PD.XN, D.d, PD.Y, qd + 2 * kd, 0, 0, st); ++*cnt;
+    pdm_launch_gemv(pl, wqkv, nqkv, 3, D.d, PD.XN, D.d, PD.Y, qd + 2 * kd, 0, 0, st); *cnt += pl->PD.use_tc ? 2 : 1;
     k_pdm_rope_append<<<R, 256, 0, st>>>(P, PD, l); ++*cnt;
     dim3 ga(P.nsplit_max, D.Hkv, R);
     if (D.hd == 128) k_pdm_attn_partial<128><<<ga, group * 32, 0, st>>>(P, PD, l);
@@ -411,20 +481,20 @@ static void pdm_enqueue_body(const DevPtrs &P, const PdmPlan *pl, bool head, cud
     k_pdm_attn_merge<<<dim3(D.Hq, R), D.hd, 0, st>>>(P, PD); ++*cnt;
     const uint16_t *wo[1] = {pl->w[4][l]};
     const int nd[1] = {D.d};
-    pdm_launch_gemv(pl, wo, nd, 1, qd, PD.ATT, qd, PD.X, D.d, 1, 0, st); ++*cnt;
+    pdm_launch_gemv(pl, wo, nd, 1, qd, PD.ATT, qd, PD.X, D.d, 1, 0, st); *cnt += pl->PD.use_tc ? 2 : 1;
     k_pdm_norm<<<R, 256, 0, st>>>(P, PD, pl->w[5][l], 0); ++*cnt;
     const uint16_t *wgu[2] = {pl->w[6][l], pl->w[7][l]};
     const int ngu[2] = {D.F, D.F};
-    pdm_launch_gemv(pl, wgu, ngu, 2, D.d, PD.XN, D.d, PD.Y, 2 * D.F, 0, 0, st); ++*cnt;
+    pdm_launch_gemv(pl, wgu, ngu, 2, D.d, PD.XN, D.d, PD.Y, 2 * D.F, 0, 0, st); *cnt += pl->PD.use_tc ? 2 : 1;
     k_pdm_silu<<<dim3((D.F + 255) / 256, R), 256, 0, st>>>(P, PD); ++*cnt;
     const uint16_t *wd[1] = {pl->w[8][l]};
-    pdm_launch_gemv(pl, wd, nd, 1, D.F, PD.ACT, D.F, PD.X, D.d, 1, 0, st); ++*cnt;
+    pdm_launch_gemv(pl, wd, nd, 1, D.F, PD.ACT, D.F, PD.X, D.d, 1, 0, st); *cnt += pl->PD.use_tc ? 2 : 1;
   }
   if (head) {
     k_pdm_norm<<<1, 256, 0, st>>>(P, PD, nullptr, 1); ++*cnt;
     const uint16_t *wh[1] = {PD.head};
     const int nv[1] = {pl->Vs};
-    pdm_launch_gemv(pl, wh, nv, 1, D.d, PD.z, D.d, PD.logits, pl->Vs, 0, 1, st); ++*cnt;
+    pdm_launch_gemv(pl, wh, nv, 1, D.d, PD.z, D.d, PD.logits, pl->Vs, 0, 1, st); *cnt += pl->PD.use_tc ? 2 : 1;
     k_pdm_argmax_cand<<<kPdmCand, 256, 0, st>>>(PD); ++*cnt;
     k_pdm_argmax_final<<<1, 32, 0, st>>>(P, PD); ++*cnt;
   }
@@ -440,9 +510,16 @@ int pdm_enqueue_draft(const DevPtrs &P, const PdmPlan *pl, cudaStream_t st, long
 }
 
 // After the target's prefill: the full-depth rows of positions 0 .. n_tokens - 1, then F = n_tokens.
-int pdm_prefill(const DevPtrs &P, const PdmPlan *pl, int n_tokens, cudaStream_t st, long long *launches) {
+int pdm_prefill(const DevPtrs &P, const PdmPlan *pl, int n_tokens, int batched, cudaStream_t st, long long *launches) {
   long long cnt = 0;
-  const int RB = 32;
+  // tensor-core path: the same GEMMs and prefill attention as the target's batched prefill, over the PDM's layers
+  if (batched && prefill_pdm_rows(P, pl->w, pl->Ls, pl->PD.kv, pl->fc_full, n_tokens, st, &cnt) == 0) {
+    k_pdm_set_final<<<1, 1, 0, st>>>(pl->PD, n_tokens, 0); ++cnt;
+    if (launches) *launches += cnt;
+    return cudaGetLastError() == cudaSuccess ? 0 : -1;
+  }
+  cudaGetLastError();
+  const int RB = pl->PD.use_tc ? (pl->NB < 32 ? pl->NB : 32) : 32;
   for (int p0 = 0; p0 < n_tokens; p0 += RB) {
     const int rows = n_tokens - p0 < RB ? n_tokens - p0 : RB;
     k_pdm_begin<<<1, 32, 0, st>>>(P, pl->PD, p0, rows); ++cnt;

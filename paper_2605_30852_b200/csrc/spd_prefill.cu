@@ -214,6 +214,140 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_pf_gemm(const __grid_consta
   }
 }
 
+// ------------------------------------------------------------------ the skinny GEMM (M = a few rows) ------------
+// The paper PDM's per-cycle products (spd_pdm.cu): up to 48 activation rows against a weight matrix that has to be
+// STREAMED once — HBM-bound like the GEMVs of the cycle kernel, but with M = n + 1 rows per weight tile.  The operands
+// swap roles: the 128 x 64 weight tile is the MMA's A operand (weight rows = TMEM lanes), the activation rows — three
+// exact bf16 parts of NB <= 48 rows — are the B operand (N = NB), so a 16 KB weight tile is multiplied into every row
+// while it sits in shared memory, 8 stages (176 KB) of TMA loads are in flight per SM, and K is split over gridDim.y so
+// that narrow matrices still fill 148 SMs.  Output: partial sums part[ks][row][column]; k_pf_skinny_reduce adds them in
+// ks order (deterministic) into the destination (optionally on top of the residual).
+constexpr int kSkMaxStages = 8;
+constexpr int kSkMaxNB = 48;
+// a stage = the 16 KB weight tile + three NB x 128-byte activation tiles: 8 stages of 22 KB at NB = 16 (176 KB in flight),
+// 7 x 28 KB at NB = 32, 6 x 34 KB at NB = 48
+__host__ __device__ constexpr int sk_stage_bytes(int NB) { return kGemmBM * 128 + 3 * NB * 128; }
+__host__ __device__ constexpr int sk_stages(int NB) { return NB <= 16 ? 8 : (NB <= 32 ? 7 : 6); }
+
+struct SkinnyArgs {
+  CUtensorMap w[3];                // [N_seg, K] bf16, box {64, 128}
+  CUtensorMap x[3];                // the three bf16 parts of the activation rows: [48, K], box {64, NB}
+  int seg_tiles[3], seg_n[3], seg_col0[3];
+  int K, NB, ldp;                  // ldp = columns of one partial row (sum of the segments' rows)
+  float *part;                     // [gridDim.y][NB][ldp]
+};
+
+__device__ __forceinline__ void tc_ld_32x16(uint32_t taddr, float (&v)[16]) {
+  uint32_t r[16];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+__global__ void __launch_bounds__(kGemmThreads, 1) k_pf_gemm_skinny(const __grid_constant__ SkinnyArgs A) {
+  extern __shared__ uint8_t pf_smem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>(((uintptr_t)pf_smem_raw + 1023) & ~(uintptr_t)1023);
+  const int NB = A.NB, kSkStages = sk_stages(NB), kSkStageBytes = sk_stage_bytes(NB);
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + kSkStages * kSkStageBytes);
+  uint64_t *empty = full + kSkMaxStages;
+  uint64_t *tmem_full = empty + kSkMaxStages;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_full + 1);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int seg = 0, tile = blockIdx.x;
+  while (seg < 2 && tile >= A.seg_tiles[seg]) { tile -= A.seg_tiles[seg]; ++seg; }
+  const int n0 = tile * kGemmBM;
+  const int nkb_all = A.K / kGemmBK, per = (nkb_all + gridDim.y - 1) / gridDim.y;
+  const int kb0 = blockIdx.y * per, kb1 = min(nkb_all, kb0 + per), nkb = max(0, kb1 - kb0);
+  const uint32_t stage_tx = (uint32_t)(kGemmBM * 128 + 3 * NB * 128);
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kSkStages; ++s) { pf_mbar_init(&full[s], 1); pf_mbar_init(&empty[s], 1); }
+    pf_mbar_init(tmem_full, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(pf_smem_u32(tmem_slot)), "r"(64u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_d = *tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      for (int i = 0; i < nkb; ++i) {
+        const int s = i % kSkStages, it = i / kSkStages, kb = kb0 + i;
+        pf_mbar_wait(&empty[s], (it & 1) ^ 1);
+        uint8_t *st = smem + (size_t)s * kSkStageBytes;
+        pf_mbar_expect_tx(&full[s], stage_tx);
+        pf_tma_load_2d(st, &A.w[seg], kb * kGemmBK, n0, &full[s]);
+#pragma unroll
+        for (int p = 0; p < 3; ++p) pf_tma_load_2d(st + kGemmBM * 128 + p * NB * 128, &A.x[p], kb * kGemmBK, 0, &full[s]);
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      const uint32_t idesc = tc_idesc_bf16(kGemmBM, NB);
+      for (int i = 0; i < nkb; ++i) {
+        const int s = i % kSkStages, it = i / kSkStages;
+        pf_mbar_wait(&full[s], it & 1);
+        tc_fence_after();
+        const uint32_t a = pf_smem_u32(smem + (size_t)s * kSkStageBytes), b = a + kGemmBM * 128;
+#pragma unroll
+        for (int k = 0; k < kGemmBK / 16; ++k) {
+          const uint64_t ad = tc_smem_desc(a + k * 32);
+#pragma unroll
+          for (int p = 0; p < 3; ++p)
+            tc_mma_bf16(tmem_d, ad, tc_smem_desc(b + p * NB * 128 + k * 32), idesc, (i | k | p) ? 1u : 0u);
+        }
+        tc_commit(&empty[s]);
+      }
+      tc_commit(tmem_full);
+    }
+  } else {
+    pf_mbar_wait(tmem_full, 0);
+    tc_fence_after();
+    const int lg = warp & 3;
+    const int n = n0 + lg * 32 + lane;               // this thread's weight row = output column
+    const bool ok = n < A.seg_n[seg] && nkb > 0;
+    float *prow = A.part + ((size_t)blockIdx.y * NB) * A.ldp + A.seg_col0[seg] + n;
+    for (int c = 0; c < NB; c += 16) {
+      float v[16];
+      if (nkb > 0) tc_ld_32x16(tmem_d + ((uint32_t)(lg * 32) << 16) + (uint32_t)c, v);
+#pragma unroll
+      for (int r = 0; r < 16; ++r)
+        if (n < A.seg_n[seg]) prow[(size_t)(c + r) * A.ldp] = ok ? v[r] : 0.f;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"(64u) : "memory");
+  }
+}
+
+// dst[r][c] (+)= sum over ks (in order) of part[ks][r][c], r < *rows_ptr (clamped to NB), c < ncol
+__global__ void k_pf_skinny_reduce(const float *part, int ksplit, int NB, int ldp, const int *rows_ptr, int rows_fixed,
+                                   float *dst, int ldd, int ncol, int residual) {
+  const int rows = min(NB, rows_fixed > 0 ? rows_fixed : *rows_ptr);
+  const size_t n = (size_t)rows * ncol;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t r = i / ncol, c = i - r * ncol;
+    float v = 0.f;
+    for (int ks = 0; ks < ksplit; ++ks) v += part[((size_t)ks * NB + r) * ldp + c];
+    float *d = dst + r * ldd + c;
+    *d = residual ? *d + v : v;
+  }
+}
+
 // ------------------------------------------------------------------ elementwise kernels ------------------------
 // x = hi + mid + lo exactly (finite x; each residual is exact in fp32 and the last one fits 8 mantissa bits)
 struct Split3 { uint16_t hi, mid, lo; };
@@ -530,6 +664,47 @@ static int pf_launch_gemm(PfEncodeFn enc, const uint16_t *x3, size_t plane, int 
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 
+// Skinny GEMM launcher: x3 = three bf16 planes of [48][K] rows (plane stride in elements), rows on the device
+// (rows_ptr) or fixed.  part: scratch of >= ksplit * NB * ncol floats.
+int skinny_gemm(const uint16_t *x3, size_t plane, int K, int NB, const uint16_t *const *w, const int *w_rows, int nseg,
+                float *part, size_t part_floats, const int *rows_ptr, int rows_fixed, float *dst, int ldd, int residual,
+                cudaStream_t st, long long *launches) {
+  static PfEncodeFn enc = nullptr;
+  static bool attr = false;
+  if (!enc) enc = pf_encoder();
+  if (!enc || K % kGemmBK || NB % 16 || NB < 16 || NB > kSkMaxNB) return -1;
+  if (!attr) {
+    if (cudaFuncSetAttribute(k_pf_gemm_skinny, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) != cudaSuccess) return -1;
+    attr = true;
+  }
+  const int sk_smem = sk_stages(NB) * sk_stage_bytes(NB) + 1024 + 256;
+  SkinnyArgs A;
+  memset(&A, 0, sizeof A);
+  int tiles = 0, col = 0;
+  for (int s = 0; s < nseg; ++s) {
+    if (pf_make_map(enc, &A.w[s], w[s], w_rows[s], K, kGemmBM)) return -1;
+    A.seg_tiles[s] = (w_rows[s] + kGemmBM - 1) / kGemmBM;
+    A.seg_n[s] = w_rows[s];
+    A.seg_col0[s] = col;
+    col += w_rows[s];
+    tiles += A.seg_tiles[s];
+  }
+  for (int p = 0; p < 3; ++p)
+    if (pf_make_map(enc, &A.x[p], x3 + p * plane, kSkMaxNB, K, NB)) return -1;
+  const int nkb = K / kGemmBK;
+  int ksplit = (2 * 148 + tiles - 1) / tiles;          // about two CTAs per SM in total
+  if (ksplit > nkb / 4) ksplit = nkb / 4 > 0 ? nkb / 4 : 1;
+  if (ksplit > 16) ksplit = 16;
+  if ((size_t)ksplit * NB * col > part_floats) ksplit = (int)(part_floats / ((size_t)NB * col));
+  if (ksplit < 1) return -1;
+  A.K = K; A.NB = NB; A.ldp = col; A.part = part;
+  k_pf_gemm_skinny<<<dim3(tiles, ksplit), kGemmThreads, sk_smem, st>>>(A);
+  const int rb = (int)(((size_t)NB * col + 255) / 256);
+  k_pf_skinny_reduce<<<rb < 1184 ? rb : 1184, 256, 0, st>>>(part, ksplit, NB, col, rows_ptr, rows_fixed, dst, ldd, col, residual);
+  if (launches) *launches += 2;
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
 bool prefill_supported(const Dims &D) {
   const int qd = D.Hq * D.hd;
   const int G = D.Hq / D.Hkv;
@@ -565,8 +740,12 @@ int prefill_create(const DevPtrs &P, const uint16_t *const *const *src, PrefillP
 }
 
 // Runs positions [0, n_tokens) through all layers (KV rows appended, Hfin written).  Tokens are in P.pf_tokens.
-int prefill_run(const DevPtrs &P, const PrefillPlan &plan, int n_tokens, cudaStream_t st, long long *launches) {
-  if (!plan.available) return -1;
+// One stack of decoder layers over the prompt, chunk by chunk.  Target: rows start as embeddings, the paper PDM's anchors
+// are captured on the way, Hfin is written.  PDM (fc_full != nullptr): rows start as the full-depth features
+// g^n = FC_{m-1} . Concat(H^b0 .. H^b(m-1)) (Eq. 4; P.anch IS the [position, m d] fp32 matrix of those concatenations),
+// the layers / cache are the PDM's (P.kv points at its cache), nothing else is written.
+static int prefill_stack(const DevPtrs &P, const uint16_t *const (*w)[kPrefillMaxLayers], int n_layers, const uint16_t *fc_full,
+                         int n_tokens, cudaStream_t st, long long *launches) {
   PfEncodeFn enc = pf_encoder();
   if (!enc) return -1;
   const Dims &D = P.dim;
@@ -577,40 +756,63 @@ int prefill_run(const DevPtrs &P, const PrefillPlan &plan, int n_tokens, cudaStr
   for (int p0 = 0; p0 < n_tokens; p0 += Mc) {
     const int M = n_tokens - p0 < Mc ? n_tokens - p0 : Mc;
     const int eb = (int)(((size_t)M * D.F + 255) / 256 < 4096 ? ((size_t)M * D.F + 255) / 256 : 4096);
-    k_pf_embed<<<M, 256, 0, st>>>(P.embed, P.pf_tokens, p0, D.d, P.pf_H);
+    if (fc_full) {
+      const int K5 = P.pdm_m * D.d;
+      k_pf_split<<<2048, 256, 0, st>>>(P.anch + (size_t)p0 * K5, (size_t)M * K5, P.pf_x3, P.pf_plane);
+      const uint16_t *wf[1] = {fc_full};
+      const int nf[1] = {D.d};
+      if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, K5, wf, nf, 1, P.pf_H, D.d, st, &cnt)) return -1;
+    } else {
+      k_pf_embed<<<M, 256, 0, st>>>(P.embed, P.pf_tokens, p0, D.d, P.pf_H);
+    }
     ++cnt;
-    for (int l = 0; l < D.L; ++l) {
+    for (int l = 0; l < n_layers; ++l) {
       // spd_weights order: 0 attn_norm 1 wq 2 wk 3 wv 4 wo 5 mlp_norm 6 w_gate 7 w_up 8 w_down
-      if (P.paper_pdm)
+      if (P.paper_pdm && !fc_full)
         for (int ai = 0; ai < P.pdm_m; ++ai)
           if (P.pdm_anchor[ai] == l) { k_pf_store_anchor<<<eb, 256, 0, st>>>(P.pf_H, P.anch, p0, D.d, M, P.pdm_m, ai); ++cnt; }
-      k_pf_norm_split<<<M, 256, 0, st>>>(P.pf_H, plan.w[0][l], D.d, D.eps, P.pf_x3, P.pf_plane);
-      const uint16_t *wqkv[3] = {plan.w[1][l], plan.w[2][l], plan.w[3][l]};
+      k_pf_norm_split<<<M, 256, 0, st>>>(P.pf_H, w[0][l], D.d, D.eps, P.pf_x3, P.pf_plane);
+      const uint16_t *wqkv[3] = {w[1][l], w[2][l], w[3][l]};
       const int nqkv[3] = {qd, kd, kd};
       if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, D.d, wqkv, nqkv, 3, P.pf_Y, qd + 2 * kd, st, &cnt)) return -1;
       k_pf_rope_append<<<M, 256, 0, st>>>(P.pf_Y, qd + 2 * kd, P, l, p0, P.pf_Q);
       dim3 ag((M + TQ - 1) / TQ, D.Hkv);
       if (D.hd == 128) k_pf_attention<128><<<ag, 256, att_smem, st>>>(P, l, p0, M, P.pf_Q, P.pf_x3, P.pf_plane);
       else k_pf_attention<64><<<ag, 256, att_smem, st>>>(P, l, p0, M, P.pf_Q, P.pf_x3, P.pf_plane);
-      const uint16_t *wo[1] = {plan.w[4][l]};
+      const uint16_t *wo[1] = {w[4][l]};
       const int no[1] = {D.d};
       if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, qd, wo, no, 1, P.pf_Y, D.d, st, &cnt)) return -1;
       k_pf_residual<<<eb, 256, 0, st>>>(P.pf_H, P.pf_Y, D.d, D.d, M);
-      k_pf_norm_split<<<M, 256, 0, st>>>(P.pf_H, plan.w[5][l], D.d, D.eps, P.pf_x3, P.pf_plane);
-      const uint16_t *wgu[2] = {plan.w[6][l], plan.w[7][l]};
+      k_pf_norm_split<<<M, 256, 0, st>>>(P.pf_H, w[5][l], D.d, D.eps, P.pf_x3, P.pf_plane);
+      const uint16_t *wgu[2] = {w[6][l], w[7][l]};
       const int ngu[2] = {D.F, D.F};
       if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, D.d, wgu, ngu, 2, P.pf_Y, 2 * D.F, st, &cnt)) return -1;
       k_pf_silu_split<<<eb, 256, 0, st>>>(P.pf_Y, 2 * D.F, D.F, M, P.pf_x3, P.pf_plane);
-      const uint16_t *wd[1] = {plan.w[8][l]};
+      const uint16_t *wd[1] = {w[8][l]};
       if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, D.F, wd, no, 1, P.pf_Y, D.d, st, &cnt)) return -1;
       k_pf_residual<<<eb, 256, 0, st>>>(P.pf_H, P.pf_Y, D.d, D.d, M);
       cnt += 7;
     }
-    k_pf_store_hfin<<<eb, 256, 0, st>>>(P.pf_H, P.hfin, p0, D.d, M);
-    ++cnt;
+    if (!fc_full) { k_pf_store_hfin<<<eb, 256, 0, st>>>(P.pf_H, P.hfin, p0, D.d, M); ++cnt; }
   }
   if (launches) *launches += cnt;
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+int prefill_run(const DevPtrs &P, const PrefillPlan &plan, int n_tokens, cudaStream_t st, long long *launches) {
+  if (!plan.available) return -1;
+  return prefill_stack(P, plan.w, P.dim.L, nullptr, n_tokens, st, launches);
+}
+
+// The paper PDM's full-depth rows of positions 0 .. n_tokens - 1 (its prefill): the same tensor-core GEMMs and prefill
+// attention over ITS layers and ITS cache.  Needs the batched-prefill scratch (P.pf_*) sized for K = m d.
+int prefill_pdm_rows(const DevPtrs &P, const uint16_t *const (*w)[kPrefillMaxLayers], int n_layers, uint16_t *pdm_kv,
+                     const uint16_t *fc_full, int n_tokens, cudaStream_t st, long long *launches) {
+  const Dims &D = P.dim;
+  if (!prefill_supported(D) || !P.pf_H || (size_t)P.pf_chunk * P.pdm_m * D.d > P.pf_plane) return -1;
+  DevPtrs Q = P;
+  Q.kv = pdm_kv;
+  return prefill_stack(Q, w, n_layers, fc_full, n_tokens, st, launches);
 }
 
 // spd_op_gemm: Y[M, N] = X[M, K] . W[N, K]^T with the prefill GEMM (X fp32 -> bf16 hi + mid + lo, exact).  scratch: 3 * M * K bf16.
