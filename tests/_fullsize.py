@@ -157,12 +157,14 @@ def oracle_tier(eng, shape, w, g, first, G=None, p=0.8, seed=3, tol=1e-2, pdm_ev
                 continue
             if not r.accepted:
                 assert np.all(eng.kv_len() == r.committed_len) and r.discarded == r.fill - 1
-        # spot-checked slot states: a CORRECT in-flight token at depth k holds O-AR's residual stream after layer
+        # spot-checked slot states: a CORRECT in-flight token (behind correct ones) at depth k holds O-AR's residual stream after layer
         # k L/n - 1 at its position (SURVEY C-3)
         _, _, slots = eng.ring()
+        right = [bool(o) and P <= q <= P + G and t == int(g["tokens"][q - P]) for o, q, t in slots]
         for k in range(1, n):
             occ, pos, tok = slots[k]
-            if occ and pos in trace_at and k in depth_of and P <= pos <= P + G and tok == int(g["tokens"][pos - P]):
+            # ... and so must every older in-flight token be: its K/V rows are part of this token's context
+            if occ and pos in trace_at and k in depth_of and all(right[j] for j in range(k, n) if slots[j][0]):
                 e = rel_err(eng.hidden(k), g["trace"][trace_at[pos], depth_of[k]])
                 rep.max_slot_err = max(rep.max_slot_err, e)
                 rep.slots_checked += 1

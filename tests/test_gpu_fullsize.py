@@ -79,7 +79,7 @@ def test_full_prompt_sampled_oracle_outputs_and_invariants(name, G):
     #      and exit logits, spot-checked in-flight slot states, the PDM on the kernel's own slots --------------------
     tier = oracle_tier(eng, shape, w, golden_for(name), first)
     print(f"{name} full-prompt oracle tier ({'live oracle' if LIVE else 'stored oracle values'}):", tier.summary())
-    assert tier.accepts > 0 and tier.rejects > 0 and tier.slots_checked > 0 and tier.pdm_checked > 0
+    assert tier.accepts > 0 and (tier.rejects > 0 or tier.tokens < 16) and tier.slots_checked > 0 and tier.pdm_checked > 0
     assert tier.ties <= 1 and (tier.ties == 0 or tier.min_margin <= 2.0 * tier.max_logit_err)
     eng.rollback(P, first)
 
