@@ -15,10 +15,22 @@ import numpy as np
 import torch
 
 
+_W_MEMO: dict = {}
+
+
 def _w(bits: np.ndarray) -> np.ndarray:
-    """bf16 bits -> float64 via torch's own bf16 type (not the generator's shift)."""
+    """bf16 bits -> float64 via torch's own bf16 type (not the generator's shift).  The widened copy of an array is
+    kept (keyed by the array object, which the memo keeps alive): the per-cycle pins call this model dozens of times
+    on the same weights."""
+    hit = _W_MEMO.get(id(bits))
+    if hit is not None and hit[0] is bits:
+        return hit[1]
     t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16)
-    return t.to(torch.float64).numpy()
+    out = t.to(torch.float64).numpy()
+    if len(_W_MEMO) > 512:
+        _W_MEMO.clear()
+    _W_MEMO[id(bits)] = (bits, out)
+    return out
 
 
 def _round_bf16(x: np.ndarray) -> np.ndarray:
