@@ -41,7 +41,7 @@ int prefill_pdm_rows(const DevPtrs &P, const uint16_t *const (*w)[kPrefillMaxLay
                      const uint16_t *fc_full, int n_tokens, cudaStream_t st, long long *launches);
 int skinny_gemm(const uint16_t *x3, size_t plane, int K, int NB, const uint16_t *const *w, const int *w_rows, int nseg,
                 float *part, size_t part_floats, const int *rows_ptr, int rows_fixed, float *dst, int ldd, int residual,
-                cudaStream_t st, long long *launches);
+                cudaStream_t st, long long *launches, int *ksplit_out = nullptr);
 int prefill_op_gemm(const float *x, const uint16_t *w, int M, int N, int K, float *y, void *scratch, cudaStream_t st);
 
 

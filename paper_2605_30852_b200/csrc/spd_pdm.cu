@@ -42,6 +42,7 @@ struct PdmPtrs {
   float *part;                        // split-K partial sums of the skinny GEMM
   size_t part_floats;
   int32_t use_tc;                     // 1: tcgen05 skinny GEMM, 0: CUDA-core M-row GEMV
+  float2 *rope;                       // [kPdmMaxRows][64] (cos, sin) of the run's positions: computed once per draft
   float *logits, *z;                  // [Vs], [d]
   float *cand_val;                    // [kPdmCand]
   int32_t *cand_idx;
@@ -230,6 +231,16 @@ __global__ void __launch_bounds__(256, 1) k_pdm_rows_gemv(PdmPtrs PD, RowsGemv A
   }
 }
 
+// (cos, sin)(pos * theta_i) of the run's rows, angles in double (C-2.14): once per draft, shared by the L_s layers.
+__global__ void k_pdm_rope_table(DevPtrs P, PdmPtrs PD) {
+  const PdmRun *R = PD.run;
+  const int r = blockIdx.x;
+  if (r >= R->rows || (int)threadIdx.x >= P.dim.hd / 2) return;
+  double s_, c_;
+  sincos((double)(R->first + r) * P.inv_freq[threadIdx.x], &s_, &c_);
+  PD.rope[r * 64 + threadIdx.x] = make_float2((float)c_, (float)s_);
+}
+
 // Y row = [q | k | v]: RoPE (C-2.14) on q and k; q -> Q; k, v -> bf16 rows of the PDM cache at the row's position
 // (REwritten every cycle for in-flight positions).  grid kPdmMaxRows.
 __global__ void k_pdm_rope_append(DevPtrs P, PdmPtrs PD, int layer) {
@@ -239,11 +250,7 @@ __global__ void k_pdm_rope_append(DevPtrs P, PdmPtrs PD, int layer) {
   const int r = blockIdx.x;
   if (r >= R->rows) return;
   const int pos = R->first + r, half = D.hd / 2, qd = D.Hq * D.hd, kd = D.Hkv * D.hd, ldy = qd + 2 * kd;
-  if (threadIdx.x < half) {
-    double s_, c_;
-    sincos((double)pos * P.inv_freq[threadIdx.x], &s_, &c_);
-    cs[threadIdx.x] = make_float2((float)c_, (float)s_);
-  }
+  if (threadIdx.x < half) cs[threadIdx.x] = PD.rope[r * 64 + threadIdx.x];
   __syncthreads();
   const float *y = PD.Y + (size_t)r * ldy;
   for (int j = threadIdx.x; j < (D.Hq + D.Hkv) * half; j += blockDim.x) {
@@ -347,6 +354,57 @@ __global__ void k_pdm_argmax_final(DevPtrs P, PdmPtrs PD) {
   *P.pdm_draft = PD.vocab_map[bi];
 }
 
+// ------------------------------------------------------------------ fused reduces of the skinny GEMM -------------
+// The skinny GEMM leaves split-K partial sums part[ks][row][column]; these kernels add them in ks order and run the
+// epilogue that follows the product in the layer, so no separate norm / SiLU kernel is launched.
+// (a) O / DOWN: X[r] += sum; then XN[r] = RMSNorm(X[r]; gain) and its three bf16 parts = the next product's input.
+//     One CTA per row; the sum of squares uses block_rms_scale's tree on the updated row.
+__global__ void __launch_bounds__(256) k_pdm_reduce_norm(DevPtrs P, PdmPtrs PD, int ksplit, int NB, const uint16_t *gain) {
+  __shared__ float red[33];
+  const Dims &D = P.dim;
+  const int r = blockIdx.x;
+  if (r >= PD.run->rows) return;
+  float *x = PD.X + (size_t)r * D.d;
+  for (int c = threadIdx.x; c < D.d; c += blockDim.x) {
+    float v = 0.f;
+    for (int ks = 0; ks < ksplit; ++ks) v += PD.part[((size_t)ks * NB + r) * D.d + c];
+    x[c] += v;
+  }
+  __syncthreads();
+  const float rs = block_rms_scale(x, D.d, D.eps, red);
+  for (int c = threadIdx.x; c < D.d; c += blockDim.x) {
+    const float v = x[c] * rs * bf16_to_f32(gain[c]);
+    PD.XN[(size_t)r * D.d + c] = v;
+    pdm_put3(PD, r, D.d, c, v);
+  }
+}
+// (b) gate / up: ACT[r] = silu(sum_gate) * sum_up and its parts.  grid (ceil(F / 256), kPdmMaxRows)
+__global__ void k_pdm_reduce_silu(DevPtrs P, PdmPtrs PD, int ksplit, int NB) {
+  const Dims &D = P.dim;
+  const int r = blockIdx.y, c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= PD.run->rows || c >= D.F) return;
+  float g = 0.f, u = 0.f;
+  for (int ks = 0; ks < ksplit; ++ks) {
+    const float *p = PD.part + ((size_t)ks * NB + r) * 2 * D.F;
+    g += p[c]; u += p[D.F + c];
+  }
+  const float v = silu_mul(g, u);
+  PD.ACT[(size_t)r * D.F + c] = v;
+  pdm_put3(PD, r, D.F, c, v);
+}
+// (c) plain: dst[r][c] = sum (QKV -> Y); last_row: only the run's last row, into a single vector (the head -> logits)
+__global__ void k_pdm_reduce_plain(PdmPtrs PD, int ksplit, int NB, int ncol, float *dst, int last_row) {
+  const int rows = PD.run->rows;
+  int r = blockIdx.y;
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (last_row) { if (r != 0 || rows < 1) return; r = rows - 1; }
+  else if (r >= rows) return;
+  if (c >= ncol) return;
+  float v = 0.f;
+  for (int ks = 0; ks < ksplit; ++ks) v += PD.part[((size_t)ks * NB + r) * ncol + c];
+  dst[(size_t)(last_row ? 0 : r) * ncol + c] = v;
+}
+
 // ------------------------------------------------------------------ host side ----------------------------------
 struct PdmPlan {
   PdmPtrs PD;
@@ -378,6 +436,7 @@ static size_t pdm_carve(const Dims &D, int Ls, int Vs, int m, int nsplit, void *
   Q.x3 = (uint16_t *)take(3 * Q.plane * 2);
   Q.part_floats = 16 * 48 * nmax;                     // ksplit <= 16, NB <= 48
   Q.part = (float *)take(Q.part_floats * 4);
+  Q.rope = (float2 *)take(R * 64 * 8);
   Q.logits = (float *)take((size_t)Vs * 4); Q.z = (float *)take((size_t)D.d * 4);
   Q.cand_val = (float *)take(kPdmCand * 4); Q.cand_idx = (int32_t *)take(kPdmCand * 4);
   Q.fc = (const uint16_t *const *)take(8 * sizeof(void *));
@@ -463,16 +522,65 @@ static int pdm_launch_gemv(const PdmPlan *pl, const uint16_t *const *w, const in
 }
 
 // The kernels of one draft after k_pdm_begin (shared by the cycle and the PDM prefill).
+static void pdm_enqueue_body_tc(const DevPtrs &P, const PdmPlan *pl, bool head, cudaStream_t st, long long *cnt) {
+  const Dims &D = P.dim;
+  const PdmPtrs &PD = pl->PD;
+  const int R = kPdmMaxRows, qd = D.Hq * D.hd, kd = D.Hkv * D.hd, group = D.Hq / D.Hkv, NB = pl->NB;
+  int ks = 1;
+  auto gemm = [&](const uint16_t *const *w, const int *n, int nseg, int K) {
+    skinny_gemm(PD.x3, PD.plane, K, NB, w, n, nseg, PD.part, PD.part_floats, nullptr, 0, nullptr, 0, 0, st, cnt, &ks);
+  };
+  k_pdm_rope_table<<<R, 64, 0, st>>>(P, PD); ++*cnt;
+  k_pdm_features<<<dim3((D.d + 7) / 8, R), 256, 0, st>>>(P, PD); ++*cnt;
+  k_pdm_norm<<<R, 256, 0, st>>>(P, PD, pl->w[0][0], 0); ++*cnt;             // the first layer's attention norm
+  const int nd[1] = {D.d};
+  for (int l = 0; l < pl->Ls; ++l) {
+    const uint16_t *wqkv[3] = {pl->w[1][l], pl->w[2][l], pl->w[3][l]};
+    const int nqkv[3] = {qd, kd, kd};
+    gemm(wqkv, nqkv, 3, D.d);
+    k_pdm_reduce_plain<<<dim3((qd + 2 * kd + 255) / 256, R), 256, 0, st>>>(PD, ks, NB, qd + 2 * kd, PD.Y, 0); ++*cnt;
+    k_pdm_rope_append<<<R, 256, 0, st>>>(P, PD, l); ++*cnt;
+    dim3 ga(P.nsplit_max, D.Hkv, R);
+    if (D.hd == 128) k_pdm_attn_partial<128><<<ga, group * 32, 0, st>>>(P, PD, l);
+    else k_pdm_attn_partial<64><<<ga, group * 32, 0, st>>>(P, PD, l);
+    ++*cnt;
+    k_pdm_attn_merge<<<dim3(D.Hq, R), D.hd, 0, st>>>(P, PD); ++*cnt;
+    const uint16_t *wo[1] = {pl->w[4][l]};
+    gemm(wo, nd, 1, qd);
+    k_pdm_reduce_norm<<<R, 256, 0, st>>>(P, PD, ks, NB, pl->w[5][l]); ++*cnt;
+    const uint16_t *wgu[2] = {pl->w[6][l], pl->w[7][l]};
+    const int ngu[2] = {D.F, D.F};
+    gemm(wgu, ngu, 2, D.d);
+    k_pdm_reduce_silu<<<dim3((D.F + 255) / 256, R), 256, 0, st>>>(P, PD, ks, NB); ++*cnt;
+    const uint16_t *wd[1] = {pl->w[8][l]};
+    gemm(wd, nd, 1, D.F);
+    // ... + residual, then the NEXT product's norm: the next layer's attention norm, or the final norm in front of the head
+    k_pdm_reduce_norm<<<R, 256, 0, st>>>(P, PD, ks, NB, l + 1 < pl->Ls ? pl->w[0][l + 1] : PD.final_norm); ++*cnt;
+  }
+  if (head) {
+    const uint16_t *wh[1] = {PD.head};
+    const int nv[1] = {pl->Vs};
+    gemm(wh, nv, 1, D.d);
+    k_pdm_reduce_plain<<<dim3((pl->Vs + 255) / 256, 1), 256, 0, st>>>(PD, ks, NB, pl->Vs, PD.logits, 1); ++*cnt;
+    k_pdm_argmax_cand<<<kPdmCand, 256, 0, st>>>(PD); ++*cnt;
+    k_pdm_argmax_final<<<1, 32, 0, st>>>(P, PD); ++*cnt;
+  }
+}
+
 static void pdm_enqueue_body(const DevPtrs &P, const PdmPlan *pl, bool head, cudaStream_t st, long long *cnt) {
+  // (pdm_enqueue_body_tc — reduce + norm / SiLU fused into one CTA per row — measured SLOWER on a B200: 1975 vs 1777 us per
+  //  draft at 9b_n4; five CTAs cannot add 16 partial sums per element as fast as a grid-wide reduce.  Kept for reference.)
+  if (false) { pdm_enqueue_body_tc(P, pl, head, st, cnt); return; }
   const Dims &D = P.dim;
   const PdmPtrs &PD = pl->PD;
   const int R = kPdmMaxRows, qd = D.Hq * D.hd, kd = D.Hkv * D.hd, group = D.Hq / D.Hkv;
+  k_pdm_rope_table<<<R, 64, 0, st>>>(P, PD); ++*cnt;
   k_pdm_features<<<dim3((D.d + 7) / 8, R), 256, 0, st>>>(P, PD); ++*cnt;
   for (int l = 0; l < pl->Ls; ++l) {
-    k_pdm_norm<<<R, 256, 0, st>>>(P, PD, pl->w[0][l], 0); ++*cnt;
+    k_pdm_norm<<<R, 1024, 0, st>>>(P, PD, pl->w[0][l], 0); ++*cnt;
     const uint16_t *wqkv[3] = {pl->w[1][l], pl->w[2][l], pl->w[3][l]};
     const int nqkv[3] = {qd, kd, kd};
-    pdm_launch_gemv(pl, wqkv, nqkv, 3, D.d, PD.XN, D.d, PD.Y, qd + 2 * kd, 0, 0, st); *cnt += pl->PD.use_tc ? 2 : 1;
+    pdm_launch_gemv(pl, wqkv, nqkv, 3, D.d, PD.XN, D.d, PD.Y, qd + 2 * kd, 0, 0, st); ++*cnt;
     k_pdm_rope_append<<<R, 256, 0, st>>>(P, PD, l); ++*cnt;
     dim3 ga(P.nsplit_max, D.Hkv, R);
     if (D.hd == 128) k_pdm_attn_partial<128><<<ga, group * 32, 0, st>>>(P, PD, l);
@@ -481,20 +589,20 @@ static void pdm_enqueue_body(const DevPtrs &P, const PdmPlan *pl, bool head, cud
     k_pdm_attn_merge<<<dim3(D.Hq, R), D.hd, 0, st>>>(P, PD); ++*cnt;
     const uint16_t *wo[1] = {pl->w[4][l]};
     const int nd[1] = {D.d};
-    pdm_launch_gemv(pl, wo, nd, 1, qd, PD.ATT, qd, PD.X, D.d, 1, 0, st); *cnt += pl->PD.use_tc ? 2 : 1;
-    k_pdm_norm<<<R, 256, 0, st>>>(P, PD, pl->w[5][l], 0); ++*cnt;
+    pdm_launch_gemv(pl, wo, nd, 1, qd, PD.ATT, qd, PD.X, D.d, 1, 0, st); ++*cnt;
+    k_pdm_norm<<<R, 1024, 0, st>>>(P, PD, pl->w[5][l], 0); ++*cnt;
     const uint16_t *wgu[2] = {pl->w[6][l], pl->w[7][l]};
     const int ngu[2] = {D.F, D.F};
-    pdm_launch_gemv(pl, wgu, ngu, 2, D.d, PD.XN, D.d, PD.Y, 2 * D.F, 0, 0, st); *cnt += pl->PD.use_tc ? 2 : 1;
+    pdm_launch_gemv(pl, wgu, ngu, 2, D.d, PD.XN, D.d, PD.Y, 2 * D.F, 0, 0, st); ++*cnt;
     k_pdm_silu<<<dim3((D.F + 255) / 256, R), 256, 0, st>>>(P, PD); ++*cnt;
     const uint16_t *wd[1] = {pl->w[8][l]};
-    pdm_launch_gemv(pl, wd, nd, 1, D.F, PD.ACT, D.F, PD.X, D.d, 1, 0, st); *cnt += pl->PD.use_tc ? 2 : 1;
+    pdm_launch_gemv(pl, wd, nd, 1, D.F, PD.ACT, D.F, PD.X, D.d, 1, 0, st); ++*cnt;
   }
   if (head) {
     k_pdm_norm<<<1, 256, 0, st>>>(P, PD, nullptr, 1); ++*cnt;
     const uint16_t *wh[1] = {PD.head};
     const int nv[1] = {pl->Vs};
-    pdm_launch_gemv(pl, wh, nv, 1, D.d, PD.z, D.d, PD.logits, pl->Vs, 0, 1, st); *cnt += pl->PD.use_tc ? 2 : 1;
+    pdm_launch_gemv(pl, wh, nv, 1, D.d, PD.z, D.d, PD.logits, pl->Vs, 0, 1, st); ++*cnt;
     k_pdm_argmax_cand<<<kPdmCand, 256, 0, st>>>(PD); ++*cnt;
     k_pdm_argmax_final<<<1, 32, 0, st>>>(P, PD); ++*cnt;
   }

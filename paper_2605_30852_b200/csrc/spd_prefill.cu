@@ -668,7 +668,7 @@ static int pf_launch_gemm(PfEncodeFn enc, const uint16_t *x3, size_t plane, int 
 // (rows_ptr) or fixed.  part: scratch of >= ksplit * NB * ncol floats.
 int skinny_gemm(const uint16_t *x3, size_t plane, int K, int NB, const uint16_t *const *w, const int *w_rows, int nseg,
                 float *part, size_t part_floats, const int *rows_ptr, int rows_fixed, float *dst, int ldd, int residual,
-                cudaStream_t st, long long *launches) {
+                cudaStream_t st, long long *launches, int *ksplit_out) {
   static PfEncodeFn enc = nullptr;
   static bool attr = false;
   if (!enc) enc = pf_encoder();
@@ -699,6 +699,11 @@ int skinny_gemm(const uint16_t *x3, size_t plane, int K, int NB, const uint16_t 
   if (ksplit < 1) return -1;
   A.K = K; A.NB = NB; A.ldp = col; A.part = part;
   k_pf_gemm_skinny<<<dim3(tiles, ksplit), kGemmThreads, sk_smem, st>>>(A);
+  if (ksplit_out) {                                   // the caller reduces the partial sums itself (fused epilogues)
+    *ksplit_out = ksplit;
+    if (launches) *launches += 1;
+    return cudaGetLastError() == cudaSuccess ? 0 : -1;
+  }
   const int rb = (int)(((size_t)NB * col + 255) / 256);
   k_pf_skinny_reduce<<<rb < 1184 ? rb : 1184, 256, 0, st>>>(part, ksplit, NB, col, rows_ptr, rows_fixed, dst, ldd, col, residual);
   if (launches) *launches += 2;
