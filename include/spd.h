@@ -90,6 +90,8 @@ typedef struct {
 typedef struct {
   void *repack, *kv, *work;        /* DEVICE, >= the sizes above, 256-byte aligned            */
   void *stream_main, *stream_pdm;  /* cudaStream_t handles (e.g. torch.cuda.Stream.cuda_stream) */
+  size_t repack_bytes, kv_bytes, work_bytes; /* what the caller allocated: spd_create returns SPD_ENOMEM if any is
+                                      smaller than spd_query_sizes reports (an undersized buffer never reaches a kernel) */
 } spd_buffers;
 
 /* What one cycle did.  step_index = K after the step (K counts cycles since prefill);

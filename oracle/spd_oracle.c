@@ -925,6 +925,7 @@ int ora_rollback(ora_ctx *o, int32_t new_len, int32_t reseed_token) {
   o->c = new_len;
   if (o->pdm_final > new_len) o->pdm_final = new_len;
   o->emitted = new_len - o->prompt_len + 1; /* tokens emitted up to and including the reseed token */
+  if (o->emitted < 1) o->emitted = 1;       /* a rollback into the prompt: the reseed token is the first emitted one */
   for (int l = 0; l < o->cfg.n_layers; ++l)
     if (o->len[l] > new_len) o->len[l] = new_len;
   ring_set_single(o, new_len, reseed_token);

@@ -76,7 +76,8 @@ class _Sizes(C.Structure):
 
 class _Buffers(C.Structure):
     _fields_ = [("repack", C.c_void_p), ("kv", C.c_void_p), ("work", C.c_void_p),
-                ("stream_main", C.c_void_p), ("stream_pdm", C.c_void_p)]
+                ("stream_main", C.c_void_p), ("stream_pdm", C.c_void_p),
+                ("repack_bytes", C.c_size_t), ("kv_bytes", C.c_size_t), ("work_bytes", C.c_size_t)]
 
 
 class _PdmWeights(C.Structure):
@@ -231,7 +232,8 @@ class SPD:
             self._tabs.append(tab)
             setattr(w, name, C.cast(tab, _PP))
         bufs = _Buffers(self._repack.data_ptr(), self._kv.data_ptr(), self._work.data_ptr(),
-                        self.stream_main.cuda_stream, self.stream_pdm.cuda_stream)
+                        self.stream_main.cuda_stream, self.stream_pdm.cuda_stream,
+                        self._repack.numel(), self._kv.numel(), self._work.numel())
         torch.cuda.synchronize(dev)
         h = C.c_void_p()
         rc = L.spd_create(C.byref(cfg), C.byref(w), C.byref(bufs), C.byref(h))

@@ -205,7 +205,8 @@ __global__ void k_rollback(DevPtrs P, int new_len, int tok) {
   __syncthreads();
   if (threadIdx.x == 0) {
     st->c = new_len;
-    st->N = (long long)new_len - st->prompt_len + 1;   // tokens emitted up to and including the reseed token
+    const long long nn = (long long)new_len - st->prompt_len + 1;   // tokens emitted up to and including the reseed token
+    st->N = nn > 1 ? nn : 1;                           // a rollback into the prompt: the reseed token is the first emitted one
     for (int k = 1; k < P.dim.n; ++k) st->occ[k] = 0;
     st->occ[0] = 1; st->pos[0] = new_len; st->tok[0] = tok;
   }
@@ -215,6 +216,18 @@ __global__ void k_rollback(DevPtrs P, int new_len, int tok) {
 }  // namespace spd
 
 // ------------------------------------------------------------------ create / destroy -----------
+// Everything a half-built context may own (events, pinned buffers, plans): one exit for every failure of spd_create.
+static void create_cleanup(spd_ctx *ctx) {
+  if (!ctx) return;
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+  if (ctx->h_results) cudaFreeHost(ctx->h_results);
+  if (ctx->h_state) cudaFreeHost(ctx->h_state);
+  free(ctx->pf);
+  free(ctx);
+  cudaGetLastError();
+}
+
 extern "C" int spd_create(const spd_config *cfg, const spd_weights *w, const spd_buffers *bufs, spd_ctx **out) {
   if (!out) return SPD_EINVAL;
   if (!validate(cfg) || !w || !bufs) return SPD_EINVAL;
@@ -226,6 +239,8 @@ extern "C" int spd_create(const spd_config *cfg, const spd_weights *w, const spd
   spd_sizes need;
   spd_query_sizes(cfg, &need);
   if (!bufs->kv || !bufs->work || (need.repack_bytes && !bufs->repack)) return SPD_ENOMEM;
+  if (bufs->kv_bytes < need.kv_bytes || bufs->work_bytes < need.work_bytes || bufs->repack_bytes < need.repack_bytes)
+    return SPD_ENOMEM;
   spd_ctx *ctx = (spd_ctx *)calloc(1, sizeof(spd_ctx));
   if (!ctx) return SPD_ENOMEM;
   ctx->cfg = *cfg; ctx->bufs = *bufs; ctx->sizes = need;
@@ -233,7 +248,7 @@ extern "C" int spd_create(const spd_config *cfg, const spd_weights *w, const spd
 #define CUC(call)                                                                                         \
   do {                                                                                                    \
     cudaError_t e_ = (call);                                                                              \
-    if (e_ != cudaSuccess) { fprintf(stderr, "spd_create: %s\n", cudaGetErrorString(e_)); free(ctx); return SPD_ECUDA; } \
+    if (e_ != cudaSuccess) { fprintf(stderr, "spd_create: %s\n", cudaGetErrorString(e_)); create_cleanup(ctx); return SPD_ECUDA; } \
   } while (0)
   CUC(cudaSetDevice(cfg->device));
   const uint16_t **tables[9];
@@ -245,7 +260,7 @@ extern "C" int spd_create(const spd_config *cfg, const spd_weights *w, const spd
   const uint16_t *const *src[9] = {w->attn_norm, w->wq, w->wk, w->wv, w->wo, w->mlp_norm, w->w_gate, w->w_up, w->w_down};
   for (int i = 0; i < 9; ++i) {
     for (int l = 0; l < cfg->n_layers; ++l)
-      if (!src[i][l]) { free(ctx); return SPD_EINVAL; }
+      if (!src[i][l]) { create_cleanup(ctx); return SPD_EINVAL; }
     CUC(cudaMemcpyAsync((void *)tables[i], src[i], sizeof(void *) * cfg->n_layers, cudaMemcpyHostToDevice, ctx->sm));
   }
   int half = cfg->head_dim / 2;
