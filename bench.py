@@ -274,6 +274,10 @@ def run_gpu(args, shape):
     ctx_mid = (res[0].committed_len + res[-1].committed_len) // 2 + n // 2
     by = step_bytes(shape, ctx_mid)
 
+    phases = None
+    if args.phase_profile:     # per-phase stamps of saturated cycles (the pipeline is still saturated at p = 1)
+        phases = phase_table(eng, shape)
+
     # ---- e2e: one host call per cycle, result D2H + sync inside the timed region -----------------
     ke = min(args.steps, max(50, args.steps // 4))
     torch.cuda.synchronize()
@@ -438,7 +442,7 @@ def run_gpu(args, shape):
         "step_us_stats": {**percentiles(timed_lat), "unit": "us",
                           "source": "finish-stamp differences (%globaltimer, SPD_DBG_CYCLE_TIMES) of the timed back-to-back cycles"},
         "by_fill": by_fill_table(shape, fill_samples, peak),
-        "prefill": prefill_report(shape, P, prefill_ms), "paper_pdm": paper,
+        "prefill": prefill_report(shape, P, prefill_ms), "paper_pdm": paper, "phase_profile": phases,
         "gpu_launches": int(tot["gpu_launches"]), "clocks": clk, "p_sweep": sweep, "sampling": sampling,
         "setup_s": t_setup,
     }
@@ -449,6 +453,45 @@ def run_gpu(args, shape):
                                           f"of length {ctx_mid}"}
     print(json.dumps(line), flush=True)
     eng.close()
+
+
+PHASE_NAMES = {0: "PDM", 1: "QKV", 2: "ATTN", 3: "O", 4: "GATEUP", 5: "DOWN", 6: "HEAD"}
+
+
+def phase_table(eng, shape, cycles: int = 8) -> dict:
+    """Per-phase breakdown of the fused cycle kernel from its own clock stamps (SPD_OPT_PHASE_PROFILE; not under a
+    profiler): mean over CTAs and over `cycles` saturated cycles of wait (this CTA's last tile of the previous phase ->
+    its group's barrier open), stage (activation vector into shared memory, RMSNorm) and consume (streaming the phase's
+    tiles), in us, per phase type; `per_cycle_us` = (wait + stage + consume) x occurrences."""
+    import paper_2605_30852_b200 as spd
+    per = shape.n_layers // shape.n_stages
+    npz = 2 + 5 * per
+    eng.set_option(spd.OPT.PHASE_PROFILE, 1)
+    acc = {}
+    for _ in range(cycles):
+        eng.step()
+        pr = eng.phase_profile().astype(np.int64)                 # [cta, phase, stamp]
+        c0, g0, c1, g1 = pr[0, 167, 0], pr[0, 167, 1], pr[0, 167, 4], pr[0, 167, 5]
+        mhz = (c1 - c0) / max(g1 - g0, 1) * 1e3                   # SM clocks per us
+        ncta = int(np.count_nonzero(pr[:, npz - 1, 2]))
+        for p in range(npz):
+            t = 0 if p == 0 else (6 if p == npz - 1 else 1 + (p - 1) % 5)
+            s0, s1, s2 = pr[:ncta, p, 0], pr[:ncta, p, 1], pr[:ncta, p, 2]
+            prev = pr[:ncta, p - 1, 2] if p > 0 else pr[:ncta, 167, 0]
+            ok = (s0 > 0) & (s2 >= s1) & (s1 >= s0) & (prev > 0)
+            if not ok.any():
+                continue
+            a = acc.setdefault(t, {"wait": [], "stage": [], "consume": []})
+            a["wait"].append(float(np.mean((s0 - prev)[ok])) / mhz)
+            a["stage"].append(float(np.mean((s1 - s0)[ok])) / mhz)
+            a["consume"].append(float(np.mean((s2 - s1)[ok])) / mhz)
+    eng.set_option(spd.OPT.PHASE_PROFILE, 0)
+    out = {}
+    for t, a in sorted(acc.items()):
+        count = 1 if t in (0, 6) else per
+        w, st, co = (float(np.mean(a[k])) for k in ("wait", "stage", "consume"))
+        out[PHASE_NAMES[t]] = {"count": count, "wait_us": w, "stage_us": st, "consume_us": co, "per_cycle_us": (w + st + co) * count}
+    return out
 
 
 def percentiles(x) -> dict:
@@ -527,6 +570,7 @@ def main():
     ap.add_argument("--engine", type=int, default=None, help="0 reference engine, 1 fused engine (default: library default)")
     ap.add_argument("--seed", type=int, default=1234)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--phase-profile", action="store_true", help="add the fused kernel's per-phase breakdown (its own clock stamps)")
     ap.add_argument("--no-paper-pdm", action="store_true", help="skip the NEXT-1 leg (the paper's PDM in place of the simplified one)")
     args = ap.parse_args()
     shape = si.CONFIGS[args.config]

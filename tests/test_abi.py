@@ -61,6 +61,23 @@ def test_query_sizes_and_validation(lib):
         assert e.value.status == 1  # SPD_EINVAL
 
 
+def test_pdm_query_sizes_and_validation(lib):
+    """spd_pdm_query_sizes needs no GPU: the PDM's cache is L_s layers of the target's per-layer cache, the work buffer
+    holds at least the anchors H^b of every position ([max_seq][m][d] fp32, m = 5 anchors for L >= 8)."""
+    from paper_2605_30852_b200.binding import _PdmSizes, _cfg_of
+    for name in ("tiny", "9b_n4"):
+        shape = si.CONFIGS[name]
+        cfg = _cfg_of(shape, shape.max_seq, 0)
+        sz = _PdmSizes()
+        assert lib.spd_pdm_query_sizes(C.byref(cfg), 3, 300, C.byref(sz)) == 0
+        assert sz.kv_bytes == 3 * 2 * shape.n_kv_heads * shape.head_dim * 2 * shape.max_seq
+        assert sz.work_bytes > shape.max_seq * si.pdm_anchor_count(shape.n_layers) * shape.d_model * 4
+        for layers, vocab in ((0, 300), (3, 0), (3, shape.vocab + 1), (1000, 300)):
+            assert lib.spd_pdm_query_sizes(C.byref(cfg), layers, vocab, C.byref(sz)) == 1      # SPD_EINVAL
+    assert lib.spd_pdm_attach(None, None, None, None) == 1
+    assert si.pdm_anchor_count(32) == 5 and si.pdm_anchor_count(8) == 5 and si.pdm_anchor_count(4) == 4
+
+
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
 def test_no_gpu_means_no_compute_not_a_fallback(lib):
     from paper_2605_30852_b200.binding import _Cfg, _Weights, _Buffers, _cfg_of
@@ -70,7 +87,7 @@ def test_no_gpu_means_no_compute_not_a_fallback(lib):
     w = _Weights()
     for k, _ in _Weights._fields_:
         setattr(w, k, C.cast(dummy, C.POINTER(C.c_void_p)) if k not in ("embed", "final_norm", "pdm_proj", "pdm_norm") else 8)
-    bufs = _Buffers(8, 8, 8, None, None)
+    bufs = _Buffers(8, 8, 8, None, None, 1 << 40, 1 << 40, 1 << 40)
     h = C.c_void_p()
     assert lib.spd_create(C.byref(cfg), C.byref(w), C.byref(bufs), C.byref(h)) == 4  # SPD_ECUDA
     assert not h.value
