@@ -276,9 +276,15 @@ __global__ void k_pdm_rope_append(DevPtrs P, PdmPtrs PD, int layer) {
 }
 
 // Split-KV attention of every row over the PDM cache rows 0 .. pos (fixed 128-row splits merged in split order, as the
-// target's): grid (split, kv head, kPdmMaxRows), one warp per q head of the group.
+// target's): grid (split, kv head, kPdmMaxRows), one warp per q head of the group.  Written for memory-level
+// parallelism (a draft has few rows, so a warp must keep many loads in flight) with coalesced rows: scores — HD/8 lanes
+// share a K row (one 16-byte chunk each, q chunk in registers), 32/(HD/8) rows per load instruction, 8 instructions in
+// flight, a 4- or 3-step xor tree per row; softmax over the split with the scores parked in shared memory; P.V with 8 V
+// rows in flight (lane = HD/32 head-dim elements).  Fixed order per (row, head, split): batch-invariant.
 template <int HD>
 __global__ void k_pdm_attn_partial(DevPtrs P, PdmPtrs PD, int layer) {
+  constexpr int EPL = HD / 32, LPR = HD / 8, RPI = 32 / LPR, U = 8;
+  __shared__ float ps[8][kAttnSplit];
   const Dims &D = P.dim;
   const PdmRun *R = PD.run;
   const int r = blockIdx.z;
@@ -286,10 +292,70 @@ __global__ void k_pdm_attn_partial(DevPtrs P, PdmPtrs PD, int layer) {
   const int T = R->first + r + 1, split = blockIdx.x, t0 = split * kAttnSplit;
   if (t0 >= T) return;
   const int t1 = min(T, t0 + kAttnSplit), kvh = blockIdx.y, group = D.Hq / D.Hkv;
-  const int hq = kvh * group + (threadIdx.x >> 5);
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int hq = kvh * group + w;
   const uint16_t *kc = PD.kv + kv_offset(D, layer, 0, kvh), *vc = PD.kv + kv_offset(D, layer, 1, kvh);
+  const int sub = lane / LPR, hl = lane % LPR;            // which row of an instruction's RPI rows, which chunk of it
+  const float4 qa = *reinterpret_cast<const float4 *>(PD.Q + ((size_t)r * D.Hq + hq) * HD + 8 * hl);
+  const float4 qb = *reinterpret_cast<const float4 *>(PD.Q + ((size_t)r * D.Hq + hq) * HD + 8 * hl + 4);
+  const float scale = 1.0f / sqrtf((float)HD);
+  const int nrows = t1 - t0;
+  for (int i0 = 0; i0 < kAttnSplit; i0 += RPI * U) {
+    uint4 kw[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int i = i0 + RPI * u + sub;
+      kw[u] = make_uint4(0u, 0u, 0u, 0u);
+      if (i < nrows) kw[u] = __ldg(reinterpret_cast<const uint4 *>(kc + (size_t)(t0 + i) * HD) + hl);
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      float a = bf16_lo(kw[u].x) * qa.x;
+      a = fmaf(bf16_hi(kw[u].x), qa.y, a); a = fmaf(bf16_lo(kw[u].y), qa.z, a); a = fmaf(bf16_hi(kw[u].y), qa.w, a);
+      a = fmaf(bf16_lo(kw[u].z), qb.x, a); a = fmaf(bf16_hi(kw[u].z), qb.y, a);
+      a = fmaf(bf16_lo(kw[u].w), qb.z, a); a = fmaf(bf16_hi(kw[u].w), qb.w, a);
+#pragma unroll
+      for (int o = LPR / 2; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+      const int i = i0 + RPI * u + sub;
+      if (hl == 0) ps[w][i] = i < nrows ? a * scale : -INFINITY;
+    }
+  }
+  __syncwarp();
+  float sc[kAttnSplit / 32], m = -INFINITY;
+#pragma unroll
+  for (int j = 0; j < kAttnSplit / 32; ++j) { sc[j] = ps[w][lane + 32 * j]; m = fmaxf(m, sc[j]); }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  __syncwarp();
+  float l = 0.f;
+#pragma unroll
+  for (int j = 0; j < kAttnSplit / 32; ++j) {
+    const float pr = sc[j] == -INFINITY ? 0.f : expf(sc[j] - m);
+    ps[w][lane + 32 * j] = pr;
+    l += pr;
+  }
+  l = warp_sum(l);
+  __syncwarp();
+  float acc[EPL];
+#pragma unroll
+  for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
+#pragma unroll 8
+  for (int i = 0; i < nrows; ++i) {
+    const uint16_t *vr = vc + (size_t)(t0 + i) * HD + lane * EPL;
+    const float pr = ps[w][i];
+    if constexpr (EPL == 4) {
+      const uint2 vw = __ldg(reinterpret_cast<const uint2 *>(vr));
+      acc[0] = fmaf(pr, bf16_lo(vw.x), acc[0]); acc[1] = fmaf(pr, bf16_hi(vw.x), acc[1]);
+      acc[2] = fmaf(pr, bf16_lo(vw.y), acc[2]); acc[3] = fmaf(pr, bf16_hi(vw.y), acc[3]);
+    } else {
+      const uint32_t vw = __ldg(reinterpret_cast<const uint32_t *>(vr));
+      acc[0] = fmaf(pr, bf16_lo(vw), acc[0]); acc[1] = fmaf(pr, bf16_hi(vw), acc[1]);
+    }
+  }
   const size_t slot = ((size_t)r * D.Hq + hq) * P.nsplit_max + split;
-  attn_partial_warp<HD>(PD.Q + ((size_t)r * D.Hq + hq) * HD, kc, vc, t0, t1, PD.part_o + slot * HD, PD.part_ml + slot);
+#pragma unroll
+  for (int e = 0; e < EPL; ++e) PD.part_o[slot * HD + lane * EPL + e] = acc[e];
+  if (lane == 0) PD.part_ml[slot] = make_float2(m, l);
 }
 
 // grid (q head, kPdmMaxRows); block = hd threads

@@ -233,7 +233,7 @@ struct SkinnyArgs {
   CUtensorMap w[3];                // [N_seg, K] bf16, box {64, 128}
   CUtensorMap x[3];                // the three bf16 parts of the activation rows: [48, K], box {64, NB}
   int seg_tiles[3], seg_n[3], seg_col0[3];
-  int K, NB, ldp;                  // ldp = columns of one partial row (sum of the segments' rows)
+  int K, NB, ldp, ksplit;          // ldp = columns of one partial row (sum of the segments' rows)
   float *part;                     // [gridDim.y][NB][ldp]
 };
 
@@ -250,87 +250,127 @@ __device__ __forceinline__ void tc_ld_32x16(uint32_t taddr, float (&v)[16]) {
   for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 }
 
+// PERSISTENT: gridDim.x <= #SMs CTAs walk the work items (weight tile, K split) item = blockIdx.x, + gridDim.x, ...; the
+// TMA producer streams across item boundaries without draining the ring, the MMA thread alternates between two TMEM
+// accumulators so the epilogue of one item (TMEM -> partial sums) overlaps the next item's MMAs.
 __global__ void __launch_bounds__(kGemmThreads, 1) k_pf_gemm_skinny(const __grid_constant__ SkinnyArgs A) {
   extern __shared__ uint8_t pf_smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>(((uintptr_t)pf_smem_raw + 1023) & ~(uintptr_t)1023);
   const int NB = A.NB, kSkStages = sk_stages(NB), kSkStageBytes = sk_stage_bytes(NB);
   uint64_t *full = reinterpret_cast<uint64_t *>(smem + kSkStages * kSkStageBytes);
   uint64_t *empty = full + kSkMaxStages;
-  uint64_t *tmem_full = empty + kSkMaxStages;
-  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_full + 1);
+  uint64_t *tmem_full = empty + kSkMaxStages;          // [2]
+  uint64_t *tmem_empty = tmem_full + 2;                // [2]
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_empty + 2);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  int seg = 0, tile = blockIdx.x;
-  while (seg < 2 && tile >= A.seg_tiles[seg]) { tile -= A.seg_tiles[seg]; ++seg; }
-  const int n0 = tile * kGemmBM;
-  const int nkb_all = A.K / kGemmBK, per = (nkb_all + gridDim.y - 1) / gridDim.y;
-  const int kb0 = blockIdx.y * per, kb1 = min(nkb_all, kb0 + per), nkb = max(0, kb1 - kb0);
+  const int tiles = A.seg_tiles[0] + A.seg_tiles[1] + A.seg_tiles[2];
+  const int n_items = tiles * A.ksplit;
+  const int nkb_all = A.K / kGemmBK, per = (nkb_all + A.ksplit - 1) / A.ksplit;
   const uint32_t stage_tx = (uint32_t)(kGemmBM * 128 + 3 * NB * 128);
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < kSkStages; ++s) { pf_mbar_init(&full[s], 1); pf_mbar_init(&empty[s], 1); }
-    pf_mbar_init(tmem_full, 1);
+    for (int a = 0; a < 2; ++a) { pf_mbar_init(&tmem_full[a], 1); pf_mbar_init(&tmem_empty[a], 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(pf_smem_u32(tmem_slot)), "r"(64u) : "memory");
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(pf_smem_u32(tmem_slot)), "r"(128u) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_d = *tmem_slot;
+  const uint32_t tmem_base = *tmem_slot;
+
+  // item -> (segment, weight tile, K range)
+  auto decode = [&](int item, int &seg, int &n0, int &kb0, int &nkb) {
+    int tile = item / A.ksplit;
+    const int ks = item - tile * A.ksplit;
+    seg = 0;
+    while (seg < 2 && tile >= A.seg_tiles[seg]) { tile -= A.seg_tiles[seg]; ++seg; }
+    n0 = tile * kGemmBM;
+    kb0 = ks * per;
+    nkb = max(0, min(nkb_all, kb0 + per) - kb0);
+    return ks;
+  };
 
   if (warp == 0) {
-    if (lane == 0) {
-      for (int i = 0; i < nkb; ++i) {
-        const int s = i % kSkStages, it = i / kSkStages, kb = kb0 + i;
-        pf_mbar_wait(&empty[s], (it & 1) ^ 1);
-        uint8_t *st = smem + (size_t)s * kSkStageBytes;
-        pf_mbar_expect_tx(&full[s], stage_tx);
-        pf_tma_load_2d(st, &A.w[seg], kb * kGemmBK, n0, &full[s]);
+    if (lane == 0) {   // ===== TMA producer: one continuous stream over this CTA's items =====
+      uint32_t q = 0;
+      for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        int seg, n0, kb0, nkb;
+        decode(item, seg, n0, kb0, nkb);
+        for (int i = 0; i < nkb; ++i, ++q) {
+          const int s = q % kSkStages, it = q / kSkStages, kb = kb0 + i;
+          pf_mbar_wait(&empty[s], (it & 1) ^ 1);
+          uint8_t *st = smem + (size_t)s * kSkStageBytes;
+          pf_mbar_expect_tx(&full[s], stage_tx);
+          pf_tma_load_2d(st, &A.w[seg], kb * kGemmBK, n0, &full[s]);
 #pragma unroll
-        for (int p = 0; p < 3; ++p) pf_tma_load_2d(st + kGemmBM * 128 + p * NB * 128, &A.x[p], kb * kGemmBK, 0, &full[s]);
+          for (int p = 0; p < 3; ++p) pf_tma_load_2d(st + kGemmBM * 128 + p * NB * 128, &A.x[p], kb * kGemmBK, 0, &full[s]);
+        }
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
+    if (lane == 0) {   // ===== MMA issuer: two accumulators, alternating per item =====
       const uint32_t idesc = tc_idesc_bf16(kGemmBM, NB);
-      for (int i = 0; i < nkb; ++i) {
-        const int s = i % kSkStages, it = i / kSkStages;
-        pf_mbar_wait(&full[s], it & 1);
+      uint32_t q = 0;
+      int n_mine = 0;
+      for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++n_mine) {
+        int seg, n0, kb0, nkb;
+        decode(item, seg, n0, kb0, nkb);
+        const int acc = n_mine & 1, use = n_mine >> 1;
+        pf_mbar_wait(&tmem_empty[acc], (use & 1) ^ 1);   // the epilogue drained this accumulator (first use: passes)
         tc_fence_after();
-        const uint32_t a = pf_smem_u32(smem + (size_t)s * kSkStageBytes), b = a + kGemmBM * 128;
+        const uint32_t tmem_d = tmem_base + (uint32_t)(acc * 64);
+        for (int i = 0; i < nkb; ++i, ++q) {
+          const int s = q % kSkStages, it = q / kSkStages;
+          pf_mbar_wait(&full[s], it & 1);
+          tc_fence_after();
+          const uint32_t a = pf_smem_u32(smem + (size_t)s * kSkStageBytes), b = a + kGemmBM * 128;
 #pragma unroll
-        for (int k = 0; k < kGemmBK / 16; ++k) {
-          const uint64_t ad = tc_smem_desc(a + k * 32);
+          for (int k = 0; k < kGemmBK / 16; ++k) {
+            const uint64_t ad = tc_smem_desc(a + k * 32);
 #pragma unroll
-          for (int p = 0; p < 3; ++p)
-            tc_mma_bf16(tmem_d, ad, tc_smem_desc(b + p * NB * 128 + k * 32), idesc, (i | k | p) ? 1u : 0u);
+            for (int p = 0; p < 3; ++p)
+              tc_mma_bf16(tmem_d, ad, tc_smem_desc(b + p * NB * 128 + k * 32), idesc, (i | k | p) ? 1u : 0u);
+          }
+          tc_commit(&empty[s]);
         }
-        tc_commit(&empty[s]);
+        tc_commit(&tmem_full[acc]);
       }
-      tc_commit(tmem_full);
     }
-  } else {
-    pf_mbar_wait(tmem_full, 0);
-    tc_fence_after();
+  } else {             // ===== epilogue: TMEM -> split-K partial sums =====
     const int lg = warp & 3;
-    const int n = n0 + lg * 32 + lane;               // this thread's weight row = output column
-    const bool ok = n < A.seg_n[seg] && nkb > 0;
-    float *prow = A.part + ((size_t)blockIdx.y * NB) * A.ldp + A.seg_col0[seg] + n;
-    for (int c = 0; c < NB; c += 16) {
-      float v[16];
-      if (nkb > 0) tc_ld_32x16(tmem_d + ((uint32_t)(lg * 32) << 16) + (uint32_t)c, v);
+    int n_mine = 0;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++n_mine) {
+      int seg, n0, kb0, nkb;
+      const int ks = decode(item, seg, n0, kb0, nkb);
+      const int acc = n_mine & 1, use = n_mine >> 1;
+      pf_mbar_wait(&tmem_full[acc], use & 1);
+      tc_fence_after();
+      const int n = n0 + lg * 32 + lane;               // this thread's weight row = output column
+      const bool in = n < A.seg_n[seg];
+      float *prow = A.part + ((size_t)ks * NB) * A.ldp + A.seg_col0[seg] + n;
+      for (int c = 0; c < NB; c += 16) {
+        float v[16];
+        tc_ld_32x16(tmem_base + (uint32_t)(acc * 64) + ((uint32_t)(lg * 32) << 16) + (uint32_t)c, v);
 #pragma unroll
-      for (int r = 0; r < 16; ++r)
-        if (n < A.seg_n[seg]) prow[(size_t)(c + r) * A.ldp] = ok ? v[r] : 0.f;
+        for (int r = 0; r < 16; ++r)
+          if (in) prow[(size_t)(c + r) * A.ldp] = nkb > 0 ? v[r] : 0.f;
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) {
+        asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(pf_smem_u32(&tmem_empty[acc])) : "memory");
+      }
     }
   }
   tc_fence_before();
   __syncthreads();
   if (warp == 1) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"(64u) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(128u) : "memory");
   }
 }
 
@@ -692,13 +732,21 @@ int skinny_gemm(const uint16_t *x3, size_t plane, int K, int NB, const uint16_t 
   for (int p = 0; p < 3; ++p)
     if (pf_make_map(enc, &A.x[p], x3 + p * plane, kSkMaxNB, K, NB)) return -1;
   const int nkb = K / kGemmBK;
-  int ksplit = (2 * 148 + tiles - 1) / tiles;          // about two CTAs per SM in total
-  if (ksplit > nkb / 4) ksplit = nkb / 4 > 0 ? nkb / 4 : 1;
-  if (ksplit > 16) ksplit = 16;
-  if ((size_t)ksplit * NB * col > part_floats) ksplit = (int)(part_floats / ((size_t)NB * col));
-  if (ksplit < 1) return -1;
-  A.K = K; A.NB = NB; A.ldp = col; A.part = part;
-  k_pf_gemm_skinny<<<dim3(tiles, ksplit), kGemmThreads, sk_smem, st>>>(A);
+  // K split: work items of >= 8 k-blocks (>= 176 KB) whose count fills whole waves of the persistent grid
+  static int sms = 0;
+  if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms < 1) sms = 148; }
+  int ksplit = 1;
+  double best = -1.0;
+  for (int k = 1; k <= 16 && nkb / k >= 8; ++k) {
+    if ((size_t)k * NB * col > part_floats) break;
+    const int items = tiles * k, waves = (items + sms - 1) / sms;
+    const double eff = (double)items / ((double)waves * sms) - 0.01 * k;     // fuller waves first, then fewer partial sums
+    if (eff > best) { best = eff; ksplit = k; }
+  }
+  if ((size_t)ksplit * NB * col > part_floats) return -1;
+  A.K = K; A.NB = NB; A.ldp = col; A.part = part; A.ksplit = ksplit;
+  const int grid = tiles * ksplit < sms ? tiles * ksplit : sms;
+  k_pf_gemm_skinny<<<grid, kGemmThreads, sk_smem, st>>>(A);
   if (ksplit_out) {                                   // the caller reduces the partial sums itself (fused epilogues)
     *ksplit_out = ksplit;
     if (launches) *launches += 1;
