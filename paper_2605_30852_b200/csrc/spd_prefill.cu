@@ -33,6 +33,7 @@
 
 namespace spd {
 
+constexpr bool kPrefillAttnMma = true;    // prefill attention on mma.sync (false: the fp32 CUDA-core kernel)
 constexpr int kGemmBM = 128;              // tokens per tile (TMEM lanes)
 constexpr int kGemmBN = 256;              // output features per tile (TMEM fp32 columns)
 constexpr int kGemmBK = 64;               // bf16 elements per k block = one 128-byte swizzle row
@@ -653,6 +654,167 @@ __global__ void __launch_bounds__(256, 1) k_pf_attention(DevPtrs P, int layer, i
   }
 }
 
+// ------------------------------------------------------------------ prefill attention on the tensor cores -------
+// Same work split as k_pf_attention (one CTA = one kv head x 64 / G chunk tokens = 64 query rows, cache rows visited in
+// tiles of 64), but scores and P.V run as mma.sync.m16n8k16 (bf16 x bf16 -> fp32): warp w owns query rows 16 w .. 16 w + 15
+// and keeps Q (as bf16 hi + lo parts), the score / probability fragments and the 16 x HD output tile in registers
+// (flash-attention-2 layout: the score fragment of a thread IS the A fragment of P.V); K and V tiles stay bf16 in shared
+// memory, 16-byte chunks XOR-swizzled by (row & 7) so ldmatrix / ldmatrix.trans are bank-conflict-free.  q and the
+// probabilities are fp32 by contract (C-2.17): each is split into bf16 hi + lo (16 mantissa bits, products with the exact
+// bf16 K / V accumulate in fp32) — the representation the decode kernel's tensor-core attention already uses.
+__device__ __forceinline__ void pf_ldsm4(uint32_t (&r)[4], uint32_t addr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void pf_ldsm4t(uint32_t (&r)[4], uint32_t addr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void pf_mma(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void pf_split2(float x0, float x1, uint32_t &hi, uint32_t &lo) {
+  const uint16_t h0 = f32_to_bf16(x0), h1 = f32_to_bf16(x1);
+  const uint16_t l0 = f32_to_bf16(x0 - bf16_to_f32(h0)), l1 = f32_to_bf16(x1 - bf16_to_f32(h1));
+  hi = (uint32_t)h0 | ((uint32_t)h1 << 16);
+  lo = (uint32_t)l0 | ((uint32_t)l1 << 16);
+}
+
+template <int HD>
+__global__ void __launch_bounds__(128, 2) k_pf_attention_mma(DevPtrs P, int layer, int p0, int M, const float *Q,
+                                                             uint16_t *x3, size_t plane) {
+  constexpr int TK = 64, KS = HD / 16, NT = HD / 8, CPR = HD / 8;      // k steps of Q.K^T, n tiles of P.V, 16-byte chunks per row
+  const Dims &D = P.dim;
+  const int G = D.Hq / D.Hkv, TQ = 64 / G, qd = D.Hq * HD;
+  __shared__ __align__(128) uint16_t Ks[TK * HD];
+  __shared__ __align__(128) uint16_t Vs[TK * HD];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
+  const int mi = lane >> 3, mr = lane & 7;                             // ldmatrix: this lane addresses row mr of matrix mi
+  const int kvh = blockIdx.y, t0 = blockIdx.x * TQ;
+  // this thread's two query rows (of the CTA's 64): r_lo = 16 warp + g, r_hi = r_lo + 8; row = tq * G + head-in-group
+  const int r_lo = 16 * warp + g, r_hi = r_lo + 8;
+  const int tok_lo = t0 + r_lo / G, tok_hi = t0 + r_hi / G;
+  const int hq_lo = kvh * G + r_lo % G, hq_hi = kvh * G + r_hi % G;
+  const int pos_lo = p0 + tok_lo, pos_hi = p0 + tok_hi;
+  uint32_t qh[KS][4], ql[KS][4];
+#pragma unroll
+  for (int ks = 0; ks < KS; ++ks) {
+    float2 a = make_float2(0.f, 0.f), b = a, c = a, d = a;
+    if (tok_lo < M) {
+      const float *q = Q + (size_t)tok_lo * qd + (size_t)hq_lo * HD + 16 * ks + 2 * t;
+      a = *reinterpret_cast<const float2 *>(q); c = *reinterpret_cast<const float2 *>(q + 8);
+    }
+    if (tok_hi < M) {
+      const float *q = Q + (size_t)tok_hi * qd + (size_t)hq_hi * HD + 16 * ks + 2 * t;
+      b = *reinterpret_cast<const float2 *>(q); d = *reinterpret_cast<const float2 *>(q + 8);
+    }
+    pf_split2(a.x, a.y, qh[ks][0], ql[ks][0]); pf_split2(b.x, b.y, qh[ks][1], ql[ks][1]);
+    pf_split2(c.x, c.y, qh[ks][2], ql[ks][2]); pf_split2(d.x, d.y, qh[ks][3], ql[ks][3]);
+  }
+  float o[NT][4];
+#pragma unroll
+  for (int j = 0; j < NT; ++j) { o[j][0] = o[j][1] = o[j][2] = o[j][3] = 0.f; }
+  float m_lo = -INFINITY, m_hi = -INFINITY, l_lo = 0.f, l_hi = 0.f;
+  const float scale = 1.0f / sqrtf((float)HD);
+  const int last_pos = p0 + min(t0 + TQ, M) - 1;
+  const uint16_t *kc = P.kv + kv_offset(D, layer, 0, kvh), *vc = P.kv + kv_offset(D, layer, 1, kvh);
+  const uint32_t ks_base = pf_smem_u32(Ks), vs_base = pf_smem_u32(Vs);
+  for (int r0 = 0; r0 <= last_pos; r0 += TK) {
+    __syncthreads();                                                   // the previous tile is consumed
+    for (int i = tid; i < TK * CPR; i += 128) {                        // 16-byte chunks, swizzled by (row & 7)
+      const int r = i / CPR, c = i - r * CPR;
+      uint4 kw = make_uint4(0u, 0u, 0u, 0u), vw = kw;
+      if (r0 + r <= last_pos) {
+        kw = *reinterpret_cast<const uint4 *>(kc + (size_t)(r0 + r) * HD + 8 * c);
+        vw = *reinterpret_cast<const uint4 *>(vc + (size_t)(r0 + r) * HD + 8 * c);
+      }
+      const int o16 = r * CPR + (c ^ (r & 7));
+      reinterpret_cast<uint4 *>(Ks)[o16] = kw;
+      reinterpret_cast<uint4 *>(Vs)[o16] = vw;
+    }
+    __syncthreads();
+    // ---- S = Q . K^T for this warp's 16 rows x 64 cache rows: 8 n tiles, hi and lo parts of q ----
+    float s[8][4];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { s[j][0] = s[j][1] = s[j][2] = s[j][3] = 0.f; }
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj) {                                   // two n tiles (16 cache rows) per ldmatrix.x4
+      const int krow = 16 * jj + (mi >> 1) * 8 + mr;
+#pragma unroll
+      for (int ks = 0; ks < KS; ++ks) {
+        const int cc = 2 * ks + (mi & 1);
+        uint32_t b[4];
+        pf_ldsm4(b, ks_base + (uint32_t)((krow * CPR + (cc ^ (krow & 7))) * 16));
+        pf_mma(s[2 * jj], qh[ks], b[0], b[1]); pf_mma(s[2 * jj], ql[ks], b[0], b[1]);
+        pf_mma(s[2 * jj + 1], qh[ks], b[2], b[3]); pf_mma(s[2 * jj + 1], ql[ks], b[2], b[3]);
+      }
+    }
+    // ---- scale, causal mask, online softmax (rows g and g + 8 of the warp; a row's 64 columns live in one quad) ----
+    float mx_lo = -INFINITY, mx_hi = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int c0 = r0 + 8 * j + 2 * t;
+      s[j][0] = c0 <= pos_lo ? s[j][0] * scale : -INFINITY;
+      s[j][1] = c0 + 1 <= pos_lo ? s[j][1] * scale : -INFINITY;
+      s[j][2] = c0 <= pos_hi ? s[j][2] * scale : -INFINITY;
+      s[j][3] = c0 + 1 <= pos_hi ? s[j][3] * scale : -INFINITY;
+      mx_lo = fmaxf(mx_lo, fmaxf(s[j][0], s[j][1]));
+      mx_hi = fmaxf(mx_hi, fmaxf(s[j][2], s[j][3]));
+    }
+    mx_lo = fmaxf(mx_lo, __shfl_xor_sync(0xffffffffu, mx_lo, 1)); mx_lo = fmaxf(mx_lo, __shfl_xor_sync(0xffffffffu, mx_lo, 2));
+    mx_hi = fmaxf(mx_hi, __shfl_xor_sync(0xffffffffu, mx_hi, 1)); mx_hi = fmaxf(mx_hi, __shfl_xor_sync(0xffffffffu, mx_hi, 2));
+    const float mn_lo = fmaxf(m_lo, mx_lo), mn_hi = fmaxf(m_hi, mx_hi);
+    const float cr_lo = m_lo == -INFINITY ? 0.f : expf(m_lo - mn_lo), cr_hi = m_hi == -INFINITY ? 0.f : expf(m_hi - mn_hi);
+    float sum_lo = 0.f, sum_hi = 0.f;
+    uint32_t ph[4][4], pl[4][4];                                       // A fragments of P.V, one per 16 cache rows
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const float e0 = mn_lo == -INFINITY ? 0.f : expf(s[j][0] - mn_lo), e1 = mn_lo == -INFINITY ? 0.f : expf(s[j][1] - mn_lo);
+      const float e2 = mn_hi == -INFINITY ? 0.f : expf(s[j][2] - mn_hi), e3 = mn_hi == -INFINITY ? 0.f : expf(s[j][3] - mn_hi);
+      sum_lo += e0 + e1; sum_hi += e2 + e3;
+      // n tile j of S = k rows 8 j .. 8 j + 7 of P.V: tile 2 kk -> a0 (row g), a1 (row g + 8); tile 2 kk + 1 -> a2, a3
+      pf_split2(e0, e1, ph[j >> 1][(j & 1) * 2], pl[j >> 1][(j & 1) * 2]);
+      pf_split2(e2, e3, ph[j >> 1][(j & 1) * 2 + 1], pl[j >> 1][(j & 1) * 2 + 1]);
+    }
+    sum_lo += __shfl_xor_sync(0xffffffffu, sum_lo, 1); sum_lo += __shfl_xor_sync(0xffffffffu, sum_lo, 2);
+    sum_hi += __shfl_xor_sync(0xffffffffu, sum_hi, 1); sum_hi += __shfl_xor_sync(0xffffffffu, sum_hi, 2);
+    l_lo = fmaf(l_lo, cr_lo, sum_lo); l_hi = fmaf(l_hi, cr_hi, sum_hi);
+    m_lo = mn_lo; m_hi = mn_hi;
+#pragma unroll
+    for (int j = 0; j < NT; ++j) { o[j][0] *= cr_lo; o[j][1] *= cr_lo; o[j][2] *= cr_hi; o[j][3] *= cr_hi; }
+    // ---- O += P . V: k = the tile's 64 cache rows (4 k steps), n = head dims (NT tiles), V through ldmatrix.trans ----
+#pragma unroll
+    for (int kk = 0; kk < 4; ++kk) {
+      const int vrow = 16 * kk + (mi & 1) * 8 + mr;
+#pragma unroll
+      for (int jj = 0; jj < NT / 2; ++jj) {
+        const int cc = 2 * jj + (mi >> 1);
+        uint32_t b[4];
+        pf_ldsm4t(b, vs_base + (uint32_t)((vrow * CPR + (cc ^ (vrow & 7))) * 16));
+        pf_mma(o[2 * jj], ph[kk], b[0], b[1]); pf_mma(o[2 * jj], pl[kk], b[0], b[1]);
+        pf_mma(o[2 * jj + 1], ph[kk], b[2], b[3]); pf_mma(o[2 * jj + 1], pl[kk], b[2], b[3]);
+      }
+    }
+  }
+  // ---- out = O / l as three exact bf16 parts (the O projection's GEMM input) ----
+#pragma unroll
+  for (int j = 0; j < NT; ++j) {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int tok = h ? tok_hi : tok_lo;
+      if (tok >= M) continue;
+      const float l = h ? l_hi : l_lo;
+      const size_t ob = (size_t)tok * qd + (size_t)(h ? hq_hi : hq_lo) * HD + 8 * j + 2 * t;
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const Split3 sp = pf_split(o[j][2 * h + e] / l);
+        x3[ob + e] = sp.hi; x3[plane + ob + e] = sp.mid; x3[2 * plane + ob + e] = sp.lo;
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------ host side ----------------------------------
 typedef CUresult (*PfEncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -830,7 +992,10 @@ static int prefill_stack(const DevPtrs &P, const uint16_t *const (*w)[kPrefillMa
       if (pf_launch_gemm(enc, P.pf_x3, P.pf_plane, Mc, M, D.d, wqkv, nqkv, 3, P.pf_Y, qd + 2 * kd, st, &cnt)) return -1;
       k_pf_rope_append<<<M, 256, 0, st>>>(P.pf_Y, qd + 2 * kd, P, l, p0, P.pf_Q);
       dim3 ag((M + TQ - 1) / TQ, D.Hkv);
-      if (D.hd == 128) k_pf_attention<128><<<ag, 256, att_smem, st>>>(P, l, p0, M, P.pf_Q, P.pf_x3, P.pf_plane);
+      if (kPrefillAttnMma) {
+        if (D.hd == 128) k_pf_attention_mma<128><<<ag, 128, 0, st>>>(P, l, p0, M, P.pf_Q, P.pf_x3, P.pf_plane);
+        else k_pf_attention_mma<64><<<ag, 128, 0, st>>>(P, l, p0, M, P.pf_Q, P.pf_x3, P.pf_plane);
+      } else if (D.hd == 128) k_pf_attention<128><<<ag, 256, att_smem, st>>>(P, l, p0, M, P.pf_Q, P.pf_x3, P.pf_plane);
       else k_pf_attention<64><<<ag, 256, att_smem, st>>>(P, l, p0, M, P.pf_Q, P.pf_x3, P.pf_plane);
       const uint16_t *wo[1] = {w[4][l]};
       const int no[1] = {D.d};
