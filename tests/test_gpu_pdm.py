@@ -163,3 +163,38 @@ def test_full_model_dims_paper_pdm(name, pdm_layers):
     rep = run_pdm_parity(shape, w, pw, si.make_prompt(shape, 1234, 24), 10, 1, 0.7, tol=1e-2)
     print(name, rep)
     assert rep["ties"] <= 1
+
+
+@pytest.mark.parametrize("engine", [0, 1])
+def test_external_rollback_and_second_prefill_with_the_paper_pdm(engine):
+    """spd_rollback rewinds the PDM's final-row count F with the committed length (rows above are rebuilt by the next
+    draft); a second spd_prefill on the same context starts a new sequence.  Step results against the oracle."""
+    import paper_2605_30852_b200 as spd
+    shape = shape_of("tiny", 4)
+    w = si.make_weights(shape, seed=1234, std=0.08, random_gains=True)
+    pw = si.make_pdm_weights(shape, 2, 300, seed=1234, std=0.08, random_gains=True)
+    ora = Oracle(shape, w, max_seq=400)
+    ora.attach_pdm(pw)
+    gpu = spd.SPD(shape, spd.upload_weights(w), max_seq=400)
+    gpu.attach_pdm(spd.upload_pdm_weights(pw))
+    gpu.set_option(spd.OPT.ENGINE, engine)
+    rng = np.random.default_rng(5)
+    try:
+        for seq in range(2):
+            prompt = si.make_prompt(shape, 11 + seq, 37 + 20 * seq)
+            assert gpu.prefill(prompt) == ora.prefill(prompt, block=8)
+            for rnd in range(4):
+                for _ in range(9):
+                    a, b = gpu.step(), ora.step_follow(-1, -1, 0.0)
+                    assert tuple(a) == tuple(b), (seq, rnd)
+                    assert gpu.pdm_run()[2] <= ora.committed_len
+                c = ora.committed_len
+                new_len, tok = int(c - rng.integers(0, 4)), int(rng.integers(0, shape.vocab))
+                gpu.rollback(new_len, tok)
+                assert ora.rollback(new_len, tok) == 0
+                assert gpu.pdm_run()[2] <= new_len
+                fill, cc, slots = gpu.ring()
+                assert (fill, cc, slots[0]) == (1, new_len, (1, new_len, tok))
+    finally:
+        ora.close()
+        gpu.close()
