@@ -43,6 +43,7 @@ struct PdmPtrs {
   size_t part_floats;
   int32_t use_tc;                     // 1: tcgen05 skinny GEMM, 0: CUDA-core M-row GEMV
   float2 *rope;                       // [kPdmMaxRows][64] (cos, sin) of the run's positions: computed once per draft
+  float *ss_part;                     // [kPdmMaxRows][64] per-256-column partial sums of squares of a row (deferred RMSNorm)
   float *logits, *z;                  // [Vs], [d]
   float *cand_val;                    // [kPdmCand]
   int32_t *cand_idx;
@@ -420,55 +421,118 @@ __global__ void k_pdm_argmax_final(DevPtrs P, PdmPtrs PD) {
   *P.pdm_draft = PD.vocab_map[bi];
 }
 
-// ------------------------------------------------------------------ fused reduces of the skinny GEMM -------------
-// The skinny GEMM leaves split-K partial sums part[ks][row][column]; these kernels add them in ks order and run the
-// epilogue that follows the product in the layer, so no separate norm / SiLU kernel is launched.
-// (a) O / DOWN: X[r] += sum; then XN[r] = RMSNorm(X[r]; gain) and its three bf16 parts = the next product's input.
-//     One CTA per row; the sum of squares uses block_rms_scale's tree on the updated row.
-__global__ void __launch_bounds__(256) k_pdm_reduce_norm(DevPtrs P, PdmPtrs PD, int ksplit, int NB, const uint16_t *gain) {
-  __shared__ float red[33];
-  const Dims &D = P.dim;
-  const int r = blockIdx.x;
-  if (r >= PD.run->rows) return;
-  float *x = PD.X + (size_t)r * D.d;
-  for (int c = threadIdx.x; c < D.d; c += blockDim.x) {
-    float v = 0.f;
-    for (int ks = 0; ks < ksplit; ++ks) v += PD.part[((size_t)ks * NB + r) * D.d + c];
-    x[c] += v;
-  }
+// ------------------------------------------------------------------ fused epilogues of the skinny GEMM -----------
+// The skinny GEMM leaves split-K partial sums part[ks][row][column].  RMSNorm is DEFERRED so that no kernel has to see a
+// whole row before the product: y = W . (x * rs * g) = rs * (W . (x * g)) with the scalar rs = rsqrt(mean(x^2) + eps).
+// The kernel that PRODUCES a residual row writes the three bf16 parts of x * g_next and the row's sum of squares as
+// per-256-column partials (fixed block tree); the kernel that CONSUMES the next product adds those partials in order
+// and multiplies by rs.  One draft layer is then 10 launches instead of 17.
+__device__ __forceinline__ float pdm_row_rs(const PdmPtrs &PD, const Dims &D, int r) {
+  float ss = 0.f;
+  const int nb = (D.d + 255) / 256;
+  for (int b = 0; b < nb; ++b) ss += PD.ss_part[r * 64 + b];
+  return 1.0f / sqrtf(ss / (float)D.d + D.eps);
+}
+// block-wide sum of `v` over 256 threads in a fixed order -> ss_part[r][blockIdx.x] (thread 0)
+__device__ __forceinline__ void pdm_block_sumsq(const PdmPtrs &PD, int r, float v) {
+  __shared__ float red[8];
+  v = warp_sum(v);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
   __syncthreads();
-  const float rs = block_rms_scale(x, D.d, D.eps, red);
-  for (int c = threadIdx.x; c < D.d; c += blockDim.x) {
-    const float v = x[c] * rs * bf16_to_f32(gain[c]);
-    PD.XN[(size_t)r * D.d + c] = v;
-    pdm_put3(PD, r, D.d, c, v);
+  if (threadIdx.x == 0) {
+    float t = 0.f;
+    for (int w = 0; w < 8; ++w) t += red[w];
+    PD.ss_part[r * 64 + blockIdx.x] = t;
   }
 }
-// (b) gate / up: ACT[r] = silu(sum_gate) * sum_up and its parts.  grid (ceil(F / 256), kPdmMaxRows)
+// (a) after the features: x3 = parts(X * g), sum-of-squares partials.  grid (ceil(d / 256), kPdmMaxRows), 256 threads
+__global__ void __launch_bounds__(256) k_pdm_prep(DevPtrs P, PdmPtrs PD, const uint16_t *gain) {
+  const Dims &D = P.dim;
+  const int r = blockIdx.y, c = blockIdx.x * 256 + threadIdx.x;
+  if (r >= PD.run->rows) return;
+  float x = 0.f;
+  if (c < D.d) {
+    x = PD.X[(size_t)r * D.d + c];
+    pdm_put3(PD, r, D.d, c, x * bf16_to_f32(gain[c]));
+  }
+  pdm_block_sumsq(PD, r, x * x);
+}
+// (b) O / DOWN: X[r] += sum of the partials; x3 = parts(X * g_next); sum-of-squares partials.  same grid
+__global__ void __launch_bounds__(256) k_pdm_reduce_res(DevPtrs P, PdmPtrs PD, int ksplit, int NB, const uint16_t *gain_next) {
+  const Dims &D = P.dim;
+  const int r = blockIdx.y, c = blockIdx.x * 256 + threadIdx.x;
+  if (r >= PD.run->rows) return;
+  float x = 0.f;
+  if (c < D.d) {
+    float v = 0.f;
+    for (int ks = 0; ks < ksplit; ++ks) v += PD.part[((size_t)ks * NB + r) * D.d + c];
+    x = PD.X[(size_t)r * D.d + c] + v;
+    PD.X[(size_t)r * D.d + c] = x;
+    pdm_put3(PD, r, D.d, c, x * bf16_to_f32(gain_next[c]));
+  }
+  pdm_block_sumsq(PD, r, x * x);
+}
+// (c) gate / up: ACT[r] = silu(rs * sum_gate) * (rs * sum_up) and its parts.  grid (ceil(F / 256), kPdmMaxRows)
 __global__ void k_pdm_reduce_silu(DevPtrs P, PdmPtrs PD, int ksplit, int NB) {
   const Dims &D = P.dim;
   const int r = blockIdx.y, c = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= PD.run->rows || c >= D.F) return;
+  const float rs = pdm_row_rs(PD, D, r);
   float g = 0.f, u = 0.f;
   for (int ks = 0; ks < ksplit; ++ks) {
     const float *p = PD.part + ((size_t)ks * NB + r) * 2 * D.F;
     g += p[c]; u += p[D.F + c];
   }
-  const float v = silu_mul(g, u);
+  const float v = silu_mul(g * rs, u * rs);
   PD.ACT[(size_t)r * D.F + c] = v;
   pdm_put3(PD, r, D.F, c, v);
 }
-// (c) plain: dst[r][c] = sum (QKV -> Y); last_row: only the run's last row, into a single vector (the head -> logits)
-__global__ void k_pdm_reduce_plain(PdmPtrs PD, int ksplit, int NB, int ncol, float *dst, int last_row) {
-  const int rows = PD.run->rows;
-  int r = blockIdx.y;
-  const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (last_row) { if (r != 0 || rows < 1) return; r = rows - 1; }
-  else if (r >= rows) return;
-  if (c >= ncol) return;
+// (d) QKV: y = rs * sum; RoPE (C-2.14) on q and k; q -> Q; k, v -> bf16 rows of the PDM cache.  grid kPdmMaxRows
+__global__ void k_pdm_rope_append_red(DevPtrs P, PdmPtrs PD, int layer, int ksplit, int NB) {
+  const Dims &D = P.dim;
+  const PdmRun *R = PD.run;
+  __shared__ float2 cs[64];
+  const int r = blockIdx.x;
+  if (r >= R->rows) return;
+  const int pos = R->first + r, half = D.hd / 2, qd = D.Hq * D.hd, kd = D.Hkv * D.hd, ldy = qd + 2 * kd;
+  if (threadIdx.x < half) cs[threadIdx.x] = PD.rope[r * 64 + threadIdx.x];
+  __syncthreads();
+  const float rs = pdm_row_rs(PD, D, r);
+  auto y = [&](int col) {
+    float v = 0.f;
+    for (int ks = 0; ks < ksplit; ++ks) v += PD.part[((size_t)ks * NB + r) * ldy + col];
+    return v * rs;
+  };
+  for (int j = threadIdx.x; j < (D.Hq + D.Hkv) * half; j += blockDim.x) {
+    const int hh = j / half, i = j - hh * half;
+    const float2 c = cs[i];
+    if (hh < D.Hq) {
+      const float a = y(hh * D.hd + i), b = y(hh * D.hd + i + half);
+      float *q = PD.Q + (size_t)r * qd + hh * D.hd;
+      q[i] = a * c.x - b * c.y;
+      q[i + half] = b * c.x + a * c.y;
+    } else {
+      const int kh = hh - D.Hq;
+      const float a = y(qd + kh * D.hd + i), b = y(qd + kh * D.hd + i + half);
+      uint16_t *dst = PD.kv + kv_offset(D, layer, 0, kh) + (size_t)pos * D.hd;
+      dst[i] = f32_to_bf16(a * c.x - b * c.y);
+      dst[i + half] = f32_to_bf16(b * c.x + a * c.y);
+    }
+  }
+  for (int j = threadIdx.x; j < kd; j += blockDim.x) {
+    const int kh = j / D.hd, i = j - kh * D.hd;
+    PD.kv[kv_offset(D, layer, 1, kh) + (size_t)pos * D.hd + i] = f32_to_bf16(y(qd + kd + j));
+  }
+}
+// (e) the head: logits = rs * sum for the run's LAST row
+__global__ void k_pdm_reduce_logits(DevPtrs P, PdmPtrs PD, int ksplit, int NB) {
+  const int rows = PD.run->rows, c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (rows < 1 || c >= PD.Vs) return;
+  const int r = rows - 1;
+  const float rs = pdm_row_rs(PD, P.dim, r);
   float v = 0.f;
-  for (int ks = 0; ks < ksplit; ++ks) v += PD.part[((size_t)ks * NB + r) * ncol + c];
-  dst[(size_t)(last_row ? 0 : r) * ncol + c] = v;
+  for (int ks = 0; ks < ksplit; ++ks) v += PD.part[((size_t)ks * NB + r) * PD.Vs + c];
+  PD.logits[c] = v * rs;
 }
 
 // ------------------------------------------------------------------ host side ----------------------------------
@@ -503,6 +567,7 @@ static size_t pdm_carve(const Dims &D, int Ls, int Vs, int m, int nsplit, void *
   Q.part_floats = 16 * 48 * nmax;                     // ksplit <= 16, NB <= 48
   Q.part = (float *)take(Q.part_floats * 4);
   Q.rope = (float2 *)take(R * 64 * 8);
+  Q.ss_part = (float *)take(R * 64 * 4);
   Q.logits = (float *)take((size_t)Vs * 4); Q.z = (float *)take((size_t)D.d * 4);
   Q.cand_val = (float *)take(kPdmCand * 4); Q.cand_idx = (int32_t *)take(kPdmCand * 4);
   Q.fc = (const uint16_t *const *)take(8 * sizeof(void *));
@@ -568,9 +633,6 @@ void pdm_destroy(PdmPlan *plan) { free(plan); }
 
 static int pdm_launch_gemv(const PdmPlan *pl, const uint16_t *const *w, const int *n, int nseg, int K, const float *x, int ldx,
                            float *y, int ldy, int residual, int last_only, cudaStream_t st) {
-  if (pl->PD.use_tc)     // the producers of x also wrote its three bf16 parts into PD.x3 (row stride K)
-    return skinny_gemm(pl->PD.x3, pl->PD.plane, K, pl->NB, w, n, nseg, pl->PD.part, pl->PD.part_floats, &pl->PD.run->rows,
-                       last_only ? 1 : 0, y, ldy, residual, st, nullptr);
   RowsGemv A;
   memset(&A, 0, sizeof A);
   int total = 0, col = 0, nmax = 0;
@@ -587,25 +649,26 @@ static int pdm_launch_gemv(const PdmPlan *pl, const uint16_t *const *w, const in
   return 0;
 }
 
-// The kernels of one draft after k_pdm_begin (shared by the cycle and the PDM prefill).
+// The kernels of one draft after k_pdm_begin (shared by the cycle and the PDM prefill): tensor-core products with the
+// fused epilogues above.
 static void pdm_enqueue_body_tc(const DevPtrs &P, const PdmPlan *pl, bool head, cudaStream_t st, long long *cnt) {
   const Dims &D = P.dim;
   const PdmPtrs &PD = pl->PD;
   const int R = kPdmMaxRows, qd = D.Hq * D.hd, kd = D.Hkv * D.hd, group = D.Hq / D.Hkv, NB = pl->NB;
+  const dim3 gd((D.d + 255) / 256, R);
   int ks = 1;
   auto gemm = [&](const uint16_t *const *w, const int *n, int nseg, int K) {
     skinny_gemm(PD.x3, PD.plane, K, NB, w, n, nseg, PD.part, PD.part_floats, nullptr, 0, nullptr, 0, 0, st, cnt, &ks);
   };
   k_pdm_rope_table<<<R, 64, 0, st>>>(P, PD); ++*cnt;
   k_pdm_features<<<dim3((D.d + 7) / 8, R), 256, 0, st>>>(P, PD); ++*cnt;
-  k_pdm_norm<<<R, 256, 0, st>>>(P, PD, pl->w[0][0], 0); ++*cnt;             // the first layer's attention norm
+  k_pdm_prep<<<gd, 256, 0, st>>>(P, PD, pl->w[0][0]); ++*cnt;                // the first layer's attention norm (deferred)
   const int nd[1] = {D.d};
   for (int l = 0; l < pl->Ls; ++l) {
     const uint16_t *wqkv[3] = {pl->w[1][l], pl->w[2][l], pl->w[3][l]};
     const int nqkv[3] = {qd, kd, kd};
     gemm(wqkv, nqkv, 3, D.d);
-    k_pdm_reduce_plain<<<dim3((qd + 2 * kd + 255) / 256, R), 256, 0, st>>>(PD, ks, NB, qd + 2 * kd, PD.Y, 0); ++*cnt;
-    k_pdm_rope_append<<<R, 256, 0, st>>>(P, PD, l); ++*cnt;
+    k_pdm_rope_append_red<<<R, 256, 0, st>>>(P, PD, l, ks, NB); ++*cnt;
     dim3 ga(P.nsplit_max, D.Hkv, R);
     if (D.hd == 128) k_pdm_attn_partial<128><<<ga, group * 32, 0, st>>>(P, PD, l);
     else k_pdm_attn_partial<64><<<ga, group * 32, 0, st>>>(P, PD, l);
@@ -613,30 +676,29 @@ static void pdm_enqueue_body_tc(const DevPtrs &P, const PdmPlan *pl, bool head, 
     k_pdm_attn_merge<<<dim3(D.Hq, R), D.hd, 0, st>>>(P, PD); ++*cnt;
     const uint16_t *wo[1] = {pl->w[4][l]};
     gemm(wo, nd, 1, qd);
-    k_pdm_reduce_norm<<<R, 256, 0, st>>>(P, PD, ks, NB, pl->w[5][l]); ++*cnt;
+    k_pdm_reduce_res<<<gd, 256, 0, st>>>(P, PD, ks, NB, pl->w[5][l]); ++*cnt;
     const uint16_t *wgu[2] = {pl->w[6][l], pl->w[7][l]};
     const int ngu[2] = {D.F, D.F};
     gemm(wgu, ngu, 2, D.d);
     k_pdm_reduce_silu<<<dim3((D.F + 255) / 256, R), 256, 0, st>>>(P, PD, ks, NB); ++*cnt;
     const uint16_t *wd[1] = {pl->w[8][l]};
     gemm(wd, nd, 1, D.F);
-    // ... + residual, then the NEXT product's norm: the next layer's attention norm, or the final norm in front of the head
-    k_pdm_reduce_norm<<<R, 256, 0, st>>>(P, PD, ks, NB, l + 1 < pl->Ls ? pl->w[0][l + 1] : PD.final_norm); ++*cnt;
+    // ... + residual, and the NEXT product's norm (deferred): the next layer's attention norm, or the final norm before the head
+    k_pdm_reduce_res<<<gd, 256, 0, st>>>(P, PD, ks, NB, l + 1 < pl->Ls ? pl->w[0][l + 1] : PD.final_norm); ++*cnt;
   }
   if (head) {
     const uint16_t *wh[1] = {PD.head};
     const int nv[1] = {pl->Vs};
     gemm(wh, nv, 1, D.d);
-    k_pdm_reduce_plain<<<dim3((pl->Vs + 255) / 256, 1), 256, 0, st>>>(PD, ks, NB, pl->Vs, PD.logits, 1); ++*cnt;
+    k_pdm_reduce_logits<<<(pl->Vs + 255) / 256, 256, 0, st>>>(P, PD, ks, NB); ++*cnt;
     k_pdm_argmax_cand<<<kPdmCand, 256, 0, st>>>(PD); ++*cnt;
     k_pdm_argmax_final<<<1, 32, 0, st>>>(P, PD); ++*cnt;
   }
 }
 
 static void pdm_enqueue_body(const DevPtrs &P, const PdmPlan *pl, bool head, cudaStream_t st, long long *cnt) {
-  // (pdm_enqueue_body_tc — reduce + norm / SiLU fused into one CTA per row — measured SLOWER on a B200: 1975 vs 1777 us per
-  //  draft at 9b_n4; five CTAs cannot add 16 partial sums per element as fast as a grid-wide reduce.  Kept for reference.)
-  if (false) { pdm_enqueue_body_tc(P, pl, head, st, cnt); return; }
+  if (pl->PD.use_tc) { pdm_enqueue_body_tc(P, pl, head, st, cnt); return; }
+  // CUDA-core fallback (shapes the tensor path does not take): one kernel per operation, M-row GEMV
   const Dims &D = P.dim;
   const PdmPtrs &PD = pl->PD;
   const int R = kPdmMaxRows, qd = D.Hq * D.hd, kd = D.Hkv * D.hd, group = D.Hq / D.Hkv;
