@@ -468,11 +468,16 @@ def phase_table(eng, shape, cycles: int = 8) -> dict:
     npz = 2 + 5 * per
     eng.set_option(spd.OPT.PHASE_PROFILE, 1)
     acc = {}
+    two_chain = None
     for _ in range(cycles):
         eng.step()
         pr = eng.phase_profile().astype(np.int64)                 # [cta, phase, stamp]
         c0, g0, c1, g1 = pr[0, 167, 0], pr[0, 167, 1], pr[0, 167, 4], pr[0, 167, 5]
         mhz = (c1 - c0) / max(g1 - g0, 1) * 1e3                   # SM clocks per us
+        nvis = int(np.count_nonzero(pr[0, :167, 2]))
+        if nvis != npz:                                           # engine 2: stamps are filed per VISIT (phase x chain)
+            two_chain = phase_table_two_chain(pr, per, mhz, two_chain)
+            continue
         ncta = int(np.count_nonzero(pr[:, npz - 1, 2]))
         for p in range(npz):
             t = 0 if p == 0 else (6 if p == npz - 1 else 1 + (p - 1) % 5)
@@ -486,11 +491,56 @@ def phase_table(eng, shape, cycles: int = 8) -> dict:
             a["stage"].append(float(np.mean((s1 - s0)[ok])) / mhz)
             a["consume"].append(float(np.mean((s2 - s1)[ok])) / mhz)
     eng.set_option(spd.OPT.PHASE_PROFILE, 0)
+    if two_chain:
+        return finish_two_chain(two_chain)
     out = {}
     for t, a in sorted(acc.items()):
         count = 1 if t in (0, 6) else per
         w, st, co = (float(np.mean(a[k])) for k in ("wait", "stage", "consume"))
         out[PHASE_NAMES[t]] = {"count": count, "wait_us": w, "stage_us": st, "consume_us": co, "per_cycle_us": (w + st + co) * count}
+    return out
+
+
+PHASE2_NAMES = ["QKV", "ATTN", "O", "GATEUP", "DOWN_A", "DOWN_B"]
+
+
+def phase_table_two_chain(pr, per, mhz, acc):
+    """Engine 2 (spd_mega2.cu): visit v of a CTA = PDM (0), then (phase, chain) pairs, then HEAD.  `wait` = end of the previous
+    visit -> this visit's inputs handed over by the stager (dependency + staging, hidden when the stager is ahead),
+    `consume` = streaming the visit's tiles.  Accumulates sums per (phase type, chain); returns the running table."""
+    acc = acc or {"_n": 0}
+    acc["_n"] += 1
+    for cta in range(pr.shape[0]):
+        nv = int(np.count_nonzero(pr[cta, :167, 2]))
+        if nv < 2 or (nv - 2) % (6 * per):
+            continue
+        m = (nv - 2) // (6 * per)
+        for v in range(nv):
+            if v == 0:
+                name = "PDM"
+            elif v == nv - 1:
+                name = "HEAD"
+            else:
+                pl, j = divmod(v - 1, m) if m else (0, 0)
+                name = f"{PHASE2_NAMES[pl % 6]}.c{j}"
+            s0, s1, s2 = pr[cta, v, 0], pr[cta, v, 1], pr[cta, v, 2]
+            prev = pr[cta, v - 1, 2] if v > 0 else pr[cta, 167, 0]
+            a = acc.setdefault(name, {"wait_us": 0.0, "stage_us": 0.0, "consume_us": 0.0, "visits": 0})
+            a["wait_us"] += float(s0 - prev) / mhz
+            a["stage_us"] += float(s1 - s0) / mhz
+            a["consume_us"] += float(s2 - s1) / mhz
+            a["visits"] += 1
+    return acc
+
+
+def finish_two_chain(acc, ncta=148):
+    out = {}
+    n = acc.pop("_n")
+    for name, a in acc.items():
+        k = a["visits"]
+        out[name] = {"visits_per_cta_cycle": k / (n * ncta), "wait_us": a["wait_us"] / k, "stage_us": a["stage_us"] / k,
+                     "consume_us": a["consume_us"] / k,
+                     "per_cycle_us": (a["wait_us"] + a["stage_us"] + a["consume_us"]) / (n * ncta)}
     return out
 
 

@@ -19,11 +19,12 @@ struct spd_ctx {
   spd_sizes sizes;
   cudaStream_t sm, sp;
   cudaEvent_t ev_fork, ev_join;
-  cudaGraphExec_t graph[2];
-  int graph_tried[2];
+  cudaGraphExec_t graph[3];
+  int graph_tried[3];
   int engine;
-  int has_mega;
+  int has_mega, has_mega2;
   MegaPlan mega;
+  Mega2Plan mega2;
   PdmPlan *pdm;            // the paper's PDM, if attached (spd_pdm_attach)
   int prefill_mode;        // 1: batched tensor-core prefill (spd_prefill.cu), 0: the decode kernel's prefill mode
   PrefillPlan *pf;
@@ -32,7 +33,7 @@ struct spd_ctx {
   int prefilled, dead;
   int forced_on, sampling_on;   // host mirrors (the two modes exclude each other)
   long long launches;
-  long long launches_per_step[2];
+  long long launches_per_step[3];
   char err[512];
 };
 
@@ -277,6 +278,9 @@ extern "C" int spd_create(const spd_config *cfg, const spd_weights *w, const spd
   ctx->engine = 0;
   int mrc = mega_create(P, src, bufs->repack, need.repack_bytes, ctx->sm, &ctx->mega);
   if (mrc == 0) { ctx->has_mega = 1; ctx->engine = 1; }
+  // the multiplexed-chain schedule of the same building blocks (spd_mega2.cu); shares the repacked weights
+  ctx->has_mega2 = 0;
+  if (ctx->has_mega && mega2_create(P, ctx->mega, &ctx->mega2) == 0) { ctx->has_mega2 = 1; ctx->engine = SPD_DEFAULT_FUSED_ENGINE == 2 ? 2 : 1; }
   ctx->pf = (PrefillPlan *)calloc(1, sizeof(PrefillPlan));
   ctx->prefill_mode = (ctx->pf && prefill_create(P, src, ctx->pf) == 0) ? 1 : 0;
   CUC(cudaStreamSynchronize(ctx->sm));
@@ -291,7 +295,7 @@ extern "C" int spd_destroy(spd_ctx *ctx) {
   if (!ctx) return SPD_EINVAL;
   cudaStreamSynchronize(ctx->sm);
   cudaStreamSynchronize(ctx->sp);
-  for (int e = 0; e < 2; ++e) if (ctx->graph[e]) cudaGraphExecDestroy(ctx->graph[e]);
+  for (int e = 0; e < 3; ++e) if (ctx->graph[e]) cudaGraphExecDestroy(ctx->graph[e]);
   cudaEventDestroy(ctx->ev_fork);
   cudaEventDestroy(ctx->ev_join);
   cudaFreeHost(ctx->h_results);
@@ -308,6 +312,7 @@ extern "C" const char *spd_last_error(const spd_ctx *ctx) { return ctx ? ctx->er
 static int enqueue_raw(spd_ctx *ctx, long long *cnt) {
   // NEXT-1: the paper's PDM drafts from the pre-step state, in front of the cycle's kernels
   if (ctx->pdm && pdm_enqueue_draft(ctx->P, ctx->pdm, ctx->sm, cnt)) return -1;
+  if (ctx->engine == 2) return mega2_enqueue_step(ctx->P, ctx->mega, ctx->mega2, ctx->sm, cnt);
   if (ctx->engine == 1) return mega_enqueue_step(ctx->P, ctx->mega, ctx->sm, cnt);
   return ref_enqueue_step(ctx->P, ctx->sm, ctx->sp, ctx->ev_fork, ctx->ev_join, cnt);
 }
@@ -464,7 +469,7 @@ extern "C" int spd_set_forced(spd_ctx *ctx, const int32_t *truth, int32_t n_trut
 
 static void drop_graphs(spd_ctx *ctx) {   // a kernel parameter changed: captured graphs must be rebuilt
   cudaStreamSynchronize(ctx->sm);
-  for (int e = 0; e < 2; ++e) {
+  for (int e = 0; e < 3; ++e) {
     if (ctx->graph[e]) cudaGraphExecDestroy(ctx->graph[e]);
     ctx->graph[e] = nullptr; ctx->graph_tried[e] = 0;
   }
@@ -489,7 +494,7 @@ extern "C" int spd_set_sampling(spd_ctx *ctx, float temperature, int32_t top_k, 
 extern "C" int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value) {
   if (!ctx) return SPD_EINVAL;
   if (option == SPD_OPT_ENGINE) {
-    if (value == 0 || (value == 1 && ctx->has_mega)) { ctx->engine = value; return SPD_OK; }
+    if (value == 0 || (value == 1 && ctx->has_mega) || (value == 2 && ctx->has_mega2)) { ctx->engine = value; return SPD_OK; }
     return fail(ctx, SPD_EINVAL, "engine not available%s");
   }
   if (option == SPD_OPT_PREFILL) {
@@ -533,7 +538,7 @@ extern "C" int spd_debug_read(spd_ctx *ctx, int32_t what, int32_t index, void *h
       src = P.h + (size_t)st->hbuf[index] * D.d; want = sizeof(float) * D.d; break;
     case SPD_DBG_EXIT_LOGITS:
     case SPD_DBG_PDM_LOGITS:
-      if (!P.debug_logits && !P.sampling && ctx->engine == 1) return fail(ctx, SPD_ESTATE, "debug_read: enable SPD_OPT_DEBUG_LOGITS first%s");
+      if (!P.debug_logits && !P.sampling && ctx->engine >= 1) return fail(ctx, SPD_ESTATE, "debug_read: enable SPD_OPT_DEBUG_LOGITS first%s");
       src = what == SPD_DBG_EXIT_LOGITS ? P.logits_v : P.logits_p; want = sizeof(float) * D.V; break;
     case SPD_DBG_PDM_PRENORM: src = P.pdm_u; want = sizeof(float) * D.d; break;
     case SPD_DBG_PDM_FEAT: src = P.feat; want = sizeof(float) * D.d * D.n; break;

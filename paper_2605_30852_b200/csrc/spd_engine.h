@@ -1,4 +1,4 @@
-// spd_engine.h — host-side entry points of the two engines (internal to the library).
+// spd_engine.h — host-side entry points of the engines (internal to the library).
 #pragma once
 #include "spd_dev.cuh"
 
@@ -23,6 +23,18 @@ size_t mega_repack_bytes(const Dims &D);
 int mega_create(const DevPtrs &P, const uint16_t *const *const *src, void *repack, size_t repack_bytes,
                 cudaStream_t stream, MegaPlan *plan);
 int mega_enqueue_step(const DevPtrs &P, const MegaPlan &plan, cudaStream_t sm, long long *launches);
+
+// Fused persistent engine with multiplexed stage chains (spd_mega2.cu): the same repacked weights, layout and K/V tensor map
+// (MegaPlan), its own launch geometry.
+#ifndef SPD_DEFAULT_FUSED_ENGINE
+#define SPD_DEFAULT_FUSED_ENGINE 1
+#endif
+struct Mega2Plan {
+  int smem_bytes;
+  int available;
+};
+int mega2_create(const DevPtrs &P, const MegaPlan &base, Mega2Plan *plan);
+int mega2_enqueue_step(const DevPtrs &P, const MegaPlan &base, const Mega2Plan &plan, cudaStream_t sm, long long *launches);
 
 
 // Batched tensor-core prefill (spd_prefill.cu).

@@ -351,6 +351,7 @@ struct SampSmem {
   TopkSmem tk;
   SampleDist qd, pt, qs;            // this cycle's draft / target distributions, the judged token's stored one
   double w[kMaxTopK];               // residual weights max(0, P - Q) over P's support
+  int ctl[12];                      // controller_end's CTA-wide scalars
 };
 __device__ __forceinline__ double dist_prob(const SampleDist *D, int token) {
   for (int i = 0; i < D->k; ++i)
@@ -397,7 +398,10 @@ __device__ __forceinline__ int sample_residual(const SampleDist *Pt, const doubl
 // `sm`: shared-memory scratch for the sampler (may be nullptr when P.sampling == 0).
 // `with_lists`: the head pass filled the threshold lists (fused engine).
 __device__ __forceinline__ void controller_end(const DevPtrs &P, int ncand, SampSmem *sm, bool with_lists = false) {
-  __shared__ int s_y, s_draft, s_exit_buf, s_exit_pos, s_enter_tok, s_enter_buf, s_do_exit, s_do_enter, s_keep_q, s_stamp;
+  // CTA-wide scalars of the controller live in the caller's scratch (no static shared memory: the fused kernels' dynamic
+  // segment is 1024-byte aligned and has no room for a padded static one)
+  int &s_y = sm->ctl[0], &s_draft = sm->ctl[1], &s_exit_buf = sm->ctl[2], &s_exit_pos = sm->ctl[3], &s_enter_tok = sm->ctl[4],
+      &s_enter_buf = sm->ctl[5], &s_do_exit = sm->ctl[6], &s_do_enter = sm->ctl[7], &s_keep_q = sm->ctl[8], &s_stamp = sm->ctl[9];
   StepState *st = P.st;
   const Dims &D = P.dim;
   int n = D.n;
