@@ -20,7 +20,7 @@
 //   * two 24 KB activation buffers alternate between visits.  W_down is therefore streamed as TWO phases over the two
 //     K parts of the repacked matrix (residual += part a, then += part b: a fixed order), so no visit needs more than
 //     24 KB: 6 phases per pass (QKV, ATTN, O, GATEUP, DOWN_A, DOWN_B).  The ring keeps its 11 slots.
-//   * attention visits use their buffer as scratch; q is read per item (no per-visit staging: a visit has ~2 items per CTA).
+//   * attention visits use their buffer as scratch; an item's q (G heads, 2 KB) arrives through the ring behind its K/V tiles.
 //   * PDM phase (visit 0) and LM head (last visit) are the one-chain engine's (foreground staging, whole buffer).
 // Results do not depend on the grouping: every row's dot product, every attention split and every merge keep their fixed
 // mapping and order (batch invariance as in spd_mega.cu).  DOWN differs from the one-chain engine by the point where the
@@ -337,13 +337,15 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
               attn_decode(k, S.attn_ns[x.j], S.attn_nonfinal[x.j], S.pos[k], (int)next, it);
               const int item = (int)next;
               next = atomicAdd(w.ctr, 1u);
-              if (item >= S.attn_nonfinal[x.j] && !kv_ready) {
-                // the last split holds the row appended by the group's CTAs in this pass's QKV phase: wait for it
-                const unsigned int target = (unsigned int)(x.p - 1) * (unsigned int)S.gsize;
-                while (ld_acquire_u32(gbar + 32 * k) < target) {}
-                fence_proxy_async();
-                kv_ready = true;
-              }
+              auto wait_qkv = [&]() {   // this pass's QKV phase of the group: q of the stage and the row it appended
+                if (!kv_ready) {
+                  const unsigned int target = (unsigned int)(x.p - 1) * (unsigned int)S.gsize;
+                  while (ld_acquire_u32(gbar + 32 * k) < target) {}
+                  fence_proxy_async();
+                  kv_ready = true;
+                }
+              };
+              if (item >= S.attn_nonfinal[x.j]) wait_qkv();   // the last split holds the appended row
               const int layer = k * D.per + x.pass;
               const int nk = (it.rows + RPS - 1) / RPS;
               const bool boxed = ML.attn_mma && it.rows == kAttnSplit;   // full split: swizzled boxes for the MMA path
@@ -366,6 +368,18 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
                   }
                   if (first) { prof_stamp(P, cta, v, 3); first = false; }
                 }
+              }
+              {   // the item's q (G heads, fp32, contiguous) rides the ring too: no consumer ever waits on an L2 round trip
+                wait_qkv();
+                const int G = D.Hq / D.Hkv;
+                const uint32_t slot = seq % kStages, itn = seq / kStages;
+                const uint32_t bytes = (uint32_t)(G * D.hd * 4);
+                mbar_wait(&empty[slot], (itn & 1) ^ 1);
+                meta[slot] = item;
+                mbar_expect_tx(&full[slot], bytes);
+                tma_load_1d(ring + (size_t)slot * kTileBytes, P.q + ((size_t)k * D.Hq + (size_t)it.kvh * G) * D.hd, bytes, &full[slot],
+                            pol_kv);
+                ++seq;
               }
             }
           } else {
@@ -500,14 +514,16 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
             AttnItem it;
             attn_decode(k, S.attn_ns[j], S.attn_nonfinal[j], S.pos[k], item, it);
             const int nk = (it.rows + RPS - 1) / RPS;
-            for (int jj = 1; jj < 2 * nk; ++jj) mbar_wait(&full[(seq + jj) % kStages], ((seq + jj) / kStages) & 1);
+            for (int jj = 1; jj <= 2 * nk; ++jj) mbar_wait(&full[(seq + jj) % kStages], ((seq + jj) / kStages) & 1);
+            const int qslot = (int)((seq + 2 * nk) % kStages);      // K slots, V slots, then the q slot
+            const float *qsm = reinterpret_cast<const float *>(ring + (size_t)qslot * kTileBytes);
             if (ML.attn_mma && it.rows == kAttnSplit) {
-              if (G == 4) attn_item_mma<4>(P, it, ring, seq, xb, empty, nullptr);
-              else if (G == 2) attn_item_mma<2>(P, it, ring, seq, xb, empty, nullptr);
-              else attn_item_mma<1>(P, it, ring, seq, xb, empty, nullptr);
-            } else if (D.hd == 128) attn_item_g<128>(P, it, ring, seq, nk, xb, empty, G);
-            else attn_item_g<64>(P, it, ring, seq, nk, xb, empty, G);
-            seq += 2 * nk;
+              if (G == 4) attn_item_mma<4>(P, it, ring, seq, xb, empty, nullptr, qsm, qslot);
+              else if (G == 2) attn_item_mma<2>(P, it, ring, seq, xb, empty, nullptr, qsm, qslot);
+              else attn_item_mma<1>(P, it, ring, seq, xb, empty, nullptr, qsm, qslot);
+            } else if (D.hd == 128) attn_item_g<128>(P, it, ring, seq, nk, xb, empty, G, qsm, qslot);
+            else attn_item_g<64>(P, it, ring, seq, nk, xb, empty, G, qsm, qslot);
+            seq += 2 * nk + 1;
             if (tid == 0) done_list[n_done] = item;
             ++n_done;
           }

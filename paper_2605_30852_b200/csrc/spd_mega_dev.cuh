@@ -296,7 +296,7 @@ struct XReduce {
 // red[8][G][HD] per-warp partial outputs.
 template <int HD, int G>
 __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, const uint8_t *ring, uint32_t seq0, int nk,
-                                          float *scratch, uint64_t *empty) {
+                                          float *scratch, uint64_t *empty, const float *qsm = nullptr, int qslot = -1) {
   constexpr int CH = HD / 8;            // 16-byte chunks (= lanes) per K row
   constexpr int RPI = 32 / CH;          // rows covered by one warp-wide LDS.128
   constexpr int NI = 16 / RPI;          // iterations for a warp's 16 rows
@@ -316,8 +316,10 @@ __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, 
     float qv[G][8];
 #pragma unroll
     for (int h = 0; h < G; ++h) {
-      const float4 *q4 = reinterpret_cast<const float4 *>(P.q + ((size_t)it.stage * D.Hq + hq0 + h) * HD + c * 8);
-      float4 a = __ldcg(q4), b = __ldcg(q4 + 1);
+      // q of the G heads: from the ring slot the producer filled (qsm, engine 2) or from global memory (written by other CTAs)
+      const float4 *q4 = reinterpret_cast<const float4 *>((qsm ? qsm + (size_t)h * HD : P.q + ((size_t)it.stage * D.Hq + hq0 + h) * HD) + c * 8);
+      float4 a, b;
+      if (qsm) { a = q4[0]; b = q4[1]; } else { a = __ldcg(q4); b = __ldcg(q4 + 1); }
       qv[h][0] = a.x; qv[h][1] = a.y; qv[h][2] = a.z; qv[h][3] = a.w;
       qv[h][4] = b.x; qv[h][5] = b.y; qv[h][6] = b.z; qv[h][7] = b.w;
     }
@@ -350,7 +352,10 @@ __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, 
     }
   }
   consumer_sync();
-  if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + j) % kStages]);   // K slots are free
+  if (lane == 0) {
+    for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + j) % kStages]);   // K slots are free
+    if (qslot >= 0) mbar_arrive(&empty[qslot]);                               // ... and the q slot
+  }
   // ---- softmax of the split, one warp per head: m = max, p = exp(s - m), l = sum p ----
   if (warp < G) {
     float s[kAttnSplit / 32], m = -INFINITY;
@@ -446,7 +451,8 @@ __device__ __forceinline__ void attn_item(const DevPtrs &P, const AttnItem &it, 
 // after one CTA barrier, the splits in split order: results do not depend on who ran the item.
 template <int G>
 __device__ __forceinline__ void attn_item_mma(const DevPtrs &P, const AttnItem &it, const uint8_t *ring, uint32_t seq0,
-                                              float *scratch, uint64_t *empty, const uint32_t *qs) {
+                                              float *scratch, uint64_t *empty, const uint32_t *qs, const float *qsm = nullptr,
+                                              int qslot = -1) {
   constexpr int HD = 128, nk = 2;
   const Dims &D = P.dim;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -470,6 +476,15 @@ __device__ __forceinline__ void attn_item_mma(const DevPtrs &P, const AttnItem &
         for (int ks = 0; ks < 8; ++ks) {
           qh[ks][0] = h[8 * ks + t]; qh[ks][1] = h[8 * ks + 4 + t];
           ql[ks][0] = l[8 * ks + t]; ql[ks][1] = l[8 * ks + 4 + t];
+        }
+      } else if (qsm) {                           // fp32 q of the G heads in a ring slot (engine 2: brought by the producer)
+        const float *q = qsm + (size_t)g * HD;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+          const float2 x = *reinterpret_cast<const float2 *>(q + 16 * ks + 2 * t);
+          const float2 y = *reinterpret_cast<const float2 *>(q + 16 * ks + 8 + 2 * t);
+          split_bf16x2(x.x, x.y, qh[ks][0], ql[ks][0]);
+          split_bf16x2(y.x, y.y, qh[ks][1], ql[ks][1]);
         }
       } else {
         const float *q = P.q + ((size_t)it.stage * D.Hq + hq0 + g) * HD;
@@ -510,7 +525,10 @@ __device__ __forceinline__ void attn_item_mma(const DevPtrs &P, const AttnItem &
     if (g < G && t == 0) wml[warp * G + g] = make_float2(m, l);
   }
   __syncwarp();
-  if (lane == 0) for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + j) % kStages]);   // this warp is done with K
+  if (lane == 0) {
+    for (int j = 0; j < nk; ++j) mbar_arrive(&empty[(seq0 + j) % kStages]);   // this warp is done with K
+    if (qslot >= 0) mbar_arrive(&empty[qslot]);                               // ... and with q
+  }
   // ---- P.V: O[head][dim] = sum over this warp's 16 rows: A = P (k = rows), B = V via ldmatrix.trans ----
   {
     uint32_t ph[2] = {0u, 0u}, pl[2] = {0u, 0u};  // a0: rows 2t, 2t+1; a2: rows 2t+8, 2t+9 (of the warp's 16)
@@ -648,11 +666,11 @@ __device__ __forceinline__ void unit_epilogue(const DevPtrs &P, const SchedT &S,
 
 template <int HD>
 __device__ __forceinline__ void attn_item_g(const DevPtrs &P, const AttnItem &it, const uint8_t *ring, uint32_t seq0, int nk,
-                                            float *scratch, uint64_t *empty, int G) {
-  if (G == 4) attn_item<HD, 4>(P, it, ring, seq0, nk, scratch, empty);
-  else if (G == 2) attn_item<HD, 2>(P, it, ring, seq0, nk, scratch, empty);
-  else if (G == 8) attn_item<HD, 8>(P, it, ring, seq0, nk, scratch, empty);
-  else attn_item<HD, 1>(P, it, ring, seq0, nk, scratch, empty);
+                                            float *scratch, uint64_t *empty, int G, const float *qsm = nullptr, int qslot = -1) {
+  if (G == 4) attn_item<HD, 4>(P, it, ring, seq0, nk, scratch, empty, qsm, qslot);
+  else if (G == 2) attn_item<HD, 2>(P, it, ring, seq0, nk, scratch, empty, qsm, qslot);
+  else if (G == 8) attn_item<HD, 8>(P, it, ring, seq0, nk, scratch, empty, qsm, qslot);
+  else attn_item<HD, 1>(P, it, ring, seq0, nk, scratch, empty, qsm, qslot);
 }
 
 // Slot protocol of the tile-per-warp-pair mapping.  Only the owner pair of a tile reads its data, but EVERY
