@@ -281,6 +281,19 @@ int spd_op_attention(const float *q, const uint16_t *kc, const uint16_t *vc, int
                      int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, float *out, float *scratch,
                      void *stream);
 size_t spd_op_attention_scratch(int32_t t_len, int32_t n_q_heads, int32_t head_dim);
+/* spd_op_attention for callers that cannot allocate device memory (CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same operation (the stage forward's attention; fixed 128-row splits merged in
+ * split order), same arguments minus `scratch` — the split partials live in a file-scope device array of
+ * spd_op_attention_static_max_bytes() = 2 MiB inside the library (held by every GPU that loads the library until the
+ * process exits).  q, kc, vc, out: DEVICE, caller-owned, layouts as spd_op_attention.  Allocates nothing (no cudaMalloc /
+ * cudaFree / allocating library call).  Returns SPD_OK; SPD_EINVAL (bad argument); SPD_ECAPACITY when
+ * ceil(t_len / 128) * n_q_heads * (head_dim + 2) * 4 bytes exceed the array (use spd_op_attention with a caller buffer);
+ * SPD_ECUDA.  All calls on a device SHARE the array, which keeps the last call's contents (nothing needs to start at zero:
+ * every slot is written before it is read); calls that overlap on the GPU (different streams without a dependency) race
+ * on it — calls on one stream are ordered.  Asynchronous on `stream` like the other spd_op_* calls. */
+int spd_op_attention_static(const float *q, const uint16_t *kc, const uint16_t *vc, int32_t t_len, int32_t t_stride,
+                            int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, float *out, void *stream);
+size_t spd_op_attention_static_max_bytes(void);
 /* The prefill GEMM as one operation: y[M, N] = x[M, K] . W[N, K]^T, x fp32 (split exactly into three bf16 parts), W bf16 row-major,
  * y fp32, on the tcgen05 tensor cores.  K % 64 == 0, N % 4 == 0.  scratch: DEVICE, >= spd_op_gemm_scratch(M, K) bytes. */
 int spd_op_gemm(const float *x, const uint16_t *w, int32_t m, int32_t n, int32_t k, float *y, void *scratch, void *stream);

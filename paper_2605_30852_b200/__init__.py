@@ -4,8 +4,8 @@ path runs in the library's kernels.  There is no CPU fallback: importing `bindin
 CUDA library has not been built (python -m paper_2605_30852_b200.build or __graft_entry__.build()).
 """
 from .binding import (SPD, StepResult, SpdError, lib, upload_weights, upload_pdm_weights, op_rmsnorm, op_gemv, op_gemm, op_rope,
-                      op_attention, op_silu_mul, op_argmax, op_topk_softmax, DBG, OPT)
+                      op_attention, op_attention_static, op_silu_mul, op_argmax, op_topk_softmax, DBG, OPT)
 from . import reporting
 
 __all__ = ["SPD", "StepResult", "SpdError", "lib", "upload_weights", "upload_pdm_weights", "op_rmsnorm", "op_gemv", "op_gemm", "op_rope",
-           "op_attention", "op_silu_mul", "op_argmax", "op_topk_softmax", "DBG", "OPT", "reporting"]
+           "op_attention", "op_attention_static", "op_silu_mul", "op_argmax", "op_topk_softmax", "DBG", "OPT", "reporting"]

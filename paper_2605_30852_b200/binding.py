@@ -147,6 +147,9 @@ def lib():
         L.spd_op_attention.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp]
         L.spd_op_attention_scratch.argtypes = [i32, i32, i32]
         L.spd_op_attention_scratch.restype = C.c_size_t
+        L.spd_op_attention_static.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]
+        L.spd_op_attention_static_max_bytes.argtypes = []
+        L.spd_op_attention_static_max_bytes.restype = C.c_size_t
         L.spd_op_silu_mul.argtypes = [vp, vp, i32, vp, vp]
         L.spd_op_argmax.argtypes = [vp, i32, vp, vp]
         _lib = L
@@ -465,6 +468,17 @@ def op_attention(q: torch.Tensor, kc: torch.Tensor, vc: torch.Tensor, t_len: int
     scratch = torch.empty(nbytes // 4 + 1, dtype=torch.float32, device=q.device)
     _chk(lib().spd_op_attention(q.data_ptr(), kc.data_ptr(), vc.data_ptr(), t_len, t_stride, n_q_heads, n_kv_heads,
                                 head_dim, out.data_ptr(), scratch.data_ptr(), _s(stream)), "spd_op_attention")
+    return out
+
+
+def op_attention_static(q: torch.Tensor, kc: torch.Tensor, vc: torch.Tensor, t_len: int, n_q_heads: int, n_kv_heads: int,
+                        head_dim: int, out: torch.Tensor, stream=None) -> torch.Tensor:
+    """spd_op_attention_static: as op_attention, but the library allocates nothing — the caller passes `out`
+    (fp32[n_q_heads * head_dim]) and the split partials live in the library's static 2 MiB device array."""
+    rc = lib().spd_op_attention_static(q.data_ptr(), kc.data_ptr(), vc.data_ptr(), t_len, kc.shape[1], n_q_heads, n_kv_heads,
+                                       head_dim, out.data_ptr(), _s(stream))
+    if rc:
+        raise SpdError(rc, "spd_op_attention_static")
     return out
 
 
