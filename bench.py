@@ -219,6 +219,8 @@ def run_gpu(args, shape):
     eng = spd.SPD(shape, w_dev, max_seq=max_seq, device=local_rank)
     if args.engine is not None:
         eng.set_option(spd.OPT.ENGINE, args.engine)
+    if args.chains is not None:
+        eng.set_option(spd.OPT.CHAINS, args.chains)
     prompt = si.make_prompt(shape, args.seed + rank)
     first = eng.prefill(prompt)
     # the step before the path (untimed in the paper): the batched tensor-core prefill, timed once warm
@@ -356,6 +358,8 @@ def run_gpu(args, shape):
         eng2.attach_pdm(spd.upload_pdm_weights(pw, local_rank))
         if args.engine is not None:
             eng2.set_option(spd.OPT.ENGINE, args.engine)
+        if args.chains is not None:
+            eng2.set_option(spd.OPT.CHAINS, args.chains)
         s2 = eng2.stream_main
         q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         eng2.prefill(prompt)
@@ -398,6 +402,8 @@ def run_gpu(args, shape):
     eng = spd.SPD(shape, w_dev, max_seq=P + 2 * ks + 8 * n + 64, device=local_rank)
     if args.engine is not None:
         eng.set_option(spd.OPT.ENGINE, args.engine)
+    if args.chains is not None:
+        eng.set_option(spd.OPT.CHAINS, args.chains)
     stream = eng.stream_main
     eng.set_sampling(1.0, 50, args.seed)
     first_e = eng.prefill(prompt)
@@ -618,6 +624,7 @@ def main():
     ap.add_argument("--config", default="9b_n4", choices=sorted(si.CONFIGS))
     ap.add_argument("--impl", default="spd", choices=["spd", "reference"])
     ap.add_argument("--engine", type=int, default=None, help="0 reference engine, 1 fused engine (default: library default)")
+    ap.add_argument("--chains", type=int, default=None, help="engine 2: stage chains per CTA, 1..4 (default: library default)")
     ap.add_argument("--seed", type=int, default=1234)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--phase-profile", action="store_true", help="add the fused kernel's per-phase breakdown (its own clock stamps)")

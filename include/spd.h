@@ -109,6 +109,7 @@ enum {
                               step kernel (default when available)                               */
   SPD_OPT_DEBUG_LOGITS = 1,/* 1 = also write full verify/PDM logit vectors (for parity tests)    */
   SPD_OPT_PHASE_PROFILE = 2,/* 1 = the fused kernel records per-phase clock stamps (SPD_DBG_PHASE_PROFILE) */
+  SPD_OPT_CHAINS = 4,      /* engine 2 only: stage chains a CTA serves in turn, 1..4 (results do not depend on it)          */
   SPD_OPT_PREFILL = 3      /* 1 = batched tensor-core prefill (tcgen05 GEMMs over chunks of the prompt; default when the
                               configuration supports it: d_model, n_q_heads*head_dim, d_ffn multiples of 64),
                               0 = the prompt runs through the decode kernel, one token entering per cycle          */

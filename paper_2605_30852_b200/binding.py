@@ -31,6 +31,7 @@ class OPT:
     DEBUG_LOGITS = 1
     PHASE_PROFILE = 2
     PREFILL = 3
+    CHAINS = 4
 
 
 class DBG:

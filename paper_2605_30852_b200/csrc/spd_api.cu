@@ -497,6 +497,11 @@ extern "C" int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value) {
     if (value == 0 || (value == 1 && ctx->has_mega) || (value == 2 && ctx->has_mega2)) { ctx->engine = value; return SPD_OK; }
     return fail(ctx, SPD_EINVAL, "engine not available%s");
   }
+  if (option == SPD_OPT_CHAINS) {
+    if (!ctx->has_mega2 || value < 1 || value > kMega2MaxChains) return fail(ctx, SPD_EINVAL, "chains: 1..4, engine 2 only%s");
+    if (ctx->mega2.chains != value) { ctx->mega2.chains = value; drop_graphs(ctx); }
+    return SPD_OK;
+  }
   if (option == SPD_OPT_PREFILL) {
     if (value == 0 || (value == 1 && ctx->pf && ctx->pf->available)) { ctx->prefill_mode = value; return SPD_OK; }
     return fail(ctx, SPD_EINVAL, "batched prefill not available for this configuration%s");

@@ -29,9 +29,11 @@ int mega_enqueue_step(const DevPtrs &P, const MegaPlan &plan, cudaStream_t sm, l
 #ifndef SPD_DEFAULT_FUSED_ENGINE
 #define SPD_DEFAULT_FUSED_ENGINE 1
 #endif
+constexpr int kMega2DefaultChains = 2, kMega2MaxChains = 4;
 struct Mega2Plan {
   int smem_bytes;
   int available;
+  int chains;               // stage chains per CTA (SPD_OPT_CHAINS)
 };
 int mega2_create(const DevPtrs &P, const MegaPlan &base, Mega2Plan *plan);
 int mega2_enqueue_step(const DevPtrs &P, const MegaPlan &base, const Mega2Plan &plan, cudaStream_t sm, long long *launches);

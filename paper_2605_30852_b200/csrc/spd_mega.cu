@@ -494,6 +494,7 @@ static void make_layout(const Dims &D, MegaLayout *ML, size_t *total) {
   unsigned long long b_gu = (unsigned long long)ML->u_gu * ML->nc_d * kTileBytes;
   unsigned long long b_dn = (unsigned long long)ML->u_dn * ML->nc_f * kTileBytes;
   ML->off_o = b_qkv; ML->off_gu = b_qkv + b_o; ML->off_dn = b_qkv + b_o + b_gu;
+  ML->chains = 0;
   ML->nc_fa = (ML->nc_f + 1) / 2;                  // W_down as two K parts (spd_mega_dev.cuh)
   ML->off_dnb = ML->off_dn + (unsigned long long)ML->u_dn * ML->nc_fa * kTileBytes;
   ML->layer_bytes = b_qkv + b_o + b_gu + b_dn;

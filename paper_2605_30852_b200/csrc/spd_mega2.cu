@@ -33,7 +33,7 @@ constexpr int kXHalf = kXFloats / 2;                      // floats per activati
 constexpr int kStagerThreads = 64;
 constexpr int kThreads2 = kConsumerThreads + 32 + kStagerThreads + 32;   // 8 consumer warps, producer, 2 stager warps, publisher
 // (12 warps = 3 per SM sub-partition: the most that leaves the consumers their 168 registers)
-constexpr int kMaxChains = 3;
+constexpr int kMaxChains = kMega2MaxChains;               // stage chains a CTA serves at most
 constexpr int kPhasesPerPass = 6;
 
 enum Phase2 { P2_QKV = 0, P2_ATTN = 1, P2_O = 2, P2_GU = 3, P2_DNA = 4, P2_DNB = 5 };
@@ -106,6 +106,10 @@ __device__ __forceinline__ Work2 work_desc(const Visit &x, const Sched2 &S, cons
   return w;
 }
 
+// Clock stamps are filed per VISIT; slot kProfPhases - 1 holds the kernel's entry / exit stamps, later visits are not recorded.
+__device__ __forceinline__ void vstamp(const DevPtrs &P, int cta, int v, int stamp) {
+  if (v < kProfPhases - 1) prof_stamp(P, cta, v, stamp);
+}
 __device__ __forceinline__ void stager_sync() { asm volatile("bar.sync 2, 64;" ::: "memory"); }
 
 // What a visit's inputs depend on (stager): polled with ld.acquire by one lane per stager warp.
@@ -229,8 +233,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
   uint64_t *empty = full + kStages;                                      // [kStages]
   uint64_t *xfull = empty + kStages;                                     // [2] buffer b holds the visit's inputs
   uint64_t *xempty = xfull + 2;                                          // [2] the consumers are done with buffer b
-  float2 *rope_s = reinterpret_cast<float2 *>(xempty + 2);               // [kMaxChains][64]
-  float *red = reinterpret_cast<float *>(rope_s + kMaxChains * 64);      // [16]
+  float *red = reinterpret_cast<float *>(xempty + 2);                    // [16]
   float *cbest_v = red + 16;                                             // [2][8]
   int *cbest_i = reinterpret_cast<int *>(cbest_v + 16);                  // [2][8]
   int *meta = cbest_i + 16;                                              // [kStages] slot tags (+ padding to 16)
@@ -268,14 +271,18 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
     S.p_new = st->occ[0] ? st->pos[0] : -1;
     S.run_pdm = st->mode == MODE_SPD && !P.paper_pdm;
     S.run_verify = (st->mode == MODE_SPD && st->occ[D.n - 1]) || st->mode == MODE_PREFILL_FINAL;
-    // Groups: shares r = cta mod a; group g = min(r / 2, a / 2 - 1) serves the stages act[2 g], act[2 g + 1] (and act[a - 1]
-    // when it is the last group of an odd a); a == 1: one group, one chain.
+    // Groups: shares r = cta mod a; the a shares (= active stages, ascending) are cut into ng = ceil(a / chains) runs of
+    // a / ng or a / ng + 1 consecutive shares, and the CTAs of a run serve all of its stages as chains.  A dependent visit
+    // of a chain is m - 1 visits behind its producer: with m = 4 the barrier latency (skew of one visit + release /
+    // acquire + the stager's copy, ~8 us) is covered even by the short visits (ATTN, O, DOWN parts: 5-6 us each).
     S.m = 0; S.gsize = 0; S.lead = 0; S.exit_gsize = 0;
     if (a > 0) {
-      const int ng = a >= 2 ? a / 2 : 1;
+      const int cm = max(1, min(ML.chains, kMaxChains));
+      const int ng = (a + cm - 1) / cm, gb = a / ng, grem = a % ng;
       const int r = cta % a;
-      const int g = min(r / 2, ng - 1);
-      const int first = 2 * g, last = (g == ng - 1) ? a - 1 : 2 * g + 1;   // shares (= chains) of the group
+      int g = 0, first = 0;
+      while (first + gb + (g < grem ? 1 : 0) <= r) { first += gb + (g < grem ? 1 : 0); ++g; }
+      const int last = first + gb + (g < grem ? 1 : 0) - 1;               // shares (= chains) of this CTA's group
       S.m = last - first + 1;
       for (int j = 0; j < S.m; ++j) {
         const int k = act[first + j];
@@ -287,7 +294,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
       for (int rr = first; rr <= last; ++rr) S.gsize += ncta / a + (rr < ncta % a ? 1 : 0);
       S.lead = cta == first;                                               // the lowest CTA of the group
       if (st->occ[D.n - 1]) {                                              // stage n - 1 = act[a - 1]: the last group
-        const int f2 = 2 * (ng - 1);
+        const int f2 = a - (gb + (ng - 1 < grem ? 1 : 0));
         for (int rr = f2; rr <= a - 1; ++rr) S.exit_gsize += ncta / a + (rr < ncta % a ? 1 : 0);
       }
     }
@@ -305,12 +312,6 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
   if (P.prof_on && tid == 0 && cta < kProfCtas) {
     unsigned long long *pr = P.prof + ((size_t)cta * kProfPhases + (kProfPhases - 1)) * kProfStamps;
     pr[0] = (unsigned long long)clock64(); pr[1] = globaltimer_ns();
-  }
-  for (int e = tid; e < S.m * (D.hd / 2); e += kThreads2) {   // RoPE tables of this CTA's chains (C-2.14)
-    const int j = e / (D.hd / 2), i = e - j * (D.hd / 2);
-    double s_, c_;
-    sincos((double)S.pos[S.stage[j]] * P.inv_freq[i], &s_, &c_);
-    rope_s[j * 64 + i] = make_float2((float)c_, (float)s_);
   }
   __syncthreads();
   const int RPS = kTileBytes / (D.hd * 2);         // K/V rows per ring slot
@@ -366,7 +367,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
                   } else {
                     tma_load_1d(dst, src + (size_t)j * RPS * D.hd, bytes, &full[slot], pol_kv);
                   }
-                  if (first) { prof_stamp(P, cta, v, 3); first = false; }
+                  if (first) { vstamp(P, cta, v, 3); first = false; }
                 }
               }
               {   // the item's q (G heads, fp32, contiguous) rides the ring too: no consumer ever waits on an L2 round trip
@@ -394,11 +395,11 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
                 meta[slot] = u;
                 mbar_expect_tx(&full[slot], kTileBytes);
                 tma_load_1d(ring + (size_t)slot * kTileBytes, src, kTileBytes, &full[slot], pol_w);
-                if (first) { prof_stamp(P, cta, v, 3); first = false; }
+                if (first) { vstamp(P, cta, v, 3); first = false; }
               }
             }
           }
-          prof_stamp(P, cta, v, 4);
+          vstamp(P, cta, v, 4);
         }
         // END slot: closes the visit for the consumers
         uint32_t slot = seq % kStages, itn = seq / kStages;
@@ -455,6 +456,11 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
             if (ai >= 0 && S.pos[k] < D.max_seq) raw = P.anch + ((size_t)S.pos[k] * P.pdm_m + ai) * D.d;
           }
           stager_copy(dp, h, dst, D.d, ML.nc_d * kTileCols, g, D.eps, raw, sred, st);
+          if (x.type == P2_QKV && st < D.hd / 2) {   // RoPE table of the chain's position (C-2.14), behind the vector (the parked
+            double s_, c_;                         // gains are dead: every stager thread has passed stager_copy's last barrier)
+            sincos((double)S.pos[k] * P.inv_freq[st], &s_, &c_);
+            reinterpret_cast<float2 *>(dst + ML.nc_d * kTileCols)[st] = make_float2((float)c_, (float)s_);
+          }
           if (x.type == P2_QKV && S.lead && st == 0) {
             // causality / capacity precondition of the KV append, and the new length (one CTA per stage)
             const int pos = S.pos[k];
@@ -487,14 +493,14 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
       const Visit x = visit_decode(v, nv, np, m);
       mbar_wait(&xfull[b], (v >> 1) & 1);          // inputs staged, dependencies satisfied
       if (tid == 0) {
-        prof_stamp(P, cta, v, 0);
-        if (P.prof_on && cta < kProfCtas && v < kProfPhases) P.prof[((size_t)cta * kProfPhases + v) * kProfStamps + 5] = globaltimer_ns();
+        vstamp(P, cta, v, 0);
+        if (P.prof_on && cta < kProfCtas && v < kProfPhases - 1) P.prof[((size_t)cta * kProfPhases + v) * kProfStamps + 5] = globaltimer_ns();
       }
       const Work2 w = work_desc(x, S, ML, D, P.claim);
       float *xb = xs + b * kXHalf;
       if (x.kind == 1 && x.type == P2_ATTN) {
         const int j = x.j, k = S.stage[j];
-        if (tid == 0) prof_stamp(P, cta, v, 1);
+        if (tid == 0) vstamp(P, cta, v, 1);
         // ---- split-KV decode attention (as in spd_mega.cu; scratch = this visit's buffer, q read per item) ----
         int *done_list = reinterpret_cast<int *>(xb + 10 * G * kAttnSplit);   // [kAttnDoneMax] item ids
         int *merge_cnt = done_list + kAttnDoneMax;                            // [1]
@@ -556,9 +562,10 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
           }
         }
       } else if (x.kind == 1) {
-        if (tid == 0) prof_stamp(P, cta, v, 1);
+        if (tid == 0) vstamp(P, cta, v, 1);
         const int t = x.type == P2_QKV ? PH_QKV : x.type == P2_O ? PH_O : x.type == P2_GU ? PH_GATEUP : PH_DOWN;
-        gemv_stream(P, S, t, w.job, x.pass, w.nc, ring, full, empty, meta, xb, gpart, seq, rope_s + x.j * 64);
+        gemv_stream(P, S, t, w.job, x.pass, w.nc, ring, full, empty, meta, xb, gpart, seq,
+                    reinterpret_cast<const float2 *>(xb + ML.nc_d * kTileCols));   // QKV: the stager's RoPE table
         if (x.type == P2_QKV) fence_proxy_async();   // the appended K/V rows are read by TMA (async proxy) next
       } else {
         // ---- PDM phase / LM head: staged by the consumers themselves (whole buffer), as in spd_mega.cu ----
@@ -606,7 +613,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
           if (x.kind == 2) for (int i = K + tid; i < kpad; i += kConsumerThreads) xs[kXHalf + i] = 0.f;
         }
         consumer_sync();
-        if (tid == 0) prof_stamp(P, cta, v, 1);
+        if (tid == 0) vstamp(P, cta, v, 1);
         if (k < 0) {                               // nothing to stream: one END slot, read by every warp
           const uint32_t slot = seq % kStages;
           mbar_wait(&full[slot], (seq / kStages) & 1);
@@ -628,11 +635,11 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
             P.cand_idx[tid * kMaxCand + cta] = bi == 0x7fffffff ? -1 : bi;
           }
         } else {
-          gemv_stream(P, S, PH_PDM, k, 0, w.nc, ring, full, empty, meta, xs, gpart, seq, rope_s);
+          gemv_stream(P, S, PH_PDM, k, 0, w.nc, ring, full, empty, meta, xs, gpart, seq, nullptr);
         }
       }
       // ---- hand the buffer back to the stager and the visit's outputs to the publisher ------------------------
-      if (tid == 0) prof_stamp(P, cta, v, 2);
+      if (tid == 0) vstamp(P, cta, v, 2);
       consumer_sync();
       if (tid == 0) {
         mbar_arrive(&xempty[b]);
@@ -666,7 +673,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
 
 // ------------------------------------------------------------------ host side ------------------
 static int mega2_smem_bytes() {
-  return kStages * kTileBytes + kXFloats * 4 + 2 * kStages * 8 + 4 * 8 + kMaxChains * 64 * 8 + 16 * 4 + 32 * 4 + 16 * 4 + 128 * 4 +
+  return kStages * kTileBytes + kXFloats * 4 + 2 * kStages * 8 + 4 * 8 + 16 * 4 + 32 * 4 + 16 * 4 + 128 * 4 +
          4 * 4 + (int)sizeof(Sched2);   // sred[3] + vdone
 }
 
@@ -680,7 +687,7 @@ int mega2_create(const DevPtrs &P, const MegaPlan &base, Mega2Plan *plan) {
   const int G = D.Hq / D.Hkv, qd = D.Hq * D.hd;
   // every visit's vector and the attention scratch (+ its completion lists) must fit one 24 KB buffer; the claim /
   // profile tables hold 2 + 6 L/n phases
-  if (D.d > kXHalf || qd > kXHalf || ML.nc_fa * kTileCols > kXHalf || G > 4 ||
+  if (ML.nc_d * kTileCols + 2 * 64 > kXHalf || D.hd > 128 || qd > kXHalf || ML.nc_fa * kTileCols > kXHalf || G > 4 ||
       10 * G * kAttnSplit + kAttnDoneMax * 9 + 1 > kXHalf || 2 + kPhasesPerPass * D.per > kProfPhases) return -1;
   const int smem = mega2_smem_bytes();
   if (cudaFuncSetAttribute(k_spd_cycle2, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
@@ -693,6 +700,7 @@ int mega2_create(const DevPtrs &P, const MegaPlan &base, Mega2Plan *plan) {
     return -1;
   }
   plan->smem_bytes = smem;
+  plan->chains = kMega2DefaultChains;
   plan->available = 1;
   return 0;
 }
@@ -701,6 +709,7 @@ int mega2_enqueue_step(const DevPtrs &P, const MegaPlan &base, const Mega2Plan &
   if (!plan.available || !base.available) return -1;
   MegaLayout ML;
   memcpy(&ML, base.layout, sizeof ML);
+  ML.chains = plan.chains;
   DevPtrs Pc = P;
   CUtensorMap tm;
   memcpy(&tm, base.kv_tmap, sizeof tm);

@@ -38,6 +38,7 @@ struct MegaLayout {
   // off_dnb.  The one-chain engine streams a unit's tiles from both places in column order (same products, same order);
   // the two-chain engine runs the parts as two phases so that an activation buffer is 24 KB.
   int nc_fa;
+  int chains;                                   // spd_mega2.cu: stage chains a CTA serves at most (SPD_OPT_CHAINS)
 };
 
 // Per-cycle schedule, computed identically by every CTA from the device state.

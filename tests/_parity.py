@@ -88,6 +88,18 @@ def kv_compare(gpu, ora, layers, rows, rep: Report, tol: float):
     return True
 
 
+def set_engine(gpu, engine):
+    """engine: None (library default), 0 / 1 / 2, or (2, chains) = engine 2 with SPD_OPT_CHAINS = chains."""
+    from paper_2605_30852_b200 import OPT
+    if engine is None:
+        return
+    if isinstance(engine, tuple):
+        gpu.set_option(OPT.ENGINE, engine[0])
+        gpu.set_option(OPT.CHAINS, engine[1])
+    else:
+        gpu.set_option(OPT.ENGINE, engine)
+
+
 def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, engine=None, tensor_every=1,
                tensor_tol=CONTRACT, check_logits=True, prefill_block=16, max_seq=None, gpu=None, prefill_mode=None) -> Report:
     """forced = (truth tokens, p, seed) or None (the PDM's own drafts).  tensor_tol bounds hidden states,
@@ -106,8 +118,7 @@ def run_parity(shape, weights_np, dev_weights, prompt, n_tokens, forced=None, en
         return rep
 
     try:
-        if engine is not None:
-            gpu.set_option(OPT.ENGINE, engine)
+        set_engine(gpu, engine)
         if prefill_mode is not None:             # 1: batched tensor-core prefill (the default), 0: through the decode kernel
             gpu.set_option(OPT.PREFILL, prefill_mode)
         gpu.set_option(OPT.DEBUG_LOGITS, 1)      # the measured logit difference sets the tie band
@@ -270,8 +281,7 @@ def run_sampling_parity(shape, weights_np, dev_weights, prompt, n_tokens, temper
         return rep
 
     try:
-        if engine is not None:
-            gpu.set_option(OPT.ENGINE, engine)
+        set_engine(gpu, engine)
         if greedy_steps:      # greedy prefill + cycles first; sampling is switched on with tokens in flight
             gpu.set_option(OPT.DEBUG_LOGITS, 1)
         else:
