@@ -426,22 +426,23 @@ def run_gpu(args, shape):
         return
     peak, peak_src = measured_peak()
     achieved = by["full"] / tot["kernel_us"] / 1e3               # GB/s per GPU
+    kname = {1: "k_spd_cycle", 2: "k_spd_cycle2"}.get(eng.get_option(spd.OPT.ENGINE), "reference engine (kernel per op)")
     line = {
         "metric": METRIC, "value": tot["step_us"], "unit": "us", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": tot["step_us"] / 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16 weights, f32 activations/accumulation", "data": "synthetic",
         "config": {"workload": f"{shape.name}: d={shape.d_model} L={shape.n_layers} n={n} F={shape.d_ffn} V={shape.vocab}, "
                                f"prompt {P}, saturated cycles at forced p=1.0 (context ~{ctx_mid})",
-                   "engine": "fused persistent cycle kernel" if launches == args.steps else "reference (kernel per op)",
+                   "engine": ENGINE_NAMES[eng.get_option(spd.OPT.ENGINE)], "chains": eng.get_option(spd.OPT.CHAINS),
                    "l2": "working set %.1f GB per step >> 126 MB L2: no flush needed" % (by["full"] / 1e9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "tokens_per_s": tot["tokens_per_s"], "hbm_gbs": tot["hbm_gbs"],
         "frac_of_8tbs": {"strict": by["strict"] / tot["kernel_us"] / 1e3 / NOMINAL_HBM_GBS,
                          "full": by["full"] / tot["kernel_us"] / 1e3 / NOMINAL_HBM_GBS},
-        "roofline": {"bound": "hbm", "kernel": "k_spd_cycle", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "roofline": {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "peak_source": peak_src, "algorithmic_bytes": by["full"],
                      "algorithmic_bytes_strict": by["strict"], "launch_us": tot["kernel_us"],
-                     "traffic": recorded_traffic("k_spd_cycle")},
+                     "traffic": recorded_traffic(kname)},
         "e2e": {"value": tot["e2e_us"], "unit": "us", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": d2h,
                 "note": "spd_step(): launch + result/state D2H + stream sync per cycle; the cycle has no per-step host input "
                         "(ring, KV and lengths live on the device)"},
@@ -461,6 +462,8 @@ def run_gpu(args, shape):
     eng.close()
 
 
+ENGINE_NAMES = {0: "reference (kernel per op)", 1: "fused persistent cycle kernel k_spd_cycle (one stage chain per CTA)",
+                2: "fused persistent cycle kernel k_spd_cycle2 (multiplexed stage chains)"}
 PHASE_NAMES = {0: "PDM", 1: "QKV", 2: "ATTN", 3: "O", 4: "GATEUP", 5: "DOWN", 6: "HEAD"}
 
 
@@ -623,7 +626,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", default="9b_n4", choices=sorted(si.CONFIGS))
     ap.add_argument("--impl", default="spd", choices=["spd", "reference"])
-    ap.add_argument("--engine", type=int, default=None, help="0 reference engine, 1 fused engine (default: library default)")
+    ap.add_argument("--engine", type=int, default=None, help="0 reference engine, 1 / 2 fused engines (default: library default = 2)")
     ap.add_argument("--chains", type=int, default=None, help="engine 2: stage chains per CTA, 1..4 (default: library default)")
     ap.add_argument("--seed", type=int, default=1234)
     ap.add_argument("--no-cpu-baseline", action="store_true")

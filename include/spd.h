@@ -105,11 +105,13 @@ typedef struct {
 
 /* Engine options (spd_set_option). */
 enum {
-  SPD_OPT_ENGINE = 0,      /* 0 = one kernel per operation (reference engine), 1 = persistent fused
-                              step kernel (default when available)                               */
+  SPD_OPT_ENGINE = 0,      /* 0 = one kernel per operation (reference engine), 1 = persistent fused step kernel, one stage
+                              chain per CTA (spd_mega.cu), 2 = persistent fused step kernel with multiplexed stage chains
+                              (spd_mega2.cu; default when available, else 1, else 0)                                  */
   SPD_OPT_DEBUG_LOGITS = 1,/* 1 = also write full verify/PDM logit vectors (for parity tests)    */
   SPD_OPT_PHASE_PROFILE = 2,/* 1 = the fused kernel records per-phase clock stamps (SPD_DBG_PHASE_PROFILE) */
-  SPD_OPT_CHAINS = 4,      /* engine 2 only: stage chains a CTA serves in turn, 1..4 (results do not depend on it)          */
+  SPD_OPT_CHAINS = 4,      /* engine 2 only: stage chains a CTA serves in turn, 1..4 (default 2; 3 for n_stages > 8; results
+                              do not depend on it)                                                                  */
   SPD_OPT_PREFILL = 3      /* 1 = batched tensor-core prefill (tcgen05 GEMMs over chunks of the prompt; default when the
                               configuration supports it: d_model, n_q_heads*head_dim, d_ffn multiples of 64),
                               0 = the prompt runs through the decode kernel, one token entering per cycle          */
@@ -256,6 +258,9 @@ int spd_pdm_query_sizes(const spd_config *cfg, int32_t pdm_layers, int32_t pdm_v
 int spd_pdm_attach(spd_ctx *ctx, const spd_pdm_weights *w, void *pdm_kv, void *pdm_work);
 
 int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value);
+/* The option's current value (SPD_OPT_ENGINE: the engine that runs the next cycle; SPD_OPT_CHAINS: 0 when engine 2 is not
+ * available for this configuration).  Returns SPD_OK / SPD_EINVAL. */
+int spd_get_option(spd_ctx *ctx, int32_t option, int32_t *value);
 
 /* Copies internal state to HOST memory (parity tests).  bytes must match the selector's size
  * (KV selectors: a multiple of the row size, at most max_seq rows). */

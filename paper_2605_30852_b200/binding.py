@@ -129,6 +129,7 @@ def lib():
         L.spd_rollback.argtypes = [vp, i32, i32]
         L.spd_set_forced.argtypes = [vp, vp, i32, f32, u64]
         L.spd_set_option.argtypes = [vp, i32, i32]
+        L.spd_get_option.argtypes = [vp, i32, C.POINTER(i32)]
         L.spd_set_sampling.argtypes = [vp, f32, i32, u64]
         L.spd_op_topk_softmax.argtypes = [vp, i32, i32, f32, i32, vp, vp, vp]
         L.spd_op_topk_scratch.argtypes = []
@@ -348,6 +349,11 @@ class SPD:
 
     def set_option(self, option: int, value: int):
         self._check(lib().spd_set_option(self._h, option, value))
+
+    def get_option(self, option: int) -> int:
+        v = C.c_int32()
+        self._check(lib().spd_get_option(self._h, option, C.byref(v)))
+        return int(v.value)
 
     def counters(self):
         k, n, l = C.c_int64(), C.c_int64(), C.c_int64()

@@ -124,7 +124,7 @@ static size_t carve_work(const spd_config *c, void *base, DevPtrs *P, const uint
   Q.results = cv.take<StepResult>(kResultRing);
   Q.cycle_ts = cv.take<unsigned long long>(2 * (size_t)kResultRing);
   Q.bar = cv.take<unsigned int>(kBarWords);
-  Q.claim = cv.take<unsigned int>((size_t)kProfPhases * kMaxStages);
+  Q.claim = cv.take<unsigned int>((size_t)kClaimPhases * kMaxStages);
   Q.prof = cv.take<unsigned long long>((size_t)kProfCtas * kProfPhases * kProfStamps);
   Q.samp = cv.take<SampleState>(1);
   Q.samp_val = cv.take<float>(kSampCap);
@@ -516,6 +516,18 @@ extern "C" int spd_set_option(spd_ctx *ctx, int32_t option, int32_t value) {
     return SPD_OK;
   }
   return fail(ctx, SPD_EINVAL, "unknown option%s");
+}
+
+extern "C" int spd_get_option(spd_ctx *ctx, int32_t option, int32_t *value) {
+  if (!ctx || !value) return SPD_EINVAL;
+  switch (option) {
+    case SPD_OPT_ENGINE: *value = ctx->engine; return SPD_OK;
+    case SPD_OPT_DEBUG_LOGITS: *value = ctx->P.debug_logits; return SPD_OK;
+    case SPD_OPT_PHASE_PROFILE: *value = ctx->P.prof_on; return SPD_OK;
+    case SPD_OPT_PREFILL: *value = ctx->prefill_mode; return SPD_OK;
+    case SPD_OPT_CHAINS: *value = ctx->has_mega2 ? ctx->mega2.chains : 0; return SPD_OK;
+    default: return fail(ctx, SPD_EINVAL, "unknown option%s");
+  }
 }
 
 extern "C" int spd_get_counters(spd_ctx *ctx, int64_t *steps, int64_t *emitted, int64_t *kernel_launches) {

@@ -17,6 +17,7 @@ constexpr int kBarGroup0 = 64;
 constexpr int kBarWords = kBarGroup0 + 32 * (kMaxStages + 2);
 // Optional per-phase clock stamps of the fused kernel (SPD_OPT_PHASE_PROFILE): [cta][phase][stamp]
 constexpr int kProfCtas = 160, kProfPhases = 168, kProfStamps = 6;
+constexpr int kClaimPhases = 200;   // rows of the work-claim table: 2 + 6 * (L / n) phases of a cycle (engine 2 at L = 32, n = 1: 194)
 
 // Sampling verification ("under sampling we apply standard rejection
 // sampling", :141 "T=1 ... top-k=50 and top-p=1.0"; readings S-1..S-9 of DESIGN.md).
@@ -112,7 +113,7 @@ struct DevPtrs {
   StepResult *results;               // [kResultRing]
   unsigned long long *cycle_ts;      // [kResultRing][2] %globaltimer (ns) when the cycle's controller began / ended, filed like results
   unsigned int *bar;                 // grid-barrier words (fused engine)
-  unsigned int *claim;               // [kProfPhases][kMaxStages] work-claim counters of one cycle (fused engine)
+  unsigned int *claim;               // [kClaimPhases][kMaxStages] work-claim counters of one cycle (fused engine)
   uint16_t *kv;                      // K/V cache
   const uint16_t *embed, *final_norm, *pdm_proj, *pdm_norm;
   const uint16_t *const *attn_norm, *const *wq, *const *wk, *const *wv, *const *wo, *const *mlp_norm,

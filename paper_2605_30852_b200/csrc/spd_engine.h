@@ -27,7 +27,7 @@ int mega_enqueue_step(const DevPtrs &P, const MegaPlan &plan, cudaStream_t sm, l
 // Fused persistent engine with multiplexed stage chains (spd_mega2.cu): the same repacked weights, layout and K/V tensor map
 // (MegaPlan), its own launch geometry.
 #ifndef SPD_DEFAULT_FUSED_ENGINE
-#define SPD_DEFAULT_FUSED_ENGINE 1
+#define SPD_DEFAULT_FUSED_ENGINE 2
 #endif
 constexpr int kMega2DefaultChains = 2, kMega2MaxChains = 4;
 struct Mega2Plan {

@@ -507,7 +507,7 @@ static void make_layout(const Dims &D, MegaLayout *ML, size_t *total) {
 static bool mega_supported(const Dims &D) {
   int qd = D.Hq * D.hd;
   int G = D.Hq / D.Hkv;
-  // 2 + 5 * (L / n) phases must fit the claim-counter / profile tables (P.claim is [kProfPhases][kMaxStages])
+  // 2 + 5 * (L / n) phases must fit the claim-counter table (P.claim is [kClaimPhases][kMaxStages]) and the profile table
   return D.d <= kXFloats / 2 && qd <= kXFloats && D.F <= kXFloats && (G == 1 || G == 2 || G == 4 || G == 8) &&
          (qd + 2 * D.Hkv * D.hd) % 2 == 0 && D.hd % 2 == 0 && 2 + 5 * D.per <= kProfPhases;
 }

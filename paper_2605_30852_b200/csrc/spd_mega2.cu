@@ -688,7 +688,7 @@ int mega2_create(const DevPtrs &P, const MegaPlan &base, Mega2Plan *plan) {
   // every visit's vector and the attention scratch (+ its completion lists) must fit one 24 KB buffer; the claim /
   // profile tables hold 2 + 6 L/n phases
   if (ML.nc_d * kTileCols + 2 * 64 > kXHalf || D.hd > 128 || qd > kXHalf || ML.nc_fa * kTileCols > kXHalf || G > 4 ||
-      10 * G * kAttnSplit + kAttnDoneMax * 9 + 1 > kXHalf || 2 + kPhasesPerPass * D.per > kProfPhases) return -1;
+      10 * G * kAttnSplit + kAttnDoneMax * 9 + 1 > kXHalf || 2 + kPhasesPerPass * D.per > kClaimPhases) return -1;
   const int smem = mega2_smem_bytes();
   if (cudaFuncSetAttribute(k_spd_cycle2, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
     cudaGetLastError();
@@ -700,7 +700,7 @@ int mega2_create(const DevPtrs &P, const MegaPlan &base, Mega2Plan *plan) {
     return -1;
   }
   plan->smem_bytes = smem;
-  plan->chains = kMega2DefaultChains;
+  plan->chains = D.n > 8 ? 3 : kMega2DefaultChains;   // measured: 2 at n = 4 and 8, 3 at n = 16
   plan->available = 1;
   return 0;
 }

@@ -26,7 +26,7 @@ def _state_equal(gpu, ora, what):
     assert (K, N) == (ora.steps, ora.emitted), what
 
 
-@pytest.mark.parametrize("engine", [0, 1])
+@pytest.mark.parametrize("engine", [0, 1, 2])
 @pytest.mark.parametrize("n,seed", [(1, 0), (2, 1), (4, 2), (4, 3), (8, 4), (2, 5), (4, 6), (8, 7), (1, 8), (4, 9), (2, 10),
                                     (8, 11)])
 def test_random_call_sequences_match_the_oracle(engine, n, seed):

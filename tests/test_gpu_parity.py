@@ -1,5 +1,6 @@
-"""GPU-vs-oracle parity of the whole SPD path (-m gpu), through the C ABI, for both engines
-(0 = one kernel per op, 1 = the fused persistent kernel).
+"""GPU-vs-oracle parity of the whole SPD path (-m gpu), through the C ABI, for all engines
+(0 = one kernel per op, 1 = the fused persistent kernel with one stage chain per CTA, 2 = the fused persistent kernel with
+multiplexed stage chains — the library's default; (2, c) = engine 2 with SPD_OPT_CHAINS = c).
 
 Token ids, accept bits, fills, committed lengths and KV lengths: exact (ties within the logit tolerance
 follow tests/_parity.py's protocol and are counted).  Hidden states, PDM vector and logits: max relative
@@ -15,25 +16,25 @@ from tests._util import TINY, shape_of
 
 pytestmark = pytest.mark.gpu
 
-ENGINES = [0, 1]
-_HAS_MEGA = None
+ENGINES = [0, 1, 2]
+_HAS_MEGA = {}
 
 
 def _need_engine(engine):
-    global _HAS_MEGA
-    if engine == 0:
+    e = engine[0] if isinstance(engine, tuple) else engine
+    if e == 0:
         return
-    if _HAS_MEGA is None:
+    if e not in _HAS_MEGA:
         import paper_2605_30852_b200 as spd
         g = spd.SPD(TINY, spd.upload_weights(si.make_weights(TINY)))
         try:
-            g.set_option(spd.OPT.ENGINE, 1)
-            _HAS_MEGA = True
+            g.set_option(spd.OPT.ENGINE, e)
+            _HAS_MEGA[e] = True
         except spd.SpdError:
-            _HAS_MEGA = False
+            _HAS_MEGA[e] = False
         finally:
             g.close()
-    assert _HAS_MEGA, "the fused engine must be available on a B200 (spd_create could not set it up)"
+    assert _HAS_MEGA[e], f"fused engine {e} must be available on a B200 (spd_create could not set it up)"
 
 
 def _inputs(shape, prompt_len, seed=1234, std=0.02, random_gains=False, attention_heavy=False):
@@ -107,17 +108,36 @@ def test_full_model_dims_short_prompt(engine, name, prompt_len, gen):
     assert rep.max_hidden_err < CONTRACT and rep.max_logit_err < CONTRACT
 
 
+@pytest.mark.parametrize("engine", [1, 2])
 @pytest.mark.parametrize("hq,hkv", [(8, 2), (8, 1), (4, 2), (2, 2)])
-def test_tensor_core_attention_path_midsize(hq, hkv):
+def test_tensor_core_attention_path_midsize(hq, hkv, engine):
     """head_dim 128 with a 300-token prompt: two full 128-row splits per head go through the fused engine's
     mma.sync attention (swizzled K/V boxes, q and probabilities split into bf16 hi + lo), the ragged third
     split through the scalar path; G = 4, 8 (q read from global), 2, 1.  Attention-heavy weights (C-4) make an
     attention error visible in the hidden state; compared with the oracle cycle by cycle at 5e-4."""
-    _need_engine(1)
+    _need_engine(engine)
+    if engine == 2 and hq // hkv > 4:
+        pytest.skip("engine 2 takes G <= 4 (spd_create falls back to engine 1 for this shape)")
     shape = si.ModelShape("mid", 512, 4, 2, hq, hkv, 128, 1024, 2048, 300, 24, ())
     inp = _inputs(shape, 300, std=0.04, attention_heavy=True)
-    rep = run_parity(**inp, n_tokens=24, engine=1, tensor_tol=5e-4, prefill_mode=0)   # the decode kernel's attention, prompt included
+    rep = run_parity(**inp, n_tokens=24, engine=engine, tensor_tol=5e-4, prefill_mode=0)   # the decode kernel's attention, prompt included
     print(f"mid Hq={hq} Hkv={hkv}:", rep.summary())
     assert rep.status == "ok", rep.detail
     assert_ties(rep)
     assert rep.max_hidden_err < 5e-4 and rep.max_logit_err < 5e-4
+
+
+@pytest.mark.parametrize("chains", [1, 3, 4])
+@pytest.mark.parametrize("n,p", [(4, 0.6), (8, 0.8), (8, None)])
+def test_tiny_engine2_chain_counts(n, p, chains):
+    """Engine 2 with 1, 3 and 4 stage chains per CTA (the default is 2): odd splits of the active stages into CTA groups
+    (3 + 3 + 2 at n = 8, a single chain, bubbles after rejects) — results do not depend on the grouping."""
+    _need_engine(2)
+    shape = shape_of("tiny", n)
+    inp = _inputs(shape, 32)
+    G = 40
+    forced = None if p is None else (_truth(shape, inp, G + 8), p, 7)
+    rep = run_parity(**inp, n_tokens=G, forced=forced, engine=(2, chains), tensor_tol=5e-3)
+    print(f"tiny n={n} p={p} chains={chains}:", rep.summary())
+    assert rep.status == "ok", rep.detail
+    assert_ties(rep)

@@ -120,7 +120,7 @@ def run_pdm_parity(shape, w, pw, prompt, n_tokens, engine, forced_p=None, tol=5e
         gpu.close()
 
 
-@pytest.mark.parametrize("engine", [0, 1])
+@pytest.mark.parametrize("engine", [0, 1, 2])
 @pytest.mark.parametrize("n,pdm_layers,forced_p", [(1, 1, None), (2, 2, None), (4, 3, 0.7), (8, 2, 0.8), (4, 1, 1.0)])
 def test_tiny_paper_pdm(engine, n, pdm_layers, forced_p):
     shape = shape_of("tiny", n)
@@ -165,7 +165,7 @@ def test_full_model_dims_paper_pdm(name, pdm_layers):
     assert rep["ties"] <= 1
 
 
-@pytest.mark.parametrize("engine", [0, 1])
+@pytest.mark.parametrize("engine", [0, 1, 2])
 def test_external_rollback_and_second_prefill_with_the_paper_pdm(engine):
     """spd_rollback rewinds the PDM's final-row count F with the committed length (rows above are rebuilt by the next
     draft); a second spd_prefill on the same context starts a new sequence.  Step results against the oracle."""

@@ -89,7 +89,7 @@ def test_batched_prefill_against_the_oracle(name, n, P, kw, tol):
     o.close(); g.close(); h.close()
 
 
-@pytest.mark.parametrize("engine", [0, 1])
+@pytest.mark.parametrize("engine", [0, 1, 2])
 def test_decode_after_batched_prefill_matches_the_oracle(engine):
     """run_parity uses the library's default prefill (the batched one): cycles that start from its state."""
     import paper_2605_30852_b200 as spd

@@ -12,7 +12,7 @@ from tests._parity import run_sampling_parity
 from tests._util import TINY, shape_of
 
 pytestmark = pytest.mark.gpu
-ENGINES = [0, 1]
+ENGINES = [0, 1, 2]
 
 
 def _inputs(shape, prompt_len, seed=1234, std=0.02, random_gains=False):
@@ -182,7 +182,7 @@ def test_full_model_dims_paper_setting(engine, name, prompt_len, gen):
     print(f"sampling {name} engine={engine}:", rep.summary())
     assert rep.status == "ok", rep.detail
     assert rep.exact_rounds == 0          # the threshold paths were the ones that ran
-    if engine == 1:                       # most selections came from the head pass's own list, without a scan
+    if engine >= 1:                       # fused engines: most selections came from the head pass's own list, without a scan
         assert rep.prefiltered >= rep.steps // 2, rep.summary()
     else:
         assert rep.prefiltered == 0
