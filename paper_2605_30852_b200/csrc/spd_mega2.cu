@@ -19,7 +19,9 @@
 //     never touch global memory for their inputs and never poll a global counter.
 //   * two 24 KB activation buffers alternate between visits.  W_down is therefore streamed as TWO phases over the two
 //     K parts of the repacked matrix (residual += part a, then += part b: a fixed order), so no visit needs more than
-//     24 KB: 6 phases per pass (QKV, ATTN, O, GATEUP, DOWN_A, DOWN_B).  The ring keeps its 11 slots.
+//     24 KB: 6 phases per pass (QKV, ATTN, O, GATEUP, DOWN_A, DOWN_B).  The ring keeps its 11 slots.  A CTA streams
+//     DOWN_B for exactly the units it claimed in DOWN_A, so the two residual updates of a row are local and ordered and
+//     DOWN_B has no dependency on other CTAs' DOWN_A.
 //   * attention visits use their buffer as scratch; an item's q (G heads, 2 KB) arrives through the ring behind its K/V tiles.
 //   * PDM phase (visit 0) and LM head (last visit) are the one-chain engine's (foreground staging, whole buffer).
 // Results do not depend on the grouping: every row's dot product, every attention split and every merge keep their fixed
@@ -35,6 +37,10 @@ constexpr int kThreads2 = kConsumerThreads + 32 + kStagerThreads + 32;   // 8 co
 // (12 warps = 3 per SM sub-partition: the most that leaves the consumers their 168 registers)
 constexpr int kMaxChains = kMega2MaxChains;               // stage chains a CTA serves at most
 constexpr int kPhasesPerPass = 6;
+// W_down's second K part (DOWN_B) is streamed for the SAME units a CTA claimed in DOWN_A: both residual updates of a row
+// then happen in one CTA, in program order, and DOWN_B needs no cross-CTA dependency on DOWN_A (its input, the second half
+// of the SwiGLU vector, is complete since GATEUP).  A CTA stops claiming at kDnCap units; the rest of its group takes them.
+constexpr int kDnCap = 96;
 
 enum Phase2 { P2_QKV = 0, P2_ATTN = 1, P2_O = 2, P2_GU = 3, P2_DNA = 4, P2_DNB = 5 };
 
@@ -240,7 +246,8 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
   float *gpart = reinterpret_cast<float *>(meta + 16);                   // [2][8][8] warp partials of a unit
   float *sred = gpart + 128;                                             // [3] stager: warp sums of squares
   unsigned int *vdone = reinterpret_cast<unsigned int *>(sred + 3);      // [1] visits the consumers have finished
-  Sched2 *Sp = reinterpret_cast<Sched2 *>(sred + 4);
+  unsigned short *dnl = reinterpret_cast<unsigned short *>(sred + 4);    // [kMaxChains][kDnCap] W_down units this CTA claimed
+  Sched2 *Sp = reinterpret_cast<Sched2 *>(dnl + kMaxChains * kDnCap);
 
   const Dims &D = P.dim;
   const int cta = blockIdx.x, ncta = gridDim.x;
@@ -325,10 +332,27 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
       asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_w));
       asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol_kv));
       uint32_t seq = 0;
+      int dn_cnt[kMaxChains];
+      for (int j = 0; j < kMaxChains; ++j) dn_cnt[j] = 0;
       for (int v = 0; v < nv; ++v) {
         const Visit x = visit_decode(v, nv, np, m);
         const Work2 w = work_desc(x, S, ML, D, P.claim);
-        if (w.job >= 0 && w.U > 0) {
+        if (x.kind == 1 && x.type == P2_DNB) {
+          bool first = true;
+          for (int i = 0; i < dn_cnt[x.j] && w.nc > 0; ++i) {     // the units of this CTA's DOWN_A visit, in the same order
+            const int u = dnl[x.j * kDnCap + i];
+            const uint8_t *src = w.base + (unsigned long long)u * w.nc * kTileBytes;
+            for (int t = 0; t < w.nc; ++t, ++seq, src += kTileBytes) {
+              uint32_t slot = seq % kStages, itn = seq / kStages;
+              mbar_wait(&empty[slot], (itn & 1) ^ 1);
+              meta[slot] = u;
+              mbar_expect_tx(&full[slot], kTileBytes);
+              tma_load_1d(ring + (size_t)slot * kTileBytes, src, kTileBytes, &full[slot], pol_w);
+              if (first) { vstamp(P, cta, v, 3); first = false; }
+            }
+          }
+          vstamp(P, cta, v, 4);
+        } else if (w.job >= 0 && w.U > 0) {
           unsigned int next = atomicAdd(w.ctr, 1u);
           if (x.kind == 1 && x.type == P2_ATTN) {
             const int k = w.job;
@@ -385,9 +409,13 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
             }
           } else {
             bool first = true;
+            const bool is_dna = x.kind == 1 && x.type == P2_DNA;
+            int ndn = 0;
             while (next < (unsigned int)w.U) {
               const int u = (int)next;
-              next = atomicAdd(w.ctr, 1u);         // claim ahead: its latency hides behind this unit's tiles
+              if (is_dna) dnl[x.j * kDnCap + ndn++] = (unsigned short)u;
+              next = (is_dna && ndn == kDnCap) ? (unsigned int)w.U   // full list: leave the rest to the group
+                                               : atomicAdd(w.ctr, 1u);   // claim ahead: its latency hides behind this unit's tiles
               const uint8_t *src = w.base + (unsigned long long)u * w.nc * kTileBytes;
               for (int i = 0; i < w.nc; ++i, ++seq, src += kTileBytes) {
                 uint32_t slot = seq % kStages, itn = seq / kStages;
@@ -398,6 +426,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
                 if (first) { vstamp(P, cta, v, 3); first = false; }
               }
             }
+            if (is_dna) dn_cnt[x.j] = ndn;
           }
           vstamp(P, cta, v, 4);
         }
@@ -440,7 +469,10 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
         if (S.run_verify && S.exit_gsize > 0) { dp.c0 = gbar + 32 * (D.n - 1); dp.t0 = (unsigned int)(np - 2) * (unsigned int)S.exit_gsize; }
         if (S.run_pdm) { dp.c1 = pdm_done; dp.t1 = (unsigned int)ncta; }
       } else if (x.kind == 1) {
-        if (x.p >= 2) { dp.c0 = gbar + 32 * S.stage[x.j]; dp.t0 = (unsigned int)(x.p - 1) * (unsigned int)S.gsize; }
+        // DOWN_B reads the second half of the SwiGLU vector (complete since GATEUP) and updates only rows this CTA updated
+        // in DOWN_A: it waits for GATEUP (two phases back), not for DOWN_A
+        const int back = x.type == P2_DNB ? 2 : 1;
+        if (x.p >= 2) { dp.c0 = gbar + 32 * S.stage[x.j]; dp.t0 = (unsigned int)(x.p - back) * (unsigned int)S.gsize; }
         if (x.p == 1 + P2_O && S.run_pdm) { dp.c1 = pdm_staged; dp.t1 = (unsigned int)ncta; }
       }
       if (x.kind == 1 && x.type != P2_ATTN) {
@@ -674,7 +706,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
 // ------------------------------------------------------------------ host side ------------------
 static int mega2_smem_bytes() {
   return kStages * kTileBytes + kXFloats * 4 + 2 * kStages * 8 + 4 * 8 + 16 * 4 + 32 * 4 + 16 * 4 + 128 * 4 +
-         4 * 4 + (int)sizeof(Sched2);   // sred[3] + vdone
+         4 * 4 + kMaxChains * kDnCap * 2 + (int)sizeof(Sched2);   // sred[3] + vdone, dnl
 }
 
 // Shares the one-chain engine's plan (repacked weights, layout, K/V tensor map); adds only the launch geometry.
@@ -687,6 +719,10 @@ int mega2_create(const DevPtrs &P, const MegaPlan &base, Mega2Plan *plan) {
   const int G = D.Hq / D.Hkv, qd = D.Hq * D.hd;
   // every visit's vector and the attention scratch (+ its completion lists) must fit one 24 KB buffer; the claim /
   // profile tables hold 2 + 6 L/n phases
+  int sms = 0, dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (kDnCap * (sms / kMaxStages) < ML.u_dn || ML.u_dn > 65535) return -1;   // DOWN_A claims are capped per CTA (kDnCap)
   if (ML.nc_d * kTileCols + 2 * 64 > kXHalf || D.hd > 128 || qd > kXHalf || ML.nc_fa * kTileCols > kXHalf || G > 4 ||
       10 * G * kAttnSplit + kAttnDoneMax * 9 + 1 > kXHalf || 2 + kPhasesPerPass * D.per > kClaimPhases) return -1;
   const int smem = mega2_smem_bytes();
