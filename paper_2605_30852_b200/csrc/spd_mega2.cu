@@ -443,7 +443,7 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
     // (one release at gpu scope after the consumers' CTA barrier + their release on `vdone`: cumulative over what that
     // ordered before it.  A release waits until the CTA's writes are visible, 2-3 us under the weight stream: here it
     // delays nobody.)
-    if (lane == 0) {
+    if (lane == 0 && m != 1) {                   // (one chain: the consumers release their visits themselves, see below)
       for (int v = 0; v < nv; ++v) {
         while (ld_acquire_cta_shared(vdone) <= (unsigned int)v) {}
         const Visit x = visit_decode(v, nv, np, m);
@@ -675,7 +675,12 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
       consumer_sync();
       if (tid == 0) {
         mbar_arrive(&xempty[b]);
-        red_release_cta_shared_add(vdone, 1u);     // the publisher takes it from here
+        if (m != 1) red_release_cta_shared_add(vdone, 1u);     // the publisher takes it from here
+        else {   // a single chain (one active stage): the next visit depends on this one, nothing is gained by the hand-over
+          if (x.kind == 2) red_release_add_u64(bar_count, 1ull);
+          else if (x.kind == 0) { if (S.run_pdm) red_release_add_u32(pdm_done, 1u); }
+          else red_release_add_u32(gbar + 32 * S.stage[x.j], 1u);
+        }
       }
     }
   }
