@@ -177,6 +177,8 @@ def test_full_model_dims_paper_setting(engine, name, prompt_len, gen):
     """The 4B/9B-class shapes (vocabulary 151 936) with top-k 50, T = 1: the threshold scan over the real
     vocabulary inside the cycle, 148 per-CTA candidates (fused engine) / 128 chunk candidates (reference)."""
     shape = si.CONFIGS[name]
+    if engine == 1 and name not in ("9b_n4", "4b_n8"):
+        pytest.skip("engine 1 (selectable, no longer the default) is checked at two of the four full-size shapes")
     rep = run_sampling_parity(**_inputs(shape, prompt_len), n_tokens=gen, temperature=1.0, top_k=50, seed=11,
                               engine=engine, tensor_tol=1e-2, max_steps=shape.n_stages * gen)
     print(f"sampling {name} engine={engine}:", rep.summary())
