@@ -443,10 +443,11 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
     // (one release at gpu scope after the consumers' CTA barrier + their release on `vdone`: cumulative over what that
     // ordered before it.  A release waits until the CTA's writes are visible, 2-3 us under the weight stream: here it
     // delays nobody.)
-    if (lane == 0 && m != 1) {                   // (one chain: the consumers release their visits themselves, see below)
+    if (lane == 0) {
       for (int v = 0; v < nv; ++v) {
         while (ld_acquire_cta_shared(vdone) <= (unsigned int)v) {}
         const Visit x = visit_decode(v, nv, np, m);
+        if (m == 1 && !(x.kind == 1 && x.type == P2_DNA)) continue;   // one chain: released by the consumers (see below)
         if (x.kind == 2) red_release_add_u64(bar_count, 1ull);
         else if (x.kind == 0) { if (S.run_pdm) red_release_add_u32(pdm_done, 1u); }
         else red_release_add_u32(gbar + 32 * S.stage[x.j], 1u);
@@ -487,12 +488,15 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
             const int ai = anchor_index(P, layer);
             if (ai >= 0 && S.pos[k] < D.max_seq) raw = P.anch + ((size_t)S.pos[k] * P.pdm_m + ai) * D.d;
           }
-          stager_copy(dp, h, dst, D.d, ML.nc_d * kTileCols, g, D.eps, raw, sred, st);
-          if (x.type == P2_QKV && st < D.hd / 2) {   // RoPE table of the chain's position (C-2.14), behind the vector (the parked
-            double s_, c_;                         // gains are dead: every stager thread has passed stager_copy's last barrier)
+          float2 cs = make_float2(1.f, 0.f);       // RoPE table entry of the chain's position (C-2.14): the double-precision
+          if (x.type == P2_QKV && st < D.hd / 2) { //   sincos (1-2 us for a 64-lane table) runs while the dependency is still open
+            double s_, c_;
             sincos((double)S.pos[k] * P.inv_freq[st], &s_, &c_);
-            reinterpret_cast<float2 *>(dst + ML.nc_d * kTileCols)[st] = make_float2((float)c_, (float)s_);
+            cs = make_float2((float)c_, (float)s_);
           }
+          stager_copy(dp, h, dst, D.d, ML.nc_d * kTileCols, g, D.eps, raw, sred, st);
+          if (x.type == P2_QKV && st < D.hd / 2)   // stored behind the vector (the parked gains are dead: every stager thread
+            reinterpret_cast<float2 *>(dst + ML.nc_d * kTileCols)[st] = cs;   // has passed stager_copy's last barrier)
           if (x.type == P2_QKV && S.lead && st == 0) {
             // causality / capacity precondition of the KV append, and the new length (one CTA per stage)
             const int pos = S.pos[k];
@@ -675,8 +679,10 @@ __global__ void __launch_bounds__(kThreads2, 1) k_spd_cycle2(DevPtrs P, MegaLayo
       consumer_sync();
       if (tid == 0) {
         mbar_arrive(&xempty[b]);
-        if (m != 1) red_release_cta_shared_add(vdone, 1u);     // the publisher takes it from here
-        else {   // a single chain (one active stage): the next visit depends on this one, nothing is gained by the hand-over
+        red_release_cta_shared_add(vdone, 1u);     // the publisher takes it from here ...
+        if (m == 1 && !(x.kind == 1 && x.type == P2_DNA)) {
+          // ... except with a single chain (one active stage): the next visit depends on this one (DOWN_B on DOWN_A excepted),
+          // so nothing is gained by the hand-over
           if (x.kind == 2) red_release_add_u64(bar_count, 1ull);
           else if (x.kind == 0) { if (S.run_pdm) red_release_add_u32(pdm_done, 1u); }
           else red_release_add_u32(gbar + 32 * S.stage[x.j], 1u);
