@@ -143,3 +143,20 @@ def test_tiny_engine2_chain_counts(n, p, chains):
     print(f"tiny n={n} p={p} chains={chains}:", rep.summary())
     assert rep.status == "ok", rep.detail
     assert_ties(rep)
+
+
+@pytest.mark.parametrize("engine", [2, (2, 3)])
+@pytest.mark.parametrize("n,p", [(4, 0.5), (8, 0.9)])
+def test_tiny_long_generation_with_rejects(engine, n, p):
+    """600 tokens (1000-2700 cycles, hundreds of rejects and refills, the context growing over five attention splits) cycle by
+    cycle against the oracle: a soak of engine 2's stager / publisher / ring hand-overs at every fill level."""
+    _need_engine(engine)
+    shape = shape_of("tiny", n)
+    inp = _inputs(shape, 32, seed=77)
+    G = 600
+    rep = run_parity(**inp, n_tokens=G, forced=(_truth(shape, inp, G + 16), p, 5), engine=engine, tensor_tol=5e-3,
+                     tensor_every=16, max_seq=32 + 2 * G + 64)
+    print(f"tiny long n={n} p={p} engine={engine}:", rep.summary())
+    assert rep.status == "ok", rep.detail
+    assert_ties(rep)
+    assert rep.rejects > 20
