@@ -46,6 +46,21 @@ def ar_tokens(name: str = "tiny", n_tokens: int = 64, prompt_seed: int = 1, seed
     return tuple(toks)
 
 
+_LAST = {}
+
+
+def cached_last(slot: str, key, make):
+    """One-entry cache per slot: consecutive test cases that differ only in the engine reuse the seeded inputs (weights of
+    the 4B / 9B-class shapes take 10-30 s to generate and ~18 GB on the device) and the oracle's greedy continuation; a new
+    key drops the previous entry first."""
+    ent = _LAST.get(slot)
+    if ent is None or ent[0] != key:
+        _LAST.pop(slot, None)
+        ent = (key, make())
+        _LAST[slot] = ent
+    return ent[1]
+
+
 def rel_err(a: np.ndarray, b: np.ndarray) -> float:
     """SURVEY C-2.18: max_i |a_i - b_i| / max_i |b_i|."""
     a = np.asarray(a, dtype=np.float64)

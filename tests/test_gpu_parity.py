@@ -12,7 +12,7 @@ import pytest
 
 import spd_inputs as si
 from tests._parity import run_parity, assert_ties, CONTRACT
-from tests._util import TINY, shape_of
+from tests._util import TINY, shape_of, cached_last
 
 pytestmark = pytest.mark.gpu
 
@@ -39,16 +39,22 @@ def _need_engine(engine):
 
 def _inputs(shape, prompt_len, seed=1234, std=0.02, random_gains=False, attention_heavy=False):
     import paper_2605_30852_b200 as spd
-    w = si.make_weights(shape, seed=seed, std=std, random_gains=random_gains, attention_heavy=attention_heavy)
-    return dict(shape=shape, weights_np=w, dev_weights=spd.upload_weights(w), prompt=si.make_prompt(shape, seed, prompt_len))
+
+    def make():
+        w = si.make_weights(shape, seed=seed, std=std, random_gains=random_gains, attention_heavy=attention_heavy)
+        return dict(shape=shape, weights_np=w, dev_weights=spd.upload_weights(w), prompt=si.make_prompt(shape, seed, prompt_len))
+    return dict(cached_last("parity_inputs", (shape, prompt_len, seed, std, random_gains, attention_heavy), make))   # a shallow copy: callers may replace entries
 
 
 def _truth(shape, inp, n, block=16):
     from oracle import Oracle
-    o = Oracle(shape, inp["weights_np"], max_seq=len(inp["prompt"]) + n + 8)
-    t = [o.prefill(inp["prompt"], block=block)] + [o.ar_step() for _ in range(n)]
-    o.close()
-    return np.array(t, np.int32)
+
+    def make():
+        o = Oracle(shape, inp["weights_np"], max_seq=len(inp["prompt"]) + n + 8)
+        t = [o.prefill(inp["prompt"], block=block)] + [o.ar_step() for _ in range(n)]
+        o.close()
+        return np.array(t, np.int32)
+    return cached_last("parity_truth", (id(inp["weights_np"]), shape, len(inp["prompt"]), n, block), make)
 
 
 @pytest.mark.parametrize("engine", ENGINES)

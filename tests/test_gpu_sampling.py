@@ -9,7 +9,7 @@ import torch
 import oracle as ora
 import spd_inputs as si
 from tests._parity import run_sampling_parity
-from tests._util import TINY, shape_of
+from tests._util import TINY, shape_of, cached_last
 
 pytestmark = pytest.mark.gpu
 ENGINES = [0, 1, 2]
@@ -17,8 +17,11 @@ ENGINES = [0, 1, 2]
 
 def _inputs(shape, prompt_len, seed=1234, std=0.02, random_gains=False):
     import paper_2605_30852_b200 as spd
-    w = si.make_weights(shape, seed=seed, std=std, random_gains=random_gains)
-    return dict(shape=shape, weights_np=w, dev_weights=spd.upload_weights(w), prompt=si.make_prompt(shape, seed, prompt_len))
+
+    def make():
+        w = si.make_weights(shape, seed=seed, std=std, random_gains=random_gains)
+        return dict(shape=shape, weights_np=w, dev_weights=spd.upload_weights(w), prompt=si.make_prompt(shape, seed, prompt_len))
+    return dict(cached_last("sampling_inputs", (shape, prompt_len, seed, std, random_gains), make))   # a shallow copy: callers may replace entries
 
 
 # ------------------------------------------------------------------ the filter as one operation ---
